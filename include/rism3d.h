@@ -1,0 +1,154 @@
+/* rism3d.h -- C ABI of the B200-native 3D-RISM solver core (librism3d.so).
+ *
+ * The library runs the self-consistent 3D-RISM iteration of arxiv 2403.01039 (RISMiCal),
+ * PAPER.md:222-254 "numerical procedure", on one GPU in fp64:
+ *
+ *   setup (once per solute)   w_g(r) = -beta u_g(r) + f_g(r)      Eq. 22 + Eq. 29
+ *                             phi~(k), f~_g = q_g phi~             Eq. 30
+ *   loop  step 2              g = closure(w + tau),  c_sr = g-1-tau  Eq. 15-16, 31
+ *         step 3              c_sr(k) = FFT3D[c_sr] on the half-integer k grid
+ *                             c(k) = c_sr(k) - f~(k)                Eq. 32
+ *         step 4              h_g(k) = sum_g' c_g'(k) chi_g'g(|k|)  Eq. 13
+ *         step 5              tau' = FFT3D^-1[h(k) - c_sr(k)]       Eq. 33
+ *         step 6              MDIIS over M stored (tau, R = tau' - tau) pairs  Eq. 40
+ *         step 7              rms = sqrt(sum R^2 / (N n_v)) < tol    Eq. 41
+ *   post                      solvation free energy                 Eq. 17-18
+ *
+ * tau_g(r) = t_g(r) - f_g(r) is the short-range part of the paper's iteration variable t = h - c.
+ * The readings of the places where the paper is garbled or silent (KH branches, Eq. 40, Eq. 41,
+ * PSE-n, chi interpolation, units) are listed in DESIGN.md "Readings" Q1-Q16.
+ *
+ * Conventions
+ *   - Units: Angstrom, e, kcal/mol, K.  k_B = 0.001987204259 kcal/(mol K), Coulomb constant
+ *     332.06371 kcal A/(mol e^2).
+ *   - Every function returns RISM3D_OK (0) or a negative rism3d_status; nothing throws or aborts.
+ *     rism3d_last_error() gives the message of the last failure on that context.
+ *   - HOST pointers are borrowed for the duration of the call and copied.  DEVICE pointers are
+ *     said so explicitly.  The caller owns the device workspace and the CUDA stream (PyTorch
+ *     allocates them); the library owns only its small host-side context.
+ *   - All GPU work is enqueued on the stream given to rism3d_init; calls that return host values
+ *     synchronise that stream before returning.
+ *   - Real 3D fields are laid out [site][ix][iy][iz], iz fastest, n_sites*nx*ny*nz doubles;
+ *     grid point (ix,iy,iz) sits at origin + spacing*(ix,iy,iz).
+ *   - There is no CPU fallback: without a CUDA device rism3d_init fails with RISM3D_ERR_CUDA.
+ */
+#ifndef RISM3D_H
+#define RISM3D_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rism3d_ctx rism3d_ctx;   /* opaque; created by rism3d_init, freed by rism3d_destroy */
+
+typedef enum {
+  RISM3D_OK            =  0,
+  RISM3D_ERR_ARG       = -1,   /* NULL pointer, negative count, unknown enum value                 */
+  RISM3D_ERR_SIZE      = -2,   /* grid not cubic / not a power of two in 8..512, n_sites not 1,2,4,8,
+                                  mdiis_nvec outside 1..16                                         */
+  RISM3D_ERR_ORDER     = -3,   /* call out of order (set_solute before set_solvent_chi, ...)       */
+  RISM3D_ERR_CHI_RANGE = -4,   /* chi table does not cover the 3D |k| range, or is too coarse      */
+  RISM3D_ERR_NEUTRAL   = -5,   /* sum_g rho_g q_g != 0 (1e-12)                                     */
+  RISM3D_ERR_WORKSPACE = -6,   /* workspace smaller than rism3d_workspace_bytes()                  */
+  RISM3D_ERR_CUDA      = -7,   /* a CUDA call failed; message carries cudaGetErrorString           */
+  RISM3D_ERR_DIVERGED  = -8    /* non-finite residual; tau is left at the last input               */
+} rism3d_status;
+
+typedef enum { RISM3D_KH = 1, RISM3D_PSE = 2, RISM3D_HNC = 3 } rism3d_closure;
+
+/* which-codes of rism3d_get_field */
+typedef enum {
+  RISM3D_FIELD_G    = 0,   /* g = closure(w + tau)                                                 */
+  RISM3D_FIELD_H    = 1,   /* g - 1                                                                */
+  RISM3D_FIELD_C_SR = 2,   /* g - 1 - tau                         (Eq. 31)                         */
+  RISM3D_FIELD_T    = 3,   /* t = tau + q_g phi(r)                (the paper's variable)           */
+  RISM3D_FIELD_TAU  = 4,   /* the iteration variable as stored                                     */
+  RISM3D_FIELD_W    = 5,   /* -beta u + f                                                          */
+  RISM3D_FIELD_PHI  = 6    /* phi(r) of Eq. 29 (site argument ignored)                             */
+} rism3d_field;
+
+typedef struct {
+  int    nx, ny, nz;        /* grid points per axis; this build: nx == ny == nz, power of two, 8..512 */
+  double spacing;           /* grid spacing, A                                                     */
+  double origin[3];         /* position of grid index (0,0,0), A                                   */
+  int    n_sites;           /* n_v, number of solvent site TYPES: 1, 2, 4 or 8                     */
+  int    closure;           /* rism3d_closure                                                      */
+  int    pse_order;         /* n of PSE-n (>= 1; 1 is KH); ignored for KH / HNC                    */
+  double temperature;       /* K                                                                   */
+  int    mdiis_nvec;        /* M, 1..16 (1 = damped Picard iteration)                              */
+  double mdiis_b;           /* damping b of Eq. 40                                                 */
+  double mdiis_restart;     /* restart when rms > this * (smallest rms in the history); <= 0: never */
+  double kappa;             /* kappa of Eq. 29-30, 1/A (the paper: 1)                              */
+  double r_min;             /* distance clamp of the short-range potential, A (Q11)      */
+  int    device;            /* CUDA device ordinal                                                 */
+} rism3d_params;
+
+/* Bytes of DEVICE memory the caller must provide to rism3d_init (0 if the parameters are invalid). */
+size_t rism3d_workspace_bytes(const rism3d_params* params);
+
+/* Create a context.  d_workspace: DEVICE pointer, 256-byte aligned, `bytes` long, owned by the
+ * caller and kept alive until rism3d_destroy.  cuda_stream: a cudaStream_t (NULL = legacy default
+ * stream).  Builds the twiddle tables; no field is valid before set_solvent_chi + set_solute. */
+int rism3d_init(rism3d_ctx** out, const rism3d_params* params, void* d_workspace, size_t bytes,
+                void* cuda_stream);
+
+/* Solvent description (X_g'g = omega_g'g + rho_g' h_g'g from a 1D-RISM solve).
+ * HOST arrays.  q, sigma, eps, rho: [n_sites] (rho = number density of the site type, 1/A^3).
+ * chi: [n_k][n_sites][n_sites] with chi[m][g'][g] tabulated at k_m = k0 + m*dk (g' is the index
+ * summed in Eq. 13).  chi(|k|) is taken from the table by 4-point Lagrange interpolation
+ * (Q6), evaluated once per distinct |k| of the grid into a device table. */
+int rism3d_set_solvent_chi(rism3d_ctx* ctx, const double* q, const double* sigma, const double* eps,
+                           const double* rho, int n_k, double dk, double k0, const double* chi);
+
+/* Solute (Eq. 22).  HOST arrays xyz [n_atoms][3], q, sigma, eps [n_atoms].
+ * rcut <= 0: all pairs (the paper's definition); rcut > 0: the short-range remainder
+ * -beta [C q q exp(-kappa r)/r + LJ] only counts pairs with r < rcut (Q12); the
+ * long-range functions phi, phi~ are never cut.  Runs the setup kernels, sets tau = 0 (the paper's
+ * initial guess t = f) and clears the MDIIS history.  setup_ms (may be NULL)
+ * receives the GPU time of the setup kernels in milliseconds (CUDA events). */
+int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz, const double* q,
+                      const double* sigma, const double* eps, double rcut, float* setup_ms);
+
+/* Run the loop.  tol <= 0: exactly max_iter iterations.  tol > 0: stop after the first iteration
+ * whose rms residual is below tol (tau is then left unchanged by that iteration) or after max_iter.
+ * n_done (may be NULL): iterations performed by this call; rms (may be NULL): last residual.
+ * Returns RISM3D_ERR_DIVERGED when the residual became non-finite. */
+int rism3d_iterate(rism3d_ctx* ctx, int max_iter, double tol, int* n_done, double* rms);
+
+/* Solvation free energy of the current tau (Eq. 18 KH / Eq. 17 HNC / PSE-n, Q2, Q10),
+ * kcal/mol.  dmu_site: HOST [n_sites] or NULL. */
+int rism3d_free_energy(rism3d_ctx* ctx, double* dmu_total, double* dmu_site);
+
+/* Copy one field of one site (nx*ny*nz doubles, [ix][iy][iz]) to dst; dst_is_device selects a
+ * DEVICE or HOST destination. */
+int rism3d_get_field(rism3d_ctx* ctx, int which, int site, double* dst, int dst_is_device);
+
+/* Overwrite tau of one site (warm start); clears the MDIIS history. */
+int rism3d_set_tau(rism3d_ctx* ctx, int site, const double* src, int src_is_device);
+
+/* rms residual of every iteration since the last set_solute (at most the last 65536), HOST dst. */
+int rism3d_get_rms_history(rism3d_ctx* ctx, double* dst, int cap, int* n);
+
+/* Number of kernels the library has launched on this context so far (for bench.py's gpu_launches). */
+long long rism3d_launch_count(const rism3d_ctx* ctx);
+
+/* Debug / test hooks: run the shifted 3D transform pair alone on a caller-supplied field.
+ * forward: real DEVICE field [n_sites][nx][ny][nz] -> complex DEVICE spectrum
+ *   [jx][jy][p][site] (re, im interleaved), p = 0..nz/2-1 standing for jz = 2p, holding
+ *   sum_n f(r_n) exp(-i k_j.(r_n - origin)) with k_j = dk (j + 1/2) per axis (no dV factor).
+ * inverse: the exact inverse of that map (includes 1/(nx ny nz)). */
+int rism3d_debug_fft_forward(rism3d_ctx* ctx, const double* d_real_in, double* d_spec_out);
+int rism3d_debug_fft_inverse(rism3d_ctx* ctx, const double* d_spec_in, double* d_real_out);
+
+const char* rism3d_last_error(const rism3d_ctx* ctx);   /* valid until the next call on ctx */
+const char* rism3d_status_string(int status);           /* static strings                    */
+
+/* Frees the host context (not the workspace).  NULL is allowed. */
+void rism3d_destroy(rism3d_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RISM3D_H */

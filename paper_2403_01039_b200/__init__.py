@@ -1,0 +1,14 @@
+"""B200-native 3D-RISM solver core (arxiv 2403.01039, RISMiCal): Python binding of librism3d.so.
+
+Everything numerical runs in the hand-written sm_100a kernels behind the C ABI of include/rism3d.h;
+this package only marshals arguments (ctypes) and uses PyTorch for device memory and streams.
+There is no CPU fallback: importing works anywhere, but creating a solver without the built library
+or without a CUDA device raises.
+"""
+from .binding import (  # noqa: F401
+    CLOSURES, FIELDS, Rism3dError, Rism3dParams, Solver, library_path, load_library,
+    rism3d_workspace_bytes, rism3d_init, rism3d_set_solvent_chi, rism3d_set_solute, rism3d_iterate,
+    rism3d_free_energy, rism3d_get_field, rism3d_set_tau, rism3d_get_rms_history, rism3d_launch_count,
+    rism3d_debug_fft_forward, rism3d_debug_fft_inverse, rism3d_last_error, rism3d_status_string,
+    rism3d_destroy, EXPORTED_SYMBOLS,
+)

@@ -1,0 +1,295 @@
+"""ctypes binding of librism3d.so -- same names as include/rism3d.h, argument marshalling only.
+
+`Solver` is a thin convenience object that owns the device workspace (a torch uint8 tensor) and the
+opaque context; every method is one C call.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB = None
+
+CLOSURES = {"KH": 1, "PSE": 2, "HNC": 3}
+FIELDS = {"G": 0, "H": 1, "C_SR": 2, "T": 3, "TAU": 4, "W": 5, "PHI": 6}
+
+EXPORTED_SYMBOLS = [
+    "rism3d_workspace_bytes", "rism3d_init", "rism3d_set_solvent_chi", "rism3d_set_solute",
+    "rism3d_iterate", "rism3d_free_energy", "rism3d_get_field", "rism3d_set_tau",
+    "rism3d_get_rms_history", "rism3d_launch_count", "rism3d_debug_fft_forward",
+    "rism3d_debug_fft_inverse", "rism3d_last_error", "rism3d_status_string", "rism3d_destroy",
+]
+
+
+class Rism3dError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"rism3d status {status}: {message}")
+        self.status = status
+
+
+class Rism3dParams(C.Structure):
+    _fields_ = [
+        ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int),
+        ("spacing", C.c_double),
+        ("origin", C.c_double * 3),
+        ("n_sites", C.c_int),
+        ("closure", C.c_int),
+        ("pse_order", C.c_int),
+        ("temperature", C.c_double),
+        ("mdiis_nvec", C.c_int),
+        ("mdiis_b", C.c_double),
+        ("mdiis_restart", C.c_double),
+        ("kappa", C.c_double),
+        ("r_min", C.c_double),
+        ("device", C.c_int),
+    ]
+
+
+def library_path() -> str:
+    return os.path.join(_HERE, "librism3d.so")
+
+
+def load_library():
+    """Load librism3d.so; raises (never falls back) when it has not been built."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = library_path()
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} not found: build it with `python -m paper_2403_01039_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(path)
+    dp, ip = C.POINTER(C.c_double), C.POINTER(C.c_int)
+    lib.rism3d_workspace_bytes.restype = C.c_size_t
+    lib.rism3d_workspace_bytes.argtypes = [C.POINTER(Rism3dParams)]
+    lib.rism3d_init.restype = C.c_int
+    lib.rism3d_init.argtypes = [C.POINTER(C.c_void_p), C.POINTER(Rism3dParams), C.c_void_p, C.c_size_t, C.c_void_p]
+    lib.rism3d_set_solvent_chi.restype = C.c_int
+    lib.rism3d_set_solvent_chi.argtypes = [C.c_void_p, dp, dp, dp, dp, C.c_int, C.c_double, C.c_double, dp]
+    lib.rism3d_set_solute.restype = C.c_int
+    lib.rism3d_set_solute.argtypes = [C.c_void_p, C.c_int, dp, dp, dp, dp, C.c_double, C.POINTER(C.c_float)]
+    lib.rism3d_iterate.restype = C.c_int
+    lib.rism3d_iterate.argtypes = [C.c_void_p, C.c_int, C.c_double, ip, dp]
+    lib.rism3d_free_energy.restype = C.c_int
+    lib.rism3d_free_energy.argtypes = [C.c_void_p, dp, dp]
+    lib.rism3d_get_field.restype = C.c_int
+    lib.rism3d_get_field.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]
+    lib.rism3d_set_tau.restype = C.c_int
+    lib.rism3d_set_tau.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int]
+    lib.rism3d_get_rms_history.restype = C.c_int
+    lib.rism3d_get_rms_history.argtypes = [C.c_void_p, dp, C.c_int, ip]
+    lib.rism3d_launch_count.restype = C.c_longlong
+    lib.rism3d_launch_count.argtypes = [C.c_void_p]
+    lib.rism3d_debug_fft_forward.restype = C.c_int
+    lib.rism3d_debug_fft_forward.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.rism3d_debug_fft_inverse.restype = C.c_int
+    lib.rism3d_debug_fft_inverse.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.rism3d_last_error.restype = C.c_char_p
+    lib.rism3d_last_error.argtypes = [C.c_void_p]
+    lib.rism3d_status_string.restype = C.c_char_p
+    lib.rism3d_status_string.argtypes = [C.c_int]
+    lib.rism3d_destroy.restype = None
+    lib.rism3d_destroy.argtypes = [C.c_void_p]
+    _LIB = lib
+    return lib
+
+
+def _dptr(a: np.ndarray):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+
+
+def _check(ctx, status: int):
+    if status != 0:
+        lib = load_library()
+        msg = lib.rism3d_last_error(ctx).decode() if ctx else ""
+        raise Rism3dError(status, msg or lib.rism3d_status_string(status).decode())
+
+
+# ---- the C calls, one Python function each -------------------------------------------------------
+def rism3d_status_string(status: int) -> str:
+    return load_library().rism3d_status_string(int(status)).decode()
+
+
+def rism3d_last_error(ctx) -> str:
+    return load_library().rism3d_last_error(ctx).decode()
+
+
+def rism3d_workspace_bytes(params: Rism3dParams) -> int:
+    return int(load_library().rism3d_workspace_bytes(C.byref(params)))
+
+
+def rism3d_init(params: Rism3dParams, d_workspace: int, nbytes: int, cuda_stream: int):
+    ctx = C.c_void_p()
+    st = load_library().rism3d_init(C.byref(ctx), C.byref(params), C.c_void_p(d_workspace), nbytes,
+                                    C.c_void_p(cuda_stream))
+    if st != 0:
+        raise Rism3dError(st, rism3d_status_string(st))
+    return ctx
+
+
+def rism3d_set_solvent_chi(ctx, q, sigma, eps, rho, k0: float, dk: float, chi):
+    q, sigma, eps, rho, chi = _f64(q), _f64(sigma), _f64(eps), _f64(rho), _f64(chi)
+    _check(ctx, load_library().rism3d_set_solvent_chi(ctx, _dptr(q), _dptr(sigma), _dptr(eps), _dptr(rho),
+                                                      int(chi.shape[0]), float(dk), float(k0), _dptr(chi)))
+
+
+def rism3d_set_solute(ctx, xyz, q, sigma, eps, rcut: float = 0.0) -> float:
+    xyz, q, sigma, eps = _f64(xyz), _f64(q), _f64(sigma), _f64(eps)
+    ms = C.c_float(0.0)
+    _check(ctx, load_library().rism3d_set_solute(ctx, int(len(q)), _dptr(xyz), _dptr(q), _dptr(sigma), _dptr(eps),
+                                                 float(rcut), C.byref(ms)))
+    return float(ms.value)
+
+
+def rism3d_iterate(ctx, max_iter: int, tol: float = 0.0):
+    n, rms = C.c_int(0), C.c_double(0.0)
+    _check(ctx, load_library().rism3d_iterate(ctx, int(max_iter), float(tol), C.byref(n), C.byref(rms)))
+    return int(n.value), float(rms.value)
+
+
+def rism3d_free_energy(ctx, n_sites: int):
+    tot = C.c_double(0.0)
+    site = np.zeros(n_sites)
+    _check(ctx, load_library().rism3d_free_energy(ctx, C.byref(tot), _dptr(site)))
+    return float(tot.value), site
+
+
+def rism3d_get_field(ctx, which: int, site: int, dst_ptr: int, dst_is_device: bool):
+    _check(ctx, load_library().rism3d_get_field(ctx, int(which), int(site), C.c_void_p(dst_ptr), int(dst_is_device)))
+
+
+def rism3d_set_tau(ctx, site: int, src_ptr: int, src_is_device: bool):
+    _check(ctx, load_library().rism3d_set_tau(ctx, int(site), C.c_void_p(src_ptr), int(src_is_device)))
+
+
+def rism3d_get_rms_history(ctx, cap: int = 65536) -> np.ndarray:
+    buf = np.zeros(cap)
+    n = C.c_int(0)
+    _check(ctx, load_library().rism3d_get_rms_history(ctx, _dptr(buf), cap, C.byref(n)))
+    return buf[: n.value].copy()
+
+
+def rism3d_launch_count(ctx) -> int:
+    return int(load_library().rism3d_launch_count(ctx))
+
+
+def rism3d_debug_fft_forward(ctx, d_in: int, d_out: int):
+    _check(ctx, load_library().rism3d_debug_fft_forward(ctx, C.c_void_p(d_in), C.c_void_p(d_out)))
+
+
+def rism3d_debug_fft_inverse(ctx, d_in: int, d_out: int):
+    _check(ctx, load_library().rism3d_debug_fft_inverse(ctx, C.c_void_p(d_in), C.c_void_p(d_out)))
+
+
+def rism3d_destroy(ctx):
+    load_library().rism3d_destroy(ctx)
+
+
+# ---- convenience object --------------------------------------------------------------------------
+class Solver:
+    """Owns the workspace tensor and the context; each method is one C-ABI call."""
+
+    def __init__(self, n, spacing, n_sites, closure="KH", pse_order=1, temperature=298.0, mdiis_nvec=5,
+                 mdiis_b=0.5, mdiis_restart=10.0, kappa=1.0, r_min=1e-3, origin=None, device=0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2403_01039_b200 needs a CUDA device (no CPU fallback)")
+        load_library()
+        self.n, self.n_sites, self.spacing = int(n), int(n_sites), float(spacing)
+        p = Rism3dParams()
+        p.nx = p.ny = p.nz = self.n
+        p.spacing = self.spacing
+        org = [-(self.n // 2) * self.spacing] * 3 if origin is None else list(origin)
+        p.origin = (C.c_double * 3)(*org)
+        p.n_sites = self.n_sites
+        p.closure = CLOSURES[closure]
+        p.pse_order = int(pse_order)
+        p.temperature = float(temperature)
+        p.mdiis_nvec = int(mdiis_nvec)
+        p.mdiis_b = float(mdiis_b)
+        p.mdiis_restart = float(mdiis_restart)
+        p.kappa = float(kappa)
+        p.r_min = float(r_min)
+        p.device = int(device)
+        self.params = p
+        nbytes = rism3d_workspace_bytes(p)
+        if nbytes == 0:
+            raise Rism3dError(-2, "unsupported grid / site count / MDIIS size")
+        self.device = torch.device("cuda", device)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.stream = torch.cuda.current_stream(self.device)
+        self.ctx = rism3d_init(p, self.workspace.data_ptr(), nbytes, self.stream.cuda_stream)
+
+    def close(self):
+        if getattr(self, "ctx", None) is not None:
+            rism3d_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_solvent_chi(self, q, sigma, eps, rho, k0, dk, chi):
+        rism3d_set_solvent_chi(self.ctx, q, sigma, eps, rho, k0, dk, chi)
+
+    def set_solute(self, xyz, q, sigma, eps, rcut=0.0) -> float:
+        return rism3d_set_solute(self.ctx, xyz, q, sigma, eps, rcut)
+
+    def iterate(self, max_iter, tol=0.0):
+        return rism3d_iterate(self.ctx, max_iter, tol)
+
+    def free_energy(self):
+        return rism3d_free_energy(self.ctx, self.n_sites)
+
+    def get_field(self, which: str, site=None) -> np.ndarray:
+        """Host copy: [n][n][n] for one site, or [n_sites][n][n][n] when site is None."""
+        sites = range(self.n_sites) if site is None else [site]
+        out = np.empty((len(sites), self.n, self.n, self.n))
+        for i, s in enumerate(sites):
+            rism3d_get_field(self.ctx, FIELDS[which], s, out[i].ctypes.data, False)
+        return out if site is None else out[0]
+
+    def get_field_device(self, which: str, site: int):
+        import torch
+        out = torch.empty((self.n, self.n, self.n), dtype=torch.float64, device=self.device)
+        rism3d_get_field(self.ctx, FIELDS[which], site, out.data_ptr(), True)
+        return out
+
+    def set_tau(self, site: int, src):
+        import torch
+        if isinstance(src, torch.Tensor) and src.is_cuda:
+            src = src.contiguous()
+            rism3d_set_tau(self.ctx, site, src.data_ptr(), True)
+        else:
+            a = _f64(src)
+            rism3d_set_tau(self.ctx, site, a.ctypes.data, False)
+
+    def rms_history(self) -> np.ndarray:
+        return rism3d_get_rms_history(self.ctx)
+
+    def launch_count(self) -> int:
+        return rism3d_launch_count(self.ctx)
+
+    def fft_forward(self, real_dev):
+        """debug: real device tensor [n_sites][n][n][n] -> complex device tensor [n][n][n/2][n_sites]."""
+        import torch
+        real_dev = real_dev.contiguous()
+        out = torch.empty((self.n, self.n, self.n // 2, self.n_sites), dtype=torch.complex128, device=self.device)
+        rism3d_debug_fft_forward(self.ctx, real_dev.data_ptr(), out.data_ptr())
+        return out
+
+    def fft_inverse(self, spec_dev):
+        import torch
+        spec_dev = spec_dev.contiguous()
+        out = torch.empty((self.n_sites, self.n, self.n, self.n), dtype=torch.float64, device=self.device)
+        rism3d_debug_fft_inverse(self.ctx, spec_dev.data_ptr(), out.data_ptr())
+        return out

@@ -1,0 +1,427 @@
+// api.cu -- the C ABI of librism3d.so (include/rism3d.h): context, workspace carving, argument checks, and
+// the launch sequence of one iteration.  No arithmetic of the method lives here except
+// the host-side preparation of small input tables (twiddles, mixed LJ parameters).
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <vector>
+
+#include "rism3d_internal.h"
+
+using namespace r3d;
+
+struct rism3d_ctx {
+  rism3d_params p;
+  Grid g;
+  Buffers b;
+  SolverParams sp;
+  cudaStream_t stream;
+  char* ws;
+  size_t ws_bytes;
+  size_t scratch_bytes;      // bytes of the X..work span that set_* may use for uploads
+  bool have_solvent, have_solute;
+  double qv[MAX_NV], sigv[MAX_NV], epsv[MAX_NV], rhov[MAX_NV];
+  long long launches;
+  StateHeader* h_hdr;        // pinned
+  double* d_out;             // small device array for scalar results (inside workspace)
+  char err[512];
+};
+
+static int fail(rism3d_ctx* c, int code, const char* fmt, ...) {
+  if (c) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(c->err, sizeof(c->err), fmt, ap);
+    va_end(ap);
+  }
+  return code;
+}
+
+#define CU(call)                                                                                        \
+  do {                                                                                                  \
+    cudaError_t e_ = (call);                                                                            \
+    if (e_ != cudaSuccess) return fail(ctx, RISM3D_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+static bool valid_params(const rism3d_params* p) {
+  if (!p) return false;
+  const int n = p->nx;
+  if (p->ny != n || p->nz != n) return false;
+  if (n < 8 || n > 512 || (n & (n - 1))) return false;
+  const int nv = p->n_sites;
+  if (!(nv == 1 || nv == 2 || nv == 4 || nv == 8)) return false;
+  if (((n / 2) * nv) % 8) return false;             // tile rows are 8 complex wide
+  if (p->mdiis_nvec < 1 || p->mdiis_nvec > MAX_M) return false;
+  if (!(p->spacing > 0.0) || !(p->temperature > 0.0) || !(p->kappa > 0.0)) return false;
+  if (p->closure != RISM3D_KH && p->closure != RISM3D_PSE && p->closure != RISM3D_HNC) return false;
+  if (p->closure == RISM3D_PSE && p->pse_order < 1) return false;
+  return true;
+}
+
+static int n_shells(int n) { const int hn = n / 2; return 3 * (hn - 1) * hn / 2 + 1; }
+
+// carve the workspace; with base == nullptr only the total size is computed
+static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_out, size_t* scratch_bytes) {
+  const size_t n = p->nx, nv = p->n_sites, M = p->mdiis_nvec;
+  const size_t npts = n * n * n, field = npts * nv;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { char* ptr = base ? base + off : nullptr; off += align256(bytes); return ptr; };
+  char* st = take(sizeof(DevState));
+  const size_t off_x = off;
+  char* X = take(M * field * 8);
+  char* R = take(M * field * 8);
+  char* w = take(field * 8);
+  char* work = take(field * 8);
+  const size_t scr = off - off_x;
+  char* phi = take(npts * 8);
+  char* phik = take(npts * 8);
+  char* chis = take((size_t)n_shells((int)n) * nv * nv * 8);
+  char* tw = take(2 * n * 16);
+  char* gp = take((size_t)GRAM_BLOCKS_MAX * (MAX_M + 1) * 2 * 8);
+  char* fp = take((size_t)GRAM_BLOCKS_MAX * MAX_NV * 2 * 8);
+  char* qv = take(MAX_NV * 8);
+  char* rv = take(MAX_NV * 8);
+  char* out = take(64 * 8);
+  if (b) {
+    b->state = (DevState*)st;
+    b->X = (double*)X; b->R = (double*)R; b->w = (double*)w; b->work = (double2*)work;
+    b->phi = (double*)phi; b->phik = (double2*)phik; b->chi_shell = (double*)chis; b->tw = (double2*)tw;
+    b->gram_part = (double*)gp; b->fe_part = (double*)fp; b->qv = (double*)qv; b->rhov = (double*)rv;
+    b->scratch = (double*)work;
+  }
+  if (d_out) *d_out = (double*)out;
+  if (scratch_bytes) *scratch_bytes = scr;
+  return off;
+}
+
+extern "C" size_t rism3d_workspace_bytes(const rism3d_params* p) {
+  if (!valid_params(p)) return 0;
+  return carve(p, nullptr, nullptr, nullptr, nullptr);
+}
+
+extern "C" const char* rism3d_status_string(int s) {
+  switch (s) {
+    case RISM3D_OK: return "ok";
+    case RISM3D_ERR_ARG: return "bad argument";
+    case RISM3D_ERR_SIZE: return "unsupported size";
+    case RISM3D_ERR_ORDER: return "call out of order";
+    case RISM3D_ERR_CHI_RANGE: return "chi table does not cover the grid's |k| range";
+    case RISM3D_ERR_NEUTRAL: return "solvent not neutral";
+    case RISM3D_ERR_WORKSPACE: return "workspace too small";
+    case RISM3D_ERR_CUDA: return "CUDA error";
+    case RISM3D_ERR_DIVERGED: return "iteration diverged";
+    default: return "unknown status";
+  }
+}
+
+extern "C" const char* rism3d_last_error(const rism3d_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+extern "C" long long rism3d_launch_count(const rism3d_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_workspace, size_t bytes, void* stream) {
+  if (!out || !p || !d_workspace) return RISM3D_ERR_ARG;
+  *out = nullptr;
+  if (!valid_params(p)) return RISM3D_ERR_SIZE;
+  const size_t need = carve(p, nullptr, nullptr, nullptr, nullptr);
+  if (bytes < need) return RISM3D_ERR_WORKSPACE;
+  if (((uintptr_t)d_workspace) & 255) return RISM3D_ERR_ARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= p->device || p->device < 0) return RISM3D_ERR_CUDA;
+  if (cudaSetDevice(p->device) != cudaSuccess) return RISM3D_ERR_CUDA;
+  rism3d_ctx* ctx = new rism3d_ctx();
+  memset(ctx, 0, sizeof(*ctx));
+  ctx->p = *p;
+  ctx->stream = (cudaStream_t)stream;
+  ctx->ws = (char*)d_workspace;
+  ctx->ws_bytes = bytes;
+  carve(p, ctx->ws, &ctx->b, &ctx->d_out, &ctx->scratch_bytes);
+  Grid& g = ctx->g;
+  g.n = p->nx; g.nv = p->n_sites; g.h = p->spacing;
+  for (int i = 0; i < 3; ++i) g.origin[i] = p->origin[i];
+  g.npts = (size_t)g.n * g.n * g.n;
+  g.field = g.npts * g.nv;
+  SolverParams& sp = ctx->sp;
+  sp.closure = p->closure;
+  sp.pse_order = p->closure == RISM3D_PSE ? p->pse_order : 1;
+  sp.M = p->mdiis_nvec; sp.b = p->mdiis_b; sp.restart = p->mdiis_restart;
+  sp.kT = K_BOLTZMANN * p->temperature;
+  sp.beta = 1.0 / sp.kT;
+  sp.kappa = p->kappa; sp.r_min = p->r_min;
+  // twiddle table exp(-i pi j / n), j < 2n, from long double
+  std::vector<double> tw(4 * (size_t)g.n);
+  for (int j = 0; j < 2 * g.n; ++j) {
+    const long double a = 3.14159265358979323846264338327950288L * (long double)j / (long double)g.n;
+    tw[2 * j] = (double)cosl(a);
+    tw[2 * j + 1] = (double)(-sinl(a));
+  }
+  cudaError_t e = cudaMallocHost((void**)&ctx->h_hdr, sizeof(StateHeader));
+  if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->b.tw, tw.data(), tw.size() * 8, cudaMemcpyHostToDevice, ctx->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(ctx->b.state, 0, sizeof(DevState), ctx->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+  if (e != cudaSuccess) {
+    if (ctx->h_hdr) cudaFreeHost(ctx->h_hdr);
+    delete ctx;
+    return RISM3D_ERR_CUDA;
+  }
+  *out = ctx;
+  return RISM3D_OK;
+}
+
+extern "C" void rism3d_destroy(rism3d_ctx* ctx) {
+  if (!ctx) return;
+  cudaStreamSynchronize(ctx->stream);
+  if (ctx->h_hdr) cudaFreeHost(ctx->h_hdr);
+  delete ctx;
+}
+
+extern "C" int rism3d_set_solvent_chi(rism3d_ctx* ctx, const double* q, const double* sigma, const double* eps,
+                                      const double* rho, int n_k, double dk, double k0, const double* chi) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (!q || !sigma || !eps || !rho || !chi || n_k < 4 || !(dk > 0.0)) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
+  const Grid& g = ctx->g;
+  double neutral = 0.0;
+  for (int i = 0; i < g.nv; ++i) neutral += rho[i] * q[i];
+  if (fabs(neutral) > 1e-12) return fail(ctx, RISM3D_ERR_NEUTRAL, "sum rho_g q_g = %.3e", neutral);
+  const double dkg = 2.0 * M_PI / (g.n * g.h);
+  const double kmin = dkg * sqrt(0.75), kmax = dkg * sqrt(2.0 * (n_shells(g.n) - 1) + 0.75);
+  if ((kmin - k0) / dk < 0.0 || (kmax - k0) / dk > (double)(n_k - 1))
+    return fail(ctx, RISM3D_ERR_CHI_RANGE, "table covers [%.4f, %.4f], grid needs [%.4f, %.4f]", k0,
+                k0 + (n_k - 1) * dk, kmin, kmax);
+  const size_t tbytes = (size_t)n_k * g.nv * g.nv * 8;
+  if (tbytes > ctx->scratch_bytes) return fail(ctx, RISM3D_ERR_WORKSPACE, "chi table larger than the scratch span");
+  for (int i = 0; i < g.nv; ++i) { ctx->qv[i] = q[i]; ctx->sigv[i] = sigma[i]; ctx->epsv[i] = eps[i]; ctx->rhov[i] = rho[i]; }
+  double* d_table = ctx->b.X;                      // scratch: the history is rebuilt by set_solute anyway
+  CU(cudaMemcpyAsync(d_table, chi, tbytes, cudaMemcpyHostToDevice, ctx->stream));
+  CU(cudaMemcpyAsync(ctx->b.qv, ctx->qv, g.nv * 8, cudaMemcpyHostToDevice, ctx->stream));
+  CU(cudaMemcpyAsync(ctx->b.rhov, ctx->rhov, g.nv * 8, cudaMemcpyHostToDevice, ctx->stream));
+  ctx->launches += launch_chi_shell(g, ctx->b, d_table, n_k, k0, dk, ctx->stream);
+  CU(cudaGetLastError());
+  CU(cudaStreamSynchronize(ctx->stream));
+  ctx->have_solvent = true;
+  ctx->have_solute = false;
+  return RISM3D_OK;
+}
+
+static int reset_state(rism3d_ctx* ctx) {
+  CU(cudaMemsetAsync(ctx->b.state, 0, sizeof(DevState), ctx->stream));
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz, const double* q,
+                                 const double* sigma, const double* eps, double rcut, float* setup_ms) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (n_atoms < 0 || (n_atoms > 0 && (!xyz || !q || !sigma || !eps))) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
+  if (!ctx->have_solvent) return fail(ctx, RISM3D_ERR_ORDER, "set_solvent_chi must come before set_solute");
+  const Grid& g = ctx->g;
+  const SolverParams& sp = ctx->sp;
+  const int nv = g.nv;
+  // host-side input tables: atom records (x, y, z, beta C q), raw charges, mixed pair parameters
+  const size_t na = (size_t)n_atoms;
+  std::vector<double> atoms(na * 5), pair(na * nv * 3);
+  for (size_t a = 0; a < na; ++a) {
+    atoms[4 * a + 0] = xyz[3 * a + 0];
+    atoms[4 * a + 1] = xyz[3 * a + 1];
+    atoms[4 * a + 2] = xyz[3 * a + 2];
+    atoms[4 * a + 3] = sp.beta * COULOMB * q[a];
+    atoms[4 * na + a] = q[a];
+    for (int s = 0; s < nv; ++s) {
+      const double sg = 0.5 * (sigma[a] + ctx->sigv[s]);           // Lorentz-Berthelot (Q4)
+      const double ep = sqrt(eps[a] * ctx->epsv[s]);
+      pair[(a * nv + s) * 3 + 0] = sp.beta * COULOMB * q[a] * ctx->qv[s];
+      pair[(a * nv + s) * 3 + 1] = sg * sg;
+      pair[(a * nv + s) * 3 + 2] = 4.0 * sp.beta * ep;
+    }
+  }
+  const size_t b_atoms = align256(atoms.size() * 8 + 8), b_pair = align256(pair.size() * 8 + 8);
+  const size_t b_phase = align256((size_t)3 * na * g.n * 16 + 16);
+  if (b_atoms + b_pair + b_phase > ctx->scratch_bytes)
+    return fail(ctx, RISM3D_ERR_WORKSPACE, "%d atoms need %zu scratch bytes, workspace has %zu", n_atoms,
+                b_atoms + b_pair + b_phase, ctx->scratch_bytes);
+  char* scr = (char*)ctx->b.X;                      // X, R, w, work are contiguous; w is written last-to-first safe:
+  // place the tables at the END of the span's X/R part so that w (written by the potential kernel) is not touched
+  const size_t xr_bytes = (size_t)((char*)ctx->b.w - (char*)ctx->b.X);
+  if (b_atoms + b_pair + b_phase > xr_bytes)
+    return fail(ctx, RISM3D_ERR_WORKSPACE, "%d atoms need %zu scratch bytes, history span has %zu", n_atoms,
+                b_atoms + b_pair + b_phase, xr_bytes);
+  double* d_atoms = (double*)scr;
+  double* d_pair = (double*)(scr + b_atoms);
+  double2* d_phase = (double2*)(scr + b_atoms + b_pair);
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0));
+  CU(cudaEventCreate(&e1));
+  if (na) {
+    CU(cudaMemcpyAsync(d_atoms, atoms.data(), atoms.size() * 8, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(d_pair, pair.data(), pair.size() * 8, cudaMemcpyHostToDevice, ctx->stream));
+  }
+  CU(cudaEventRecord(e0, ctx->stream));
+  ctx->launches += launch_potential(g, ctx->b, sp, n_atoms, d_atoms, d_pair, rcut, ctx->stream);
+  CU(cudaGetLastError());
+  ctx->launches += launch_phi_tilde(g, ctx->b, sp, n_atoms, d_atoms, d_phase, ctx->stream);
+  CU(cudaGetLastError());
+  CU(cudaEventRecord(e1, ctx->stream));
+  // tau = 0 (t = f) in slot 0; empty history
+  CU(cudaMemsetAsync(ctx->b.X, 0, g.field * 8, ctx->stream));
+  int rc = reset_state(ctx);
+  if (rc) return rc;
+  CU(cudaStreamSynchronize(ctx->stream));
+  float ms = 0.f;
+  CU(cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (setup_ms) *setup_ms = ms;
+  ctx->have_solute = true;
+  return RISM3D_OK;
+}
+
+__global__ void iterate_begin_kernel(DevState* st, double tol) {
+  st->tol = tol;
+  st->done = 0;
+  st->status = 0;
+  st->n_done = 0;
+}
+
+static int enqueue_iteration(rism3d_ctx* ctx) {
+  const Grid& g = ctx->g;
+  const Buffers& b = ctx->b;
+  cudaStream_t s = ctx->stream;
+  int k = 0;
+  k += launch_closure_zfwd(g, b, ctx->sp, nullptr, s);     // step 2 + z of step 3
+  k += launch_y_fwd(g, b, true, s);                        // step 3
+  k += launch_kspace_x(g, b, s);                           // step 3 (x), Eq. 32, step 4, x of step 5
+  k += launch_y_inv(g, b, true, s);                        // step 5
+  k += launch_zinv_residual(g, b, ctx->sp, nullptr, s);    // step 5 (z), Eq. 33, Gram row
+  k += launch_mdiis_solve(g, b, ctx->sp, s);               // step 6-7
+  k += launch_mdiis_update(g, b, ctx->sp, s);              // step 6
+  ctx->launches += k;
+  return k;
+}
+
+static int read_header(rism3d_ctx* ctx) {
+  CU(cudaMemcpyAsync(ctx->h_hdr, ctx->b.state, sizeof(StateHeader), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_iterate(rism3d_ctx* ctx, int max_iter, double tol, int* n_done, double* rms) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (max_iter < 0) return fail(ctx, RISM3D_ERR_ARG, "max_iter < 0");
+  if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before iterate");
+  iterate_begin_kernel<<<1, 1, 0, ctx->stream>>>(ctx->b.state, tol);
+  ctx->launches += 1;
+  const int check_every = 8;
+  for (int it = 0; it < max_iter; ++it) {
+    enqueue_iteration(ctx);
+    if (tol > 0.0 && ((it + 1) % check_every == 0)) {
+      int rc = read_header(ctx);
+      if (rc) return rc;
+      if (ctx->h_hdr->done) break;
+    }
+  }
+  CU(cudaGetLastError());
+  int rc = read_header(ctx);
+  if (rc) return rc;
+  if (n_done) *n_done = ctx->h_hdr->n_done;
+  if (rms) *rms = ctx->h_hdr->rms_last;
+  if (ctx->h_hdr->status == RISM3D_ERR_DIVERGED)
+    return fail(ctx, RISM3D_ERR_DIVERGED, "non-finite residual after %d iterations", ctx->h_hdr->n_done);
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_free_energy(rism3d_ctx* ctx, double* dmu_total, double* dmu_site) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (!dmu_total) return fail(ctx, RISM3D_ERR_ARG, "dmu_total is NULL");
+  if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before free_energy");
+  ctx->launches += launch_free_energy(ctx->g, ctx->b, ctx->sp, ctx->d_out, ctx->stream);
+  CU(cudaGetLastError());
+  double host[MAX_NV];
+  CU(cudaMemcpyAsync(host, ctx->d_out, ctx->g.nv * 8, cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  double tot = 0.0;
+  for (int i = 0; i < ctx->g.nv; ++i) {
+    tot += host[i];
+    if (dmu_site) dmu_site[i] = host[i];
+  }
+  *dmu_total = tot;
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_get_field(rism3d_ctx* ctx, int which, int site, double* dst, int dst_is_device) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (!dst || which < 0 || which > RISM3D_FIELD_PHI || site < 0 || site >= ctx->g.nv)
+    return fail(ctx, RISM3D_ERR_ARG, "bad argument");
+  if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before get_field");
+  double* d = dst_is_device ? dst : ctx->b.scratch;
+  ctx->launches += launch_get_field(ctx->g, ctx->b, ctx->sp, which, site, d, ctx->stream);
+  CU(cudaGetLastError());
+  if (!dst_is_device) CU(cudaMemcpyAsync(dst, d, ctx->g.npts * 8, cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_set_tau(rism3d_ctx* ctx, int site, const double* src, int src_is_device) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (!src || site < 0 || site >= ctx->g.nv) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
+  if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before set_tau");
+  int rc = read_header(ctx);
+  if (rc) return rc;
+  const int cur = ctx->h_hdr->cur;
+  const Grid& g = ctx->g;
+  // move the current tau to slot 0, overwrite the requested site, clear the history
+  if (cur != 0)
+    CU(cudaMemcpyAsync(ctx->b.X, ctx->b.X + (size_t)cur * g.field, g.field * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+  CU(cudaMemcpyAsync(ctx->b.X + (size_t)site * g.npts, src, g.npts * 8,
+                     src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ctx->stream));
+  rc = reset_state(ctx);
+  if (rc) return rc;
+  CU(cudaStreamSynchronize(ctx->stream));
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_get_rms_history(rism3d_ctx* ctx, double* dst, int cap, int* n) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (!dst || cap < 0 || !n) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
+  int rc = read_header(ctx);
+  if (rc) return rc;
+  int total = ctx->h_hdr->hist_n;
+  int avail = total < RMS_HIST_CAP ? total : RMS_HIST_CAP;
+  int cnt = avail < cap ? avail : cap;
+  std::vector<double> tmp(RMS_HIST_CAP);
+  CU(cudaMemcpyAsync(tmp.data(), (char*)ctx->b.state + offsetof(DevState, rms_hist), (size_t)RMS_HIST_CAP * 8,
+                     cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  for (int i = 0; i < cnt; ++i) dst[i] = tmp[(size_t)(total - cnt + i) % RMS_HIST_CAP];
+  *n = cnt;
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_debug_fft_forward(rism3d_ctx* ctx, const double* d_in, double* d_out) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (!d_in || !d_out) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
+  const Grid& g = ctx->g;
+  int k = launch_closure_zfwd(g, ctx->b, ctx->sp, d_in, ctx->stream);
+  k += launch_y_fwd(g, ctx->b, false, ctx->stream);
+  k += launch_x_fwd(g, ctx->b, ctx->stream);
+  ctx->launches += k;
+  CU(cudaGetLastError());
+  CU(cudaMemcpyAsync(d_out, ctx->b.work, g.field * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_debug_fft_inverse(rism3d_ctx* ctx, const double* d_in, double* d_out) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (!d_in || !d_out) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
+  const Grid& g = ctx->g;
+  CU(cudaMemcpyAsync(ctx->b.work, d_in, g.field * 8, cudaMemcpyDeviceToDevice, ctx->stream));
+  int k = launch_x_inv(g, ctx->b, ctx->stream);
+  k += launch_y_inv(g, ctx->b, false, ctx->stream);
+  k += launch_zinv_residual(g, ctx->b, ctx->sp, d_out, ctx->stream);
+  ctx->launches += k;
+  CU(cudaGetLastError());
+  CU(cudaStreamSynchronize(ctx->stream));
+  return RISM3D_OK;
+}

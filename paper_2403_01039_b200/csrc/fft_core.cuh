@@ -1,0 +1,218 @@
+// fft_core.cuh -- fp64 complex FFT building blocks for sm_100a: in-register radix-2/4/8/16 DFTs and
+// the multi-pass Stockham-free (in-place, digit-indexed) line transforms that the 3D passes share.
+//
+// The transform is the SHIFTED DFT of the paper's half-integer k grid:
+//     forward   F_j = sum_m f_m exp(-2 pi i (j + 1/2) m / N)
+//     inverse   f_m = (1/N) sum_j F_j exp(+2 pi i (j + 1/2) m / N)
+// (HALF = true) or the plain DFT (HALF = false, used for the z axis where the half shift is folded
+// into the real<->half-spectrum packing).  Forward lines run decimation-in-frequency, inverse lines
+// the mirrored decimation-in-time, so that both read and write NATURAL order in global memory and
+// exchange data through one shared-memory tile in place:
+//     N = R1*R2(*R3),  m = m1*S1 + r  (S1 = N/R1),  j = k1 + R1*k2 (+ R1*R2*k3)
+//     forward pass A : DFT_R1 over m1 (odd-frequency when HALF), twiddle exp(-2 pi i (k1+1/2) r / N)
+//     forward pass B : DFT_R2 over m2 inside block k1 (, twiddle, pass C: DFT_R3)
+//     inverse        : the conjugate transpose of the above, stage by stage.
+// Nothing here is shared with the CPU oracle (oracle/ is numpy).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace r3d {
+
+typedef double2 cplx;
+
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cplx csub(cplx a, cplx b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cplx cmul(cplx a, cplx b) {
+  return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ cplx cmulc(cplx a, cplx b) {   // a * conj(b)
+  return make_double2(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y);
+}
+__device__ __forceinline__ cplx cscale(cplx a, double s) { return make_double2(a.x * s, a.y * s); }
+
+// multiply by exp(DIR * 2 pi i * idx / 16), idx a compile-time-foldable integer in [0, 8)
+template <int DIR>
+__device__ __forceinline__ cplx mul_w16(cplx v, int idx) {
+  const double C1 = 0.92387953251128673848;   // cos(pi/8)
+  const double S1 = 0.38268343236508978178;   // sin(pi/8)
+  const double H = 0.70710678118654752440;    // sqrt(1/2)
+  const double d = (double)DIR;
+  switch (idx) {
+    case 0: return v;
+    case 4: return make_double2(-d * v.y, d * v.x);                                  // * (DIR i)
+    case 2: return make_double2(H * (v.x - d * v.y), H * (v.y + d * v.x));           // * (1 + DIR i)/sqrt2
+    case 6: return make_double2(-H * (v.x + d * v.y), H * (d * v.x - v.y));          // * (-1 + DIR i)/sqrt2
+    case 1: return make_double2(C1 * v.x - d * S1 * v.y, C1 * v.y + d * S1 * v.x);
+    case 3: return make_double2(S1 * v.x - d * C1 * v.y, S1 * v.y + d * C1 * v.x);
+    case 5: return make_double2(-S1 * v.x - d * C1 * v.y, -S1 * v.y + d * C1 * v.x);
+    default: return make_double2(-C1 * v.x - d * S1 * v.y, -C1 * v.y + d * S1 * v.x);  // 7
+  }
+}
+
+// In-register DFT, natural order in and out:  X[k] = sum_m x[m] exp(DIR 2 pi i m k / R),  R in {1,2,4,8,16}
+template <int R, int DIR>
+struct Dft {
+  static __device__ __forceinline__ void run(cplx (&x)[R]) {
+    cplx e[R / 2], o[R / 2];
+#pragma unroll
+    for (int k = 0; k < R / 2; ++k) { e[k] = x[2 * k]; o[k] = x[2 * k + 1]; }
+    Dft<R / 2, DIR>::run(e);
+    Dft<R / 2, DIR>::run(o);
+#pragma unroll
+    for (int k = 0; k < R / 2; ++k) {
+      cplx t = mul_w16<DIR>(o[k], k * (16 / R));
+      x[k] = cadd(e[k], t);
+      x[k + R / 2] = csub(e[k], t);
+    }
+  }
+};
+template <int DIR>
+struct Dft<1, DIR> {
+  static __device__ __forceinline__ void run(cplx (&)[1]) {}
+};
+
+// Twiddle table of one grid axis: tab[j] = exp(-i pi j / n), j = 0 .. 2n-1 (device memory, built by the host
+// in long double).  For a line transform of length N = n / mul:  exp(-2 pi i a / (2N)) = tab[(a * mul) mod 2n].
+struct Twiddle {
+  const cplx* tab;
+  int mul;
+  int mask;   // 2n - 1
+  __device__ __forceinline__ cplx operator()(int a) const { return __ldg(tab + ((a * mul) & mask)); }
+};
+
+// ---------------------------------------------------------------------------------------------
+// Forward (DIR = -1) decimation-in-frequency passes.  Ld(idx) -> cplx, St(idx, cplx).
+// t = index of this thread within its column, T = threads per column.
+// ---------------------------------------------------------------------------------------------
+template <int N, int R1, bool HALF, class Ld, class St>
+__device__ __forceinline__ void fwd_pass_a(int t, int T, const Twiddle& tw, Ld ld, St st) {
+  constexpr int S1 = N / R1;
+  for (int r = t; r < S1; r += T) {
+    cplx x[R1];
+#pragma unroll
+    for (int m1 = 0; m1 < R1; ++m1) x[m1] = ld(m1 * S1 + r);
+    if (HALF) {
+#pragma unroll
+      for (int m1 = 1; m1 < R1; ++m1) x[m1] = cmul(x[m1], tw(m1 * S1));   // exp(-i pi m1 / R1)
+    }
+    Dft<R1, -1>::run(x);
+#pragma unroll
+    for (int k1 = 0; k1 < R1; ++k1) {
+      const int a = HALF ? (2 * k1 + 1) * r : 2 * k1 * r;                 // exp(-2 pi i (k1 [+1/2]) r / N)
+      st(k1 * S1 + r, (a == 0) ? x[k1] : cmul(x[k1], tw(a)));
+    }
+  }
+}
+
+// middle pass of a 3-pass transform: DFT_R2 inside block k1 over m2 (stride S2), twiddle exp(-2 pi i k2 r2 / S1)
+template <int N, int R1, int R2, class Ld, class St>
+__device__ __forceinline__ void fwd_pass_mid(int t, int T, const Twiddle& tw, Ld ld, St st) {
+  constexpr int S1 = N / R1, S2 = S1 / R2;
+  for (int b = t; b < N / R2; b += T) {
+    const int k1 = b / S2, r2 = b % S2;
+    cplx x[R2];
+#pragma unroll
+    for (int m2 = 0; m2 < R2; ++m2) x[m2] = ld(k1 * S1 + m2 * S2 + r2);
+    Dft<R2, -1>::run(x);
+#pragma unroll
+    for (int k2 = 0; k2 < R2; ++k2) {
+      const int a = 2 * R1 * k2 * r2;
+      st(k1 * S1 + k2 * S2 + r2, (a == 0) ? x[k2] : cmul(x[k2], tw(a)));
+    }
+  }
+}
+
+// last pass: DFT_RL over the unit-stride digit of block `blk` (blk = k1 for 2 passes, k1*R2+k2 for 3).
+// Out(j, value) receives NATURAL frequency index j.  JMUL = product of the earlier radices.
+template <int N, int RL, int R1, class Ld, class Out>
+__device__ __forceinline__ void fwd_pass_last(int t, int T, Ld ld, Out out) {
+  constexpr int NB = N / RL;          // number of blocks
+  constexpr int RMID = NB / R1;       // R2 of a 3-pass transform, 1 otherwise
+  for (int blk = t; blk < NB; blk += T) {
+    cplx x[RL];
+#pragma unroll
+    for (int m = 0; m < RL; ++m) x[m] = ld(blk * RL + m);
+    Dft<RL, -1>::run(x);
+    const int k1 = blk / RMID, k2 = blk % RMID;
+    const int j0 = k1 + R1 * k2;
+#pragma unroll
+    for (int k = 0; k < RL; ++k) out(j0 + NB * k, x[k]);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Inverse (DIR = +1) decimation-in-time stages: the mirror image of the passes above.
+// ---------------------------------------------------------------------------------------------
+// first stage: In(j) reads NATURAL frequency index j; DFT_RL over the last digit; twiddle (3-pass only); St(idx)
+template <int N, int RL, int R1, class In, class St>
+__device__ __forceinline__ void inv_stage_first(int t, int T, const Twiddle& tw, bool half2, In in, St st) {
+  constexpr int NB = N / RL;
+  constexpr int RMID = NB / R1;
+  for (int blk = t; blk < NB; blk += T) {
+    const int k1 = blk / RMID, k2 = blk % RMID;
+    const int j0 = k1 + R1 * k2;
+    cplx x[RL];
+#pragma unroll
+    for (int k = 0; k < RL; ++k) x[k] = in(j0 + NB * k);
+    Dft<RL, +1>::run(x);
+#pragma unroll
+    for (int r = 0; r < RL; ++r) {
+      // 2-pass: this stage's output index r is the r of pass A: twiddle exp(+2 pi i (k1 [+1/2]) r / N)
+      // 3-pass: mirror of the middle pass: exp(+2 pi i k2 r / S1)
+      int a;
+      if (RMID == 1) a = half2 ? (2 * k1 + 1) * r : 2 * k1 * r;
+      else a = 2 * R1 * k2 * r;
+      st(blk * RL + r, (a == 0) ? x[r] : cmulc(x[r], tw(a)));
+    }
+  }
+}
+
+// middle stage of a 3-pass inverse: DFT_R2 over k2 (stride S2) inside block k1, twiddle exp(+2 pi i (k1[+1/2]) r / N)
+template <int N, int R1, int R2, bool HALF, class Ld, class St>
+__device__ __forceinline__ void inv_stage_mid(int t, int T, const Twiddle& tw, Ld ld, St st) {
+  constexpr int S1 = N / R1, S2 = S1 / R2;
+  for (int b = t; b < N / R2; b += T) {
+    const int k1 = b / S2, r2 = b % S2;
+    cplx x[R2];
+#pragma unroll
+    for (int k2 = 0; k2 < R2; ++k2) x[k2] = ld(k1 * S1 + k2 * S2 + r2);
+    Dft<R2, +1>::run(x);
+#pragma unroll
+    for (int m2 = 0; m2 < R2; ++m2) {
+      const int r = m2 * S2 + r2;
+      const int a = HALF ? (2 * k1 + 1) * r : 2 * k1 * r;
+      st(k1 * S1 + r, (a == 0) ? x[m2] : cmulc(x[m2], tw(a)));
+    }
+  }
+}
+
+// last stage: DFT_R1 over k1 (stride S1); when HALF the outputs get exp(+i pi m1 / R1); Out(m, value), m natural.
+template <int N, int R1, bool HALF, class Ld, class Out>
+__device__ __forceinline__ void inv_stage_last(int t, int T, const Twiddle& tw, Ld ld, Out out) {
+  constexpr int S1 = N / R1;
+  for (int r = t; r < S1; r += T) {
+    cplx x[R1];
+#pragma unroll
+    for (int k1 = 0; k1 < R1; ++k1) x[k1] = ld(k1 * S1 + r);
+    Dft<R1, +1>::run(x);
+#pragma unroll
+    for (int m1 = 0; m1 < R1; ++m1) {
+      cplx v = x[m1];
+      if (HALF && m1 > 0) v = cmulc(v, tw(m1 * S1));
+      out(m1 * S1 + r, v);
+    }
+  }
+}
+
+// Radix plan per line length.  T = threads per column, G = column groups (tiles) per CTA.
+template <int N> struct FftCfg;
+template <> struct FftCfg<4>   { enum { R1 = 2,  R2 = 2,  R3 = 1, T = 2,  G = 8 }; };
+template <> struct FftCfg<8>   { enum { R1 = 4,  R2 = 2,  R3 = 1, T = 2,  G = 8 }; };
+template <> struct FftCfg<16>  { enum { R1 = 4,  R2 = 4,  R3 = 1, T = 4,  G = 8 }; };
+template <> struct FftCfg<32>  { enum { R1 = 8,  R2 = 4,  R3 = 1, T = 4,  G = 8 }; };
+template <> struct FftCfg<64>  { enum { R1 = 8,  R2 = 8,  R3 = 1, T = 8,  G = 4 }; };
+template <> struct FftCfg<128> { enum { R1 = 16, R2 = 8,  R3 = 1, T = 8,  G = 2 }; };
+template <> struct FftCfg<256> { enum { R1 = 16, R2 = 16, R3 = 1, T = 16, G = 1 }; };
+template <> struct FftCfg<512> { enum { R1 = 8,  R2 = 8,  R3 = 8, T = 64, G = 1 }; };
+
+}  // namespace r3d

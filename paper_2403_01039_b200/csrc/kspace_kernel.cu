@@ -1,0 +1,140 @@
+// kspace_kernel.cu -- steps 3b-5a of the loop in ONE pass over the k-space work array:
+//   forward FFT along x  ->  c(k) = c_sr(k) - q_g phi~(k)          (Eq. 32)
+//                        ->  h_g(k) = sum_g' c_g'(k) chi_g'g(|k|)   (Eq. 13)
+//                        ->  tau'(k) = h(k) - c_sr(k)               (Eq. 33 in k space; Q14)
+//                        ->  inverse FFT along x, in place.
+// The last forward pass and the first inverse stage work on the same register set (decimation in frequency
+// forward, decimation in time inverse), so the k-space arithmetic happens in registers between them; the n_v
+// sites of one k point sit in n_v adjacent lanes (site-interleaved layout) and are exchanged by warp shuffles.
+// chi(|k|) comes from the per-shell table built in set_solvent_chi: |k|^2 = dk^2 (s + 3/4) with
+// s = sum_axis j'(j'+1), j' the folded index.
+#include "fft_core.cuh"
+#include "rism3d_internal.h"
+
+namespace r3d {
+
+extern __shared__ double2 smem_dyn[];
+constexpr int COLS = 8;
+
+template <int N, int NV>
+__global__ void __launch_bounds__(FftCfg<N>::T* FftCfg<N>::G* COLS)
+    kspace_x_kernel(cplx* __restrict__ data, const cplx* __restrict__ phik, const double* __restrict__ chi_shell,
+                    const double* __restrict__ qv, Twiddle tw, const DevState* __restrict__ st) {
+  if (st->done) return;
+  using Cfg = FftCfg<N>;
+  constexpr int T = Cfg::T, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS;
+  constexpr int RL = (R3 == 1) ? R2 : R3;            // radix of the innermost digit
+  constexpr int NB = N / RL, RMID = NB / R1;
+  constexpr int NZ = N / 2;
+  constexpr size_t Q = (size_t)NZ * NV;              // complex elements per (jx, jy) row
+  constexpr size_t ES = (size_t)N * Q;               // stride of the x axis
+  const int tid = threadIdx.x;
+  const int col = tid % C, t = (tid / C) % T, grp = tid / (C * T);
+  const size_t chunk = (size_t)blockIdx.x * Cfg::G + grp;
+  cplx* sm = smem_dyn + grp * (N * C) + col;
+  const size_t q2 = chunk * C + col;                 // flattened (jy, p, site)
+  cplx* base = data + q2;
+  const int jy = (int)(q2 / Q);
+  const int p = (int)((q2 % Q) / NV);
+  const int site = col % NV;
+  const int lane = tid & 31;
+  const int lane0 = lane & ~(NV - 1);
+  const int jyf = jy < NZ ? jy : N - 1 - jy;         // folded indices: |k_axis| = dk (j' + 1/2)
+  const int jzf = (2 * p) < NZ ? 2 * p : N - 1 - 2 * p;
+  const int s_yz = jyf * (jyf + 1) + jzf * (jzf + 1);
+  const double qg = qv[site];
+  const cplx* phrow = phik + (size_t)jy * NZ + p;    // + jx * N * NZ
+  auto ld_sm = [&](int i) { return sm[i * C]; };
+  auto st_sm = [&](int i, cplx v) { sm[i * C] = v; };
+
+  fwd_pass_a<N, R1, true>(t, T, tw, [&](int m) { return base[m * ES]; }, st_sm);
+  __syncthreads();
+  if constexpr (R3 != 1) {
+    fwd_pass_mid<N, R1, R2>(t, T, tw, ld_sm, st_sm);
+    __syncthreads();
+  }
+  // innermost digit: forward DFT, k-space arithmetic, inverse DFT, all on the same registers
+  for (int blk = t; blk < NB; blk += T) {
+    cplx x[RL];
+#pragma unroll
+    for (int m = 0; m < RL; ++m) x[m] = ld_sm(blk * RL + m);
+    Dft<RL, -1>::run(x);
+    const int k1 = blk / RMID, k2 = blk % RMID;
+    const int j0 = k1 + R1 * k2;
+#pragma unroll
+    for (int k = 0; k < RL; ++k) {
+      const int jx = j0 + NB * k;
+      const int jxf = jx < NZ ? jx : N - 1 - jx;
+      const int shell = (jxf * (jxf + 1) + s_yz) >> 1;
+      const cplx ph = __ldg(phrow + (size_t)jx * N * NZ);
+      const cplx csr = x[k];
+      const cplx c = make_double2(csr.x - qg * ph.x, csr.y - qg * ph.y);     // Eq. 32
+      const double* ch = chi_shell + (size_t)shell * (NV * NV) + site * NV;  // chi_{g' site}, g' = 0..NV-1
+      double hx = 0.0, hy = 0.0;
+#pragma unroll
+      for (int gp = 0; gp < NV; ++gp) {
+        const double cx = __shfl_sync(0xffffffffu, c.x, lane0 + gp);
+        const double cy = __shfl_sync(0xffffffffu, c.y, lane0 + gp);
+        const double chv = __ldg(ch + gp);
+        hx += cx * chv;                                                       // Eq. 13
+        hy += cy * chv;
+      }
+      x[k] = make_double2(hx - csr.x, hy - csr.y);                            // tau'(k) = h - c_sr
+    }
+    Dft<RL, +1>::run(x);
+#pragma unroll
+    for (int r = 0; r < RL; ++r) {
+      int a;
+      if (RMID == 1) a = (2 * k1 + 1) * r;
+      else a = 2 * R1 * k2 * r;
+      st_sm(blk * RL + r, (a == 0) ? x[r] : cmulc(x[r], tw(a)));
+    }
+  }
+  __syncthreads();
+  if constexpr (R3 != 1) {
+    inv_stage_mid<N, R1, R2, true>(t, T, tw, ld_sm, st_sm);
+    __syncthreads();
+  }
+  const double scale = 1.0 / (double)N;
+  inv_stage_last<N, R1, true>(t, T, tw, ld_sm, [&](int m, cplx v) { base[m * ES] = cscale(v, scale); });
+}
+
+template <int N, int NV>
+static int launch_kspace_nv(const Grid& gr, const Buffers& b, cudaStream_t s) {
+  using Cfg = FftCfg<N>;
+  const size_t Q = (size_t)(gr.n / 2) * gr.nv;
+  const size_t nchunks = (size_t)gr.n * Q / COLS;
+  const int threads = Cfg::T * Cfg::G * COLS;
+  const size_t shm = (size_t)Cfg::G * N * COLS * sizeof(cplx);
+  auto kern = kspace_x_kernel<N, NV>;
+  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
+  Twiddle tw{b.tw, 1, 2 * gr.n - 1};
+  kern<<<(unsigned)(nchunks / Cfg::G), threads, shm, s>>>(b.work, b.phik, b.chi_shell, b.qv, tw, b.state);
+  return 1;
+}
+
+template <int N>
+static int launch_kspace_n(const Grid& g, const Buffers& b, cudaStream_t s) {
+  switch (g.nv) {
+    case 1: return launch_kspace_nv<N, 1>(g, b, s);
+    case 2: return launch_kspace_nv<N, 2>(g, b, s);
+    case 4: return launch_kspace_nv<N, 4>(g, b, s);
+    case 8: return launch_kspace_nv<N, 8>(g, b, s);
+    default: return 0;
+  }
+}
+
+int launch_kspace_x(const Grid& g, const Buffers& b, cudaStream_t s) {
+  switch (g.n) {
+    case 8: return launch_kspace_n<8>(g, b, s);
+    case 16: return launch_kspace_n<16>(g, b, s);
+    case 32: return launch_kspace_n<32>(g, b, s);
+    case 64: return launch_kspace_n<64>(g, b, s);
+    case 128: return launch_kspace_n<128>(g, b, s);
+    case 256: return launch_kspace_n<256>(g, b, s);
+    case 512: return launch_kspace_n<512>(g, b, s);
+    default: return 0;
+  }
+}
+
+}  // namespace r3d

@@ -1,0 +1,195 @@
+// mdiis_kernels.cu -- step 6 of the loop (Q7, Q8): MDIIS with M stored
+// (input, residual) pairs.  R_i = Y_i - X_i; c = argmin |sum c_i R_i|^2 with sum c_i = 1 (Lagrange multiplier);
+// X_new = sum_i c_i (X_i + b R_i).
+//
+//   mdiis_solve_kernel  : one CTA.  Finishes the Gram row (fixed-order double-double reduction of the per-CTA
+//                         partial sums of zinv_residual), rms and convergence test (Eq. 41 as read in Q9), history
+//                         bookkeeping (circular overwrite, restart rule), the bordered (m+1)x(m+1) solve by Gaussian
+//                         elimination with partial pivoting, and the choice of the slot the update writes.
+//   mdiis_update_kernel : streaming linear combination over the stored slots.
+#include "rism3d_internal.h"
+
+namespace r3d {
+
+__global__ void __launch_bounds__(256)
+    mdiis_solve_kernel(DevState* __restrict__ st, const double* __restrict__ gram_part, int nblocks, int M, double b,
+                       double restart, double npts_total) {
+  if (st->done) return;
+  __shared__ double s_hi[256], s_lo[256];
+  __shared__ double s_row[MAX_M + 1];
+  const int tid = threadIdx.x;
+  const int m_old = st->m;
+  const int skip = (m_old == M) ? 1 : 0;
+  const int nother = m_old - skip;
+
+  // Gram row: entry j < nother is <R_new, R_other[j]>, entry MAX_M is <R_new, R_new>
+  for (int jj = 0; jj <= nother; ++jj) {
+    const int j = (jj == nother) ? MAX_M : jj;
+    double hi = 0.0, lo = 0.0;
+    for (int blk = tid; blk < nblocks; blk += 256) {
+      const double* p = gram_part + ((size_t)blk * (MAX_M + 1) + j) * 2;
+      dd_add(hi, lo, p[0], p[1]);
+    }
+    s_hi[tid] = hi;
+    s_lo[tid] = lo;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+      if (tid < o) {
+        double h = s_hi[tid], l = s_lo[tid];
+        dd_add(h, l, s_hi[tid + o], s_lo[tid + o]);
+        s_hi[tid] = h;
+        s_lo[tid] = l;
+      }
+      __syncthreads();
+    }
+    if (tid == 0) s_row[jj] = s_hi[0] + s_lo[0];
+    __syncthreads();
+  }
+  if (tid != 0) return;
+
+  const double self = s_row[nother];
+  const double rms = sqrt(self / npts_total);          // Eq. 41 (Q9)
+  st->rms_last = rms;
+  st->n_done += 1;
+  st->rms_hist[st->hist_n % RMS_HIST_CAP] = rms;
+  st->hist_n += 1;
+  st->upd_m = 0;
+  if (!isfinite(rms)) { st->done = 1; st->status = RISM3D_ERR_DIVERGED; return; }
+  if (st->tol > 0.0 && rms < st->tol) { st->done = 1; return; }   // converged: tau stays as it is
+
+  // append (cur, R_new) to the history, dropping the oldest entry of a full history
+  int m = m_old;
+  if (skip) {
+    for (int i = 0; i + 1 < m; ++i) {
+      st->list[i] = st->list[i + 1];
+      st->rms[i] = st->rms[i + 1];
+      for (int j = 0; j + 1 < m; ++j) st->S[i][j] = st->S[i + 1][j + 1];
+    }
+    m -= 1;
+  }
+  const int cur = st->cur;
+  st->list[m] = cur;
+  st->rms[m] = rms;
+  for (int i = 0; i < m; ++i) st->S[m][i] = st->S[i][m] = s_row[i];
+  st->S[m][m] = self;
+  m += 1;
+
+  // restart rule (Q8): keep only the entry with the smallest rms (first minimum)
+  if (restart > 0.0) {
+    double rmin = st->rms[0];
+    int best = 0;
+    for (int i = 1; i < m; ++i)
+      if (st->rms[i] < rmin) { rmin = st->rms[i]; best = i; }
+    if (rms > restart * rmin) {
+      st->list[0] = st->list[best];
+      st->rms[0] = st->rms[best];
+      st->S[0][0] = st->S[best][best];
+      m = 1;
+    }
+  }
+  st->m = m;
+
+  // bordered system [[S/smax, 1], [1^T, 0]] [c; lambda] = [0; 1]; every product and difference is rounded
+  // separately (no FMA contraction) so the elimination takes the same steps as the oracle's
+  double c[MAX_M];
+  for (int i = 0; i < m; ++i) c[i] = (i == m - 1) ? 1.0 : 0.0;     // fallback: unit vector on the newest entry
+  double smax = st->S[0][0];
+  for (int i = 1; i < m; ++i) smax = fmax(smax, st->S[i][i]);
+  if (smax > 0.0) {
+    const int n = m + 1;
+    double A[MAX_M + 1][MAX_M + 2];
+    for (int i = 0; i < n; ++i)
+      for (int j = 0; j <= n; ++j) A[i][j] = 0.0;
+    for (int i = 0; i < m; ++i) {
+      for (int j = 0; j < m; ++j) A[i][j] = st->S[i][j] / smax;
+      A[i][m] = 1.0;
+      A[m][i] = 1.0;
+    }
+    A[m][n] = 1.0;
+    bool ok = true;
+    for (int colx = 0; colx < n && ok; ++colx) {
+      int piv = colx;
+      for (int r = colx + 1; r < n; ++r)
+        if (fabs(A[r][colx]) > fabs(A[piv][colx])) piv = r;
+      if (A[piv][colx] == 0.0) { ok = false; break; }
+      if (piv != colx)
+        for (int j = 0; j <= n; ++j) { const double tmp = A[colx][j]; A[colx][j] = A[piv][j]; A[piv][j] = tmp; }
+      for (int r = colx + 1; r < n; ++r) {
+        const double fac = A[r][colx] / A[colx][colx];
+        for (int j = colx; j <= n; ++j) A[r][j] = __dsub_rn(A[r][j], __dmul_rn(fac, A[colx][j]));
+      }
+    }
+    if (ok) {
+      double xs[MAX_M + 1];
+      for (int r = n - 1; r >= 0; --r) {
+        double acc = A[r][n];
+        for (int j = r + 1; j < n; ++j) acc = __dsub_rn(acc, __dmul_rn(A[r][j], xs[j]));
+        xs[r] = acc / A[r][r];
+      }
+      for (int i = 0; i < m; ++i) c[i] = xs[i];
+    }
+  }
+
+  // where the update writes: a full history overwrites its oldest input in place (it is dropped next iteration)
+  int dst;
+  if (m == M) {
+    dst = st->list[0];
+  } else {
+    unsigned used = 0;
+    for (int i = 0; i < m; ++i) used |= 1u << st->list[i];
+    dst = 0;
+    while (used & (1u << dst)) ++dst;
+  }
+  st->upd_m = m;
+  for (int i = 0; i < m; ++i) { st->upd_list[i] = st->list[i]; st->upd_coef[i] = c[i]; }
+  st->upd_dst = dst;
+  st->cur = dst;
+}
+
+int launch_mdiis_solve(const Grid& g, const Buffers& b, const SolverParams& sp, cudaStream_t s) {
+  mdiis_solve_kernel<<<1, 256, 0, s>>>(b.state, b.gram_part, gram_blocks(g), sp.M, sp.b, sp.restart,
+                                       (double)g.field);
+  return 1;
+}
+
+// X[dst] = sum_i c_i (X[i] + b R[i]) over the stored entries.  dst may alias the oldest X (elementwise in place).
+__global__ void __launch_bounds__(256)
+    mdiis_update_kernel(const DevState* __restrict__ st, double* X, const double* __restrict__ R, size_t field,
+                        double b) {
+  if (st->done) return;
+  __shared__ int s_list[MAX_M];
+  __shared__ double s_c[MAX_M];
+  __shared__ int s_m, s_dst;
+  if (threadIdx.x == 0) {
+    s_m = st->upd_m;
+    s_dst = st->upd_dst;
+    for (int i = 0; i < st->upd_m; ++i) { s_list[i] = st->upd_list[i]; s_c[i] = st->upd_coef[i]; }
+  }
+  __syncthreads();
+  const int m = s_m;
+  if (m == 0) return;
+  double2* dst = reinterpret_cast<double2*>(X + (size_t)s_dst * field);
+  const size_t n2 = field / 2;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += (size_t)gridDim.x * blockDim.x) {
+    double2 acc = make_double2(0.0, 0.0);
+    for (int k = 0; k < m; ++k) {
+      const double2 xv = reinterpret_cast<const double2*>(X + (size_t)s_list[k] * field)[i];
+      const double2 rv = reinterpret_cast<const double2*>(R + (size_t)s_list[k] * field)[i];
+      const double ck = s_c[k];
+      acc.x = acc.x + ck * (xv.x + b * rv.x);
+      acc.y = acc.y + ck * (xv.y + b * rv.y);
+    }
+    dst[i] = acc;
+  }
+}
+
+int launch_mdiis_update(const Grid& g, const Buffers& b, const SolverParams& sp, cudaStream_t s) {
+  const size_t n2 = g.field / 2;
+  size_t blocks = (n2 + 255) / 256;
+  const size_t cap = 148 * 8 * 4;
+  if (blocks > cap) blocks = cap;
+  mdiis_update_kernel<<<(unsigned)blocks, 256, 0, s>>>(b.state, b.X, b.R, g.field, sp.b);
+  return 1;
+}
+
+}  // namespace r3d

@@ -1,0 +1,141 @@
+// rism3d_internal.h -- shared declarations of the CUDA side of librism3d.so (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/rism3d.h"
+
+namespace r3d {
+
+constexpr int MAX_M = 16;            // MDIIS history slots (rism3d_params.mdiis_nvec <= 16)
+constexpr int MAX_NV = 8;            // solvent site types
+constexpr int RMS_HIST_CAP = 65536;
+constexpr int GRAM_BLOCKS_MAX = 148 * 8;
+
+constexpr double K_BOLTZMANN = 0.001987204259;   // kcal/(mol K)     (Q3)
+constexpr double COULOMB = 332.06371;            // kcal A/(mol e^2) (Q3)
+
+// Device-resident solver state: the whole MDIIS bookkeeping lives on the GPU so that an iteration is a
+// fixed sequence of launches (graph-capturable) and `iterate` never has to synchronise per iteration.
+struct DevState {
+  // ---- header: the first 64 bytes are what rism3d_iterate copies back to the host ----
+  int done;                    // 1: converged or diverged -> all loop kernels return immediately
+  int status;                  // rism3d_status
+  int n_done;                  // iterations completed by the current rism3d_iterate call
+  int hist_n;                  // total iterations since set_solute
+  int m;                       // filled history entries
+  int cur;                     // physical slot that holds the current input tau (not yet in `list`)
+  int upd_m;                   // entries to combine in the update kernel (0: skip)
+  int upd_dst;                 // physical slot the update writes (== new cur)
+  double tol;
+  double rms_last;
+  double pad_[2];
+  // ---- MDIIS bookkeeping ----
+  int list[MAX_M];             // physical slot of each entry, oldest first
+  int upd_list[MAX_M];
+  double upd_coef[MAX_M];
+  double S[MAX_M][MAX_M];      // Gram matrix of the stored residuals, indexed like `list`
+  double rms[MAX_M];           // rms of each entry
+  double rms_hist[RMS_HIST_CAP];
+};
+struct StateHeader {           // mirrors the first 64 bytes of DevState
+  int done, status, n_done, hist_n, m, cur, upd_m, upd_dst;
+  double tol, rms_last, pad_[2];
+};
+
+struct Grid {
+  int n;                 // points per axis (cubic)
+  int nv;                // site types
+  double h;              // spacing
+  double origin[3];
+  size_t npts;           // n^3
+  size_t field;          // nv * n^3 doubles in one field-set
+};
+
+// Device pointers carved from the caller's workspace.
+struct Buffers {
+  DevState* state;
+  double* X;             // [M][field]   MDIIS inputs  (tau)
+  double* R;             // [M][field]   MDIIS residuals
+  double* w;             // [field]      -beta u + f
+  double2* work;         // [n][n][n/2][nv] complex   k-space work array
+  double* phi;           // [npts]       phi(r)
+  double2* phik;         // [n][n][n/2]  phi~(k) exp(+i k.r0) / dV
+  double* chi_shell;     // [nshell][nv][nv]   chi_shell[s][g][g'] = chi_{g' g}(k_s)
+  double2* tw;           // [2n]         exp(-i pi j / n)
+  double* gram_part;     // [GRAM_BLOCKS_MAX][MAX_M+1][2]  double-double partial sums
+  double* scratch;       // [field] temporary (get_field, setup tables); aliases `work`
+  double* qv;            // [nv] solvent charges
+  double* rhov;          // [nv]
+  double* fe_part;       // [GRAM_BLOCKS_MAX][MAX_NV][2]
+};
+
+struct SolverParams {
+  int closure;           // rism3d_closure
+  int pse_order;
+  int M;
+  double b;
+  double restart;
+  double beta, kT, kappa, r_min;
+};
+
+// ---- launchers (each returns the number of kernels it launched; errors surface via cudaGetLastError) ----
+// fft_kernels.cu
+int launch_closure_zfwd(const Grid&, const Buffers&, const SolverParams&, const double* d_raw_in, cudaStream_t);
+int launch_y_fwd(const Grid&, const Buffers&, bool use_state, cudaStream_t);
+int launch_x_fwd(const Grid&, const Buffers&, cudaStream_t);
+int launch_x_inv(const Grid&, const Buffers&, cudaStream_t);
+int launch_kspace_x(const Grid&, const Buffers&, cudaStream_t);
+int launch_y_inv(const Grid&, const Buffers&, bool use_state, cudaStream_t);
+int launch_zinv_residual(const Grid&, const Buffers&, const SolverParams&, double* d_raw_out, cudaStream_t);
+int gram_blocks(const Grid&);
+// mdiis_kernels.cu
+int launch_mdiis_solve(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);
+int launch_mdiis_update(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);
+// setup_kernels.cu
+int launch_chi_shell(const Grid&, const Buffers&, const double* d_chi_table, int n_k, double k0, double dk,
+                     cudaStream_t);
+int launch_potential(const Grid&, const Buffers&, const SolverParams&, int n_atoms, const double* d_atoms,
+                     const double* d_pair, double rcut, cudaStream_t);
+int launch_phi_tilde(const Grid&, const Buffers&, const SolverParams&, int n_atoms, const double* d_atoms,
+                     double2* d_phase, cudaStream_t);
+int launch_free_energy(const Grid&, const Buffers&, const SolverParams&, double* d_out, cudaStream_t);
+int launch_get_field(const Grid&, const Buffers&, const SolverParams&, int which, int site, double* d_dst,
+                     cudaStream_t);
+
+// double-double helpers (used by the Gram and free-energy reductions)
+__device__ __forceinline__ void dd_add_prod(double& hi, double& lo, double a, double b) {
+  const double p = __dmul_rn(a, b);        // kept out of FMA contraction: the error-free split needs the rounded product
+  const double e = __fma_rn(a, b, -p);
+  const double s = hi + p;
+  const double bb = s - hi;
+  const double err = (hi - (s - bb)) + (p - bb);
+  hi = s;
+  lo += err + e;
+}
+__device__ __forceinline__ void dd_add(double& hi, double& lo, double h2, double l2) {
+  const double s = hi + h2;
+  const double bb = s - hi;
+  const double err = (hi - (s - bb)) + (h2 - bb);
+  hi = s;
+  lo += err + l2;
+}
+__device__ __forceinline__ void dd_norm(double& hi, double& lo) {
+  const double s = hi + lo;
+  lo = lo - (s - hi);
+  hi = s;
+}
+
+// closure g(d) (Q1, Q2): HNC exp(d); KH/PSE-n: exp(d) for d <= 0, sum_{i<=n} d^i/i! for d > 0
+__device__ __forceinline__ double closure_g(double d, int closure, int order) {
+  if (closure == RISM3D_HNC) return exp(d);
+  if (d > 0.0) {
+    double s = 1.0;
+    for (int i = order; i >= 1; --i) s = 1.0 + s * d / (double)i;
+    return s;
+  }
+  return exp(d);
+}
+
+}  // namespace r3d

@@ -1,0 +1,312 @@
+// setup_kernels.cu -- everything outside the iteration loop:
+//   potential_kernel   : w_g(r) = -beta u_g(r) + f_g(r) and phi(r)       (Eq. 22 + Eq. 29)
+//   phase / phi_tilde  : phi~(k) exp(+i k.r0)/dV on the stored half of the half-integer k grid (Eq. 30)
+//   chi_shell_kernel   : chi_{g'g}(|k|) for every distinct |k| of the grid, by 4-point Lagrange interpolation of
+//                        the radial table (Q6)
+//   free_energy_kernel : Eq. 17 / 18 / PSE-n grid sum (Q2, Q10)
+//   get_field_kernel   : g, h, c_sr, t, tau, w, phi of one site
+#include "rism3d_internal.h"
+
+namespace r3d {
+
+// ------------------------------------------------------------------------------------------------
+// Grid potential, all pairs (optionally with the sharp cutoff of Q12 on the short-range remainder).
+// One thread per grid point, atoms staged through shared memory in chunks.
+// atoms: [n_atoms] (x, y, z, beta*C*q_a);  pair: [n_atoms][nv] (beta C q_a q_g, sigma_ag^2, 4 beta eps_ag)
+// ------------------------------------------------------------------------------------------------
+constexpr int ATOM_CHUNK = 64;
+
+template <int NV>
+__global__ void __launch_bounds__(128)
+    potential_kernel(double* __restrict__ w, double* __restrict__ phi, const double4* __restrict__ atoms,
+                     const double* __restrict__ pair, int n_atoms, int n, double h, double ox, double oy, double oz,
+                     double kappa, double r_min, double rcut2, size_t npts) {
+  __shared__ double4 s_atom[ATOM_CHUNK];
+  __shared__ double s_pair[ATOM_CHUNK * NV * 3];
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;   // npts is a multiple of blockDim
+  const int iz = (int)(idx % n), iy = (int)((idx / n) % n), ix = (int)(idx / ((size_t)n * n));
+  // r_n = origin + spacing * index, each operation rounded separately (the pair set of a cutoff must not depend
+  // on contraction)
+  const double x = __dadd_rn(ox, __dmul_rn(h, (double)ix));
+  const double y = __dadd_rn(oy, __dmul_rn(h, (double)iy));
+  const double z = __dadd_rn(oz, __dmul_rn(h, (double)iz));
+  double acc[NV];
+#pragma unroll
+  for (int g = 0; g < NV; ++g) acc[g] = 0.0;
+  double ph = 0.0;
+  const bool cut = rcut2 > 0.0;
+  for (int a0 = 0; a0 < n_atoms; a0 += ATOM_CHUNK) {
+    const int na = min(ATOM_CHUNK, n_atoms - a0);
+    __syncthreads();
+    for (int i = threadIdx.x; i < na; i += blockDim.x) s_atom[i] = atoms[a0 + i];
+    for (int i = threadIdx.x; i < na * NV * 3; i += blockDim.x) s_pair[i] = pair[(size_t)a0 * NV * 3 + i];
+    __syncthreads();
+    for (int a = 0; a < na; ++a) {
+      const double4 at = s_atom[a];
+      const double dx = x - at.x, dy = y - at.y, dz = z - at.z;
+      const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+      const double rt = sqrt(r2);
+      const double kr = kappa * rt;
+      const double em = expm1(-kr);
+      const double lr = (kr < 1e-8) ? kappa : -em / rt;      // (1 - exp(-kappa r)) / r and its limit
+      ph += at.w * lr;
+      if (!cut || r2 < rcut2) {
+        const double rc = fmax(rt, r_min);
+        double sc;                                            // 1/r - (1 - exp(-kappa r))/r
+        if (rt >= r_min) sc = (1.0 + em) / rt;
+        else sc = cut ? exp(-kappa * rc) / rc : 1.0 / rc - lr;
+        const double inv2 = 1.0 / (rc * rc);
+        const double* pp = s_pair + a * NV * 3;
+#pragma unroll
+        for (int g = 0; g < NV; ++g) {
+          const double s2 = pp[g * 3 + 1] * inv2;
+          const double s6 = s2 * s2 * s2;
+          acc[g] -= pp[g * 3 + 0] * sc + pp[g * 3 + 2] * (s6 * s6 - s6);
+        }
+      }
+    }
+  }
+  phi[idx] = ph;
+#pragma unroll
+  for (int g = 0; g < NV; ++g) w[(size_t)g * npts + idx] = acc[g];
+}
+
+int launch_potential(const Grid& g, const Buffers& b, const SolverParams& sp, int n_atoms, const double* d_atoms,
+                     const double* d_pair, double rcut, cudaStream_t s) {
+  const unsigned blocks = (unsigned)(g.npts / 128);
+  const double rcut2 = rcut > 0.0 ? rcut * rcut : 0.0;
+  const double4* at = reinterpret_cast<const double4*>(d_atoms);
+#define POT(NV)                                                                                                   \
+  potential_kernel<NV><<<blocks, 128, 0, s>>>(b.w, b.phi, at, d_pair, n_atoms, g.n, g.h, g.origin[0], g.origin[1], \
+                                              g.origin[2], sp.kappa, sp.r_min, rcut2, g.npts)
+  switch (g.nv) {
+    case 1: POT(1); break;
+    case 2: POT(2); break;
+    case 4: POT(4); break;
+    case 8: POT(8); break;
+    default: return 0;
+  }
+#undef POT
+  return 1;
+}
+
+// ------------------------------------------------------------------------------------------------
+// phi~(k): separable phase tables E_axis[a][j] = exp(-i k_j (R_a,axis - r0,axis)), then
+//   phik[jx][jy][p] = (4 pi beta C / dV) kappa^2 / (k^2 (k^2 + kappa^2)) sum_a q_a Ex[a][jx] Ey[a][jy] Ez[a][2p]
+// d_phase: [3][n_atoms][n] complex (z table holds only the even j at index p, n/2 entries used)
+// ------------------------------------------------------------------------------------------------
+__global__ void phase_kernel(double2* __restrict__ phase, const double4* __restrict__ atoms, int n_atoms, int n,
+                             double h, double ox, double oy, double oz) {
+  const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t total = (size_t)3 * n_atoms * n;
+  if (idx >= total) return;
+  const int j = (int)(idx % n);
+  const int a = (int)((idx / n) % n_atoms);
+  const int axis = (int)(idx / ((size_t)n * n_atoms));
+  const double4 at = atoms[a];
+  const double d = axis == 0 ? at.x - ox : (axis == 1 ? at.y - oy : at.z - oz);
+  int jj = j;
+  if (axis == 2) { if (j >= n / 2) { phase[idx] = make_double2(0.0, 0.0); return; } jj = 2 * j; }
+  const double f = (jj < n / 2) ? (jj + 0.5) : (jj + 0.5 - n);          // k = dk * f, dk = 2 pi / (n h)
+  double sn, cs;
+  sincospi(2.0 * f * (d / (n * h)), &sn, &cs);
+  phase[idx] = make_double2(cs, -sn);
+}
+
+constexpr int PT_JY = 8;      // jy values per thread
+constexpr int PT_AC = 32;     // atoms per shared-memory chunk
+
+__global__ void __launch_bounds__(64)
+    phi_tilde_kernel(double2* __restrict__ phik, const double2* __restrict__ phase, const double* __restrict__ qa,
+                     int n_atoms, int n, double h, double kappa, double pref) {
+  __shared__ double2 s_a[PT_AC][PT_JY];
+  const int nz = n / 2;
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  const int jy0 = blockIdx.y * PT_JY;
+  const int jx = blockIdx.z;
+  const double2* Ex = phase;
+  const double2* Ey = phase + (size_t)n_atoms * n;
+  const double2* Ez = phase + (size_t)2 * n_atoms * n;
+  double2 acc[PT_JY];
+#pragma unroll
+  for (int i = 0; i < PT_JY; ++i) acc[i] = make_double2(0.0, 0.0);
+  for (int a0 = 0; a0 < n_atoms; a0 += PT_AC) {
+    const int na = min(PT_AC, n_atoms - a0);
+    __syncthreads();
+    for (int i = threadIdx.x; i < na * PT_JY; i += blockDim.x) {
+      const int a = a0 + i / PT_JY, jy = jy0 + i % PT_JY;
+      const double2 ex = Ex[(size_t)a * n + jx], ey = Ey[(size_t)a * n + jy];
+      const double q = qa[a];
+      s_a[i / PT_JY][i % PT_JY] = make_double2(q * (ex.x * ey.x - ex.y * ey.y), q * (ex.x * ey.y + ex.y * ey.x));
+    }
+    __syncthreads();
+    if (p < nz) {
+      for (int a = 0; a < na; ++a) {
+        const double2 ez = Ez[(size_t)(a0 + a) * n + p];
+#pragma unroll
+        for (int i = 0; i < PT_JY; ++i) {
+          const double2 v = s_a[a][i];
+          acc[i].x += v.x * ez.x - v.y * ez.y;
+          acc[i].y += v.x * ez.y + v.y * ez.x;
+        }
+      }
+    }
+  }
+  if (p >= nz) return;
+  const double dk = 2.0 * 3.14159265358979323846 / (n * h);
+  auto kof = [&](int j) { return dk * ((j < nz) ? (j + 0.5) : (j + 0.5 - n)); };
+  const double kx = kof(jx), kz = kof(2 * p);
+#pragma unroll
+  for (int i = 0; i < PT_JY; ++i) {
+    const double ky = kof(jy0 + i);
+    const double k2 = kx * kx + ky * ky + kz * kz;
+    const double f = pref * kappa * kappa / (k2 * (k2 + kappa * kappa));
+    phik[((size_t)jx * n + (jy0 + i)) * nz + p] = make_double2(f * acc[i].x, f * acc[i].y);
+  }
+}
+
+int launch_phi_tilde(const Grid& g, const Buffers& b, const SolverParams& sp, int n_atoms, const double* d_atoms,
+                     double2* d_phase, cudaStream_t s) {
+  const size_t total = (size_t)3 * n_atoms * g.n;
+  const double4* at = reinterpret_cast<const double4*>(d_atoms);
+  phase_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(d_phase, at, n_atoms, g.n, g.h, g.origin[0],
+                                                              g.origin[1], g.origin[2]);
+  // charges q_a live in a separate array right after the atom records (set up by the API layer)
+  const double* qa = d_atoms + (size_t)4 * n_atoms;
+  const int nz = g.n / 2;
+  const int bx = nz < 64 ? nz : 64;
+  dim3 grid((nz + bx - 1) / bx, g.n / PT_JY, g.n);
+  const double pref = 4.0 * 3.14159265358979323846 * sp.beta * COULOMB / (g.h * g.h * g.h);
+  phi_tilde_kernel<<<grid, bx, 0, s>>>(b.phik, d_phase, qa, n_atoms, g.n, g.h, sp.kappa, pref);
+  return 2;
+}
+
+// ------------------------------------------------------------------------------------------------
+// chi per |k| shell.  table: [n_k][nv][nv] (chi[m][g'][g]);  out: [nshell][g][g']
+// ------------------------------------------------------------------------------------------------
+__global__ void chi_shell_kernel(double* __restrict__ out, const double* __restrict__ table, int n_k, double k0,
+                                 double dkt, int nv, double dk_grid, int nshell) {
+  const int sidx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (sidx >= nshell) return;
+  const double kmag = dk_grid * sqrt(2.0 * sidx + 0.75);
+  const double xk = (kmag - k0) / dkt;
+  int m = (int)floor(xk);
+  int first = m - 1;
+  if (first < 0) first = 0;
+  if (first > n_k - 4) first = n_k - 4;
+  const double u = xk - first;
+  const double l0 = -(u - 1.0) * (u - 2.0) * (u - 3.0) / 6.0;
+  const double l1 = u * (u - 2.0) * (u - 3.0) / 2.0;
+  const double l2 = -u * (u - 1.0) * (u - 3.0) / 2.0;
+  const double l3 = u * (u - 1.0) * (u - 2.0) / 6.0;
+  const size_t st = (size_t)nv * nv;
+  for (int gp = 0; gp < nv; ++gp)
+    for (int g = 0; g < nv; ++g) {
+      const double* t = table + (size_t)first * st + gp * nv + g;
+      out[(size_t)sidx * st + g * nv + gp] = l0 * t[0] + l1 * t[st] + l2 * t[2 * st] + l3 * t[3 * st];
+    }
+}
+
+int launch_chi_shell(const Grid& g, const Buffers& b, const double* d_table, int n_k, double k0, double dk,
+                     cudaStream_t s) {
+  const int hn = g.n / 2;
+  const int nshell = 3 * (hn - 1) * hn / 2 + 1;
+  const double dk_grid = 2.0 * 3.14159265358979323846 / (g.n * g.h);
+  chi_shell_kernel<<<(nshell + 127) / 128, 128, 0, s>>>(b.chi_shell, d_table, n_k, k0, dk, g.nv, dk_grid, nshell);
+  return 1;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Solvation free energy:  dmu_g = kT dV rho_g sum_n [ -c_sr - h c / 2 + h^2 / 2 - B ],  c = c_sr - q_g phi
+//   B = h^2/2 Theta(h) (KH), Theta(d) d^(n+1)/(n+1)! (PSE-n), 0 (HNC)
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+    free_energy_kernel(double* __restrict__ part, const double* __restrict__ X, const double* __restrict__ w,
+                       const double* __restrict__ phi, const double* __restrict__ qv,
+                       const DevState* __restrict__ st, int nv, size_t npts, size_t field, int closure, int order) {
+  const double* tau = X + (size_t)st->cur * field;
+  __shared__ double s_red[8][2];
+  double inv_fact = 1.0;
+  for (int i = 2; i <= order + 1; ++i) inv_fact /= (double)i;
+  for (int g = 0; g < nv; ++g) {
+    double hi = 0.0, lo = 0.0;
+    const double q = qv[g];
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < npts; i += (size_t)gridDim.x * blockDim.x) {
+      const double t = tau[(size_t)g * npts + i];
+      const double d = w[(size_t)g * npts + i] + t;
+      const double gg = closure_g(d, closure, order);
+      const double hh = gg - 1.0;
+      const double csr = gg - 1.0 - t;
+      const double c = csr - q * phi[i];
+      double B = 0.0;
+      if (closure == RISM3D_KH) B = hh > 0.0 ? 0.5 * hh * hh : 0.0;
+      else if (closure == RISM3D_PSE) B = d > 0.0 ? pow(d, order + 1) * inv_fact : 0.0;
+      const double v = -csr - 0.5 * hh * c + 0.5 * hh * hh - B;
+      dd_add(hi, lo, v, 0.0);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+      const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
+      dd_add(hi, lo, h2, l2);
+    }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) { s_red[wid][0] = hi; s_red[wid][1] = lo; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      hi = 0.0; lo = 0.0;
+      for (int k = 0; k < 8; ++k) dd_add(hi, lo, s_red[k][0], s_red[k][1]);
+      part[((size_t)blockIdx.x * MAX_NV + g) * 2 + 0] = hi;
+      part[((size_t)blockIdx.x * MAX_NV + g) * 2 + 1] = lo;
+    }
+  }
+}
+
+__global__ void free_energy_final_kernel(double* __restrict__ out, const double* __restrict__ part, int nblocks,
+                                         const double* __restrict__ rhov, int nv, double scale) {
+  const int g = threadIdx.x;
+  if (g >= nv) return;
+  double hi = 0.0, lo = 0.0;
+  for (int b = 0; b < nblocks; ++b) dd_add(hi, lo, part[((size_t)b * MAX_NV + g) * 2], part[((size_t)b * MAX_NV + g) * 2 + 1]);
+  out[g] = scale * rhov[g] * (hi + lo);
+}
+
+int launch_free_energy(const Grid& g, const Buffers& b, const SolverParams& sp, double* d_out, cudaStream_t s) {
+  const int blocks = 148 * 4;
+  free_energy_kernel<<<blocks, 256, 0, s>>>(b.fe_part, b.X, b.w, b.phi, b.qv, b.state, g.nv, g.npts, g.field,
+                                            sp.closure, sp.pse_order);
+  free_energy_final_kernel<<<1, 32, 0, s>>>(d_out, b.fe_part, blocks, b.rhov, g.nv, sp.kT * g.h * g.h * g.h);
+  return 2;
+}
+
+// ------------------------------------------------------------------------------------------------
+__global__ void get_field_kernel(double* __restrict__ dst, const double* __restrict__ X, const double* __restrict__ w,
+                                 const double* __restrict__ phi, const double* __restrict__ qv,
+                                 const DevState* __restrict__ st, int which, int site, size_t npts, size_t field,
+                                 int closure, int order) {
+  const double* tau = X + (size_t)st->cur * field + (size_t)site * npts;
+  const double* ws = w + (size_t)site * npts;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < npts; i += (size_t)gridDim.x * blockDim.x) {
+    double v;
+    if (which == RISM3D_FIELD_PHI) v = phi[i];
+    else if (which == RISM3D_FIELD_W) v = ws[i];
+    else if (which == RISM3D_FIELD_TAU) v = tau[i];
+    else if (which == RISM3D_FIELD_T) v = tau[i] + qv[site] * phi[i];
+    else {
+      const double t = tau[i];
+      const double gg = closure_g(ws[i] + t, closure, order);
+      v = which == RISM3D_FIELD_G ? gg : (which == RISM3D_FIELD_H ? gg - 1.0 : gg - 1.0 - t);
+    }
+    dst[i] = v;
+  }
+}
+
+int launch_get_field(const Grid& g, const Buffers& b, const SolverParams& sp, int which, int site, double* d_dst,
+                     cudaStream_t s) {
+  size_t blocks = (g.npts + 255) / 256;
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  get_field_kernel<<<(unsigned)blocks, 256, 0, s>>>(d_dst, b.X, b.w, b.phi, b.qv, b.state, which, site, g.npts,
+                                                    g.field, sp.closure, sp.pse_order);
+  return 1;
+}
+
+}  // namespace r3d
