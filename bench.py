@@ -1,0 +1,386 @@
+"""bench.py -- 3D-RISM iteration throughput of librism3d.so on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C4]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A "step" is ONE 3D-RISM iteration = one pass of the loop rows S1-S7 of DESIGN.md (closure, forward 3D FFT,
+tail subtraction + chi mat-vec, inverse 3D FFT, residual + Gram row, MDIIS solve, MDIIS update) over the whole
+grid of the workload, with a FULL MDIIS history (the warm-up runs at least M iterations so that every timed
+step reads all 2M history fields).  The setup kernel (S0) and the free energy (S8) are timed separately and
+are part of the end-to-end solve (`e2e`).  One JSON line on stdout (rank 0); DESIGN.md "Measurement" explains
+every key.  N > 1 runs N independent replicas (one solute per GPU, no data-path collective: DESIGN.md
+"Multi-GPU").
+
+`--impl reference` times the CPU oracle (oracle/, numpy fp64, as it stands) on a bounded sample of the same
+workload; it is the only other place besides `cpu_baseline` where this file executes oracle code.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "3D-RISM iterations/s"
+UNIT = "iterations/s"
+CPU_SAMPLE_N = 64            # grid of the oracle's bounded sample (same box as the workload, coarser spacing)
+CPU_SAMPLE_ATOMS = 64        # the loop cost does not depend on the atom count; the (untimed) setup does
+
+
+# ---------------------------------------------------------------------------------------------------------
+# algorithmic HBM words per grid-point*site and iteration of each loop kernel
+# ---------------------------------------------------------------------------------------------------------
+def kernel_words(n_v: int, m_hist: int) -> dict:
+    """m_hist = stored MDIIS entries during the timed steps (= M once the history is full)."""
+    return {
+        "closure_zfwd": 3.0,                    # read tau, w; write c_sr(z-transformed)
+        "y_fwd": 2.0,                           # in place
+        "kspace_x": 2.0 + 1.0 / n_v,            # in place + phi~ (one complex per 2 points, shared by the sites)
+        "y_inv": 2.0,
+        "zinv_residual": m_hist + 2.0,          # read work, tau, M-1 old residuals; write R
+        "mdiis_solve": 0.0,
+        "mdiis_update": 2.0 * m_hist + 1.0,     # read M inputs + M residuals; write the new input
+    }
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ---------------------------------------------------------------------------------------------------------
+# clocks: nvidia-smi sampled DURING the timed region
+# ---------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device_index: int):
+        self.path = tempfile.mktemp(prefix="rism3d_clocks_", suffix=".csv")
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(device_index), f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            with open(self.path) as f:
+                for line in f:
+                    parts = [x.strip() for x in line.split(",")]
+                    if len(parts) < 7:
+                        continue
+                    try:
+                        sm.append(float(parts[0])); smax.append(float(parts[1])); power.append(float(parts[2]))
+                    except ValueError:
+                        continue
+                    for nm, v in zip(names, parts[3:7]):
+                        if v.lower().startswith("active"):
+                            reasons.add(nm)
+            os.unlink(self.path)
+        except OSError:
+            pass
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(power)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------------
+# distributed plumbing (replicas: a barrier and a max / sum over ranks of scalars, nothing on the data path)
+# ---------------------------------------------------------------------------------------------------------
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def dist_init(backend: str):
+    import torch.distributed as dist
+    rank, _, world = dist_env()
+    if world > 1 and not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29511")
+        dist.init_process_group(backend=backend, rank=rank, world_size=world)
+    return rank, world
+
+
+def reduce_scalars(values, op: str, device):
+    """max / sum over ranks of a list of floats -> list of floats (identity when world size is 1)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX if op == "max" else dist.ReduceOp.SUM)
+    return [float(v) for v in t.cpu()]
+
+
+def aggregate_throughput(units_local: float, ms_local: float, device):
+    """Whole-job throughput of a replicated run: units of ALL ranks / the slowest rank's time.
+    -> (units_total / s, max ms)"""
+    (ms_max,) = reduce_scalars([ms_local], "max", device)
+    (units,) = reduce_scalars([units_local], "sum", device)
+    return units / (ms_max * 1e-3), ms_max
+
+
+# ---------------------------------------------------------------------------------------------------------
+# workload
+# ---------------------------------------------------------------------------------------------------------
+def workload_inputs(name: str, rank: int = 0):
+    """-> (cfg, solvent, solute, (k0, dk, chi)).  Replica r of a multi-GPU run gets its own seeded solute."""
+    from workloads import get_config, load_chi, make_solute, solvent_by_name
+    from workloads import solutes as _sol
+    cfg = get_config(name)
+    sv = solvent_by_name(cfg.solvent)
+    if rank == 0 or name in ("C1",):
+        sol = make_solute(name)
+    else:
+        base_seed = {"C2": 2, "C3": 3, "C4": 4, "C5": 5}[name]
+        sol = getattr(_sol, "make_" + name.lower())(seed=base_seed + 100 * rank)
+    return cfg, sv, sol, load_chi(sv.name)
+
+
+def workload_label(cfg, sol) -> str:
+    return (f"{cfg.name}: {sol.n_atoms}-atom synthetic solute ({sol.name}), {cfg.solvent}, grid {cfg.n}^3 at "
+            f"{cfg.spacing} A, {cfg.closure}{'-%d' % cfg.pse_order if cfg.closure == 'PSE' else ''}, "
+            f"MDIIS {cfg.mdiis_nvec} vectors, fp64")
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the oracle on a bounded sample (cpu_baseline leg and --impl reference)
+# ---------------------------------------------------------------------------------------------------------
+class OracleSample:
+    """The workload's box, solvent, closure and MDIIS settings on a CPU_SAMPLE_N^3 grid (coarser spacing, same
+    box edge) with the first CPU_SAMPLE_ATOMS atoms of its solute.  One oracle iteration costs the same per
+    grid-point*site whatever the atoms are, so iterations/s at the full grid = measured point*site rate /
+    (n^3 n_v)."""
+
+    def __init__(self, name: str):
+        from oracle import rism3d as o3
+        cfg, sv, sol, (k0, dk, chi) = workload_inputs(name)
+        self.cfg, self.sv = cfg, sv
+        self.n = min(CPU_SAMPLE_N, cfg.n)
+        self.spacing = cfg.spacing * cfg.n / self.n
+        na = min(CPU_SAMPLE_ATOMS, sol.n_atoms)
+        self.orc = o3.Rism3dOracle(self.n, self.spacing, sv.n_v, closure=cfg.closure, pse_order=cfg.pse_order,
+                                   mdiis_nvec=cfg.mdiis_nvec, mdiis_b=cfg.mdiis_b, mdiis_restart=cfg.mdiis_restart)
+        self.orc.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+        self.orc.set_solute(sol.xyz[:na], sol.q[:na], sol.sigma[:na], sol.eps[:na], rcut=cfg.rcut)
+        self.pt_sites_sample = float(self.n ** 3 * sv.n_v)
+        self.pt_sites_full = float(cfg.n ** 3 * sv.n_v)
+        self.label = (f"{cfg.name} settings ({sv.n_v} sites, {cfg.closure}, MDIIS {cfg.mdiis_nvec}) on a {self.n}^3 grid at "
+                      f"{self.spacing:g} A (same {cfg.n * cfg.spacing:g} A box, 1/{int(self.pt_sites_full / self.pt_sites_sample)} "
+                      f"of the points), first {na} atoms; rate scaled by grid-point*site count")
+
+    def run(self, steps: int, warmup: int):
+        """-> seconds per oracle iteration on the sample (history filled during the warm-up)."""
+        self.orc.iterate(max(warmup, 0), 0.0)
+        t0, c0 = time.perf_counter(), time.process_time()
+        self.orc.iterate(steps, 0.0)
+        wall = time.perf_counter() - t0
+        self.threads_used = max(1, int(round((time.process_time() - c0) / wall)))   # CPU time / wall time
+        return wall / steps
+
+    def iterations_per_s_full(self, s_per_iter_sample: float) -> float:
+        return (self.pt_sites_sample / s_per_iter_sample) / self.pt_sites_full
+
+
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    smp = OracleSample(args.workload)
+    s_per = smp.run(args.steps, max(args.warmup, smp.cfg.mdiis_nvec))
+    val = smp.iterations_per_s_full(s_per)
+    cfg = smp.cfg
+    from workloads import make_solute
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": s_per * 1e3 * smp.pt_sites_full / smp.pt_sites_sample,
+        "ms_per_step_sample": s_per * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_label(cfg, make_solute(cfg.name)), "timing": "host perf_counter (CPU program)"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": smp.threads_used, "kind": "oracle", "sample": smp.label,
+                         "host_cores_available": os.cpu_count()},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------------
+# the CUDA path
+# ---------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device for --impl ours (there is no CPU fallback)")
+    import paper_2403_01039_b200 as lib
+    rank, local_rank, world = dist_env()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist_init("nccl")
+    import torch.distributed as dist
+
+    cfg, sv, sol, (k0, dk, chi) = workload_inputs(args.workload, rank)
+    M, n_v = cfg.mdiis_nvec, sv.n_v
+    pt_sites = float(cfg.n ** 3 * n_v)
+    solver = lib.Solver(cfg.n, cfg.spacing, n_v, closure=cfg.closure, pse_order=cfg.pse_order, mdiis_nvec=M,
+                        mdiis_b=cfg.mdiis_b, mdiis_restart=cfg.mdiis_restart, temperature=cfg.temperature,
+                        kappa=cfg.kappa, r_min=cfg.r_min, device=local_rank)
+    solver.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+    setup_ms = solver.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=cfg.rcut)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # ---- device-resident throughput: K iterations with a full history -------------------------------------
+    warm = max(args.warmup, M, 3)
+    solver.iterate(warm, 0.0)
+    launches0 = solver.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    barrier()
+    ev0.record(solver.stream)
+    n_done, rms_end = solver.iterate(args.steps, 0.0)
+    ev1.record(solver.stream)
+    barrier()
+    ms_local = ev0.elapsed_time(ev1)
+    launches = solver.launch_count() - launches0
+    value, ms_max = aggregate_throughput(float(args.steps), ms_local, dev)
+
+    # ---- per-kernel CUDA-event times (second pass over the same number of steps) -----------------------------
+    solver.set_profiling(True)
+    solver.iterate(args.steps, 0.0)
+    kern_ms, prof_n = solver.timings()
+    solver.set_profiling(False)
+    clocks = sampler.stop() if sampler else None
+    peak, peak_src = load_peaks()
+    words = kernel_words(n_v, M)
+    kernels = {}
+    for name, ms in kern_ms.items():
+        gb = words[name] * 8.0 * pt_sites / 1e9
+        kernels[name] = {"ms": ms, "algorithmic_gb": gb, "gbs": (gb / (ms * 1e-3) if ms > 0 else 0.0),
+                         "frac": (gb / (ms * 1e-3) / peak if ms > 0 else 0.0)}
+    dominant = max(kernels, key=lambda k: kernels[k]["ms"])
+    traffic = ncu_traffic(dominant, args.workload)
+    roofline = {"bound": "hbm", "kernel": dominant, "achieved": kernels[dominant]["gbs"], "peak": peak, "unit": "GB/s",
+                "frac": kernels[dominant]["frac"], "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": kernels[dominant]["algorithmic_gb"] * 1e9,
+                "iteration": {"ms_sum_of_kernels": sum(k["ms"] for k in kernels.values()),
+                              "algorithmic_gb": sum(k["algorithmic_gb"] for k in kernels.values()),
+                              "frac": sum(k["algorithmic_gb"] for k in kernels.values()) /
+                              (sum(k["ms"] for k in kernels.values()) * 1e-3) / peak},
+                "kernels": kernels}
+
+    # ---- end to end: one whole solve from HOST inputs to HOST results through the C ABI ------------------------
+    e2e = None
+    if not args.no_e2e:
+        g_host = torch.empty((n_v, cfg.n, cfg.n, cfg.n), dtype=torch.float64, pin_memory=True)
+        g_np = g_host.numpy()
+        barrier()
+        t0 = time.perf_counter()
+        setup_ms_e2e = solver.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=cfg.rcut)    # H2D atoms + S0
+        it_conv, rms_conv = solver.iterate(args.max_iter, cfg.tol)                              # S1-S7 to 1e-6
+        t1 = time.perf_counter()
+        mu, mu_site = solver.free_energy()                                                      # S8 + D2H scalars
+        t2 = time.perf_counter()
+        for s in range(n_v):
+            lib.rism3d_get_field(solver.ctx, lib.FIELDS["G"], s, g_np[s].ctypes.data, False)    # D2H g
+        torch.cuda.synchronize(dev)
+        t3 = time.perf_counter()
+        (e2e_s,) = reduce_scalars([t3 - t0], "max", dev)
+        (it_total,) = reduce_scalars([float(it_conv)], "sum", dev)
+        e2e = {"value": it_total / e2e_s, "unit": UNIT,
+               "h2d_bytes_per_step": int(sol.n_atoms * 6 * 8), "d2h_bytes_per_step": int(g_np.nbytes + 8 * (n_v + 1) + 64),
+               "what": "one whole solve per replica: set_solute (host atom arrays -> device, S0) + iterate to rms < tol + "
+                       "free_energy + g of every site copied to pinned host memory; a 'step' of this leg is the solve",
+               "seconds_to_converge": e2e_s, "iterations_to_converge": int(it_conv), "converged": bool(rms_conv < cfg.tol),
+               "tol": cfg.tol, "rms": rms_conv, "setup_ms": setup_ms_e2e, "loop_s": t1 - t0 - setup_ms_e2e * 1e-3,
+               "free_energy_ms": (t2 - t1) * 1e3, "get_g_ms": (t3 - t2) * 1e3, "dmu_kcal_mol": mu,
+               "g_max": float(g_np.max())}
+
+    # ---- the oracle on the host cores (rank 0, single-GPU runs only) --------------------------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        smp = OracleSample(args.workload)
+        s_per = smp.run(args.cpu_steps, M)
+        cpu = {"value": smp.iterations_per_s_full(s_per), "unit": UNIT, "cores": smp.threads_used, "kind": "oracle",
+               "sample": smp.label + f"; {args.cpu_steps} timed iterations after {M} warm-up",
+               "s_per_iteration_sample": s_per, "host_cores_available": os.cpu_count()}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_label(cfg, sol), "parallelism": f"replicas x{world} (no collective on the data path)",
+                       "l2": "inputs larger than L2 (working set %.1f GB per replica)" % (solver.workspace.numel() / 1e9),
+                       "mdiis_history": "full (M entries) during the timed steps", "rcut_A": cfg.rcut},
+            "pt_site_updates_per_s": value * pt_sites, "setup_ms": setup_ms, "rms_after_timed_steps": rms_end,
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        }
+        print(json.dumps(line), flush=True)
+    solver.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def ncu_traffic(kernel: str, workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel`, from the committed ncu --set full summary
+    (profiles/traffic.json, written by hand from the capture named there); None when no capture covers it."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        t = json.load(f)
+    return t.get(workload, {}).get(kernel)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
+    ap.add_argument("--max-iter", type=int, default=1500, help="iteration cap of the end-to-end solve")
+    ap.add_argument("--cpu-steps", type=int, default=4, help="timed oracle iterations of the cpu_baseline leg")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.steps < 1:
+        ap.error("--steps must be >= 1")
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -134,6 +134,16 @@ int rism3d_get_rms_history(rism3d_ctx* ctx, double* dst, int cap, int* n);
 /* Number of kernels the library has launched on this context so far (for bench.py's gpu_launches). */
 long long rism3d_launch_count(const rism3d_ctx* ctx);
 
+/* Per-kernel GPU time of the loop kernels (CUDA events on the context's stream, one before and one after
+ * every kernel of an iteration).  set_profiling(1) clears the sums and switches the events on,
+ * set_profiling(0) switches them off; both synchronise the stream.  get_timings synchronises, then writes
+ * ms_total[k], k < RISM3D_N_LOOP_KERNELS (HOST, cap >= RISM3D_N_LOOP_KERNELS): the summed milliseconds of
+ * loop kernel k over *n_iterations profiled iterations, in launch order (names: rism3d_loop_kernel_name). */
+#define RISM3D_N_LOOP_KERNELS 7
+int rism3d_set_profiling(rism3d_ctx* ctx, int enable);
+int rism3d_get_timings(rism3d_ctx* ctx, double* ms_total, int cap, long long* n_iterations);
+const char* rism3d_loop_kernel_name(int k);             /* static strings; "" when k is out of range */
+
 /* Debug / test hooks: run the shifted 3D transform pair alone on a caller-supplied field.
  * forward: real DEVICE field [n_sites][nx][ny][nz] -> complex DEVICE spectrum
  *   [jx][jy][p][site] (re, im interleaved), p = 0..nz/2-1 standing for jz = 2p, holding

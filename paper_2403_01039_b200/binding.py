@@ -19,7 +19,8 @@ FIELDS = {"G": 0, "H": 1, "C_SR": 2, "T": 3, "TAU": 4, "W": 5, "PHI": 6}
 EXPORTED_SYMBOLS = [
     "rism3d_workspace_bytes", "rism3d_init", "rism3d_set_solvent_chi", "rism3d_set_solute",
     "rism3d_iterate", "rism3d_free_energy", "rism3d_get_field", "rism3d_set_tau",
-    "rism3d_get_rms_history", "rism3d_launch_count", "rism3d_debug_fft_forward",
+    "rism3d_get_rms_history", "rism3d_launch_count", "rism3d_set_profiling", "rism3d_get_timings",
+    "rism3d_loop_kernel_name", "rism3d_debug_fft_forward",
     "rism3d_debug_fft_inverse", "rism3d_last_error", "rism3d_status_string", "rism3d_destroy",
 ]
 
@@ -83,6 +84,12 @@ def load_library():
     lib.rism3d_get_rms_history.argtypes = [C.c_void_p, dp, C.c_int, ip]
     lib.rism3d_launch_count.restype = C.c_longlong
     lib.rism3d_launch_count.argtypes = [C.c_void_p]
+    lib.rism3d_set_profiling.restype = C.c_int
+    lib.rism3d_set_profiling.argtypes = [C.c_void_p, C.c_int]
+    lib.rism3d_get_timings.restype = C.c_int
+    lib.rism3d_get_timings.argtypes = [C.c_void_p, dp, C.c_int, C.POINTER(C.c_longlong)]
+    lib.rism3d_loop_kernel_name.restype = C.c_char_p
+    lib.rism3d_loop_kernel_name.argtypes = [C.c_int]
     lib.rism3d_debug_fft_forward.restype = C.c_int
     lib.rism3d_debug_fft_forward.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
     lib.rism3d_debug_fft_inverse.restype = C.c_int
@@ -178,6 +185,25 @@ def rism3d_get_rms_history(ctx, cap: int = 65536) -> np.ndarray:
 
 def rism3d_launch_count(ctx) -> int:
     return int(load_library().rism3d_launch_count(ctx))
+
+
+N_LOOP_KERNELS = 7
+
+
+def rism3d_set_profiling(ctx, enable: bool):
+    _check(ctx, load_library().rism3d_set_profiling(ctx, int(bool(enable))))
+
+
+def rism3d_get_timings(ctx):
+    """-> (ms_total[N_LOOP_KERNELS], n_iterations)"""
+    ms = np.zeros(N_LOOP_KERNELS)
+    n = C.c_longlong(0)
+    _check(ctx, load_library().rism3d_get_timings(ctx, _dptr(ms), N_LOOP_KERNELS, C.byref(n)))
+    return ms, int(n.value)
+
+
+def rism3d_loop_kernel_name(k: int) -> str:
+    return load_library().rism3d_loop_kernel_name(int(k)).decode()
 
 
 def rism3d_debug_fft_forward(ctx, d_in: int, d_out: int):
@@ -278,6 +304,14 @@ class Solver:
 
     def launch_count(self) -> int:
         return rism3d_launch_count(self.ctx)
+
+    def set_profiling(self, enable: bool):
+        rism3d_set_profiling(self.ctx, enable)
+
+    def timings(self):
+        """-> ({kernel name: mean ms per iteration}, n_iterations) of the profiled iterations"""
+        ms, n = rism3d_get_timings(self.ctx)
+        return {rism3d_loop_kernel_name(k): (ms[k] / n if n else 0.0) for k in range(N_LOOP_KERNELS)}, n
 
     def fft_forward(self, real_dev):
         """debug: real device tensor [n_sites][n][n][n] -> complex device tensor [n][n][n/2][n_sites]."""

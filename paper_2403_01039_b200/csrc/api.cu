@@ -24,6 +24,11 @@ struct rism3d_ctx {
   bool have_solvent, have_solute;
   double qv[MAX_NV], sigv[MAX_NV], epsv[MAX_NV], rhov[MAX_NV];
   long long launches;
+  bool profiling;            // per-kernel CUDA-event timing of the loop kernels (rism3d_set_profiling)
+  std::vector<cudaEvent_t>* ev_pool;
+  size_t ev_used;
+  double prof_ms[RISM3D_N_LOOP_KERNELS];
+  long long prof_iters;
   StateHeader* h_hdr;        // pinned
   double* d_out;             // small device array for scalar results (inside workspace)
   char err[512];
@@ -174,6 +179,10 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
 extern "C" void rism3d_destroy(rism3d_ctx* ctx) {
   if (!ctx) return;
   cudaStreamSynchronize(ctx->stream);
+  if (ctx->ev_pool) {
+    for (cudaEvent_t e : *ctx->ev_pool) cudaEventDestroy(e);
+    delete ctx->ev_pool;
+  }
   if (ctx->h_hdr) cudaFreeHost(ctx->h_hdr);
   delete ctx;
 }
@@ -284,20 +293,81 @@ __global__ void iterate_begin_kernel(DevState* st, double tol) {
   st->n_done = 0;
 }
 
+// profiling: one event before the first loop kernel and one after each (RISM3D_N_LOOP_KERNELS + 1 per iteration)
+static void prof_mark(rism3d_ctx* ctx) {
+  if (!ctx->profiling) return;
+  if (!ctx->ev_pool) ctx->ev_pool = new std::vector<cudaEvent_t>();
+  if (ctx->ev_used == ctx->ev_pool->size()) {
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) { ctx->profiling = false; return; }
+    ctx->ev_pool->push_back(e);
+  }
+  cudaEventRecord((*ctx->ev_pool)[ctx->ev_used++], ctx->stream);
+}
+
+// after the stream has been synchronised: fold the recorded events into the per-kernel sums
+static void prof_collect(rism3d_ctx* ctx) {
+  if (!ctx->ev_pool) return;
+  const size_t per = RISM3D_N_LOOP_KERNELS + 1;
+  for (size_t i = 0; i + per <= ctx->ev_used; i += per) {
+    for (int k = 0; k < RISM3D_N_LOOP_KERNELS; ++k) {
+      float ms = 0.f;
+      if (cudaEventElapsedTime(&ms, (*ctx->ev_pool)[i + k], (*ctx->ev_pool)[i + k + 1]) == cudaSuccess)
+        ctx->prof_ms[k] += ms;
+    }
+    ctx->prof_iters += 1;
+  }
+  ctx->ev_used = 0;
+}
+
 static int enqueue_iteration(rism3d_ctx* ctx) {
   const Grid& g = ctx->g;
   const Buffers& b = ctx->b;
   cudaStream_t s = ctx->stream;
   int k = 0;
+  prof_mark(ctx);
   k += launch_closure_zfwd(g, b, ctx->sp, nullptr, s);     // step 2 + z of step 3
+  prof_mark(ctx);
   k += launch_y_fwd(g, b, true, s);                        // step 3
+  prof_mark(ctx);
   k += launch_kspace_x(g, b, s);                           // step 3 (x), Eq. 32, step 4, x of step 5
+  prof_mark(ctx);
   k += launch_y_inv(g, b, true, s);                        // step 5
+  prof_mark(ctx);
   k += launch_zinv_residual(g, b, ctx->sp, nullptr, s);    // step 5 (z), Eq. 33, Gram row
+  prof_mark(ctx);
   k += launch_mdiis_solve(g, b, ctx->sp, s);               // step 6-7
+  prof_mark(ctx);
   k += launch_mdiis_update(g, b, ctx->sp, s);              // step 6
+  prof_mark(ctx);
   ctx->launches += k;
   return k;
+}
+
+extern "C" int rism3d_set_profiling(rism3d_ctx* ctx, int enable) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  CU(cudaStreamSynchronize(ctx->stream));
+  ctx->ev_used = 0;
+  ctx->profiling = enable != 0;
+  for (int k = 0; k < RISM3D_N_LOOP_KERNELS; ++k) ctx->prof_ms[k] = 0.0;
+  ctx->prof_iters = 0;
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_get_timings(rism3d_ctx* ctx, double* ms_total, int cap, long long* n_iterations) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (!ms_total || cap < RISM3D_N_LOOP_KERNELS) return fail(ctx, RISM3D_ERR_ARG, "ms_total needs %d entries", RISM3D_N_LOOP_KERNELS);
+  CU(cudaStreamSynchronize(ctx->stream));
+  prof_collect(ctx);
+  for (int k = 0; k < RISM3D_N_LOOP_KERNELS; ++k) ms_total[k] = ctx->prof_ms[k];
+  if (n_iterations) *n_iterations = ctx->prof_iters;
+  return RISM3D_OK;
+}
+
+extern "C" const char* rism3d_loop_kernel_name(int k) {
+  static const char* names[RISM3D_N_LOOP_KERNELS] = {"closure_zfwd", "y_fwd", "kspace_x", "y_inv", "zinv_residual",
+                                                     "mdiis_solve", "mdiis_update"};
+  return (k >= 0 && k < RISM3D_N_LOOP_KERNELS) ? names[k] : "";
 }
 
 static int read_header(rism3d_ctx* ctx) {
@@ -324,6 +394,7 @@ extern "C" int rism3d_iterate(rism3d_ctx* ctx, int max_iter, double tol, int* n_
   CU(cudaGetLastError());
   int rc = read_header(ctx);
   if (rc) return rc;
+  prof_collect(ctx);
   if (n_done) *n_done = ctx->h_hdr->n_done;
   if (rms) *rms = ctx->h_hdr->rms_last;
   if (ctx->h_hdr->status == RISM3D_ERR_DIVERGED)
