@@ -86,8 +86,8 @@ static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_o
   char* phik = take(npts * 8);
   char* chis = take((size_t)n_shells((int)n) * nv * nv * 8);
   char* tw = take(2 * n * 16);
-  char* gp = take((size_t)GRAM_BLOCKS_MAX * (MAX_M + 1) * 2 * 8);
-  char* fp = take((size_t)GRAM_BLOCKS_MAX * MAX_NV * 2 * 8);
+  char* gp = take((size_t)gram_blocks_for((int)n, (int)nv) * (MAX_M + 1) * 2 * 8);
+  char* fp = take((size_t)FE_BLOCKS * MAX_NV * 2 * 8);
   char* qv = take(MAX_NV * 8);
   char* rv = take(MAX_NV * 8);
   char* out = take(64 * 8);

@@ -144,35 +144,70 @@ int launch_x_inv(const Grid& g, const Buffers& b, cudaStream_t s) {
 // ------------------------------------------------------------------------------------------------
 constexpr int ZP = COLS + 1;
 
-template <int NZ>
-__global__ void __launch_bounds__(FftCfg<NZ>::T* FftCfg<NZ>::G* COLS)
+// Column groups per CTA of the z kernels (more than the strided passes use: these kernels stream whole fields and
+// want >= 256 threads with many independent loads in flight).
+template <int NZ> struct ZGroups { enum { G = FftCfg<NZ>::G }; };
+template <> struct ZGroups<64>  { enum { G = 4 }; };    // 8 * 4 * 8 = 256 threads
+template <> struct ZGroups<128> { enum { G = 4 }; };    // 8 * 4 * 8 = 256 threads, 72 KB tile
+template <> struct ZGroups<256> { enum { G = 2 }; };    // 16 * 2 * 8 = 256 threads, 72 KB tile
+
+__device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
+__device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
+
+// closure + forward z.  One tile per CTA.  Stage-in with 16-byte loads (two adjacent z points of both half lines
+// per thread, two such quads in flight), closure, packing u_m = (c_m - i c_{m+n/2}) exp(-i pi m / n) into the
+// shared-memory tile, then the n/2-point complex line FFTs.
+template <int NZ, int G>
+__global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
     closure_zfwd_kernel(const double* __restrict__ X, const double* __restrict__ w, const double* __restrict__ raw,
                         cplx* __restrict__ work, Twiddle tw_shift, Twiddle tw, const DevState* __restrict__ st,
                         int nv, size_t npts, size_t field, int closure, int order) {
   if (raw == nullptr && st->done) return;
   using Cfg = FftCfg<NZ>;
-  constexpr int T = Cfg::T, G = Cfg::G, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS, n = 2 * NZ;
+  constexpr int T = Cfg::T, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS, n = 2 * NZ;
+  constexpr int NT = T * G * C, HP = NZ / 2, U = 2;
   const int tid = threadIdx.x;
-  const int LP = C / nv, GL = G * LP;                 // lines per tile, lines per CTA
+  const int LP = C / nv, GL = G * LP;                 // lines per column group, lines per CTA
   const size_t line0 = (size_t)blockIdx.x * GL;
-  const double* tau = raw ? nullptr : X + (size_t)st->cur * field;
+  const double* tau = raw ? raw : X + (size_t)st->cur * field;
+  const int total = GL * nv * HP;
 
-  // stage in: closure, pack u_m = (c_m - i c_{m+n/2}) exp(-i pi m / n)
-  for (int e = tid; e < GL * nv * NZ; e += blockDim.x) {
-    const int m = e % NZ, lc = e / NZ;
-    const int site = lc / GL, l = lc % GL;
-    const size_t off = (size_t)site * npts + (line0 + l) * n + m;
-    double c0, c1;
-    if (raw) {
-      c0 = raw[off];
-      c1 = raw[off + NZ];
-    } else {
-      const double t0 = tau[off], t1 = tau[off + NZ];
-      c0 = closure_g(w[off] + t0, closure, order) - 1.0 - t0;
-      c1 = closure_g(w[off + NZ] + t1, closure, order) - 1.0 - t1;
+  for (int e0 = tid; e0 < total; e0 += U * NT) {
+    double2 t0[U], t1[U], w0[U], w1[U];
+    size_t off[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int e = e0 + u * NT;
+      if (e < total) {
+        const int mp = e % HP, lc = e / HP;
+        const int site = lc / GL, l = lc % GL;
+        off[u] = (size_t)site * npts + (line0 + l) * n + 2 * mp;
+        t0[u] = ld2(tau + off[u]);
+        t1[u] = ld2(tau + off[u] + NZ);
+        if (!raw) {
+          w0[u] = ld2(w + off[u]);
+          w1[u] = ld2(w + off[u] + NZ);
+        }
+      }
     }
-    const cplx u = cmul(make_double2(c0, -c1), tw_shift(m));
-    smem_dyn[(l / LP) * (NZ * ZP) + m * ZP + (l % LP) * nv + site] = u;
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      const int e = e0 + u * NT;
+      if (e < total) {
+        const int mp = e % HP, lc = e / HP;
+        const int site = lc / GL, l = lc % GL;
+        double2 c0 = t0[u], c1 = t1[u];
+        if (!raw) {                                    // g = closure(w + tau), c_sr = g - 1 - tau  (Eq. 15-16, 31)
+          c0.x = closure_g(w0[u].x + t0[u].x, closure, order) - 1.0 - t0[u].x;
+          c0.y = closure_g(w0[u].y + t0[u].y, closure, order) - 1.0 - t0[u].y;
+          c1.x = closure_g(w1[u].x + t1[u].x, closure, order) - 1.0 - t1[u].x;
+          c1.y = closure_g(w1[u].y + t1[u].y, closure, order) - 1.0 - t1[u].y;
+        }
+        cplx* tile = smem_dyn + (l / LP) * (NZ * ZP) + (l % LP) * nv + site;
+        tile[(2 * mp) * ZP] = cmul(make_double2(c0.x, -c1.x), tw_shift(2 * mp));
+        tile[(2 * mp + 1) * ZP] = cmul(make_double2(c0.y, -c1.y), tw_shift(2 * mp + 1));
+      }
+    }
   }
   __syncthreads();
 
@@ -198,11 +233,12 @@ template <int NZ>
 static int launch_closure_zfwd_n(const Grid& gr, const Buffers& b, const SolverParams& sp, const double* raw,
                                  cudaStream_t s) {
   using Cfg = FftCfg<NZ>;
-  const int LP = COLS / gr.nv, GL = Cfg::G * LP;
+  constexpr int G = ZGroups<NZ>::G;
+  const int LP = COLS / gr.nv, GL = G * LP;
   const size_t nlines = (size_t)gr.n * gr.n;
-  const int threads = Cfg::T * Cfg::G * COLS;
-  const size_t shm = (size_t)Cfg::G * NZ * ZP * sizeof(cplx);
-  auto kern = closure_zfwd_kernel<NZ>;
+  const int threads = Cfg::T * G * COLS;
+  const size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
+  auto kern = closure_zfwd_kernel<NZ, G>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
   kern<<<(unsigned)(nlines / GL), threads, shm, s>>>(b.X, b.w, raw, b.work, tws, tw, b.state, gr.nv, gr.npts,
@@ -225,21 +261,24 @@ int launch_closure_zfwd(const Grid& g, const Buffers& b, const SolverParams& sp,
   return k;
 }
 
-// inverse z + residual + Gram row.  Persistent over tiles so that the Gram accumulators stay in registers.
-template <int NZ>
-__global__ void __launch_bounds__(FftCfg<NZ>::T* FftCfg<NZ>::G* COLS)
+// inverse z + residual + Gram row.  One tile per CTA: inverse line FFTs in shared memory, the last stage leaves
+// (f_m, f_{m+n/2}) in place of complex element m, then a streaming phase with 16-byte accesses forms R = tau' - tau,
+// stores it and accumulates <R, R> and <R, R_i> per thread in plain fp64 over the thread's <= 64 elements; the
+// per-thread sums are then combined in double-double (warp shuffles) into one partial per CTA, and mdiis_solve adds
+// the partials of all CTAs in double-double in a fixed order.
+template <int NZ, int G>
+__global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
     zinv_residual_kernel(const cplx* __restrict__ work, const double* __restrict__ X, double* __restrict__ R,
                          double* __restrict__ raw_out, double* __restrict__ gram_part, Twiddle tw_shift,
-                         Twiddle tw, const DevState* __restrict__ st, int nv, size_t npts, size_t field, int M,
-                         unsigned ntiles) {
+                         Twiddle tw, const DevState* __restrict__ st, int nv, size_t npts, size_t field, int M) {
   if (raw_out == nullptr && st->done) return;
   using Cfg = FftCfg<NZ>;
-  constexpr int T = Cfg::T, G = Cfg::G, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS, n = 2 * NZ;
-  constexpr int RP = n + 2;                            // real tile pitch (doubles)
+  constexpr int T = Cfg::T, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS, n = 2 * NZ;
+  constexpr int NT = T * G * C;
+  constexpr int HP = NZ / 2;                           // pairs (m, m+1) per half line
   const int tid = threadIdx.x;
   const int LP = C / nv, GL = G * LP;
   cplx* smc = smem_dyn;                                // [G][NZ][ZP] complex
-  double* smr = reinterpret_cast<double*>(smem_dyn + G * NZ * ZP);   // [G][C][RP] real
 
   // MDIIS bookkeeping: the entries the new residual is dotted with
   __shared__ int s_other[MAX_M];
@@ -251,24 +290,14 @@ __global__ void __launch_bounds__(FftCfg<NZ>::T* FftCfg<NZ>::G* COLS)
     s_cur = st->cur;
     for (int i = 0; i < m - skip; ++i) s_other[i] = st->list[i + skip];
   }
-  __syncthreads();
-  const int nother = raw_out ? 0 : s_nother;
-  const double* Xc = raw_out ? nullptr : X + (size_t)s_cur * field;
-  double* Rc = raw_out ? nullptr : R + (size_t)s_cur * field;
-
-  double acc_hi[MAX_M + 1], acc_lo[MAX_M + 1];
-#pragma unroll
-  for (int j = 0; j <= MAX_M; ++j) acc_hi[j] = acc_lo[j] = 0.0;
 
   const int col = tid % C, t = (tid / C) % T, grp = tid / (C * T);
   cplx* sm = smc + grp * (NZ * ZP) + col;
-  double* sr = smr + (grp * C + col) * RP;
   auto ld_sm = [&](int i) { return sm[i * ZP]; };
   auto st_sm = [&](int i, cplx v) { sm[i * ZP] = v; };
   const double scale = 1.0 / (double)NZ;
-
-  for (unsigned tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-    const size_t line0 = (size_t)tile * GL;
+  const size_t line0 = (size_t)blockIdx.x * GL;
+  {
     const size_t line = line0 + (size_t)grp * LP + col / nv;
     const cplx* src = work + line * NZ * nv + (col % nv);
     auto in = [&](int p) { return src[(size_t)p * nv]; };
@@ -281,70 +310,79 @@ __global__ void __launch_bounds__(FftCfg<NZ>::T* FftCfg<NZ>::G* COLS)
       inv_stage_mid<NZ, R1, R2, false>(t, T, tw, ld_sm, st_sm);
       __syncthreads();
     }
-    // u_m exp(+i pi m/n) / NZ = f_m - i f_{m+n/2}
+    // u_m exp(+i pi m/n) / NZ = f_m - i f_{m+n/2}; every thread rewrites exactly the elements it has just read
     auto out = [&](int m, cplx v) {
       const cplx f = cscale(cmulc(v, tw_shift(m)), scale);
-      sr[m] = f.x;
-      sr[m + NZ] = -f.y;
+      sm[m * ZP] = make_double2(f.x, -f.y);
     };
     inv_stage_last<NZ, R1, false>(t, T, tw, ld_sm, out);
-    __syncthreads();
+  }
+  __syncthreads();
 
-    // streaming phase: coalesced over z, sites outermost
-    for (int e = tid; e < GL * nv * n; e += blockDim.x) {
-      const int m = e % n, lc = e / n;
-      const int site = lc / GL, l = lc % GL;
-      const size_t off = (size_t)site * npts + (line0 + l) * n + m;
-      const double tnew = smr[((l / LP) * C + (l % LP) * nv + site) * RP + m];
-      if (raw_out) {
-        raw_out[off] = tnew;
-      } else {
-        const double r = tnew - Xc[off];               // R = tau' - tau  (Eq. 33)
-        Rc[off] = r;
-        dd_add_prod(acc_hi[MAX_M], acc_lo[MAX_M], r, r);
+  const int nother = raw_out ? 0 : s_nother;
+  const double* Xc = raw_out ? nullptr : X + (size_t)s_cur * field;
+  double* Rc = raw_out ? nullptr : R + (size_t)s_cur * field;
+  double acc[MAX_M + 1];
 #pragma unroll
-        for (int j = 0; j < MAX_M; ++j)
-          if (j < nother) dd_add_prod(acc_hi[j], acc_lo[j], r, R[(size_t)s_other[j] * field + off]);
-      }
+  for (int j = 0; j <= MAX_M; ++j) acc[j] = 0.0;
+
+  // streaming phase: thread <-> (site, line, pair of adjacent z points); 16-byte accesses, z fastest
+  for (int e = tid; e < GL * nv * HP; e += NT) {
+    const int mp = e % HP, lc = e / HP;
+    const int site = lc / GL, l = lc % GL;
+    const size_t off = (size_t)site * npts + (line0 + l) * n + 2 * mp;
+    const cplx* tile = smc + (l / LP) * (NZ * ZP) + (l % LP) * nv + site;
+    const cplx a = tile[(2 * mp) * ZP], b = tile[(2 * mp + 1) * ZP];
+    const double2 tlo = make_double2(a.x, b.x), thi = make_double2(a.y, b.y);   // tau' at off.., off+NZ..
+    if (raw_out) {
+      st2(raw_out + off, tlo);
+      st2(raw_out + off + NZ, thi);
+    } else {
+      const double2 xlo = ld2(Xc + off), xhi = ld2(Xc + off + NZ);
+      const double2 rlo = make_double2(tlo.x - xlo.x, tlo.y - xlo.y);          // R = tau' - tau  (Eq. 33)
+      const double2 rhi = make_double2(thi.x - xhi.x, thi.y - xhi.y);
+      st2(Rc + off, rlo);
+      st2(Rc + off + NZ, rhi);
+      acc[MAX_M] = fma(rlo.x, rlo.x, fma(rlo.y, rlo.y, fma(rhi.x, rhi.x, fma(rhi.y, rhi.y, acc[MAX_M]))));
+#pragma unroll
+      for (int j = 0; j < MAX_M - 1; ++j)
+        if (j < nother) {
+          const double* Rj = R + (size_t)s_other[j] * field + off;
+          const double2 qlo = ld2(Rj), qhi = ld2(Rj + NZ);
+          acc[j] = fma(rlo.x, qlo.x, fma(rlo.y, qlo.y, fma(rhi.x, qhi.x, fma(rhi.y, qhi.y, acc[j]))));
+        }
     }
-    __syncthreads();
   }
   if (raw_out) return;
+  __syncthreads();                                     // the tile is dead: reuse it for the block reduction
 
-  // block reduction of the double-double partial sums: warp shuffles, then one warp over the warp results
-  __shared__ double s_red[32][2];
-  const int lane = tid & 31, wid = tid >> 5, nw = blockDim.x >> 5;
+  // block reduction: s_part[j][tid], then warp w sums entries j = w, w + nwarps, ... in double-double
+  double* s_part = reinterpret_cast<double*>(smem_dyn);
+  constexpr int NW = NT / 32;
 #pragma unroll
-  for (int j = 0; j <= MAX_M; ++j) {
-    if (j < nother || j == MAX_M) {
-      double hi = acc_hi[j], lo = acc_lo[j];
-      for (int o = 16; o > 0; o >>= 1) {
-        const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
-        dd_add(hi, lo, h2, l2);
-      }
-      if (lane == 0) { s_red[wid][0] = hi; s_red[wid][1] = lo; }
-      __syncthreads();
-      if (wid == 0) {
-        hi = lane < nw ? s_red[lane][0] : 0.0;
-        lo = lane < nw ? s_red[lane][1] : 0.0;
-        for (int o = 16; o > 0; o >>= 1) {
-          const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
-          dd_add(hi, lo, h2, l2);
-        }
-        if (lane == 0) {
-          dd_norm(hi, lo);
-          gram_part[((size_t)blockIdx.x * (MAX_M + 1) + j) * 2 + 0] = hi;
-          gram_part[((size_t)blockIdx.x * (MAX_M + 1) + j) * 2 + 1] = lo;
-        }
-      }
-      __syncthreads();
+  for (int j = 0; j <= MAX_M; ++j)
+    if (j < nother || j == MAX_M) s_part[(j == MAX_M ? nother : j) * NT + tid] = acc[j];
+  __syncthreads();
+  const int lane = tid & 31, wid = tid >> 5;
+  for (int jj = wid; jj <= nother; jj += NW) {
+    double hi = 0.0, lo = 0.0;
+    for (int i = lane; i < NT; i += 32) dd_add(hi, lo, s_part[jj * NT + i], 0.0);
+    for (int o = 16; o > 0; o >>= 1) {
+      const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
+      dd_add(hi, lo, h2, l2);
+    }
+    if (lane == 0) {
+      dd_norm(hi, lo);
+      const int j = (jj == nother) ? MAX_M : jj;
+      gram_part[((size_t)blockIdx.x * (MAX_M + 1) + j) * 2 + 0] = hi;
+      gram_part[((size_t)blockIdx.x * (MAX_M + 1) + j) * 2 + 1] = lo;
     }
   }
 }
 
 template <int NZ>
 static unsigned zinv_tiles(const Grid& gr) {
-  const int LP = COLS / gr.nv, GL = FftCfg<NZ>::G * LP;
+  const int LP = COLS / gr.nv, GL = ZGroups<NZ>::G * LP;
   return (unsigned)((size_t)gr.n * gr.n / GL);
 }
 
@@ -361,23 +399,28 @@ static unsigned zinv_tiles_rt(const Grid& g) {
   }
 }
 
-int gram_blocks(const Grid& g) {
-  const unsigned tiles = zinv_tiles_rt(g);
-  const unsigned cap = 148 * 4;
-  return (int)(tiles < cap ? tiles : cap);
+// number of per-CTA Gram partials (= CTAs of zinv_residual)
+int gram_blocks(const Grid& g) { return (int)zinv_tiles_rt(g); }
+int gram_blocks_for(int n, int nv) {
+  Grid g{};
+  g.n = n;
+  g.nv = nv;
+  return gram_blocks(g);
 }
 
 template <int NZ>
 static int launch_zinv_n(const Grid& gr, const Buffers& b, const SolverParams& sp, double* raw_out, cudaStream_t s) {
   using Cfg = FftCfg<NZ>;
-  const int threads = Cfg::T * Cfg::G * COLS;
-  const size_t shm = (size_t)Cfg::G * NZ * ZP * sizeof(cplx) + (size_t)Cfg::G * COLS * (2 * NZ + 2) * sizeof(double);
-  auto kern = zinv_residual_kernel<NZ>;
+  constexpr int G = ZGroups<NZ>::G;
+  const int threads = Cfg::T * G * COLS;
+  size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
+  const size_t red = (size_t)(MAX_M + 1) * threads * sizeof(double);
+  if (shm < red) shm = red;
+  auto kern = zinv_residual_kernel<NZ, G>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
-  const unsigned tiles = zinv_tiles<NZ>(gr);
-  kern<<<gram_blocks(gr), threads, shm, s>>>(b.work, b.X, b.R, raw_out, b.gram_part, tws, tw, b.state, gr.nv,
-                                             gr.npts, gr.field, sp.M, tiles);
+  kern<<<zinv_tiles<NZ>(gr), threads, shm, s>>>(b.work, b.X, b.R, raw_out, b.gram_part, tws, tw, b.state, gr.nv,
+                                               gr.npts, gr.field, sp.M);
   return 1;
 }
 

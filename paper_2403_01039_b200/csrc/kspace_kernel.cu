@@ -70,14 +70,24 @@ __global__ void __launch_bounds__(FftCfg<N>::T* FftCfg<N>::G* COLS)
       const cplx csr = x[k];
       const cplx c = make_double2(csr.x - qg * ph.x, csr.y - qg * ph.y);     // Eq. 32
       const double* ch = chi_shell + (size_t)shell * (NV * NV) + site * NV;  // chi_{g' site}, g' = 0..NV-1
+      double chv[NV];                                                         // one 8*NV-byte row, 16-byte loads
+      if constexpr (NV == 1) {
+        chv[0] = __ldg(ch);
+      } else {
+#pragma unroll
+        for (int i = 0; i < NV / 2; ++i) {
+          const double2 v = __ldg(reinterpret_cast<const double2*>(ch) + i);
+          chv[2 * i] = v.x;
+          chv[2 * i + 1] = v.y;
+        }
+      }
       double hx = 0.0, hy = 0.0;
 #pragma unroll
       for (int gp = 0; gp < NV; ++gp) {
         const double cx = __shfl_sync(0xffffffffu, c.x, lane0 + gp);
         const double cy = __shfl_sync(0xffffffffu, c.y, lane0 + gp);
-        const double chv = __ldg(ch + gp);
-        hx += cx * chv;                                                       // Eq. 13
-        hy += cy * chv;
+        hx += cx * chv[gp];                                                   // Eq. 13
+        hy += cy * chv[gp];
       }
       x[k] = make_double2(hx - csr.x, hy - csr.y);                            // tau'(k) = h - c_sr
     }

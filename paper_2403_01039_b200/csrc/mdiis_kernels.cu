@@ -11,11 +11,13 @@
 
 namespace r3d {
 
-__global__ void __launch_bounds__(256)
+constexpr int SOLVE_THREADS = 1024;
+
+__global__ void __launch_bounds__(SOLVE_THREADS)
     mdiis_solve_kernel(DevState* __restrict__ st, const double* __restrict__ gram_part, int nblocks, int M, double b,
                        double restart, double npts_total) {
   if (st->done) return;
-  __shared__ double s_hi[256], s_lo[256];
+  __shared__ double s_hi[SOLVE_THREADS], s_lo[SOLVE_THREADS];
   __shared__ double s_row[MAX_M + 1];
   const int tid = threadIdx.x;
   const int m_old = st->m;
@@ -26,14 +28,14 @@ __global__ void __launch_bounds__(256)
   for (int jj = 0; jj <= nother; ++jj) {
     const int j = (jj == nother) ? MAX_M : jj;
     double hi = 0.0, lo = 0.0;
-    for (int blk = tid; blk < nblocks; blk += 256) {
+    for (int blk = tid; blk < nblocks; blk += SOLVE_THREADS) {
       const double* p = gram_part + ((size_t)blk * (MAX_M + 1) + j) * 2;
       dd_add(hi, lo, p[0], p[1]);
     }
     s_hi[tid] = hi;
     s_lo[tid] = lo;
     __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
+    for (int o = SOLVE_THREADS / 2; o > 0; o >>= 1) {
       if (tid < o) {
         double h = s_hi[tid], l = s_lo[tid];
         dd_add(h, l, s_hi[tid + o], s_lo[tid + o]);
@@ -147,7 +149,7 @@ __global__ void __launch_bounds__(256)
 }
 
 int launch_mdiis_solve(const Grid& g, const Buffers& b, const SolverParams& sp, cudaStream_t s) {
-  mdiis_solve_kernel<<<1, 256, 0, s>>>(b.state, b.gram_part, gram_blocks(g), sp.M, sp.b, sp.restart,
+  mdiis_solve_kernel<<<1, SOLVE_THREADS, 0, s>>>(b.state, b.gram_part, gram_blocks(g), sp.M, sp.b, sp.restart,
                                        (double)g.field);
   return 1;
 }

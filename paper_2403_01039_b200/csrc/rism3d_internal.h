@@ -11,7 +11,7 @@ namespace r3d {
 constexpr int MAX_M = 16;            // MDIIS history slots (rism3d_params.mdiis_nvec <= 16)
 constexpr int MAX_NV = 8;            // solvent site types
 constexpr int RMS_HIST_CAP = 65536;
-constexpr int GRAM_BLOCKS_MAX = 148 * 8;
+constexpr int FE_BLOCKS = 148 * 4;        // CTAs of the free-energy reduction
 
 constexpr double K_BOLTZMANN = 0.001987204259;   // kcal/(mol K)     (Q3)
 constexpr double COULOMB = 332.06371;            // kcal A/(mol e^2) (Q3)
@@ -64,11 +64,11 @@ struct Buffers {
   double2* phik;         // [n][n][n/2]  phi~(k) exp(+i k.r0) / dV
   double* chi_shell;     // [nshell][nv][nv]   chi_shell[s][g][g'] = chi_{g' g}(k_s)
   double2* tw;           // [2n]         exp(-i pi j / n)
-  double* gram_part;     // [GRAM_BLOCKS_MAX][MAX_M+1][2]  double-double partial sums
+  double* gram_part;     // [gram_blocks][MAX_M+1][2]  double-double partial sums, one per zinv_residual CTA
   double* scratch;       // [field] temporary (get_field, setup tables); aliases `work`
   double* qv;            // [nv] solvent charges
   double* rhov;          // [nv]
-  double* fe_part;       // [GRAM_BLOCKS_MAX][MAX_NV][2]
+  double* fe_part;       // [FE_BLOCKS][MAX_NV][2]
 };
 
 struct SolverParams {
@@ -90,6 +90,7 @@ int launch_kspace_x(const Grid&, const Buffers&, cudaStream_t);
 int launch_y_inv(const Grid&, const Buffers&, bool use_state, cudaStream_t);
 int launch_zinv_residual(const Grid&, const Buffers&, const SolverParams&, double* d_raw_out, cudaStream_t);
 int gram_blocks(const Grid&);
+int gram_blocks_for(int n, int nv);
 // mdiis_kernels.cu
 int launch_mdiis_solve(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);
 int launch_mdiis_update(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);

@@ -271,7 +271,7 @@ __global__ void free_energy_final_kernel(double* __restrict__ out, const double*
 }
 
 int launch_free_energy(const Grid& g, const Buffers& b, const SolverParams& sp, double* d_out, cudaStream_t s) {
-  const int blocks = 148 * 4;
+  const int blocks = FE_BLOCKS;
   free_energy_kernel<<<blocks, 256, 0, s>>>(b.fe_part, b.X, b.w, b.phi, b.qv, b.state, g.nv, g.npts, g.field,
                                             sp.closure, sp.pse_order);
   free_energy_final_kernel<<<1, 32, 0, s>>>(d_out, b.fe_part, blocks, b.rhov, g.nv, sp.kT * g.h * g.h * g.h);
