@@ -47,9 +47,9 @@ def kernel_words(n_v: int, m_hist: int) -> dict:
         "y_fwd": 2.0,                           # in place
         "kspace_x": 2.0 + 1.0 / n_v,            # in place + phi~ (one complex per 2 points, shared by the sites)
         "y_inv": 2.0,
-        "zinv_residual": m_hist + 2.0,          # read work, tau, M-1 old residuals; write R
+        "zinv_residual": m_hist + 3.0,          # read work, tau, M-1 old residuals; write R and Z = tau + b R
         "mdiis_solve": 0.0,
-        "mdiis_update": 2.0 * m_hist + 1.0,     # read M inputs + M residuals; write the new input
+        "mdiis_update": m_hist + 1.0,           # read M stored Z_i; write the new input tau
     }
 
 

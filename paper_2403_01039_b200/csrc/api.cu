@@ -77,8 +77,9 @@ static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_o
   auto take = [&](size_t bytes) { char* ptr = base ? base + off : nullptr; off += align256(bytes); return ptr; };
   char* st = take(sizeof(DevState));
   const size_t off_x = off;
-  char* X = take(M * field * 8);
+  char* Z = take(M * field * 8);
   char* R = take(M * field * 8);
+  char* tau = take(field * 8);
   char* w = take(field * 8);
   char* work = take(field * 8);
   const size_t scr = off - off_x;
@@ -87,15 +88,16 @@ static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_o
   char* chis = take((size_t)n_shells((int)n) * nv * nv * 8);
   char* tw = take(2 * n * 16);
   char* gp = take((size_t)gram_blocks_for((int)n, (int)nv) * (MAX_M + 1) * 2 * 8);
+  char* gp2 = take((size_t)SOLVE_BLOCKS * (MAX_M + 1) * 2 * 8);
   char* fp = take((size_t)FE_BLOCKS * MAX_NV * 2 * 8);
   char* qv = take(MAX_NV * 8);
   char* rv = take(MAX_NV * 8);
   char* out = take(64 * 8);
   if (b) {
     b->state = (DevState*)st;
-    b->X = (double*)X; b->R = (double*)R; b->w = (double*)w; b->work = (double2*)work;
+    b->Z = (double*)Z; b->R = (double*)R; b->tau = (double*)tau; b->w = (double*)w; b->work = (double2*)work;
     b->phi = (double*)phi; b->phik = (double2*)phik; b->chi_shell = (double*)chis; b->tw = (double2*)tw;
-    b->gram_part = (double*)gp; b->fe_part = (double*)fp; b->qv = (double*)qv; b->rhov = (double*)rv;
+    b->gram_part = (double*)gp; b->gram_part2 = (double*)gp2; b->fe_part = (double*)fp; b->qv = (double*)qv; b->rhov = (double*)rv;
     b->scratch = (double*)work;
   }
   if (d_out) *d_out = (double*)out;
@@ -203,7 +205,7 @@ extern "C" int rism3d_set_solvent_chi(rism3d_ctx* ctx, const double* q, const do
   const size_t tbytes = (size_t)n_k * g.nv * g.nv * 8;
   if (tbytes > ctx->scratch_bytes) return fail(ctx, RISM3D_ERR_WORKSPACE, "chi table larger than the scratch span");
   for (int i = 0; i < g.nv; ++i) { ctx->qv[i] = q[i]; ctx->sigv[i] = sigma[i]; ctx->epsv[i] = eps[i]; ctx->rhov[i] = rho[i]; }
-  double* d_table = ctx->b.X;                      // scratch: the history is rebuilt by set_solute anyway
+  double* d_table = ctx->b.Z;                      // scratch: the history is rebuilt by set_solute anyway
   CU(cudaMemcpyAsync(d_table, chi, tbytes, cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaMemcpyAsync(ctx->b.qv, ctx->qv, g.nv * 8, cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaMemcpyAsync(ctx->b.rhov, ctx->rhov, g.nv * 8, cudaMemcpyHostToDevice, ctx->stream));
@@ -250,9 +252,9 @@ extern "C" int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz
   if (b_atoms + b_pair + b_phase > ctx->scratch_bytes)
     return fail(ctx, RISM3D_ERR_WORKSPACE, "%d atoms need %zu scratch bytes, workspace has %zu", n_atoms,
                 b_atoms + b_pair + b_phase, ctx->scratch_bytes);
-  char* scr = (char*)ctx->b.X;                      // X, R, w, work are contiguous; w is written last-to-first safe:
-  // place the tables at the END of the span's X/R part so that w (written by the potential kernel) is not touched
-  const size_t xr_bytes = (size_t)((char*)ctx->b.w - (char*)ctx->b.X);
+  char* scr = (char*)ctx->b.Z;                      // Z, R, tau, w, work are contiguous; the tables live in the
+  // history part of the span (rebuilt by the iteration anyway), clear of tau and w, which the setup writes
+  const size_t xr_bytes = (size_t)((char*)ctx->b.tau - (char*)ctx->b.Z);
   if (b_atoms + b_pair + b_phase > xr_bytes)
     return fail(ctx, RISM3D_ERR_WORKSPACE, "%d atoms need %zu scratch bytes, history span has %zu", n_atoms,
                 b_atoms + b_pair + b_phase, xr_bytes);
@@ -272,8 +274,8 @@ extern "C" int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz
   ctx->launches += launch_phi_tilde(g, ctx->b, sp, n_atoms, d_atoms, d_phase, ctx->stream);
   CU(cudaGetLastError());
   CU(cudaEventRecord(e1, ctx->stream));
-  // tau = 0 (t = f) in slot 0; empty history
-  CU(cudaMemsetAsync(ctx->b.X, 0, g.field * 8, ctx->stream));
+  // tau = 0 (t = f); empty history
+  CU(cudaMemsetAsync(ctx->b.tau, 0, g.field * 8, ctx->stream));
   int rc = reset_state(ctx);
   if (rc) return rc;
   CU(cudaStreamSynchronize(ctx->stream));
@@ -437,15 +439,10 @@ extern "C" int rism3d_set_tau(rism3d_ctx* ctx, int site, const double* src, int 
   if (!ctx) return RISM3D_ERR_ARG;
   if (!src || site < 0 || site >= ctx->g.nv) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before set_tau");
-  int rc = read_header(ctx);
-  if (rc) return rc;
-  const int cur = ctx->h_hdr->cur;
   const Grid& g = ctx->g;
-  // move the current tau to slot 0, overwrite the requested site, clear the history
-  if (cur != 0)
-    CU(cudaMemcpyAsync(ctx->b.X, ctx->b.X + (size_t)cur * g.field, g.field * 8, cudaMemcpyDeviceToDevice, ctx->stream));
-  CU(cudaMemcpyAsync(ctx->b.X + (size_t)site * g.npts, src, g.npts * 8,
+  CU(cudaMemcpyAsync(ctx->b.tau + (size_t)site * g.npts, src, g.npts * 8,
                      src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, ctx->stream));
+  int rc;
   rc = reset_state(ctx);
   if (rc) return rc;
   CU(cudaStreamSynchronize(ctx->stream));

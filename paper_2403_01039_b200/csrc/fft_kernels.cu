@@ -159,7 +159,7 @@ __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<do
 // shared-memory tile, then the n/2-point complex line FFTs.
 template <int NZ, int G>
 __global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
-    closure_zfwd_kernel(const double* __restrict__ X, const double* __restrict__ w, const double* __restrict__ raw,
+    closure_zfwd_kernel(const double* __restrict__ tau_cur, const double* __restrict__ w, const double* __restrict__ raw,
                         cplx* __restrict__ work, Twiddle tw_shift, Twiddle tw, const DevState* __restrict__ st,
                         int nv, size_t npts, size_t field, int closure, int order) {
   if (raw == nullptr && st->done) return;
@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
   const int tid = threadIdx.x;
   const int LP = C / nv, GL = G * LP;                 // lines per column group, lines per CTA
   const size_t line0 = (size_t)blockIdx.x * GL;
-  const double* tau = raw ? raw : X + (size_t)st->cur * field;
+  const double* tau = raw ? raw : tau_cur;
   const int total = GL * nv * HP;
 
   for (int e0 = tid; e0 < total; e0 += U * NT) {
@@ -241,7 +241,7 @@ static int launch_closure_zfwd_n(const Grid& gr, const Buffers& b, const SolverP
   auto kern = closure_zfwd_kernel<NZ, G>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
-  kern<<<(unsigned)(nlines / GL), threads, shm, s>>>(b.X, b.w, raw, b.work, tws, tw, b.state, gr.nv, gr.npts,
+  kern<<<(unsigned)(nlines / GL), threads, shm, s>>>(b.tau, b.w, raw, b.work, tws, tw, b.state, gr.nv, gr.npts,
                                                        gr.field, sp.closure, sp.pse_order);
   return 1;
 }
@@ -268,9 +268,10 @@ int launch_closure_zfwd(const Grid& g, const Buffers& b, const SolverParams& sp,
 // the partials of all CTAs in double-double in a fixed order.
 template <int NZ, int G>
 __global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
-    zinv_residual_kernel(const cplx* __restrict__ work, const double* __restrict__ X, double* __restrict__ R,
-                         double* __restrict__ raw_out, double* __restrict__ gram_part, Twiddle tw_shift,
-                         Twiddle tw, const DevState* __restrict__ st, int nv, size_t npts, size_t field, int M) {
+    zinv_residual_kernel(const cplx* __restrict__ work, const double* __restrict__ tau_cur, double* __restrict__ Z,
+                         double* __restrict__ R, double* __restrict__ raw_out, double* __restrict__ gram_part,
+                         Twiddle tw_shift, Twiddle tw, const DevState* __restrict__ st, int nv, size_t npts,
+                         size_t field, int M, double bdamp) {
   if (raw_out == nullptr && st->done) return;
   using Cfg = FftCfg<NZ>;
   constexpr int T = Cfg::T, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS, n = 2 * NZ;
@@ -320,8 +321,9 @@ __global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
   __syncthreads();
 
   const int nother = raw_out ? 0 : s_nother;
-  const double* Xc = raw_out ? nullptr : X + (size_t)s_cur * field;
+  const double* Xc = tau_cur;
   double* Rc = raw_out ? nullptr : R + (size_t)s_cur * field;
+  double* Zc = raw_out ? nullptr : Z + (size_t)s_cur * field;
   double acc[MAX_M + 1];
 #pragma unroll
   for (int j = 0; j <= MAX_M; ++j) acc[j] = 0.0;
@@ -343,6 +345,9 @@ __global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
       const double2 rhi = make_double2(thi.x - xhi.x, thi.y - xhi.y);
       st2(Rc + off, rlo);
       st2(Rc + off + NZ, rhi);
+      // Z = X + b R, the form in which the MDIIS update needs this entry (Eq. 40 / Q7); mul and add rounded separately
+      st2(Zc + off, make_double2(__dadd_rn(xlo.x, __dmul_rn(bdamp, rlo.x)), __dadd_rn(xlo.y, __dmul_rn(bdamp, rlo.y))));
+      st2(Zc + off + NZ, make_double2(__dadd_rn(xhi.x, __dmul_rn(bdamp, rhi.x)), __dadd_rn(xhi.y, __dmul_rn(bdamp, rhi.y))));
       acc[MAX_M] = fma(rlo.x, rlo.x, fma(rlo.y, rlo.y, fma(rhi.x, rhi.x, fma(rhi.y, rhi.y, acc[MAX_M]))));
 #pragma unroll
       for (int j = 0; j < MAX_M - 1; ++j)
@@ -374,8 +379,7 @@ __global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
     if (lane == 0) {
       dd_norm(hi, lo);
       const int j = (jj == nother) ? MAX_M : jj;
-      gram_part[((size_t)blockIdx.x * (MAX_M + 1) + j) * 2 + 0] = hi;
-      gram_part[((size_t)blockIdx.x * (MAX_M + 1) + j) * 2 + 1] = lo;
+      st2(gram_part + ((size_t)j * gridDim.x + blockIdx.x) * 2, make_double2(hi, lo));
     }
   }
 }
@@ -419,8 +423,8 @@ static int launch_zinv_n(const Grid& gr, const Buffers& b, const SolverParams& s
   auto kern = zinv_residual_kernel<NZ, G>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
-  kern<<<zinv_tiles<NZ>(gr), threads, shm, s>>>(b.work, b.X, b.R, raw_out, b.gram_part, tws, tw, b.state, gr.nv,
-                                               gr.npts, gr.field, sp.M);
+  kern<<<zinv_tiles<NZ>(gr), threads, shm, s>>>(b.work, b.tau, b.Z, b.R, raw_out, b.gram_part, tws, tw, b.state, gr.nv,
+                                               gr.npts, gr.field, sp.M, sp.b);
   return 1;
 }
 

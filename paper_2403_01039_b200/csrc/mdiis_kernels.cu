@@ -2,52 +2,86 @@
 // (input, residual) pairs.  R_i = Y_i - X_i; c = argmin |sum c_i R_i|^2 with sum c_i = 1 (Lagrange multiplier);
 // X_new = sum_i c_i (X_i + b R_i).
 //
-//   mdiis_solve_kernel  : one CTA.  Finishes the Gram row (fixed-order double-double reduction of the per-CTA
-//                         partial sums of zinv_residual), rms and convergence test (Eq. 41 as read in Q9), history
-//                         bookkeeping (circular overwrite, restart rule), the bordered (m+1)x(m+1) solve by Gaussian
-//                         elimination with partial pivoting, and the choice of the slot the update writes.
-//   mdiis_update_kernel : streaming linear combination over the stored slots.
+// The history stores Z_i = X_i + b R_i (written by zinv_residual next to R_i) instead of X_i: Eq. 40 needs X_i
+// in no other form, and the update then reads M fields instead of 2M.  The current input lives in its own field.
+//
+//   mdiis_solve_kernel  : finishes the Gram row (fixed-order double-double reduction of the per-CTA partial sums
+//                         of zinv_residual), rms and convergence test (Eq. 41 as read in Q9), history bookkeeping
+//                         (circular overwrite, restart rule), the bordered (m+1)x(m+1) solve by Gaussian
+//                         elimination with partial pivoting, and the choice of the slot the next pair goes to.
+//   mdiis_update_kernel : streaming linear combination tau = sum_i c_i Z_i over the stored slots.
 #include "rism3d_internal.h"
 
 namespace r3d {
 
-constexpr int SOLVE_THREADS = 1024;
+constexpr int SOLVE_THREADS = 256;
 
+// Grid = SOLVE_BLOCKS CTAs.  Every CTA adds its contiguous share of the per-CTA partials of zinv_residual
+// (double-double, fixed order), the CTA that finishes last (ticket counter) adds the SOLVE_BLOCKS second-level
+// partials, again in a fixed order, and runs the bookkeeping and the small solve on one thread.
 __global__ void __launch_bounds__(SOLVE_THREADS)
-    mdiis_solve_kernel(DevState* __restrict__ st, const double* __restrict__ gram_part, int nblocks, int M, double b,
-                       double restart, double npts_total) {
+    mdiis_solve_kernel(DevState* __restrict__ st, const double* __restrict__ gram_part, double* __restrict__ part2,
+                       int nblocks, int M, double b, double restart, double npts_total) {
   if (st->done) return;
-  __shared__ double s_hi[SOLVE_THREADS], s_lo[SOLVE_THREADS];
+  __shared__ double s_hi[SOLVE_THREADS / 32], s_lo[SOLVE_THREADS / 32];
   __shared__ double s_row[MAX_M + 1];
-  const int tid = threadIdx.x;
+  __shared__ bool s_last;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int m_old = st->m;
   const int skip = (m_old == M) ? 1 : 0;
   const int nother = m_old - skip;
+  const int per = (nblocks + SOLVE_BLOCKS - 1) / SOLVE_BLOCKS;
+  const int b0 = blockIdx.x * per, b1 = min(nblocks, b0 + per);
 
   // Gram row: entry j < nother is <R_new, R_other[j]>, entry MAX_M is <R_new, R_new>
   for (int jj = 0; jj <= nother; ++jj) {
     const int j = (jj == nother) ? MAX_M : jj;
     double hi = 0.0, lo = 0.0;
-    for (int blk = tid; blk < nblocks; blk += SOLVE_THREADS) {
-      const double* p = gram_part + ((size_t)blk * (MAX_M + 1) + j) * 2;
-      dd_add(hi, lo, p[0], p[1]);
+    for (int blk = b0 + tid; blk < b1; blk += SOLVE_THREADS) {
+      const double2 p = *reinterpret_cast<const double2*>(gram_part + ((size_t)j * nblocks + blk) * 2);
+      dd_add(hi, lo, p.x, p.y);
     }
-    s_hi[tid] = hi;
-    s_lo[tid] = lo;
-    __syncthreads();
-    for (int o = SOLVE_THREADS / 2; o > 0; o >>= 1) {
-      if (tid < o) {
-        double h = s_hi[tid], l = s_lo[tid];
-        dd_add(h, l, s_hi[tid + o], s_lo[tid + o]);
-        s_hi[tid] = h;
-        s_lo[tid] = l;
-      }
-      __syncthreads();
+    for (int o = 16; o > 0; o >>= 1) {
+      const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
+      dd_add(hi, lo, h2, l2);
     }
-    if (tid == 0) s_row[jj] = s_hi[0] + s_lo[0];
     __syncthreads();
+    if (lane == 0) { s_hi[wid] = hi; s_lo[wid] = lo; }
+    __syncthreads();
+    if (tid == 0) {
+      hi = 0.0; lo = 0.0;
+      for (int k = 0; k < SOLVE_THREADS / 32; ++k) dd_add(hi, lo, s_hi[k], s_lo[k]);
+      dd_norm(hi, lo);
+      part2[((size_t)j * SOLVE_BLOCKS + blockIdx.x) * 2 + 0] = hi;
+      part2[((size_t)j * SOLVE_BLOCKS + blockIdx.x) * 2 + 1] = lo;
+    }
   }
+  if (tid == 0) {
+    __threadfence();
+    const unsigned t = atomicAdd(&st->ticket, 1u);
+    s_last = (t == (unsigned)(gridDim.x - 1));
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (tid < 32) {
+    for (int jj = 0; jj <= nother; ++jj) {
+      const int j = (jj == nother) ? MAX_M : jj;
+      double hi = 0.0, lo = 0.0;
+      for (int k = lane; k < (int)gridDim.x; k += 32) {
+        const volatile double* p = part2 + ((size_t)j * SOLVE_BLOCKS + k) * 2;
+        dd_add(hi, lo, p[0], p[1]);
+      }
+      for (int o = 16; o > 0; o >>= 1) {
+        const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
+        dd_add(hi, lo, h2, l2);
+      }
+      if (lane == 0) s_row[jj] = hi + lo;
+    }
+  }
+  __syncthreads();
   if (tid != 0) return;
+  st->ticket = 0;
 
   const double self = s_row[nother];
   const double rms = sqrt(self / npts_total);          // Eq. 41 (Q9)
@@ -132,54 +166,54 @@ __global__ void __launch_bounds__(SOLVE_THREADS)
     }
   }
 
-  // where the update writes: a full history overwrites its oldest input in place (it is dropped next iteration)
-  int dst;
+  // slot of the NEXT (Z, R) pair: a full history reuses the slot of its oldest entry (dropped next iteration,
+  // and not read by the Gram row of that iteration), otherwise the first unused slot
+  int nxt;
   if (m == M) {
-    dst = st->list[0];
+    nxt = st->list[0];
   } else {
     unsigned used = 0;
     for (int i = 0; i < m; ++i) used |= 1u << st->list[i];
-    dst = 0;
-    while (used & (1u << dst)) ++dst;
+    nxt = 0;
+    while (used & (1u << nxt)) ++nxt;
   }
   st->upd_m = m;
   for (int i = 0; i < m; ++i) { st->upd_list[i] = st->list[i]; st->upd_coef[i] = c[i]; }
-  st->upd_dst = dst;
-  st->cur = dst;
+  st->cur = nxt;
 }
 
 int launch_mdiis_solve(const Grid& g, const Buffers& b, const SolverParams& sp, cudaStream_t s) {
-  mdiis_solve_kernel<<<1, SOLVE_THREADS, 0, s>>>(b.state, b.gram_part, gram_blocks(g), sp.M, sp.b, sp.restart,
-                                       (double)g.field);
+  mdiis_solve_kernel<<<SOLVE_BLOCKS, SOLVE_THREADS, 0, s>>>(b.state, b.gram_part, b.gram_part2, gram_blocks(g), sp.M,
+                                                           sp.b, sp.restart, (double)g.field);
   return 1;
 }
 
-// X[dst] = sum_i c_i (X[i] + b R[i]) over the stored entries.  dst may alias the oldest X (elementwise in place).
+// tau = sum_i c_i Z_i over the stored entries, Z_i = X_i + b R_i (Eq. 40 as read in Q7); products and sums are
+// rounded one by one, in the order of the oracle's loop.
 __global__ void __launch_bounds__(256)
-    mdiis_update_kernel(const DevState* __restrict__ st, double* X, const double* __restrict__ R, size_t field,
-                        double b) {
+    mdiis_update_kernel(const DevState* __restrict__ st, const double* __restrict__ Z, double* __restrict__ tau,
+                        size_t field) {
   if (st->done) return;
   __shared__ int s_list[MAX_M];
   __shared__ double s_c[MAX_M];
-  __shared__ int s_m, s_dst;
+  __shared__ int s_m;
   if (threadIdx.x == 0) {
     s_m = st->upd_m;
-    s_dst = st->upd_dst;
     for (int i = 0; i < st->upd_m; ++i) { s_list[i] = st->upd_list[i]; s_c[i] = st->upd_coef[i]; }
   }
   __syncthreads();
   const int m = s_m;
   if (m == 0) return;
-  double2* dst = reinterpret_cast<double2*>(X + (size_t)s_dst * field);
+  double2* dst = reinterpret_cast<double2*>(tau);
   const size_t n2 = field / 2;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += (size_t)gridDim.x * blockDim.x) {
     double2 acc = make_double2(0.0, 0.0);
+#pragma unroll 4
     for (int k = 0; k < m; ++k) {
-      const double2 xv = reinterpret_cast<const double2*>(X + (size_t)s_list[k] * field)[i];
-      const double2 rv = reinterpret_cast<const double2*>(R + (size_t)s_list[k] * field)[i];
+      const double2 zv = __ldcs(reinterpret_cast<const double2*>(Z + (size_t)s_list[k] * field) + i);
       const double ck = s_c[k];
-      acc.x = acc.x + ck * (xv.x + b * rv.x);
-      acc.y = acc.y + ck * (xv.y + b * rv.y);
+      acc.x = __dadd_rn(acc.x, __dmul_rn(ck, zv.x));
+      acc.y = __dadd_rn(acc.y, __dmul_rn(ck, zv.y));
     }
     dst[i] = acc;
   }
@@ -190,7 +224,7 @@ int launch_mdiis_update(const Grid& g, const Buffers& b, const SolverParams& sp,
   size_t blocks = (n2 + 255) / 256;
   const size_t cap = 148 * 8 * 4;
   if (blocks > cap) blocks = cap;
-  mdiis_update_kernel<<<(unsigned)blocks, 256, 0, s>>>(b.state, b.X, b.R, g.field, sp.b);
+  mdiis_update_kernel<<<(unsigned)blocks, 256, 0, s>>>(b.state, b.Z, b.tau, g.field);
   return 1;
 }
 

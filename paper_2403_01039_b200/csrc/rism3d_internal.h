@@ -12,6 +12,7 @@ constexpr int MAX_M = 16;            // MDIIS history slots (rism3d_params.mdiis
 constexpr int MAX_NV = 8;            // solvent site types
 constexpr int RMS_HIST_CAP = 65536;
 constexpr int FE_BLOCKS = 148 * 4;        // CTAs of the free-energy reduction
+constexpr int SOLVE_BLOCKS = 64;          // CTAs of mdiis_solve (second level of the Gram reduction)
 
 constexpr double K_BOLTZMANN = 0.001987204259;   // kcal/(mol K)     (Q3)
 constexpr double COULOMB = 332.06371;            // kcal A/(mol e^2) (Q3)
@@ -25,9 +26,9 @@ struct DevState {
   int n_done;                  // iterations completed by the current rism3d_iterate call
   int hist_n;                  // total iterations since set_solute
   int m;                       // filled history entries
-  int cur;                     // physical slot that holds the current input tau (not yet in `list`)
+  int cur;                     // physical history slot that receives the (Z, R) pair of the running iteration
   int upd_m;                   // entries to combine in the update kernel (0: skip)
-  int upd_dst;                 // physical slot the update writes (== new cur)
+  unsigned ticket;             // CTAs of mdiis_solve that have finished their share of the Gram reduction
   double tol;
   double rms_last;
   double pad_[2];
@@ -40,7 +41,7 @@ struct DevState {
   double rms_hist[RMS_HIST_CAP];
 };
 struct StateHeader {           // mirrors the first 64 bytes of DevState
-  int done, status, n_done, hist_n, m, cur, upd_m, upd_dst;
+  int done, status, n_done, hist_n, m, cur, upd_m; unsigned ticket;
   double tol, rms_last, pad_[2];
 };
 
@@ -56,15 +57,17 @@ struct Grid {
 // Device pointers carved from the caller's workspace.
 struct Buffers {
   DevState* state;
-  double* X;             // [M][field]   MDIIS inputs  (tau)
-  double* R;             // [M][field]   MDIIS residuals
+  double* Z;             // [M][field]   MDIIS history: Z_i = X_i + b R_i (the only form Eq. 40 needs X_i in)
+  double* R;             // [M][field]   MDIIS residuals R_i = Y_i - X_i
+  double* tau;           // [field]      current input X (tau = t - f)
   double* w;             // [field]      -beta u + f
   double2* work;         // [n][n][n/2][nv] complex   k-space work array
   double* phi;           // [npts]       phi(r)
   double2* phik;         // [n][n][n/2]  phi~(k) exp(+i k.r0) / dV
   double* chi_shell;     // [nshell][nv][nv]   chi_shell[s][g][g'] = chi_{g' g}(k_s)
   double2* tw;           // [2n]         exp(-i pi j / n)
-  double* gram_part;     // [gram_blocks][MAX_M+1][2]  double-double partial sums, one per zinv_residual CTA
+  double* gram_part;     // [MAX_M+1][gram_blocks][2]  double-double partial sums, one per zinv_residual CTA
+  double* gram_part2;    // [MAX_M+1][SOLVE_BLOCKS][2] second-level partials (mdiis_solve)
   double* scratch;       // [field] temporary (get_field, setup tables); aliases `work`
   double* qv;            // [nv] solvent charges
   double* rhov;          // [nv]

@@ -221,10 +221,9 @@ int launch_chi_shell(const Grid& g, const Buffers& b, const double* d_table, int
 //   B = h^2/2 Theta(h) (KH), Theta(d) d^(n+1)/(n+1)! (PSE-n), 0 (HNC)
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-    free_energy_kernel(double* __restrict__ part, const double* __restrict__ X, const double* __restrict__ w,
+    free_energy_kernel(double* __restrict__ part, const double* __restrict__ tau, const double* __restrict__ w,
                        const double* __restrict__ phi, const double* __restrict__ qv,
                        const DevState* __restrict__ st, int nv, size_t npts, size_t field, int closure, int order) {
-  const double* tau = X + (size_t)st->cur * field;
   __shared__ double s_red[8][2];
   double inv_fact = 1.0;
   for (int i = 2; i <= order + 1; ++i) inv_fact /= (double)i;
@@ -272,18 +271,18 @@ __global__ void free_energy_final_kernel(double* __restrict__ out, const double*
 
 int launch_free_energy(const Grid& g, const Buffers& b, const SolverParams& sp, double* d_out, cudaStream_t s) {
   const int blocks = FE_BLOCKS;
-  free_energy_kernel<<<blocks, 256, 0, s>>>(b.fe_part, b.X, b.w, b.phi, b.qv, b.state, g.nv, g.npts, g.field,
+  free_energy_kernel<<<blocks, 256, 0, s>>>(b.fe_part, b.tau, b.w, b.phi, b.qv, b.state, g.nv, g.npts, g.field,
                                             sp.closure, sp.pse_order);
   free_energy_final_kernel<<<1, 32, 0, s>>>(d_out, b.fe_part, blocks, b.rhov, g.nv, sp.kT * g.h * g.h * g.h);
   return 2;
 }
 
 // ------------------------------------------------------------------------------------------------
-__global__ void get_field_kernel(double* __restrict__ dst, const double* __restrict__ X, const double* __restrict__ w,
+__global__ void get_field_kernel(double* __restrict__ dst, const double* __restrict__ tau_all, const double* __restrict__ w,
                                  const double* __restrict__ phi, const double* __restrict__ qv,
                                  const DevState* __restrict__ st, int which, int site, size_t npts, size_t field,
                                  int closure, int order) {
-  const double* tau = X + (size_t)st->cur * field + (size_t)site * npts;
+  const double* tau = tau_all + (size_t)site * npts;
   const double* ws = w + (size_t)site * npts;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < npts; i += (size_t)gridDim.x * blockDim.x) {
     double v;
@@ -304,7 +303,7 @@ int launch_get_field(const Grid& g, const Buffers& b, const SolverParams& sp, in
                      cudaStream_t s) {
   size_t blocks = (g.npts + 255) / 256;
   if (blocks > 148 * 16) blocks = 148 * 16;
-  get_field_kernel<<<(unsigned)blocks, 256, 0, s>>>(d_dst, b.X, b.w, b.phi, b.qv, b.state, which, site, g.npts,
+  get_field_kernel<<<(unsigned)blocks, 256, 0, s>>>(d_dst, b.tau, b.w, b.phi, b.qv, b.state, which, site, g.npts,
                                                     g.field, sp.closure, sp.pse_order);
   return 1;
 }
