@@ -336,7 +336,9 @@ static int enqueue_iteration(rism3d_ctx* ctx) {
   prof_mark(ctx);
   k += launch_y_inv(g, b, true, s);                        // step 5
   prof_mark(ctx);
-  k += launch_zinv_residual(g, b, ctx->sp, nullptr, s);    // step 5 (z), Eq. 33, Gram row
+  k += launch_zinv_residual(g, b, ctx->sp, nullptr, s);    // step 5 (z), Eq. 33
+  prof_mark(ctx);
+  k += launch_gram_row(g, b, ctx->sp, s);                  // step 6: Gram row of the new residual
   prof_mark(ctx);
   k += launch_mdiis_solve(g, b, ctx->sp, s);               // step 6-7
   prof_mark(ctx);
@@ -368,7 +370,7 @@ extern "C" int rism3d_get_timings(rism3d_ctx* ctx, double* ms_total, int cap, lo
 
 extern "C" const char* rism3d_loop_kernel_name(int k) {
   static const char* names[RISM3D_N_LOOP_KERNELS] = {"closure_zfwd", "y_fwd", "kspace_x", "y_inv", "zinv_residual",
-                                                     "mdiis_solve", "mdiis_update"};
+                                                     "gram_row", "mdiis_solve", "mdiis_update"};
   return (k >= 0 && k < RISM3D_N_LOOP_KERNELS) ? names[k] : "";
 }
 

@@ -147,9 +147,22 @@ constexpr int ZP = COLS + 1;
 // Column groups per CTA of the z kernels (more than the strided passes use: these kernels stream whole fields and
 // want >= 256 threads with many independent loads in flight).
 template <int NZ> struct ZGroups { enum { G = FftCfg<NZ>::G }; };
-template <> struct ZGroups<64>  { enum { G = 4 }; };    // 8 * 4 * 8 = 256 threads
-template <> struct ZGroups<128> { enum { G = 4 }; };    // 8 * 4 * 8 = 256 threads, 72 KB tile
-template <> struct ZGroups<256> { enum { G = 2 }; };    // 16 * 2 * 8 = 256 threads, 72 KB tile
+#ifndef R3D_ZG64
+#define R3D_ZG64 4
+#endif
+#ifndef R3D_ZG128
+#define R3D_ZG128 4
+#endif
+#ifndef R3D_ZG256
+#define R3D_ZG256 2
+#endif
+template <> struct ZGroups<64>  { enum { G = R3D_ZG64 }; };     // 8 * 4 * 8 = 256 threads
+template <> struct ZGroups<128> { enum { G = R3D_ZG128 }; };    // 8 * 4 * 8 = 256 threads, 72 KB tile
+template <> struct ZGroups<256> { enum { G = R3D_ZG256 }; };    // 16 * 2 * 8 = 256 threads, 72 KB tile
+// resident CTAs per SM the z kernels are compiled for: 512 threads per SM for the large lines
+template <int NZ, int G> struct ZMinBlocks {
+  enum { NT = FftCfg<NZ>::T * G * COLS, V = (NZ < 64) ? 1 : (NT >= 256 ? 2 : (NT >= 128 ? 4 : 8)) };
+};
 
 __device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
 __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
@@ -158,7 +171,7 @@ __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<do
 // per thread, two such quads in flight), closure, packing u_m = (c_m - i c_{m+n/2}) exp(-i pi m / n) into the
 // shared-memory tile, then the n/2-point complex line FFTs.
 template <int NZ, int G>
-__global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
+__global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, ZMinBlocks<NZ, G>::V)
     closure_zfwd_kernel(const double* __restrict__ tau_cur, const double* __restrict__ w, const double* __restrict__ raw,
                         cplx* __restrict__ work, Twiddle tw_shift, Twiddle tw, const DevState* __restrict__ st,
                         int nv, size_t npts, size_t field, int closure, int order) {
@@ -261,17 +274,15 @@ int launch_closure_zfwd(const Grid& g, const Buffers& b, const SolverParams& sp,
   return k;
 }
 
-// inverse z + residual + Gram row.  One tile per CTA: inverse line FFTs in shared memory, the last stage leaves
-// (f_m, f_{m+n/2}) in place of complex element m, then a streaming phase with 16-byte accesses forms R = tau' - tau,
-// stores it and accumulates <R, R> and <R, R_i> per thread in plain fp64 over the thread's <= 64 elements; the
-// per-thread sums are then combined in double-double (warp shuffles) into one partial per CTA, and mdiis_solve adds
-// the partials of all CTAs in double-double in a fixed order.
+// inverse z + residual.  One tile per CTA: inverse line FFTs in shared memory, the last stage leaves
+// (f_m, f_{m+n/2}) in place of complex element m, then a streaming phase with 16-byte accesses forms R = tau' - tau
+// (Eq. 33) and Z = tau + b R (the form Eq. 40 needs this entry in) and stores both into history slot `cur`.
+// The Gram row <R, R_i> is a separate streaming kernel (mdiis_kernels.cu: gram_row_kernel).
 template <int NZ, int G>
-__global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
+__global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, ZMinBlocks<NZ, G>::V)
     zinv_residual_kernel(const cplx* __restrict__ work, const double* __restrict__ tau_cur, double* __restrict__ Z,
-                         double* __restrict__ R, double* __restrict__ raw_out, double* __restrict__ gram_part,
-                         Twiddle tw_shift, Twiddle tw, const DevState* __restrict__ st, int nv, size_t npts,
-                         size_t field, int M, double bdamp) {
+                         double* __restrict__ R, double* __restrict__ raw_out, Twiddle tw_shift, Twiddle tw,
+                         const DevState* __restrict__ st, int nv, size_t npts, size_t field, double bdamp) {
   if (raw_out == nullptr && st->done) return;
   using Cfg = FftCfg<NZ>;
   constexpr int T = Cfg::T, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS, n = 2 * NZ;
@@ -280,17 +291,7 @@ __global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
   const int tid = threadIdx.x;
   const int LP = C / nv, GL = G * LP;
   cplx* smc = smem_dyn;                                // [G][NZ][ZP] complex
-
-  // MDIIS bookkeeping: the entries the new residual is dotted with
-  __shared__ int s_other[MAX_M];
-  __shared__ int s_nother, s_cur;
-  if (raw_out == nullptr && tid == 0) {
-    const int m = st->m;
-    const int skip = (m == M) ? 1 : 0;                 // a full history drops its oldest entry this iteration
-    s_nother = m - skip;
-    s_cur = st->cur;
-    for (int i = 0; i < m - skip; ++i) s_other[i] = st->list[i + skip];
-  }
+  const int cur = raw_out ? 0 : st->cur;
 
   const int col = tid % C, t = (tid / C) % T, grp = tid / (C * T);
   cplx* sm = smc + grp * (NZ * ZP) + col;
@@ -320,13 +321,9 @@ __global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
   }
   __syncthreads();
 
-  const int nother = raw_out ? 0 : s_nother;
   const double* Xc = tau_cur;
-  double* Rc = raw_out ? nullptr : R + (size_t)s_cur * field;
-  double* Zc = raw_out ? nullptr : Z + (size_t)s_cur * field;
-  double acc[MAX_M + 1];
-#pragma unroll
-  for (int j = 0; j <= MAX_M; ++j) acc[j] = 0.0;
+  double* Rc = raw_out ? nullptr : R + (size_t)cur * field;
+  double* Zc = raw_out ? nullptr : Z + (size_t)cur * field;
 
   // streaming phase: thread <-> (site, line, pair of adjacent z points); 16-byte accesses, z fastest
   for (int e = tid; e < GL * nv * HP; e += NT) {
@@ -345,86 +342,25 @@ __global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, (NZ >= 64 ? 2 : 1))
       const double2 rhi = make_double2(thi.x - xhi.x, thi.y - xhi.y);
       st2(Rc + off, rlo);
       st2(Rc + off + NZ, rhi);
-      // Z = X + b R, the form in which the MDIIS update needs this entry (Eq. 40 / Q7); mul and add rounded separately
+      // Z = X + b R (Eq. 40 / Q7); mul and add rounded separately, as the oracle's X[i] + b*R[i]
       st2(Zc + off, make_double2(__dadd_rn(xlo.x, __dmul_rn(bdamp, rlo.x)), __dadd_rn(xlo.y, __dmul_rn(bdamp, rlo.y))));
       st2(Zc + off + NZ, make_double2(__dadd_rn(xhi.x, __dmul_rn(bdamp, rhi.x)), __dadd_rn(xhi.y, __dmul_rn(bdamp, rhi.y))));
-      acc[MAX_M] = fma(rlo.x, rlo.x, fma(rlo.y, rlo.y, fma(rhi.x, rhi.x, fma(rhi.y, rhi.y, acc[MAX_M]))));
-#pragma unroll
-      for (int j = 0; j < MAX_M - 1; ++j)
-        if (j < nother) {
-          const double* Rj = R + (size_t)s_other[j] * field + off;
-          const double2 qlo = ld2(Rj), qhi = ld2(Rj + NZ);
-          acc[j] = fma(rlo.x, qlo.x, fma(rlo.y, qlo.y, fma(rhi.x, qhi.x, fma(rhi.y, qhi.y, acc[j]))));
-        }
     }
   }
-  if (raw_out) return;
-  __syncthreads();                                     // the tile is dead: reuse it for the block reduction
-
-  // block reduction: s_part[j][tid], then warp w sums entries j = w, w + nwarps, ... in double-double
-  double* s_part = reinterpret_cast<double*>(smem_dyn);
-  constexpr int NW = NT / 32;
-#pragma unroll
-  for (int j = 0; j <= MAX_M; ++j)
-    if (j < nother || j == MAX_M) s_part[(j == MAX_M ? nother : j) * NT + tid] = acc[j];
-  __syncthreads();
-  const int lane = tid & 31, wid = tid >> 5;
-  for (int jj = wid; jj <= nother; jj += NW) {
-    double hi = 0.0, lo = 0.0;
-    for (int i = lane; i < NT; i += 32) dd_add(hi, lo, s_part[jj * NT + i], 0.0);
-    for (int o = 16; o > 0; o >>= 1) {
-      const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
-      dd_add(hi, lo, h2, l2);
-    }
-    if (lane == 0) {
-      dd_norm(hi, lo);
-      const int j = (jj == nother) ? MAX_M : jj;
-      st2(gram_part + ((size_t)j * gridDim.x + blockIdx.x) * 2, make_double2(hi, lo));
-    }
-  }
-}
-
-template <int NZ>
-static unsigned zinv_tiles(const Grid& gr) {
-  const int LP = COLS / gr.nv, GL = ZGroups<NZ>::G * LP;
-  return (unsigned)((size_t)gr.n * gr.n / GL);
-}
-
-static unsigned zinv_tiles_rt(const Grid& g) {
-  switch (g.n / 2) {
-    case 4: return zinv_tiles<4>(g);
-    case 8: return zinv_tiles<8>(g);
-    case 16: return zinv_tiles<16>(g);
-    case 32: return zinv_tiles<32>(g);
-    case 64: return zinv_tiles<64>(g);
-    case 128: return zinv_tiles<128>(g);
-    case 256: return zinv_tiles<256>(g);
-    default: return 0;
-  }
-}
-
-// number of per-CTA Gram partials (= CTAs of zinv_residual)
-int gram_blocks(const Grid& g) { return (int)zinv_tiles_rt(g); }
-int gram_blocks_for(int n, int nv) {
-  Grid g{};
-  g.n = n;
-  g.nv = nv;
-  return gram_blocks(g);
 }
 
 template <int NZ>
 static int launch_zinv_n(const Grid& gr, const Buffers& b, const SolverParams& sp, double* raw_out, cudaStream_t s) {
   using Cfg = FftCfg<NZ>;
   constexpr int G = ZGroups<NZ>::G;
+  const int LP = COLS / gr.nv, GL = G * LP;
   const int threads = Cfg::T * G * COLS;
-  size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
-  const size_t red = (size_t)(MAX_M + 1) * threads * sizeof(double);
-  if (shm < red) shm = red;
+  const size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
   auto kern = zinv_residual_kernel<NZ, G>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
-  kern<<<zinv_tiles<NZ>(gr), threads, shm, s>>>(b.work, b.tau, b.Z, b.R, raw_out, b.gram_part, tws, tw, b.state, gr.nv,
-                                               gr.npts, gr.field, sp.M, sp.b);
+  kern<<<(unsigned)((size_t)gr.n * gr.n / GL), threads, shm, s>>>(b.work, b.tau, b.Z, b.R, raw_out, tws, tw, b.state,
+                                                                   gr.nv, gr.npts, gr.field, sp.b);
   return 1;
 }
 

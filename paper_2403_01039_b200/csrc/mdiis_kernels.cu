@@ -5,8 +5,10 @@
 // The history stores Z_i = X_i + b R_i (written by zinv_residual next to R_i) instead of X_i: Eq. 40 needs X_i
 // in no other form, and the update then reads M fields instead of 2M.  The current input lives in its own field.
 //
+//   gram_row_kernel     : streaming pass over the new residual and the stored ones: per-CTA double-double partial
+//                         sums of <R_new, R_new> and <R_new, R_i>.
 //   mdiis_solve_kernel  : finishes the Gram row (fixed-order double-double reduction of the per-CTA partial sums
-//                         of zinv_residual), rms and convergence test (Eq. 41 as read in Q9), history bookkeeping
+//                         of gram_row_kernel), rms and convergence test (Eq. 41 as read in Q9), history bookkeeping
 //                         (circular overwrite, restart rule), the bordered (m+1)x(m+1) solve by Gaussian
 //                         elimination with partial pivoting, and the choice of the slot the next pair goes to.
 //   mdiis_update_kernel : streaming linear combination tau = sum_i c_i Z_i over the stored slots.
@@ -15,6 +17,107 @@
 namespace r3d {
 
 constexpr int SOLVE_THREADS = 256;
+
+// Gram row.  One CTA = GRAM_THREADS * GRAM_EPT consecutive double2 of every field; each thread accumulates its
+// 2 * GRAM_EPT elements per entry in plain fp64 FMAs, the per-thread sums are then combined in double-double (warp
+// shuffles, fixed order) into one partial per CTA and entry; mdiis_solve adds the partials of all CTAs in
+// double-double, again in a fixed order.  Entry j < nother: <R_new, R_other[j]>;
+// entry MAX_M: <R_new, R_new>.  MAXO = M - 1 bounds nother at compile time.
+constexpr int GRAM_THREADS = 256;
+constexpr int GRAM_EPT = 16;
+
+template <int MAXO>
+__global__ void __launch_bounds__(GRAM_THREADS)
+    gram_row_kernel(const DevState* __restrict__ st, const double* __restrict__ R, double* __restrict__ gram_part,
+                    size_t field, int M) {
+  if (st->done) return;
+  __shared__ int s_other[MAX_M];
+  __shared__ int s_nother, s_cur;
+  __shared__ double s_part[(MAX_M + 1) * (GRAM_THREADS / 32) * 2];
+  const int tid = threadIdx.x;
+  if (tid == 0) {
+    const int m = st->m;
+    const int skip = (m == M) ? 1 : 0;                 // a full history drops its oldest entry this iteration
+    s_nother = m - skip;
+    s_cur = st->cur;
+    for (int i = 0; i < m - skip; ++i) s_other[i] = st->list[i + skip];
+  }
+  __syncthreads();
+  const int nother = s_nother;
+  const size_t n2 = field / 2;
+  const double2* Rn = reinterpret_cast<const double2*>(R + (size_t)s_cur * field);
+  const double2* Ro[MAXO > 0 ? MAXO : 1];
+#pragma unroll
+  for (int j = 0; j < MAXO; ++j)
+    Ro[j] = reinterpret_cast<const double2*>(R + (size_t)s_other[j < nother ? j : 0] * field);
+  double acc[MAXO + 1];
+#pragma unroll
+  for (int j = 0; j <= MAXO; ++j) acc[j] = 0.0;
+  const size_t base = (size_t)blockIdx.x * (GRAM_THREADS * GRAM_EPT) + tid;
+#pragma unroll 2
+  for (int it = 0; it < GRAM_EPT; ++it) {
+    const size_t i = base + (size_t)it * GRAM_THREADS;
+    if (i < n2) {
+      const double2 r = __ldcs(Rn + i);
+      acc[MAXO] = fma(r.x, r.x, fma(r.y, r.y, acc[MAXO]));
+#pragma unroll
+      for (int j = 0; j < MAXO; ++j)
+        if (j < nother) {
+          const double2 q = __ldcs(Ro[j] + i);
+          acc[j] = fma(r.x, q.x, fma(r.y, q.y, acc[j]));
+        }
+    }
+  }
+  // warp level: double-double butterfly-free tree in a fixed order, then one thread per entry adds the warps
+  const int lane = tid & 31, wid = tid >> 5;
+#pragma unroll
+  for (int j = 0; j <= MAXO; ++j) {
+    if (j < nother || j == MAXO) {
+      double hi = acc[j], lo = 0.0;
+      for (int o = 16; o > 0; o >>= 1) {
+        const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
+        dd_add(hi, lo, h2, l2);
+      }
+      if (lane == 0) {
+        s_part[(j * (GRAM_THREADS / 32) + wid) * 2] = hi;
+        s_part[(j * (GRAM_THREADS / 32) + wid) * 2 + 1] = lo;
+      }
+    }
+  }
+  __syncthreads();
+  if (tid <= MAXO && (tid < nother || tid == MAXO)) {
+    double hi = 0.0, lo = 0.0;
+    for (int w = 0; w < GRAM_THREADS / 32; ++w)
+      dd_add(hi, lo, s_part[(tid * (GRAM_THREADS / 32) + w) * 2], s_part[(tid * (GRAM_THREADS / 32) + w) * 2 + 1]);
+    dd_norm(hi, lo);
+    const int j = (tid == MAXO) ? MAX_M : tid;
+    *reinterpret_cast<double2*>(gram_part + ((size_t)j * gridDim.x + blockIdx.x) * 2) = make_double2(hi, lo);
+  }
+}
+
+int gram_blocks(const Grid& g) {
+  const size_t per = (size_t)GRAM_THREADS * GRAM_EPT;
+  return (int)((g.field / 2 + per - 1) / per);
+}
+int gram_blocks_for(int n, int nv) {
+  Grid g{};
+  g.n = n;
+  g.nv = nv;
+  g.field = (size_t)n * n * n * nv;
+  return gram_blocks(g);
+}
+
+int launch_gram_row(const Grid& g, const Buffers& b, const SolverParams& sp, cudaStream_t s) {
+  const unsigned blocks = (unsigned)gram_blocks(g);
+#define R3D_GRAM(MO) case MO + 1: gram_row_kernel<MO><<<blocks, GRAM_THREADS, 0, s>>>(b.state, b.R, b.gram_part, g.field, sp.M); break
+  switch (sp.M) {
+    R3D_GRAM(0); R3D_GRAM(1); R3D_GRAM(2); R3D_GRAM(3); R3D_GRAM(4); R3D_GRAM(5); R3D_GRAM(6); R3D_GRAM(7);
+    R3D_GRAM(8); R3D_GRAM(9); R3D_GRAM(10); R3D_GRAM(11); R3D_GRAM(12); R3D_GRAM(13); R3D_GRAM(14); R3D_GRAM(15);
+    default: return 0;
+  }
+#undef R3D_GRAM
+  return 1;
+}
 
 // Grid = SOLVE_BLOCKS CTAs.  Every CTA adds its contiguous share of the per-CTA partials of zinv_residual
 // (double-double, fixed order), the CTA that finishes last (ticket counter) adds the SOLVE_BLOCKS second-level

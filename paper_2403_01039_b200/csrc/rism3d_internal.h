@@ -66,7 +66,7 @@ struct Buffers {
   double2* phik;         // [n][n][n/2]  phi~(k) exp(+i k.r0) / dV
   double* chi_shell;     // [nshell][nv][nv]   chi_shell[s][g][g'] = chi_{g' g}(k_s)
   double2* tw;           // [2n]         exp(-i pi j / n)
-  double* gram_part;     // [MAX_M+1][gram_blocks][2]  double-double partial sums, one per zinv_residual CTA
+  double* gram_part;     // [MAX_M+1][gram_blocks][2]  double-double partial sums, one per gram_row CTA
   double* gram_part2;    // [MAX_M+1][SOLVE_BLOCKS][2] second-level partials (mdiis_solve)
   double* scratch;       // [field] temporary (get_field, setup tables); aliases `work`
   double* qv;            // [nv] solvent charges
@@ -92,9 +92,10 @@ int launch_x_inv(const Grid&, const Buffers&, cudaStream_t);
 int launch_kspace_x(const Grid&, const Buffers&, cudaStream_t);
 int launch_y_inv(const Grid&, const Buffers&, bool use_state, cudaStream_t);
 int launch_zinv_residual(const Grid&, const Buffers&, const SolverParams&, double* d_raw_out, cudaStream_t);
+// mdiis_kernels.cu
 int gram_blocks(const Grid&);
 int gram_blocks_for(int n, int nv);
-// mdiis_kernels.cu
+int launch_gram_row(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);
 int launch_mdiis_solve(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);
 int launch_mdiis_update(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);
 // setup_kernels.cu
