@@ -50,6 +50,18 @@ static int fail(rism3d_ctx* c, int code, const char* fmt, ...) {
     if (e_ != cudaSuccess) return fail(ctx, RISM3D_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
   } while (0)
 
+// number of SMs of the current device (queried once; every context of this process runs on devices of one kind)
+static int g_num_sms = 0;
+int r3d::resident_ctas(int per_sm) {
+  if (g_num_sms == 0) {
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
+      n = 148;
+    g_num_sms = n;
+  }
+  return per_sm * g_num_sms;
+}
+
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 static bool valid_params(const rism3d_params* p) {

@@ -143,7 +143,8 @@ __device__ __forceinline__ void fwd_pass_last(int t, int T, Ld ld, Out out) {
 // ---------------------------------------------------------------------------------------------
 // Inverse (DIR = +1) decimation-in-time stages: the mirror image of the passes above.
 // ---------------------------------------------------------------------------------------------
-// first stage: In(j) reads NATURAL frequency index j; DFT_RL over the last digit; twiddle (3-pass only); St(idx)
+// first stage: In(j, pos) reads NATURAL frequency index j (pos = the in-place slot blk*RL + k of that value, for
+// sources staged in digit-reversed order, see inv_first_slot); DFT_RL over the last digit; twiddle (3-pass only); St(idx)
 template <int N, int RL, int R1, class In, class St>
 __device__ __forceinline__ void inv_stage_first(int t, int T, const Twiddle& tw, bool half2, In in, St st) {
   constexpr int NB = N / RL;
@@ -153,7 +154,7 @@ __device__ __forceinline__ void inv_stage_first(int t, int T, const Twiddle& tw,
     const int j0 = k1 + R1 * k2;
     cplx x[RL];
 #pragma unroll
-    for (int k = 0; k < RL; ++k) x[k] = in(j0 + NB * k);
+    for (int k = 0; k < RL; ++k) x[k] = in(j0 + NB * k, blk * RL + k);
     Dft<RL, +1>::run(x);
 #pragma unroll
     for (int r = 0; r < RL; ++r) {
@@ -165,6 +166,15 @@ __device__ __forceinline__ void inv_stage_first(int t, int T, const Twiddle& tw,
       st(blk * RL + r, (a == 0) ? x[r] : cmulc(x[r], tw(a)));
     }
   }
+}
+
+// slot of natural frequency index j in the layout inv_stage_first works on in place: j = k1 + R1*k2 + NB*k
+// -> (k1*RMID + k2)*RL + k
+template <int N, int RL, int R1>
+__device__ __forceinline__ int inv_first_slot(int j) {
+  constexpr int NB = N / RL, RMID = NB / R1;
+  const int k = j / NB, rem = j % NB;
+  return ((rem % R1) * RMID + rem / R1) * RL + k;
 }
 
 // middle stage of a 3-pass inverse: DFT_R2 over k2 (stride S2) inside block k1, twiddle exp(+2 pi i (k1[+1/2]) r / N)
@@ -213,7 +223,7 @@ template <> struct FftCfg<32>  { enum { R1 = 8,  R2 = 4,  R3 = 1, T = 4,  G = 8 
 template <> struct FftCfg<64>  { enum { R1 = 8,  R2 = 8,  R3 = 1, T = 8,  G = 4 }; };
 template <> struct FftCfg<128> { enum { R1 = 16, R2 = 8,  R3 = 1, T = 8,  G = 2 }; };
 #ifndef R3D_PLAN256
-#define R3D_PLAN256 0
+#define R3D_PLAN256 2
 #endif
 #if R3D_PLAN256 == 0
 template <> struct FftCfg<256> { enum { R1 = 16, R2 = 16, R3 = 1, T = 16, G = 1 }; };

@@ -10,6 +10,7 @@
 // f_m, m = 0..n-1, has F_{n-1-j} = conj F_j on the half-integer grid, so the even-j half is complete and
 //   F_{2p} = sum_{m<n/2} u_m exp(-2 pi i p m/(n/2)),   u_m = (f_m - i f_{m+n/2}) exp(-i pi m / n)
 // is a plain n/2-point complex FFT: no DC/Nyquist plane, same bytes as the real field.
+#include "async_copy.cuh"
 #include "fft_core.cuh"
 #include "rism3d_internal.h"
 
@@ -26,47 +27,91 @@ struct LineGeom {
 };
 
 // ------------------------------------------------------------------------------------------------
-// Strided line FFT (y or x axis), in place.  One tile = N points x COLS adjacent columns.
+// Strided line FFT (y or x axis), in place.  One tile = N points x COLS adjacent columns (128-byte rows); a CTA owns
+// G tiles at a time.  Persistent CTAs: work item i + gridDim.x streams into one shared-memory buffer (cp.async)
+// while the line FFTs of item i run in place on the other; the last radix pass stores straight to global memory.
 // ------------------------------------------------------------------------------------------------
+template <int N>
+struct StridedCfg {
+  enum { NT = FftCfg<N>::T * FftCfg<N>::G * COLS,                  // threads per CTA
+         ITEM = FftCfg<N>::G * N * COLS,                             // complex elements per work item
+         SHM = 2 * ITEM * (int)sizeof(cplx),
+         MINB = (SHM > 110 * 1024) ? 1 : ((SHM > 72 * 1024) ? 2 : 3) };
+};
+
+// stage work item `item` (G tiles) into `buf` [G][N][COLS]
+// (INV: row j goes to the slot the first inverse stage reads it from in place)
 template <int N, bool INV>
-__global__ void __launch_bounds__(FftCfg<N>::T* FftCfg<N>::G* COLS)
-    fft_strided_kernel(cplx* __restrict__ data, LineGeom g, Twiddle tw, const DevState* __restrict__ st) {
+__device__ __forceinline__ void stage_strided(cplx* buf, const cplx* data, const LineGeom& g, size_t item, int tid) {
+  using Cfg = FftCfg<N>;
+  constexpr int NT = StridedCfg<N>::NT, C = COLS;
+#pragma unroll
+  for (int k = 0; k < StridedCfg<N>::ITEM / NT; ++k) {
+    const int idx = tid + k * NT;
+    const int grp = idx / (N * C), rem = idx % (N * C), row = rem / C, col = rem % C;
+    const size_t chunk = item * Cfg::G + grp;
+    const cplx* src = data + (chunk / g.chunks_per_outer) * g.outer_stride + (chunk % g.chunks_per_outer) * C +
+                      (size_t)row * g.es + col;
+    constexpr int RL = (Cfg::R3 == 1) ? Cfg::R2 : Cfg::R3;
+    const int slot = INV ? inv_first_slot<N, RL, Cfg::R1>(row) : row;
+    cp_async16(buf + (grp * N + slot) * C + col, src);
+  }
+}
+
+template <int N, bool INV>
+__global__ void __launch_bounds__(StridedCfg<N>::NT, StridedCfg<N>::MINB)
+    fft_strided_kernel(cplx* __restrict__ data, LineGeom g, Twiddle tw, const DevState* __restrict__ st,
+                       unsigned nitems) {
   if (st != nullptr && st->done) return;
   using Cfg = FftCfg<N>;
   constexpr int T = Cfg::T, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS;
+  constexpr int ITEM = StridedCfg<N>::ITEM;
   const int tid = threadIdx.x;
   const int col = tid % C, t = (tid / C) % T, grp = tid / (C * T);
-  const size_t chunk = (size_t)blockIdx.x * Cfg::G + grp;
-  cplx* sm = smem_dyn + grp * (N * C) + col;
-  cplx* base = data + (chunk / g.chunks_per_outer) * g.outer_stride + (chunk % g.chunks_per_outer) * C + col;
   const size_t es = g.es;
-  auto ld_sm = [&](int i) { return sm[i * C]; };
-  auto st_sm = [&](int i, cplx v) { sm[i * C] = v; };
-  if (!INV) {
-    fwd_pass_a<N, R1, true>(t, T, tw, [&](int m) { return base[m * es]; }, st_sm);
+  int b = 0;
+  size_t item = blockIdx.x;
+  if (item < nitems) stage_strided<N, INV>(smem_dyn, data, g, item, tid);
+  cp_async_commit();
+  for (; item < nitems; item += gridDim.x) {
+    const size_t next = item + gridDim.x;
+    if (next < nitems) stage_strided<N, INV>(smem_dyn + (b ^ 1) * ITEM, data, g, next, tid);
+    cp_async_commit();
+    cp_async_wait<1>();
     __syncthreads();
-    auto out = [&](int j, cplx v) { base[j * es] = v; };
-    if constexpr (R3 == 1) {
-      fwd_pass_last<N, R2, R1>(t, T, ld_sm, out);
+    cplx* sm = smem_dyn + b * ITEM + grp * (N * C) + col;
+    const size_t chunk = item * Cfg::G + grp;
+    cplx* base = data + (chunk / g.chunks_per_outer) * g.outer_stride + (chunk % g.chunks_per_outer) * C + col;
+    auto ld_sm = [&](int i) { return sm[i * C]; };
+    auto st_sm = [&](int i, cplx v) { sm[i * C] = v; };
+    if (!INV) {
+      fwd_pass_a<N, R1, true>(t, T, tw, ld_sm, st_sm);
+      __syncthreads();
+      auto out = [&](int j, cplx v) { base[j * es] = v; };
+      if constexpr (R3 == 1) {
+        fwd_pass_last<N, R2, R1>(t, T, ld_sm, out);
+      } else {
+        fwd_pass_mid<N, R1, R2>(t, T, tw, ld_sm, st_sm);
+        __syncthreads();
+        fwd_pass_last<N, (R3 == 1 ? R2 : R3), R1>(t, T, ld_sm, out);
+      }
     } else {
-      fwd_pass_mid<N, R1, R2>(t, T, tw, ld_sm, st_sm);
-      __syncthreads();
-      fwd_pass_last<N, (R3 == 1 ? R2 : R3), R1>(t, T, ld_sm, out);
+      const double scale = 1.0 / (double)N;
+      auto out = [&](int m, cplx v) { base[m * es] = cscale(v, scale); };
+      auto ld_slot = [&](int, int pos) { return sm[pos * C]; };
+      if constexpr (R3 == 1) {
+        inv_stage_first<N, R2, R1>(t, T, tw, true, ld_slot, st_sm);
+        __syncthreads();
+      } else {
+        inv_stage_first<N, (R3 == 1 ? R2 : R3), R1>(t, T, tw, true, ld_slot, st_sm);
+        __syncthreads();
+        inv_stage_mid<N, R1, R2, true>(t, T, tw, ld_sm, st_sm);
+        __syncthreads();
+      }
+      inv_stage_last<N, R1, true>(t, T, tw, ld_sm, out);
     }
-  } else {
-    const double scale = 1.0 / (double)N;
-    auto in = [&](int j) { return base[j * es]; };
-    auto out = [&](int m, cplx v) { base[m * es] = cscale(v, scale); };
-    if constexpr (R3 == 1) {
-      inv_stage_first<N, R2, R1>(t, T, tw, true, in, st_sm);
-      __syncthreads();
-    } else {
-      inv_stage_first<N, (R3 == 1 ? R2 : R3), R1>(t, T, tw, true, in, st_sm);
-      __syncthreads();
-      inv_stage_mid<N, R1, R2, true>(t, T, tw, ld_sm, st_sm);
-      __syncthreads();
-    }
-    inv_stage_last<N, R1, true>(t, T, tw, ld_sm, out);
+    __syncthreads();                                   // buffer b is free again
+    b ^= 1;
   }
 }
 
@@ -87,12 +132,14 @@ static int launch_strided_n(const Grid& gr, const Buffers& b, bool x_axis, bool 
     g.chunks_per_outer = (unsigned)(Q / COLS);
     nchunks = (size_t)gr.n * g.chunks_per_outer;
   }
-  const int threads = Cfg::T * Cfg::G * COLS;
-  const size_t shm = (size_t)Cfg::G * N * COLS * sizeof(cplx);
+  const unsigned nitems = (unsigned)(nchunks / Cfg::G);
+  const size_t shm = StridedCfg<N>::SHM;
   auto kern = fft_strided_kernel<N, INV>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
   Twiddle tw{b.tw, 1, 2 * gr.n - 1};
-  kern<<<(unsigned)(nchunks / Cfg::G), threads, shm, s>>>(b.work, g, tw, use_state ? b.state : nullptr);
+  unsigned grid = (unsigned)resident_ctas(StridedCfg<N>::MINB);
+  if (grid > nitems) grid = nitems;
+  kern<<<grid, StridedCfg<N>::NT, shm, s>>>(b.work, g, tw, use_state ? b.state : nullptr, nitems);
   return 1;
 }
 
@@ -302,7 +349,7 @@ __global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, ZMinBlocks<NZ, G>::V)
   {
     const size_t line = line0 + (size_t)grp * LP + col / nv;
     const cplx* src = work + line * NZ * nv + (col % nv);
-    auto in = [&](int p) { return src[(size_t)p * nv]; };
+    auto in = [&](int p, int) { return src[(size_t)p * nv]; };
     if constexpr (R3 == 1) {
       inv_stage_first<NZ, R2, R1>(t, T, tw, false, in, st_sm);
       __syncthreads();

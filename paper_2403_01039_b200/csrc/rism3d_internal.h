@@ -83,6 +83,9 @@ struct SolverParams {
   double beta, kT, kappa, r_min;
 };
 
+// api.cu: per_sm * number of SMs of the device the context lives on (grid size of the persistent kernels)
+int resident_ctas(int per_sm);
+
 // ---- launchers (each returns the number of kernels it launched; errors surface via cudaGetLastError) ----
 // fft_kernels.cu
 int launch_closure_zfwd(const Grid&, const Buffers&, const SolverParams&, const double* d_raw_in, cudaStream_t);
