@@ -214,6 +214,138 @@ __device__ __forceinline__ void inv_stage_last(int t, int T, const Twiddle& tw, 
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Register-cached twiddles for the persistent strided passes.  A thread of a persistent CTA keeps its position
+// (t, column) for every tile, so the twiddles it needs are loop invariants: they are loaded once and stay in
+// registers.  To make forward and inverse share ONE set, the inverse applies its twiddles where a stage LOADS
+// (thread-fixed r, varying k) instead of where the previous stage stores:
+//   a[i][k1] = exp(-2 pi i (k1 + 1/2) r / N),  r = t + i T        forward pass A out  / inverse last stage in
+//   m[i][k2] = exp(-2 pi i k2 r2 / S1),  b = t + i T, r2 = b % S2  forward middle out  / inverse middle stage in
+// The pre/post factors exp(-+ i pi m1 / R1) of the half-integer grid are compile-time constants for R1 <= 8.
+// ---------------------------------------------------------------------------------------------
+// MREG = false keeps m in a small shared-memory table [S2][R2] (one per CTA, filled by fill_mid_table) instead of
+// registers, for kernels that are short of registers.
+template <int N, int R1, int R2, int R3, int T, bool MREG = true>
+struct LineTw {
+  static constexpr int S1 = N / R1, IA = S1 / T;
+  static constexpr bool THREE = (R3 != 1);
+  static constexpr int S2 = S1 / R2, IM = THREE ? (N / R2) / T : 1;
+  static constexpr int MID_TABLE = THREE ? S2 * R2 : 0;             // complex entries of the shared table
+  cplx a[IA][R1];
+  cplx m[(THREE && MREG) ? IM : 1][(THREE && MREG) ? R2 : 1];
+  const cplx* mt;
+  __device__ __forceinline__ void init(int t, const Twiddle& tw, const cplx* mid_table = nullptr) {
+#pragma unroll
+    for (int i = 0; i < IA; ++i)
+#pragma unroll
+      for (int k1 = 0; k1 < R1; ++k1) a[i][k1] = tw((2 * k1 + 1) * (t + i * T));
+    mt = mid_table;
+    if constexpr (THREE && MREG) {
+#pragma unroll
+      for (int i = 0; i < IM; ++i)
+#pragma unroll
+        for (int k2 = 0; k2 < R2; ++k2) m[i][k2] = tw(2 * R1 * k2 * ((t + i * T) % S2));
+    }
+  }
+  __device__ __forceinline__ cplx mid(int i, int r2, int k2) const {
+    if constexpr (MREG) return m[i][k2];
+    else return mt[r2 * R2 + k2];
+  }
+  // all threads of the CTA: table[r2 * R2 + k2] = exp(-2 pi i k2 r2 / S1); the caller synchronises afterwards
+  static __device__ __forceinline__ void fill_mid_table(cplx* table, const Twiddle& tw, int tid, int nthreads) {
+    for (int e = tid; e < MID_TABLE; e += nthreads) table[e] = tw(2 * R1 * (e % R2) * (e / R2));
+  }
+};
+
+// v * exp(DIR i pi m1 / R1)
+template <int R1, int DIR>
+__device__ __forceinline__ cplx half_shift(cplx v, int m1, const Twiddle& tw, int S1) {
+  if constexpr (R1 <= 8) {
+    return mul_w16<DIR>(v, m1 * (8 / R1));
+  } else {
+    return DIR < 0 ? cmul(v, tw(m1 * S1)) : cmulc(v, tw(m1 * S1));
+  }
+}
+
+template <int N, int R1, int R2, int R3, int T, bool MR, class Ld, class St>
+__device__ __forceinline__ void fwd_a_c(int t, const LineTw<N, R1, R2, R3, T, MR>& w, const Twiddle& tw, Ld ld, St st) {
+  constexpr int S1 = N / R1, IA = S1 / T;
+#pragma unroll
+  for (int i = 0; i < IA; ++i) {
+    const int r = t + i * T;
+    cplx x[R1];
+#pragma unroll
+    for (int m1 = 0; m1 < R1; ++m1) x[m1] = ld(m1 * S1 + r);
+#pragma unroll
+    for (int m1 = 1; m1 < R1; ++m1) x[m1] = half_shift<R1, -1>(x[m1], m1, tw, S1);
+    Dft<R1, -1>::run(x);
+#pragma unroll
+    for (int k1 = 0; k1 < R1; ++k1) st(k1 * S1 + r, cmul(x[k1], w.a[i][k1]));
+  }
+}
+
+template <int N, int R1, int R2, int R3, int T, bool MR, class Ld, class St>
+__device__ __forceinline__ void fwd_mid_c(int t, const LineTw<N, R1, R2, R3, T, MR>& w, Ld ld, St st) {
+  constexpr int S1 = N / R1, S2 = S1 / R2, IM = (N / R2) / T;
+#pragma unroll
+  for (int i = 0; i < IM; ++i) {
+    const int b = t + i * T, k1 = b / S2, r2 = b % S2;
+    cplx x[R2];
+#pragma unroll
+    for (int m2 = 0; m2 < R2; ++m2) x[m2] = ld(k1 * S1 + m2 * S2 + r2);
+    Dft<R2, -1>::run(x);
+    st(k1 * S1 + r2, x[0]);
+#pragma unroll
+    for (int k2 = 1; k2 < R2; ++k2) st(k1 * S1 + k2 * S2 + r2, cmul(x[k2], w.mid(i, r2, k2)));
+  }
+}
+
+// inverse first stage on slots staged by inv_first_slot: DFT_RL over the last digit, in place, no twiddle
+template <int N, int RL, int T, class Ld, class St>
+__device__ __forceinline__ void inv_first_c(int t, Ld ld, St st) {
+  constexpr int NB = N / RL;
+  for (int blk = t; blk < NB; blk += T) {
+    cplx x[RL];
+#pragma unroll
+    for (int k = 0; k < RL; ++k) x[k] = ld(blk * RL + k);
+    Dft<RL, +1>::run(x);
+#pragma unroll
+    for (int r = 0; r < RL; ++r) st(blk * RL + r, x[r]);
+  }
+}
+
+template <int N, int R1, int R2, int R3, int T, bool MR, class Ld, class St>
+__device__ __forceinline__ void inv_mid_c(int t, const LineTw<N, R1, R2, R3, T, MR>& w, Ld ld, St st) {
+  constexpr int S1 = N / R1, S2 = S1 / R2, IM = (N / R2) / T;
+#pragma unroll
+  for (int i = 0; i < IM; ++i) {
+    const int b = t + i * T, k1 = b / S2, r2 = b % S2;
+    cplx x[R2];
+    x[0] = ld(k1 * S1 + r2);
+#pragma unroll
+    for (int k2 = 1; k2 < R2; ++k2) x[k2] = cmulc(ld(k1 * S1 + k2 * S2 + r2), w.mid(i, r2, k2));
+    Dft<R2, +1>::run(x);
+#pragma unroll
+    for (int m2 = 0; m2 < R2; ++m2) st(k1 * S1 + m2 * S2 + r2, x[m2]);
+  }
+}
+
+template <int N, int R1, int R2, int R3, int T, bool MR, class Ld, class Out>
+__device__ __forceinline__ void inv_last_c(int t, const LineTw<N, R1, R2, R3, T, MR>& w, const Twiddle& tw, Ld ld, Out out) {
+  constexpr int S1 = N / R1, IA = S1 / T;
+#pragma unroll
+  for (int i = 0; i < IA; ++i) {
+    const int r = t + i * T;
+    cplx x[R1];
+#pragma unroll
+    for (int k1 = 0; k1 < R1; ++k1) x[k1] = cmulc(ld(k1 * S1 + r), w.a[i][k1]);
+    Dft<R1, +1>::run(x);
+    out(r, x[0]);
+#pragma unroll
+    for (int m1 = 1; m1 < R1; ++m1) out(m1 * S1 + r, half_shift<R1, +1>(x[m1], m1, tw, S1));
+  }
+}
+
 // Radix plan per line length.  T = threads per column, G = column groups (tiles) per CTA.
 template <int N> struct FftCfg;
 template <> struct FftCfg<4>   { enum { R1 = 2,  R2 = 2,  R3 = 1, T = 2,  G = 8 }; };

@@ -36,7 +36,7 @@ struct StridedCfg {
   enum { NT = FftCfg<N>::T * FftCfg<N>::G * COLS,                  // threads per CTA
          ITEM = FftCfg<N>::G * N * COLS,                             // complex elements per work item
          SHM = 2 * ITEM * (int)sizeof(cplx),
-         MINB = (SHM > 110 * 1024) ? 1 : ((SHM > 72 * 1024) ? 2 : 3) };
+         MINB = (SHM > 110 * 1024) ? 1 : 2 };      // <= 128 registers per thread: room for the cached twiddles
 };
 
 // stage work item `item` (G tiles) into `buf` [G][N][COLS]
@@ -69,6 +69,9 @@ __global__ void __launch_bounds__(StridedCfg<N>::NT, StridedCfg<N>::MINB)
   const int tid = threadIdx.x;
   const int col = tid % C, t = (tid / C) % T, grp = tid / (C * T);
   const size_t es = g.es;
+  constexpr int RL = (R3 == 1) ? R2 : R3;
+  LineTw<N, R1, R2, R3, T> w;                          // this thread's twiddles: the same for every tile
+  w.init(t, tw);
   int b = 0;
   size_t item = blockIdx.x;
   if (item < nitems) stage_strided<N, INV>(smem_dyn, data, g, item, tid);
@@ -85,30 +88,24 @@ __global__ void __launch_bounds__(StridedCfg<N>::NT, StridedCfg<N>::MINB)
     auto ld_sm = [&](int i) { return sm[i * C]; };
     auto st_sm = [&](int i, cplx v) { sm[i * C] = v; };
     if (!INV) {
-      fwd_pass_a<N, R1, true>(t, T, tw, ld_sm, st_sm);
+      fwd_a_c(t, w, tw, ld_sm, st_sm);
       __syncthreads();
       auto out = [&](int j, cplx v) { base[j * es] = v; };
-      if constexpr (R3 == 1) {
-        fwd_pass_last<N, R2, R1>(t, T, ld_sm, out);
-      } else {
-        fwd_pass_mid<N, R1, R2>(t, T, tw, ld_sm, st_sm);
+      if constexpr (R3 != 1) {
+        fwd_mid_c(t, w, ld_sm, st_sm);
         __syncthreads();
-        fwd_pass_last<N, (R3 == 1 ? R2 : R3), R1>(t, T, ld_sm, out);
       }
+      fwd_pass_last<N, RL, R1>(t, T, ld_sm, out);
     } else {
       const double scale = 1.0 / (double)N;
       auto out = [&](int m, cplx v) { base[m * es] = cscale(v, scale); };
-      auto ld_slot = [&](int, int pos) { return sm[pos * C]; };
-      if constexpr (R3 == 1) {
-        inv_stage_first<N, R2, R1>(t, T, tw, true, ld_slot, st_sm);
-        __syncthreads();
-      } else {
-        inv_stage_first<N, (R3 == 1 ? R2 : R3), R1>(t, T, tw, true, ld_slot, st_sm);
-        __syncthreads();
-        inv_stage_mid<N, R1, R2, true>(t, T, tw, ld_sm, st_sm);
+      inv_first_c<N, RL, T>(t, ld_sm, st_sm);
+      __syncthreads();
+      if constexpr (R3 != 1) {
+        inv_mid_c(t, w, ld_sm, st_sm);
         __syncthreads();
       }
-      inv_stage_last<N, R1, true>(t, T, tw, ld_sm, out);
+      inv_last_c(t, w, tw, ld_sm, out);
     }
     __syncthreads();                                   // buffer b is free again
     b ^= 1;

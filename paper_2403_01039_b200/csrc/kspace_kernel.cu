@@ -24,7 +24,8 @@ struct KspaceCfg {
          ITEM = FftCfg<N>::G * N * COLS,                  // complex data elements per work item
          PHI = FftCfg<N>::G * N * (COLS / NV),            // phi~ values per work item
          STAGE = ITEM + PHI,
-         SHM = 2 * STAGE * (int)sizeof(cplx),
+         MIDT = (FftCfg<N>::R3 == 1) ? 0 : (N / FftCfg<N>::R1 / FftCfg<N>::R2) * FftCfg<N>::R2,   // mid-pass twiddle table
+         SHM = (2 * STAGE + MIDT) * (int)sizeof(cplx),
          MINB = (SHM > 110 * 1024) ? 1 : ((SHM > 72 * 1024) ? 2 : 3) };
 };
 
@@ -72,6 +73,12 @@ __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
   const int lane = tid & 31;
   const int lane0 = lane & ~(NV - 1);
   const double qg = qv[site];
+  // this thread's twiddles are the same for every tile: pass-A set in registers, middle-pass set in a shared table
+  using Tw = LineTw<N, R1, R2, R3, T, false>;
+  cplx* mid_table = smem_dyn + 2 * K::STAGE;
+  Tw::fill_mid_table(mid_table, tw, tid, K::NT);
+  Tw w;
+  w.init(t, tw, mid_table);
   int b = 0;
   size_t item = blockIdx.x;
   if (item < nitems) stage_kspace<N, NV>(smem_dyn, data, phik, item, tid);
@@ -94,10 +101,10 @@ __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
     auto ld_sm = [&](int i) { return sm[i * C]; };
     auto st_sm = [&](int i, cplx v) { sm[i * C] = v; };
 
-    fwd_pass_a<N, R1, true>(t, T, tw, ld_sm, st_sm);
+    fwd_a_c(t, w, tw, ld_sm, st_sm);
     __syncthreads();
     if constexpr (R3 != 1) {
-      fwd_pass_mid<N, R1, R2>(t, T, tw, ld_sm, st_sm);
+      fwd_mid_c(t, w, ld_sm, st_sm);
       __syncthreads();
     }
     // innermost digit: forward DFT, k-space arithmetic, inverse DFT, all on the same registers
@@ -138,22 +145,17 @@ __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
         }
         x[k] = make_double2(hx - csr.x, hy - csr.y);                            // tau'(k) = h - c_sr
       }
-      Dft<RL, +1>::run(x);
+      Dft<RL, +1>::run(x);                             // first inverse stage; its twiddles are applied by the loads of the next
 #pragma unroll
-      for (int r = 0; r < RL; ++r) {
-        int a;
-        if (RMID == 1) a = (2 * k1 + 1) * r;
-        else a = 2 * R1 * k2 * r;
-        st_sm(blk * RL + r, (a == 0) ? x[r] : cmulc(x[r], tw(a)));
-      }
+      for (int r = 0; r < RL; ++r) st_sm(blk * RL + r, x[r]);
     }
     __syncthreads();
     if constexpr (R3 != 1) {
-      inv_stage_mid<N, R1, R2, true>(t, T, tw, ld_sm, st_sm);
+      inv_mid_c(t, w, ld_sm, st_sm);
       __syncthreads();
     }
     const double scale = 1.0 / (double)N;
-    inv_stage_last<N, R1, true>(t, T, tw, ld_sm, [&](int m, cplx v) { base[m * ES] = cscale(v, scale); });
+    inv_last_c(t, w, tw, ld_sm, [&](int m, cplx v) { base[m * ES] = cscale(v, scale); });
     __syncthreads();                                   // stage b is free again
     b ^= 1;
   }
