@@ -188,25 +188,26 @@ int launch_x_inv(const Grid& g, const Buffers& b, cudaStream_t s) {
 // ------------------------------------------------------------------------------------------------
 constexpr int ZP = COLS + 1;
 
-// Column groups per CTA of the z kernels (more than the strided passes use: these kernels stream whole fields and
-// want >= 256 threads with many independent loads in flight).
-template <int NZ> struct ZGroups { enum { G = FftCfg<NZ>::G }; };
-#ifndef R3D_ZG64
-#define R3D_ZG64 4
+// Configuration of the z kernels per line length NZ = n/2: radix plan (R1, R2, R3, T threads per column), column
+// groups per CTA and resident CTAs per SM the kernel is compiled for (register cap), separately for closure_zfwd
+// (GF, MBF) and zinv_residual (GI, MBI).  The large lines run 3-pass plans of small radices: few registers per thread,
+// so that 768-1024 threads per SM hide the latency of the closure's exp() chains and of the streaming loads.
+template <int NZ> struct ZPlan : FftCfg<NZ> { enum { GF = FftCfg<NZ>::G, MBF = 1, GI = FftCfg<NZ>::G, MBI = 1 }; };
+#ifndef R3D_ZGF
+#define R3D_ZGF 1
 #endif
-#ifndef R3D_ZG128
-#define R3D_ZG128 4
+#ifndef R3D_ZMBF
+#define R3D_ZMBF 8
 #endif
-#ifndef R3D_ZG256
-#define R3D_ZG256 2
+#ifndef R3D_ZGI
+#define R3D_ZGI 1
 #endif
-template <> struct ZGroups<64>  { enum { G = R3D_ZG64 }; };     // 8 * 4 * 8 = 256 threads
-template <> struct ZGroups<128> { enum { G = R3D_ZG128 }; };    // 8 * 4 * 8 = 256 threads, 72 KB tile
-template <> struct ZGroups<256> { enum { G = R3D_ZG256 }; };    // 16 * 2 * 8 = 256 threads, 72 KB tile
-// resident CTAs per SM the z kernels are compiled for: 512 threads per SM for the large lines
-template <int NZ, int G> struct ZMinBlocks {
-  enum { NT = FftCfg<NZ>::T * G * COLS, V = (NZ < 64) ? 1 : (NT >= 256 ? 2 : (NT >= 128 ? 4 : 8)) };
-};
+#ifndef R3D_ZMBI
+#define R3D_ZMBI 8
+#endif
+template <> struct ZPlan<64>  { enum { R1 = 8, R2 = 8, R3 = 1, T = 8, G = 4, GF = 4, MBF = 2, GI = 4, MBI = 2 }; };
+template <> struct ZPlan<128> { enum { R1 = 4, R2 = 4, R3 = 8, T = 16, G = 2, GF = R3D_ZGF, MBF = R3D_ZMBF, GI = R3D_ZGI, MBI = R3D_ZMBI }; };
+template <> struct ZPlan<256> { enum { R1 = 16, R2 = 16, R3 = 1, T = 16, G = 2, GF = 2, MBF = 2, GI = 2, MBI = 2 }; };
 
 __device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
 __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
@@ -214,13 +215,13 @@ __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<do
 // closure + forward z.  One tile per CTA.  Stage-in with 16-byte loads (two adjacent z points of both half lines
 // per thread, two such quads in flight), closure, packing u_m = (c_m - i c_{m+n/2}) exp(-i pi m / n) into the
 // shared-memory tile, then the n/2-point complex line FFTs.
-template <int NZ, int G>
-__global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, ZMinBlocks<NZ, G>::V)
+template <int NZ, int G, int MINB>
+__global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
     closure_zfwd_kernel(const double* __restrict__ tau_cur, const double* __restrict__ w, const double* __restrict__ raw,
                         cplx* __restrict__ work, Twiddle tw_shift, Twiddle tw, const DevState* __restrict__ st,
                         int nv, size_t npts, size_t field, int closure, int order) {
   if (raw == nullptr && st->done) return;
-  using Cfg = FftCfg<NZ>;
+  using Cfg = ZPlan<NZ>;
   constexpr int T = Cfg::T, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS, n = 2 * NZ;
   constexpr int NT = T * G * C, HP = NZ / 2, U = 2;
   const int tid = threadIdx.x;
@@ -289,13 +290,13 @@ __global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, ZMinBlocks<NZ, G>::V)
 template <int NZ>
 static int launch_closure_zfwd_n(const Grid& gr, const Buffers& b, const SolverParams& sp, const double* raw,
                                  cudaStream_t s) {
-  using Cfg = FftCfg<NZ>;
-  constexpr int G = ZGroups<NZ>::G;
+  using Cfg = ZPlan<NZ>;
+  constexpr int G = ZPlan<NZ>::GF;
   const int LP = COLS / gr.nv, GL = G * LP;
   const size_t nlines = (size_t)gr.n * gr.n;
   const int threads = Cfg::T * G * COLS;
   const size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
-  auto kern = closure_zfwd_kernel<NZ, G>;
+  auto kern = closure_zfwd_kernel<NZ, G, ZPlan<NZ>::MBF>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
   kern<<<(unsigned)(nlines / GL), threads, shm, s>>>(b.tau, b.w, raw, b.work, tws, tw, b.state, gr.nv, gr.npts,
@@ -322,13 +323,13 @@ int launch_closure_zfwd(const Grid& g, const Buffers& b, const SolverParams& sp,
 // (f_m, f_{m+n/2}) in place of complex element m, then a streaming phase with 16-byte accesses forms R = tau' - tau
 // (Eq. 33) and Z = tau + b R (the form Eq. 40 needs this entry in) and stores both into history slot `cur`.
 // The Gram row <R, R_i> is a separate streaming kernel (mdiis_kernels.cu: gram_row_kernel).
-template <int NZ, int G>
-__global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, ZMinBlocks<NZ, G>::V)
+template <int NZ, int G, int MINB>
+__global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
     zinv_residual_kernel(const cplx* __restrict__ work, const double* __restrict__ tau_cur, double* __restrict__ Z,
                          double* __restrict__ R, double* __restrict__ raw_out, Twiddle tw_shift, Twiddle tw,
                          const DevState* __restrict__ st, int nv, size_t npts, size_t field, double bdamp) {
   if (raw_out == nullptr && st->done) return;
-  using Cfg = FftCfg<NZ>;
+  using Cfg = ZPlan<NZ>;
   constexpr int T = Cfg::T, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS, n = 2 * NZ;
   constexpr int NT = T * G * C;
   constexpr int HP = NZ / 2;                           // pairs (m, m+1) per half line
@@ -395,12 +396,12 @@ __global__ void __launch_bounds__(FftCfg<NZ>::T* G* COLS, ZMinBlocks<NZ, G>::V)
 
 template <int NZ>
 static int launch_zinv_n(const Grid& gr, const Buffers& b, const SolverParams& sp, double* raw_out, cudaStream_t s) {
-  using Cfg = FftCfg<NZ>;
-  constexpr int G = ZGroups<NZ>::G;
+  using Cfg = ZPlan<NZ>;
+  constexpr int G = ZPlan<NZ>::GI;
   const int LP = COLS / gr.nv, GL = G * LP;
   const int threads = Cfg::T * G * COLS;
   const size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
-  auto kern = zinv_residual_kernel<NZ, G>;
+  auto kern = zinv_residual_kernel<NZ, G, ZPlan<NZ>::MBI>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
   kern<<<(unsigned)((size_t)gr.n * gr.n / GL), threads, shm, s>>>(b.work, b.tau, b.Z, b.R, raw_out, tws, tw, b.state,

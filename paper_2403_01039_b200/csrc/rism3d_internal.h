@@ -139,8 +139,12 @@ __device__ __forceinline__ void dd_norm(double& hi, double& lo) {
 __device__ __forceinline__ double closure_g(double d, int closure, int order) {
   if (closure == RISM3D_HNC) return exp(d);
   if (d > 0.0) {
+    // Horner form 1 + d/1 (1 + d/2 (1 + ... (1 + d/n))), every product and sum rounded separately (as the oracle's
+    // numpy expression); orders 1 and 2 need no division (x/1 and x/2 are exact as x and 0.5 x)
+    if (order == 1) return __dadd_rn(1.0, d);
+    if (order == 2) return __dadd_rn(1.0, __dmul_rn(__dadd_rn(1.0, __dmul_rn(d, 0.5)), d));
     double s = 1.0;
-    for (int i = order; i >= 1; --i) s = 1.0 + s * d / (double)i;
+    for (int i = order; i >= 1; --i) s = __dadd_rn(1.0, __ddiv_rn(__dmul_rn(s, d), (double)i));
     return s;
   }
   return exp(d);
