@@ -48,8 +48,7 @@ def kernel_words(n_v: int, m_hist: int) -> dict:
         "kspace_x": 2.0 + 1.0 / n_v,            # in place + phi~ (one complex per 2 points, shared by the sites)
         "y_inv": 2.0,
         "zinv_residual": 4.0,                   # read work, tau; write R and Z = tau + b R
-        "gram_row": float(m_hist),              # read the new residual and the M-1 stored ones it is dotted with
-        "mdiis_solve": 0.0,
+        "gram_solve": float(m_hist),            # read the new residual and the M-1 stored ones it is dotted with
         "mdiis_update": m_hist + 1.0,           # read M stored Z_i; write the new input tau
     }
 

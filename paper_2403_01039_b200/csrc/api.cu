@@ -100,7 +100,6 @@ static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_o
   char* chis = take((size_t)n_shells((int)n) * nv * nv * 8);
   char* tw = take(2 * n * 16);
   char* gp = take((size_t)gram_blocks_for((int)n, (int)nv) * (MAX_M + 1) * 2 * 8);
-  char* gp2 = take((size_t)SOLVE_BLOCKS * (MAX_M + 1) * 2 * 8);
   char* fp = take((size_t)FE_BLOCKS * MAX_NV * 2 * 8);
   char* qv = take(MAX_NV * 8);
   char* rv = take(MAX_NV * 8);
@@ -109,7 +108,7 @@ static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_o
     b->state = (DevState*)st;
     b->Z = (double*)Z; b->R = (double*)R; b->tau = (double*)tau; b->w = (double*)w; b->work = (double2*)work;
     b->phi = (double*)phi; b->phik = (double2*)phik; b->chi_shell = (double*)chis; b->tw = (double2*)tw;
-    b->gram_part = (double*)gp; b->gram_part2 = (double*)gp2; b->fe_part = (double*)fp; b->qv = (double*)qv; b->rhov = (double*)rv;
+    b->gram_part = (double*)gp; b->fe_part = (double*)fp; b->qv = (double*)qv; b->rhov = (double*)rv;
     b->scratch = (double*)work;
   }
   if (d_out) *d_out = (double*)out;
@@ -350,9 +349,7 @@ static int enqueue_iteration(rism3d_ctx* ctx) {
   prof_mark(ctx);
   k += launch_zinv_residual(g, b, ctx->sp, nullptr, s);    // step 5 (z), Eq. 33
   prof_mark(ctx);
-  k += launch_gram_row(g, b, ctx->sp, s);                  // step 6: Gram row of the new residual
-  prof_mark(ctx);
-  k += launch_mdiis_solve(g, b, ctx->sp, s);               // step 6-7
+  k += launch_gram_row(g, b, ctx->sp, s);                  // step 6-7: Gram row, rms test, MDIIS solve
   prof_mark(ctx);
   k += launch_mdiis_update(g, b, ctx->sp, s);              // step 6
   prof_mark(ctx);
@@ -382,7 +379,7 @@ extern "C" int rism3d_get_timings(rism3d_ctx* ctx, double* ms_total, int cap, lo
 
 extern "C" const char* rism3d_loop_kernel_name(int k) {
   static const char* names[RISM3D_N_LOOP_KERNELS] = {"closure_zfwd", "y_fwd", "kspace_x", "y_inv", "zinv_residual",
-                                                     "gram_row", "mdiis_solve", "mdiis_update"};
+                                                     "gram_solve", "mdiis_update"};
   return (k >= 0 && k < RISM3D_N_LOOP_KERNELS) ? names[k] : "";
 }
 

@@ -6,186 +6,21 @@
 // in no other form, and the update then reads M fields instead of 2M.  The current input lives in its own field.
 //
 //   gram_row_kernel     : streaming pass over the new residual and the stored ones: per-CTA double-double partial
-//                         sums of <R_new, R_new> and <R_new, R_i>.
-//   mdiis_solve_kernel  : finishes the Gram row (fixed-order double-double reduction of the per-CTA partial sums
-//                         of gram_row_kernel), rms and convergence test (Eq. 41 as read in Q9), history bookkeeping
-//                         (circular overwrite, restart rule), the bordered (m+1)x(m+1) solve by Gaussian
-//                         elimination with partial pivoting, and the choice of the slot the next pair goes to.
+//                         sums of <R_new, R_new> and <R_new, R_i>.  The CTA that finishes last (ticket counter)
+//                         adds the partials in a fixed order, then does rms and the convergence test (Eq. 41 as
+//                         read in Q9), the history bookkeeping (circular overwrite, restart rule), the bordered
+//                         (m+1)x(m+1) solve by Gaussian elimination with partial pivoting, and picks the slot the
+//                         next pair goes to.
 //   mdiis_update_kernel : streaming linear combination tau = sum_i c_i Z_i over the stored slots.
 #include "rism3d_internal.h"
 
 namespace r3d {
 
-constexpr int SOLVE_THREADS = 256;
-
-// Gram row.  One CTA = GRAM_THREADS * GRAM_EPT consecutive double2 of every field; each thread accumulates its
-// 2 * GRAM_EPT elements per entry in plain fp64 FMAs, the per-thread sums are then combined in double-double (warp
-// shuffles, fixed order) into one partial per CTA and entry; mdiis_solve adds the partials of all CTAs in
-// double-double, again in a fixed order (DESIGN.md "Gram accuracy").  Entry j < nother: <R_new, R_other[j]>;
-// entry MAX_M: <R_new, R_new>.  MAXO = M - 1 bounds nother at compile time.
-constexpr int GRAM_THREADS = 256;
-constexpr int GRAM_EPT = 16;
-
-template <int MAXO>
-__global__ void __launch_bounds__(GRAM_THREADS)
-    gram_row_kernel(const DevState* __restrict__ st, const double* __restrict__ R, double* __restrict__ gram_part,
-                    size_t field, int M) {
-  if (st->done) return;
-  __shared__ int s_other[MAX_M];
-  __shared__ int s_nother, s_cur;
-  __shared__ double s_part[(MAX_M + 1) * (GRAM_THREADS / 32) * 2];
-  const int tid = threadIdx.x;
-  if (tid == 0) {
-    const int m = st->m;
-    const int skip = (m == M) ? 1 : 0;                 // a full history drops its oldest entry this iteration
-    s_nother = m - skip;
-    s_cur = st->cur;
-    for (int i = 0; i < m - skip; ++i) s_other[i] = st->list[i + skip];
-  }
-  __syncthreads();
-  const int nother = s_nother;
-  const size_t n2 = field / 2;
-  const double2* Rn = reinterpret_cast<const double2*>(R + (size_t)s_cur * field);
-  const double2* Ro[MAXO > 0 ? MAXO : 1];
-#pragma unroll
-  for (int j = 0; j < MAXO; ++j)
-    Ro[j] = reinterpret_cast<const double2*>(R + (size_t)s_other[j < nother ? j : 0] * field);
-  double acc[MAXO + 1];
-#pragma unroll
-  for (int j = 0; j <= MAXO; ++j) acc[j] = 0.0;
-  const size_t base = (size_t)blockIdx.x * (GRAM_THREADS * GRAM_EPT) + tid;
-#pragma unroll 2
-  for (int it = 0; it < GRAM_EPT; ++it) {
-    const size_t i = base + (size_t)it * GRAM_THREADS;
-    if (i < n2) {
-      const double2 r = __ldcs(Rn + i);
-      acc[MAXO] = fma(r.x, r.x, fma(r.y, r.y, acc[MAXO]));
-#pragma unroll
-      for (int j = 0; j < MAXO; ++j)
-        if (j < nother) {
-          const double2 q = __ldcs(Ro[j] + i);
-          acc[j] = fma(r.x, q.x, fma(r.y, q.y, acc[j]));
-        }
-    }
-  }
-  // warp level: double-double butterfly-free tree in a fixed order, then one thread per entry adds the warps
-  const int lane = tid & 31, wid = tid >> 5;
-#pragma unroll
-  for (int j = 0; j <= MAXO; ++j) {
-    if (j < nother || j == MAXO) {
-      double hi = acc[j], lo = 0.0;
-      for (int o = 16; o > 0; o >>= 1) {
-        const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
-        dd_add(hi, lo, h2, l2);
-      }
-      if (lane == 0) {
-        s_part[(j * (GRAM_THREADS / 32) + wid) * 2] = hi;
-        s_part[(j * (GRAM_THREADS / 32) + wid) * 2 + 1] = lo;
-      }
-    }
-  }
-  __syncthreads();
-  if (tid <= MAXO && (tid < nother || tid == MAXO)) {
-    double hi = 0.0, lo = 0.0;
-    for (int w = 0; w < GRAM_THREADS / 32; ++w)
-      dd_add(hi, lo, s_part[(tid * (GRAM_THREADS / 32) + w) * 2], s_part[(tid * (GRAM_THREADS / 32) + w) * 2 + 1]);
-    dd_norm(hi, lo);
-    const int j = (tid == MAXO) ? MAX_M : tid;
-    *reinterpret_cast<double2*>(gram_part + ((size_t)j * gridDim.x + blockIdx.x) * 2) = make_double2(hi, lo);
-  }
-}
-
-int gram_blocks(const Grid& g) {
-  const size_t per = (size_t)GRAM_THREADS * GRAM_EPT;
-  return (int)((g.field / 2 + per - 1) / per);
-}
-int gram_blocks_for(int n, int nv) {
-  Grid g{};
-  g.n = n;
-  g.nv = nv;
-  g.field = (size_t)n * n * n * nv;
-  return gram_blocks(g);
-}
-
-int launch_gram_row(const Grid& g, const Buffers& b, const SolverParams& sp, cudaStream_t s) {
-  const unsigned blocks = (unsigned)gram_blocks(g);
-#define R3D_GRAM(MO) case MO + 1: gram_row_kernel<MO><<<blocks, GRAM_THREADS, 0, s>>>(b.state, b.R, b.gram_part, g.field, sp.M); break
-  switch (sp.M) {
-    R3D_GRAM(0); R3D_GRAM(1); R3D_GRAM(2); R3D_GRAM(3); R3D_GRAM(4); R3D_GRAM(5); R3D_GRAM(6); R3D_GRAM(7);
-    R3D_GRAM(8); R3D_GRAM(9); R3D_GRAM(10); R3D_GRAM(11); R3D_GRAM(12); R3D_GRAM(13); R3D_GRAM(14); R3D_GRAM(15);
-    default: return 0;
-  }
-#undef R3D_GRAM
-  return 1;
-}
-
-// Grid = SOLVE_BLOCKS CTAs.  Every CTA adds its contiguous share of the per-CTA partials of zinv_residual
-// (double-double, fixed order), the CTA that finishes last (ticket counter) adds the SOLVE_BLOCKS second-level
-// partials, again in a fixed order, and runs the bookkeeping and the small solve on one thread.
-__global__ void __launch_bounds__(SOLVE_THREADS)
-    mdiis_solve_kernel(DevState* __restrict__ st, const double* __restrict__ gram_part, double* __restrict__ part2,
-                       int nblocks, int M, double b, double restart, double npts_total) {
-  if (st->done) return;
-  __shared__ double s_hi[SOLVE_THREADS / 32], s_lo[SOLVE_THREADS / 32];
-  __shared__ double s_row[MAX_M + 1];
-  __shared__ bool s_last;
-  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  const int m_old = st->m;
+// History bookkeeping and the small solve, run by ONE thread (the last gram_row CTA) once the Gram row s_row
+// (entries 0..nother-1: <R_new, R_other[j]>, entry nother: <R_new, R_new>) is complete.
+__device__ void mdiis_bookkeeping_and_solve(DevState* __restrict__ st, const double* s_row, int m_old, int nother,
+                                            int M, double restart, double npts_total) {
   const int skip = (m_old == M) ? 1 : 0;
-  const int nother = m_old - skip;
-  const int per = (nblocks + SOLVE_BLOCKS - 1) / SOLVE_BLOCKS;
-  const int b0 = blockIdx.x * per, b1 = min(nblocks, b0 + per);
-
-  // Gram row: entry j < nother is <R_new, R_other[j]>, entry MAX_M is <R_new, R_new>
-  for (int jj = 0; jj <= nother; ++jj) {
-    const int j = (jj == nother) ? MAX_M : jj;
-    double hi = 0.0, lo = 0.0;
-    for (int blk = b0 + tid; blk < b1; blk += SOLVE_THREADS) {
-      const double2 p = *reinterpret_cast<const double2*>(gram_part + ((size_t)j * nblocks + blk) * 2);
-      dd_add(hi, lo, p.x, p.y);
-    }
-    for (int o = 16; o > 0; o >>= 1) {
-      const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
-      dd_add(hi, lo, h2, l2);
-    }
-    __syncthreads();
-    if (lane == 0) { s_hi[wid] = hi; s_lo[wid] = lo; }
-    __syncthreads();
-    if (tid == 0) {
-      hi = 0.0; lo = 0.0;
-      for (int k = 0; k < SOLVE_THREADS / 32; ++k) dd_add(hi, lo, s_hi[k], s_lo[k]);
-      dd_norm(hi, lo);
-      part2[((size_t)j * SOLVE_BLOCKS + blockIdx.x) * 2 + 0] = hi;
-      part2[((size_t)j * SOLVE_BLOCKS + blockIdx.x) * 2 + 1] = lo;
-    }
-  }
-  if (tid == 0) {
-    __threadfence();
-    const unsigned t = atomicAdd(&st->ticket, 1u);
-    s_last = (t == (unsigned)(gridDim.x - 1));
-  }
-  __syncthreads();
-  if (!s_last) return;
-  __threadfence();
-  if (tid < 32) {
-    for (int jj = 0; jj <= nother; ++jj) {
-      const int j = (jj == nother) ? MAX_M : jj;
-      double hi = 0.0, lo = 0.0;
-      for (int k = lane; k < (int)gridDim.x; k += 32) {
-        const volatile double* p = part2 + ((size_t)j * SOLVE_BLOCKS + k) * 2;
-        dd_add(hi, lo, p[0], p[1]);
-      }
-      for (int o = 16; o > 0; o >>= 1) {
-        const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
-        dd_add(hi, lo, h2, l2);
-      }
-      if (lane == 0) s_row[jj] = hi + lo;
-    }
-  }
-  __syncthreads();
-  if (tid != 0) return;
-  st->ticket = 0;
-
   const double self = s_row[nother];
   const double rms = sqrt(self / npts_total);          // Eq. 41 (Q9)
   st->rms_last = rms;
@@ -285,9 +120,149 @@ __global__ void __launch_bounds__(SOLVE_THREADS)
   st->cur = nxt;
 }
 
-int launch_mdiis_solve(const Grid& g, const Buffers& b, const SolverParams& sp, cudaStream_t s) {
-  mdiis_solve_kernel<<<SOLVE_BLOCKS, SOLVE_THREADS, 0, s>>>(b.state, b.gram_part, b.gram_part2, gram_blocks(g), sp.M,
-                                                           sp.b, sp.restart, (double)g.field);
+// Gram row.  One CTA = GRAM_THREADS * GRAM_EPT consecutive double2 of every field; each thread accumulates its
+// 2 * GRAM_EPT elements per entry in plain fp64 FMAs, the per-thread sums are then combined in double-double (warp
+// shuffles, fixed order) into one partial per CTA and entry; mdiis_solve adds the partials of all CTAs in
+// double-double, again in a fixed order (DESIGN.md "Gram accuracy").  Entry j < nother: <R_new, R_other[j]>;
+// entry MAX_M: <R_new, R_new>.  MAXO = M - 1 bounds nother at compile time.
+constexpr int GRAM_THREADS = 256;
+constexpr int GRAM_EPT = 16;
+
+template <int MAXO>
+__global__ void __launch_bounds__(GRAM_THREADS)
+    gram_row_kernel(DevState* __restrict__ st, const double* __restrict__ R, double* __restrict__ gram_part,
+                    size_t field, int M, double restart) {
+  if (st->done) return;
+  __shared__ int s_other[MAX_M];
+  __shared__ int s_nother, s_cur, s_m;
+  __shared__ bool s_last;
+  __shared__ double s_row[MAX_M + 1];
+  __shared__ double s_part[(MAX_M + 1) * (GRAM_THREADS / 32) * 2];
+  const int tid = threadIdx.x;
+  if (tid == 0) {
+    const int m = st->m;
+    const int skip = (m == M) ? 1 : 0;                 // a full history drops its oldest entry this iteration
+    s_nother = m - skip;
+    s_m = m;
+    s_cur = st->cur;
+    for (int i = 0; i < m - skip; ++i) s_other[i] = st->list[i + skip];
+  }
+  __syncthreads();
+  const int nother = s_nother;
+  const size_t n2 = field / 2;
+  const double2* Rn = reinterpret_cast<const double2*>(R + (size_t)s_cur * field);
+  const double2* Ro[MAXO > 0 ? MAXO : 1];
+#pragma unroll
+  for (int j = 0; j < MAXO; ++j)
+    Ro[j] = reinterpret_cast<const double2*>(R + (size_t)s_other[j < nother ? j : 0] * field);
+  double acc[MAXO + 1];
+#pragma unroll
+  for (int j = 0; j <= MAXO; ++j) acc[j] = 0.0;
+  const size_t base = (size_t)blockIdx.x * (GRAM_THREADS * GRAM_EPT) + tid;
+#pragma unroll 2
+  for (int it = 0; it < GRAM_EPT; ++it) {
+    const size_t i = base + (size_t)it * GRAM_THREADS;
+    if (i < n2) {
+      const double2 r = __ldcs(Rn + i);
+      acc[MAXO] = fma(r.x, r.x, fma(r.y, r.y, acc[MAXO]));
+#pragma unroll
+      for (int j = 0; j < MAXO; ++j)
+        if (j < nother) {
+          const double2 q = __ldcs(Ro[j] + i);
+          acc[j] = fma(r.x, q.x, fma(r.y, q.y, acc[j]));
+        }
+    }
+  }
+  // warp level: double-double butterfly-free tree in a fixed order, then one thread per entry adds the warps
+  const int lane = tid & 31, wid = tid >> 5;
+#pragma unroll
+  for (int j = 0; j <= MAXO; ++j) {
+    if (j < nother || j == MAXO) {
+      double hi = acc[j], lo = 0.0;
+      for (int o = 16; o > 0; o >>= 1) {
+        const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
+        dd_add(hi, lo, h2, l2);
+      }
+      if (lane == 0) {
+        s_part[(j * (GRAM_THREADS / 32) + wid) * 2] = hi;
+        s_part[(j * (GRAM_THREADS / 32) + wid) * 2 + 1] = lo;
+      }
+    }
+  }
+  __syncthreads();
+  if (tid <= MAXO && (tid < nother || tid == MAXO)) {
+    double hi = 0.0, lo = 0.0;
+    for (int w = 0; w < GRAM_THREADS / 32; ++w)
+      dd_add(hi, lo, s_part[(tid * (GRAM_THREADS / 32) + w) * 2], s_part[(tid * (GRAM_THREADS / 32) + w) * 2 + 1]);
+    dd_norm(hi, lo);
+    const int j = (tid == MAXO) ? MAX_M : tid;
+    *reinterpret_cast<double2*>(gram_part + ((size_t)j * gridDim.x + blockIdx.x) * 2) = make_double2(hi, lo);
+    __threadfence();                                   // the partial is visible before this CTA takes its ticket
+  }
+  __syncthreads();
+  if (tid == 0) {
+    const unsigned t = atomicAdd(&st->ticket, 1u);
+    s_last = (t == gridDim.x - 1);
+  }
+  __syncthreads();
+  if (!s_last) return;
+
+  // The CTA that finishes last adds the partials of all CTAs, entry by entry, in double-double and in a fixed order
+  // (thread i takes partials i, i + 256, ...; then the warp tree and the 8 warps in order), then one thread does the
+  // bookkeeping and the small solve.  Which CTA is last does not affect any value.
+  __threadfence();
+  const int nblk = (int)gridDim.x;
+  for (int jj = 0; jj <= nother; ++jj) {
+    const int j = (jj == nother) ? MAX_M : jj;
+    double hi = 0.0, lo = 0.0;
+    const double2* part = reinterpret_cast<const double2*>(gram_part) + (size_t)j * nblk;
+    for (int blk = tid; blk < nblk; blk += GRAM_THREADS) {
+      const double2 p = __ldcg(part + blk);
+      dd_add(hi, lo, p.x, p.y);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+      const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
+      dd_add(hi, lo, h2, l2);
+    }
+    if (lane == 0) {
+      s_part[(jj * (GRAM_THREADS / 32) + wid) * 2] = hi;
+      s_part[(jj * (GRAM_THREADS / 32) + wid) * 2 + 1] = lo;
+    }
+  }
+  __syncthreads();
+  if (tid <= nother) {
+    double hi = 0.0, lo = 0.0;
+    for (int w = 0; w < GRAM_THREADS / 32; ++w)
+      dd_add(hi, lo, s_part[(tid * (GRAM_THREADS / 32) + w) * 2], s_part[(tid * (GRAM_THREADS / 32) + w) * 2 + 1]);
+    s_row[tid] = hi + lo;
+  }
+  __syncthreads();
+  if (tid != 0) return;
+  st->ticket = 0;
+  mdiis_bookkeeping_and_solve(st, s_row, s_m, nother, M, restart, (double)field);
+}
+
+int gram_blocks(const Grid& g) {
+  const size_t per = (size_t)GRAM_THREADS * GRAM_EPT;
+  return (int)((g.field / 2 + per - 1) / per);
+}
+int gram_blocks_for(int n, int nv) {
+  Grid g{};
+  g.n = n;
+  g.nv = nv;
+  g.field = (size_t)n * n * n * nv;
+  return gram_blocks(g);
+}
+
+int launch_gram_row(const Grid& g, const Buffers& b, const SolverParams& sp, cudaStream_t s) {
+  const unsigned blocks = (unsigned)gram_blocks(g);
+#define R3D_GRAM(MO) case MO + 1: gram_row_kernel<MO><<<blocks, GRAM_THREADS, 0, s>>>(b.state, b.R, b.gram_part, g.field, sp.M, sp.restart); break
+  switch (sp.M) {
+    R3D_GRAM(0); R3D_GRAM(1); R3D_GRAM(2); R3D_GRAM(3); R3D_GRAM(4); R3D_GRAM(5); R3D_GRAM(6); R3D_GRAM(7);
+    R3D_GRAM(8); R3D_GRAM(9); R3D_GRAM(10); R3D_GRAM(11); R3D_GRAM(12); R3D_GRAM(13); R3D_GRAM(14); R3D_GRAM(15);
+    default: return 0;
+  }
+#undef R3D_GRAM
   return 1;
 }
 

@@ -12,7 +12,6 @@ constexpr int MAX_M = 16;            // MDIIS history slots (rism3d_params.mdiis
 constexpr int MAX_NV = 8;            // solvent site types
 constexpr int RMS_HIST_CAP = 65536;
 constexpr int FE_BLOCKS = 148 * 4;        // CTAs of the free-energy reduction
-constexpr int SOLVE_BLOCKS = 64;          // CTAs of mdiis_solve (second level of the Gram reduction)
 
 constexpr double K_BOLTZMANN = 0.001987204259;   // kcal/(mol K)     (Q3)
 constexpr double COULOMB = 332.06371;            // kcal A/(mol e^2) (Q3)
@@ -28,7 +27,7 @@ struct DevState {
   int m;                       // filled history entries
   int cur;                     // physical history slot that receives the (Z, R) pair of the running iteration
   int upd_m;                   // entries to combine in the update kernel (0: skip)
-  unsigned ticket;             // CTAs of mdiis_solve that have finished their share of the Gram reduction
+  unsigned ticket;             // CTAs of gram_row that have written their partial sums
   double tol;
   double rms_last;
   double pad_[2];
@@ -67,7 +66,6 @@ struct Buffers {
   double* chi_shell;     // [nshell][nv][nv]   chi_shell[s][g][g'] = chi_{g' g}(k_s)
   double2* tw;           // [2n]         exp(-i pi j / n)
   double* gram_part;     // [MAX_M+1][gram_blocks][2]  double-double partial sums, one per gram_row CTA
-  double* gram_part2;    // [MAX_M+1][SOLVE_BLOCKS][2] second-level partials (mdiis_solve)
   double* scratch;       // [field] temporary (get_field, setup tables); aliases `work`
   double* qv;            // [nv] solvent charges
   double* rhov;          // [nv]
@@ -99,7 +97,6 @@ int launch_zinv_residual(const Grid&, const Buffers&, const SolverParams&, doubl
 int gram_blocks(const Grid&);
 int gram_blocks_for(int n, int nv);
 int launch_gram_row(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);
-int launch_mdiis_solve(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);
 int launch_mdiis_update(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);
 // setup_kernels.cu
 int launch_chi_shell(const Grid&, const Buffers&, const double* d_chi_table, int n_k, double k0, double dk,
