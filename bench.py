@@ -43,13 +43,12 @@ CPU_SAMPLE_ATOMS = 64        # the loop cost does not depend on the atom count; 
 def kernel_words(n_v: int, m_hist: int) -> dict:
     """m_hist = stored MDIIS entries during the timed steps (= M once the history is full)."""
     return {
-        "closure_zfwd": 3.0,                    # read tau, w; write c_sr(z-transformed)
+        "closure_zfwd": m_hist + 3.0,           # read M stored Z_i (pending MDIIS update) and w; write tau and c_sr(z-transformed)
         "y_fwd": 2.0,                           # in place
         "kspace_x": 2.0 + 1.0 / n_v,            # in place + phi~ (one complex per 2 points, shared by the sites)
         "y_inv": 2.0,
         "zinv_residual": 4.0,                   # read work, tau; write R and Z = tau + b R
         "gram_solve": float(m_hist),            # read the new residual and the M-1 stored ones it is dotted with
-        "mdiis_update": m_hist + 1.0,           # read M stored Z_i; write the new input tau
     }
 
 

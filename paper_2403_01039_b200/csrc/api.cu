@@ -350,9 +350,8 @@ static int enqueue_iteration(rism3d_ctx* ctx) {
   k += launch_zinv_residual(g, b, ctx->sp, nullptr, s);    // step 5 (z), Eq. 33
   prof_mark(ctx);
   k += launch_gram_row(g, b, ctx->sp, s);                  // step 6-7: Gram row, rms test, MDIIS solve
-  prof_mark(ctx);
-  k += launch_mdiis_update(g, b, ctx->sp, s);              // step 6
-  prof_mark(ctx);
+  prof_mark(ctx);                                          // (the update tau = sum c_i Z_i is applied by the next
+                                                           //  closure_zfwd, or by iterate's trailing update pass)
   ctx->launches += k;
   return k;
 }
@@ -379,7 +378,7 @@ extern "C" int rism3d_get_timings(rism3d_ctx* ctx, double* ms_total, int cap, lo
 
 extern "C" const char* rism3d_loop_kernel_name(int k) {
   static const char* names[RISM3D_N_LOOP_KERNELS] = {"closure_zfwd", "y_fwd", "kspace_x", "y_inv", "zinv_residual",
-                                                     "gram_solve", "mdiis_update"};
+                                                     "gram_solve"};
   return (k >= 0 && k < RISM3D_N_LOOP_KERNELS) ? names[k] : "";
 }
 
@@ -404,6 +403,9 @@ extern "C" int rism3d_iterate(rism3d_ctx* ctx, int max_iter, double tol, int* n_
       if (ctx->h_hdr->done) break;
     }
   }
+  // the update of the last iteration is still pending (it rides on the next closure pass): apply it now, so that
+  // tau is the new input when this call returns
+  if (max_iter > 0) ctx->launches += launch_mdiis_update(ctx->g, ctx->b, ctx->sp, ctx->stream);
   CU(cudaGetLastError());
   int rc = read_header(ctx);
   if (rc) return rc;

@@ -197,7 +197,7 @@ template <int NZ> struct ZPlan : FftCfg<NZ> { enum { GF = FftCfg<NZ>::G, MBF = 1
 #define R3D_ZGF 1
 #endif
 #ifndef R3D_ZMBF
-#define R3D_ZMBF 8
+#define R3D_ZMBF 4
 #endif
 #ifndef R3D_ZGI
 #define R3D_ZGI 1
@@ -217,10 +217,22 @@ __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<do
 // shared-memory tile, then the n/2-point complex line FFTs.
 template <int NZ, int G, int MINB>
 __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
-    closure_zfwd_kernel(const double* __restrict__ tau_cur, const double* __restrict__ w, const double* __restrict__ raw,
-                        cplx* __restrict__ work, Twiddle tw_shift, Twiddle tw, const DevState* __restrict__ st,
-                        int nv, size_t npts, size_t field, int closure, int order) {
+    closure_zfwd_kernel(double* __restrict__ tau_cur, const double* __restrict__ w, const double* __restrict__ raw,
+                        const double* __restrict__ Z, cplx* __restrict__ work, Twiddle tw_shift, Twiddle tw,
+                        const DevState* __restrict__ st, int nv, size_t npts, size_t field, int closure, int order) {
   if (raw == nullptr && st->done) return;
+  // pending MDIIS update (step 6 of the previous iteration): tau = sum_i c_i Z_i is formed here, on the way in,
+  // and written back once, instead of by a separate pass that this kernel would then re-read
+  __shared__ int s_ulist[MAX_M];
+  __shared__ double s_ucoef[MAX_M];
+  __shared__ int s_um;
+  if (threadIdx.x == 0) {
+    const int m = raw ? 0 : st->upd_m;
+    s_um = m;
+    for (int i = 0; i < m; ++i) { s_ulist[i] = st->upd_list[i]; s_ucoef[i] = st->upd_coef[i]; }
+  }
+  __syncthreads();
+  const int um = s_um;
   using Cfg = ZPlan<NZ>;
   constexpr int T = Cfg::T, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS, n = 2 * NZ;
   constexpr int NT = T * G * C, HP = NZ / 2, U = 2;
@@ -240,8 +252,28 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
         const int mp = e % HP, lc = e / HP;
         const int site = lc / GL, l = lc % GL;
         off[u] = (size_t)site * npts + (line0 + l) * n + 2 * mp;
-        t0[u] = ld2(tau + off[u]);
-        t1[u] = ld2(tau + off[u] + NZ);
+        if (um == 0) {
+          t0[u] = ld2(tau + off[u]);
+          t1[u] = ld2(tau + off[u] + NZ);
+        } else {
+          // products and sums rounded one by one, in the order of the oracle's loop (Eq. 40 as read in Q7)
+          double2 a0 = make_double2(0.0, 0.0), a1 = make_double2(0.0, 0.0);
+#pragma unroll 5
+          for (int k = 0; k < um; ++k) {
+            const double* Zk = Z + (size_t)s_ulist[k] * field + off[u];
+            const double2 z0 = __ldcs(reinterpret_cast<const double2*>(Zk));
+            const double2 z1 = __ldcs(reinterpret_cast<const double2*>(Zk + NZ));
+            const double ck = s_ucoef[k];
+            a0.x = __dadd_rn(a0.x, __dmul_rn(ck, z0.x));
+            a0.y = __dadd_rn(a0.y, __dmul_rn(ck, z0.y));
+            a1.x = __dadd_rn(a1.x, __dmul_rn(ck, z1.x));
+            a1.y = __dadd_rn(a1.y, __dmul_rn(ck, z1.y));
+          }
+          t0[u] = a0;
+          t1[u] = a1;
+          st2(tau_cur + off[u], a0);
+          st2(tau_cur + off[u] + NZ, a1);
+        }
         if (!raw) {
           w0[u] = ld2(w + off[u]);
           w1[u] = ld2(w + off[u] + NZ);
@@ -299,7 +331,7 @@ static int launch_closure_zfwd_n(const Grid& gr, const Buffers& b, const SolverP
   auto kern = closure_zfwd_kernel<NZ, G, ZPlan<NZ>::MBF>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
-  kern<<<(unsigned)(nlines / GL), threads, shm, s>>>(b.tau, b.w, raw, b.work, tws, tw, b.state, gr.nv, gr.npts,
+  kern<<<(unsigned)(nlines / GL), threads, shm, s>>>(b.tau, b.w, raw, b.Z, b.work, tws, tw, b.state, gr.nv, gr.npts,
                                                        gr.field, sp.closure, sp.pse_order);
   return 1;
 }

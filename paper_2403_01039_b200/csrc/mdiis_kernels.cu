@@ -297,13 +297,16 @@ __global__ void __launch_bounds__(256)
   }
 }
 
+__global__ void clear_pending_update_kernel(DevState* st) { st->upd_m = 0; }
+
 int launch_mdiis_update(const Grid& g, const Buffers& b, const SolverParams& sp, cudaStream_t s) {
   const size_t n2 = g.field / 2;
   size_t blocks = (n2 + 255) / 256;
   const size_t cap = 148 * 8 * 4;
   if (blocks > cap) blocks = cap;
   mdiis_update_kernel<<<(unsigned)blocks, 256, 0, s>>>(b.state, b.Z, b.tau, g.field);
-  return 1;
+  clear_pending_update_kernel<<<1, 1, 0, s>>>(b.state);
+  return 2;
 }
 
 }  // namespace r3d
