@@ -35,6 +35,7 @@ __global__ void __launch_bounds__(128)
   for (int g = 0; g < NV; ++g) acc[g] = 0.0;
   double ph = 0.0;
   const bool cut = rcut2 > 0.0;
+  const double rmin2 = r_min * r_min, far2 = 1600.0 / (kappa * kappa);
   for (int a0 = 0; a0 < n_atoms; a0 += ATOM_CHUNK) {
     const int na = min(ATOM_CHUNK, n_atoms - a0);
     __syncthreads();
@@ -45,23 +46,62 @@ __global__ void __launch_bounds__(128)
       const double4 at = s_atom[a];
       const double dx = x - at.x, dy = y - at.y, dz = z - at.z;
       const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-      const double rt = sqrt(r2);
-      const double kr = kappa * rt;
-      const double em = expm1(-kr);
-      const double lr = (kr < 1e-8) ? kappa : -em / rt;      // (1 - exp(-kappa r)) / r and its limit
-      ph += at.w * lr;
-      if (!cut || r2 < rcut2) {
-        const double rc = fmax(rt, r_min);
-        double sc;                                            // 1/r - (1 - exp(-kappa r))/r
-        if (rt >= r_min) sc = (1.0 + em) / rt;
-        else sc = cut ? exp(-kappa * rc) / rc : 1.0 / rc - lr;
-        const double inv2 = 1.0 / (rc * rc);
-        const double* pp = s_pair + a * NV * 3;
+      // The common case first.  1/r: float rsqrt seed + two Newton steps in double (~2 ulp; r^2 is far inside the
+      // float range).  Beyond kappa r = 40, exp(-kappa r) < 5e-18 vanishes against 1 in double precision: (1 -
+      // exp(-kappa r))/r is 1/r to the last bit and the short-range Coulomb term is 0, so far pairs (most of them
+      // on the large grids) need no exp at all.
+      if (r2 >= rmin2) {
+        double rinv = (double)rsqrtf((float)r2);
+        rinv = rinv * fma(-0.5 * r2, rinv * rinv, 1.5);
+        rinv = rinv * fma(-0.5 * r2, rinv * rinv, 1.5);
+        if (r2 > far2) {
+          ph = fma(at.w, rinv, ph);
+          if (!cut) {                                         // all-pairs mode: LJ reaches further than exp(-kappa r)
+            const double inv2 = rinv * rinv;
+            const double* pp = s_pair + a * NV * 3;
 #pragma unroll
-        for (int g = 0; g < NV; ++g) {
-          const double s2 = pp[g * 3 + 1] * inv2;
-          const double s6 = s2 * s2 * s2;
-          acc[g] -= pp[g * 3 + 0] * sc + pp[g * 3 + 2] * (s6 * s6 - s6);
+            for (int g = 0; g < NV; ++g) {
+              const double s2 = pp[g * 3 + 1] * inv2;
+              const double s6 = s2 * s2 * s2;
+              acc[g] -= pp[g * 3 + 2] * (s6 * s6 - s6);
+            }
+          }
+        } else {
+          const double kr = kappa * (r2 * rinv);
+          // 1 - exp(-kappa r): expm1 where the subtraction would cancel, exp elsewhere
+          const double ex = (kr < 0.5) ? 1.0 + expm1(-kr) : exp(-kr);
+          const double om = (kr < 0.5) ? -expm1(-kr) : 1.0 - ex;
+          ph = fma(at.w, om * rinv, ph);
+          if (!cut || r2 < rcut2) {
+            const double sc = ex * rinv;                      // exp(-kappa r)/r = 1/r - (1 - exp(-kappa r))/r
+            const double inv2 = rinv * rinv;
+            const double* pp = s_pair + a * NV * 3;
+#pragma unroll
+            for (int g = 0; g < NV; ++g) {
+              const double s2 = pp[g * 3 + 1] * inv2;
+              const double s6 = s2 * s2 * s2;
+              acc[g] -= pp[g * 3 + 0] * sc + pp[g * 3 + 2] * (s6 * s6 - s6);
+            }
+          }
+        }
+      } else {
+        // grid point (almost) on an atom: distance clamped at r_min (Q11), phi at its finite limit
+        const double rt = sqrt(r2);
+        const double kr = kappa * rt;
+        const double em = expm1(-kr);
+        const double lr = (kr < 1e-8) ? kappa : -em / rt;     // (1 - exp(-kappa r)) / r and its limit
+        ph += at.w * lr;
+        if (!cut || r2 < rcut2) {
+          const double rc = fmax(rt, r_min);
+          const double sc = (rt >= r_min) ? (1.0 + em) / rt : (cut ? exp(-kappa * rc) / rc : 1.0 / rc - lr);
+          const double inv2 = 1.0 / (rc * rc);
+          const double* pp = s_pair + a * NV * 3;
+#pragma unroll
+          for (int g = 0; g < NV; ++g) {
+            const double s2 = pp[g * 3 + 1] * inv2;
+            const double s6 = s2 * s2 * s2;
+            acc[g] -= pp[g * 3 + 0] * sc + pp[g * 3 + 2] * (s6 * s6 - s6);
+          }
         }
       }
     }
