@@ -47,8 +47,7 @@ def kernel_words(n_v: int, m_hist: int) -> dict:
         "y_fwd": 2.0,                           # in place
         "kspace_x": 2.0 + 1.0 / n_v,            # in place + phi~ (one complex per 2 points, shared by the sites)
         "y_inv": 2.0,
-        "zinv_residual": 4.0,                   # read work, tau; write R and Z = tau + b R
-        "gram_solve": float(m_hist),            # read the new residual and the M-1 stored ones it is dotted with
+        "zinv_gram_solve": m_hist + 3.0,        # read work, tau, the M-1 stored residuals; write R and Z = tau + b R
     }
 
 

@@ -139,7 +139,7 @@ long long rism3d_launch_count(const rism3d_ctx* ctx);
  * set_profiling(0) switches them off; both synchronise the stream.  get_timings synchronises, then writes
  * ms_total[k], k < RISM3D_N_LOOP_KERNELS (HOST, cap >= RISM3D_N_LOOP_KERNELS): the summed milliseconds of
  * loop kernel k over *n_iterations profiled iterations, in launch order (names: rism3d_loop_kernel_name). */
-#define RISM3D_N_LOOP_KERNELS 6
+#define RISM3D_N_LOOP_KERNELS 5
 int rism3d_set_profiling(rism3d_ctx* ctx, int enable);
 int rism3d_get_timings(rism3d_ctx* ctx, double* ms_total, int cap, long long* n_iterations);
 const char* rism3d_loop_kernel_name(int k);             /* static strings; "" when k is out of range */

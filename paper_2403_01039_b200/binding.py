@@ -187,7 +187,7 @@ def rism3d_launch_count(ctx) -> int:
     return int(load_library().rism3d_launch_count(ctx))
 
 
-N_LOOP_KERNELS = 6
+N_LOOP_KERNELS = 5
 
 
 def rism3d_set_profiling(ctx, enable: bool):

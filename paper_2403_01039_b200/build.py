@@ -17,7 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "librism3d.so")
 SOURCES = ["api.cu", "fft_kernels.cu", "kspace_kernel.cu", "mdiis_kernels.cu", "setup_kernels.cu"]
-HEADERS = ["fft_core.cuh", "async_copy.cuh", "rism3d_internal.h", os.path.join("..", "..", "include", "rism3d.h")]
+HEADERS = ["fft_core.cuh", "async_copy.cuh", "mdiis_device.cuh", "rism3d_internal.h", os.path.join("..", "..", "include", "rism3d.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]

@@ -99,7 +99,13 @@ static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_o
   char* phik = take(npts * 8);
   char* chis = take((size_t)n_shells((int)n) * nv * nv * 8);
   char* tw = take(2 * n * 16);
-  char* gp = take((size_t)gram_blocks_for((int)n, (int)nv) * (MAX_M + 1) * 2 * 8);
+  Grid gq{};
+  gq.n = (int)n; gq.nv = (int)nv; gq.npts = npts; gq.field = field;
+  const size_t nblk = (size_t)zinv_ctas(gq);          // one Gram partial per zinv_residual CTA
+  const size_t ngrp = (nblk + 63) / 64;
+  char* gp = take(nblk * (MAX_M + 1) * 2 * 8);
+  char* gp2 = take(ngrp * (MAX_M + 1) * 2 * 8);
+  char* tk = take(ngrp * 4);
   char* fp = take((size_t)FE_BLOCKS * MAX_NV * 2 * 8);
   char* qv = take(MAX_NV * 8);
   char* rv = take(MAX_NV * 8);
@@ -108,7 +114,7 @@ static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_o
     b->state = (DevState*)st;
     b->Z = (double*)Z; b->R = (double*)R; b->tau = (double*)tau; b->w = (double*)w; b->work = (double2*)work;
     b->phi = (double*)phi; b->phik = (double2*)phik; b->chi_shell = (double*)chis; b->tw = (double2*)tw;
-    b->gram_part = (double*)gp; b->fe_part = (double*)fp; b->qv = (double*)qv; b->rhov = (double*)rv;
+    b->gram_part = (double*)gp; b->gram_part2 = (double*)gp2; b->tickets = (unsigned*)tk; b->n_tickets = ngrp; b->fe_part = (double*)fp; b->qv = (double*)qv; b->rhov = (double*)rv;
     b->scratch = (double*)work;
   }
   if (d_out) *d_out = (double*)out;
@@ -179,6 +185,7 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
   cudaError_t e = cudaMallocHost((void**)&ctx->h_hdr, sizeof(StateHeader));
   if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->b.tw, tw.data(), tw.size() * 8, cudaMemcpyHostToDevice, ctx->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(ctx->b.state, 0, sizeof(DevState), ctx->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(ctx->b.tickets, 0, ctx->b.n_tickets * sizeof(unsigned), ctx->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
   if (e != cudaSuccess) {
     if (ctx->h_hdr) cudaFreeHost(ctx->h_hdr);
@@ -230,6 +237,7 @@ extern "C" int rism3d_set_solvent_chi(rism3d_ctx* ctx, const double* q, const do
 
 static int reset_state(rism3d_ctx* ctx) {
   CU(cudaMemsetAsync(ctx->b.state, 0, sizeof(DevState), ctx->stream));
+  CU(cudaMemsetAsync(ctx->b.tickets, 0, ctx->b.n_tickets * sizeof(unsigned), ctx->stream));
   return RISM3D_OK;
 }
 
@@ -347,9 +355,7 @@ static int enqueue_iteration(rism3d_ctx* ctx) {
   prof_mark(ctx);
   k += launch_y_inv(g, b, true, s);                        // step 5
   prof_mark(ctx);
-  k += launch_zinv_residual(g, b, ctx->sp, nullptr, s);    // step 5 (z), Eq. 33
-  prof_mark(ctx);
-  k += launch_gram_row(g, b, ctx->sp, s);                  // step 6-7: Gram row, rms test, MDIIS solve
+  k += launch_zinv_residual(g, b, ctx->sp, nullptr, s);    // step 5 (z), Eq. 33, steps 6-7: Gram row, rms test, MDIIS solve
   prof_mark(ctx);                                          // (the update tau = sum c_i Z_i is applied by the next
                                                            //  closure_zfwd, or by iterate's trailing update pass)
   ctx->launches += k;
@@ -377,8 +383,7 @@ extern "C" int rism3d_get_timings(rism3d_ctx* ctx, double* ms_total, int cap, lo
 }
 
 extern "C" const char* rism3d_loop_kernel_name(int k) {
-  static const char* names[RISM3D_N_LOOP_KERNELS] = {"closure_zfwd", "y_fwd", "kspace_x", "y_inv", "zinv_residual",
-                                                     "gram_solve"};
+  static const char* names[RISM3D_N_LOOP_KERNELS] = {"closure_zfwd", "y_fwd", "kspace_x", "y_inv", "zinv_gram_solve"};
   return (k >= 0 && k < RISM3D_N_LOOP_KERNELS) ? names[k] : "";
 }
 

@@ -12,6 +12,7 @@
 // is a plain n/2-point complex FFT: no DC/Nyquist plane, same bytes as the real field.
 #include "async_copy.cuh"
 #include "fft_core.cuh"
+#include "mdiis_device.cuh"
 #include "rism3d_internal.h"
 
 namespace r3d {
@@ -192,7 +193,7 @@ constexpr int ZP = COLS + 1;
 // groups per CTA and resident CTAs per SM the kernel is compiled for (register cap), separately for closure_zfwd
 // (GF, MBF) and zinv_residual (GI, MBI).  The large lines run 3-pass plans of small radices: few registers per thread,
 // so that 768-1024 threads per SM hide the latency of the closure's exp() chains and of the streaming loads.
-template <int NZ> struct ZPlan : FftCfg<NZ> { enum { GF = FftCfg<NZ>::G, MBF = 1, GI = FftCfg<NZ>::G, MBI = 1 }; };
+template <int NZ> struct ZPlan : FftCfg<NZ> { enum { GF = FftCfg<NZ>::G, MBF = 1, GI = FftCfg<NZ>::G, MBI = 1, MBG = 1 }; };
 #ifndef R3D_ZGF
 #define R3D_ZGF 1
 #endif
@@ -205,9 +206,12 @@ template <int NZ> struct ZPlan : FftCfg<NZ> { enum { GF = FftCfg<NZ>::G, MBF = 1
 #ifndef R3D_ZMBI
 #define R3D_ZMBI 8
 #endif
-template <> struct ZPlan<64>  { enum { R1 = 8, R2 = 8, R3 = 1, T = 8, G = 4, GF = 4, MBF = 2, GI = 4, MBI = 2 }; };
-template <> struct ZPlan<128> { enum { R1 = 4, R2 = 4, R3 = 8, T = 16, G = 2, GF = R3D_ZGF, MBF = R3D_ZMBF, GI = R3D_ZGI, MBI = R3D_ZMBI }; };
-template <> struct ZPlan<256> { enum { R1 = 16, R2 = 16, R3 = 1, T = 16, G = 2, GF = 2, MBF = 2, GI = 2, MBI = 2 }; };
+#ifndef R3D_ZMBG
+#define R3D_ZMBG 5
+#endif
+template <> struct ZPlan<64>  { enum { R1 = 8, R2 = 8, R3 = 1, T = 8, G = 4, GF = 4, MBF = 2, GI = 4, MBI = 2, MBG = 2 }; };
+template <> struct ZPlan<128> { enum { R1 = 4, R2 = 4, R3 = 8, T = 16, G = 2, GF = R3D_ZGF, MBF = R3D_ZMBF, GI = R3D_ZGI, MBI = R3D_ZMBI, MBG = R3D_ZMBG }; };
+template <> struct ZPlan<256> { enum { R1 = 16, R2 = 16, R3 = 1, T = 16, G = 2, GF = 2, MBF = 2, GI = 2, MBI = 2, MBG = 2 }; };
 
 __device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
 __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
@@ -354,13 +358,35 @@ int launch_closure_zfwd(const Grid& g, const Buffers& b, const SolverParams& sp,
 // inverse z + residual.  One tile per CTA: inverse line FFTs in shared memory, the last stage leaves
 // (f_m, f_{m+n/2}) in place of complex element m, then a streaming phase with 16-byte accesses forms R = tau' - tau
 // (Eq. 33) and Z = tau + b R (the form Eq. 40 needs this entry in) and stores both into history slot `cur`.
-// The Gram row <R, R_i> is a separate streaming kernel (mdiis_kernels.cu: gram_row_kernel).
-template <int NZ, int G, int MINB>
+// MAXO >= 0: the Gram row <R, R_i> over the (at most MAXO = M - 1) stored residuals is accumulated in the streaming
+// phase as well, and the kernel ends with the partial-sum reduction and the MDIIS solve (mdiis_device.cuh).
+// MAXO = -1: transform only (debug hook, raw_out).
+struct GramArgs {
+  double* part1;
+  double* part2;
+  unsigned* tickets;
+  int M;
+  double restart;
+};
+
+template <int NZ, int G, int MINB, int MAXO>
 __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
     zinv_residual_kernel(const cplx* __restrict__ work, const double* __restrict__ tau_cur, double* __restrict__ Z,
                          double* __restrict__ R, double* __restrict__ raw_out, Twiddle tw_shift, Twiddle tw,
-                         const DevState* __restrict__ st, int nv, size_t npts, size_t field, double bdamp) {
+                         DevState* __restrict__ st, int nv, size_t npts, size_t field, double bdamp, GramArgs ga) {
   if (raw_out == nullptr && st->done) return;
+  constexpr bool GRAM = (MAXO >= 0);
+  constexpr int NACC = GRAM ? MAXO + 1 : 1;
+  __shared__ int s_other[MAX_M];
+  __shared__ int s_nother, s_m, s_flag;
+  __shared__ double s_row[MAX_M + 1];
+  if (GRAM && threadIdx.x == 0) {
+    const int m = st->m;
+    const int skip = (m == ga.M) ? 1 : 0;              // a full history drops its oldest entry this iteration
+    s_nother = m - skip;
+    s_m = m;
+    for (int i = 0; i < m - skip; ++i) s_other[i] = st->list[i + skip];
+  }
   using Cfg = ZPlan<NZ>;
   constexpr int T = Cfg::T, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS, n = 2 * NZ;
   constexpr int NT = T * G * C;
@@ -401,6 +427,10 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
   const double* Xc = tau_cur;
   double* Rc = raw_out ? nullptr : R + (size_t)cur * field;
   double* Zc = raw_out ? nullptr : Z + (size_t)cur * field;
+  const int nother = GRAM ? s_nother : 0;              // (written before the barriers of the transform)
+  double acc[NACC];
+#pragma unroll
+  for (int j = 0; j < NACC; ++j) acc[j] = 0.0;
 
   // streaming phase: thread <-> (site, line, pair of adjacent z points); 16-byte accesses, z fastest
   for (int e = tid; e < GL * nv * HP; e += NT) {
@@ -422,23 +452,100 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
       // Z = X + b R (Eq. 40 / Q7); mul and add rounded separately, as the oracle's X[i] + b*R[i]
       st2(Zc + off, make_double2(__dadd_rn(xlo.x, __dmul_rn(bdamp, rlo.x)), __dadd_rn(xlo.y, __dmul_rn(bdamp, rlo.y))));
       st2(Zc + off + NZ, make_double2(__dadd_rn(xhi.x, __dmul_rn(bdamp, rhi.x)), __dadd_rn(xhi.y, __dmul_rn(bdamp, rhi.y))));
+      if constexpr (GRAM) {
+        acc[MAXO] = fma(rlo.x, rlo.x, fma(rlo.y, rlo.y, fma(rhi.x, rhi.x, fma(rhi.y, rhi.y, acc[MAXO]))));
+#pragma unroll
+        for (int j = 0; j < MAXO; ++j)
+          if (j < nother) {
+            const double* Rj = R + (size_t)s_other[j] * field + off;
+            const double2 qlo = __ldcs(reinterpret_cast<const double2*>(Rj));
+            const double2 qhi = __ldcs(reinterpret_cast<const double2*>(Rj + NZ));
+            acc[j] = fma(rlo.x, qlo.x, fma(rlo.y, qlo.y, fma(rhi.x, qhi.x, fma(rhi.y, qhi.y, acc[j]))));
+          }
+      }
     }
+  }
+  if constexpr (GRAM) {
+    // per-thread fp64 sums (<= 64 elements each) -> double-double across the warp (fixed tree) and the warps
+    __syncthreads();                                   // the tile is dead: its memory holds the warp sums
+    double* s_part = reinterpret_cast<double*>(smem_dyn);
+    constexpr int NW = NT / 32;
+    const int lane = tid & 31, wid = tid >> 5;
+#pragma unroll
+    for (int j = 0; j <= MAXO; ++j) {
+      if (j < nother || j == MAXO) {
+        double hi = acc[j], lo = 0.0;
+        for (int o = 16; o > 0; o >>= 1) {
+          const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
+          dd_add(hi, lo, h2, l2);
+        }
+        if (lane == 0) {
+          s_part[(j * NW + wid) * 2] = hi;
+          s_part[(j * NW + wid) * 2 + 1] = lo;
+        }
+      }
+    }
+    __syncthreads();
+    if (tid <= MAXO && (tid < nother || tid == MAXO)) {
+      double hi = 0.0, lo = 0.0;
+      for (int w = 0; w < NW; ++w) dd_add(hi, lo, s_part[(tid * NW + w) * 2], s_part[(tid * NW + w) * 2 + 1]);
+      dd_norm(hi, lo);
+      const int j = (tid == MAXO) ? MAX_M : tid;
+      *reinterpret_cast<double2*>(ga.part1 + ((size_t)j * gridDim.x + blockIdx.x) * 2) = make_double2(hi, lo);
+      __threadfence();
+    }
+    gram_finish<NT>(st, ga.part1, ga.part2, ga.tickets, s_m, nother, ga.M, ga.restart, (double)field, s_row, &s_flag);
   }
 }
 
-template <int NZ>
-static int launch_zinv_n(const Grid& gr, const Buffers& b, const SolverParams& sp, double* raw_out, cudaStream_t s) {
+template <int NZ, int MAXO>
+static int launch_zinv_nm(const Grid& gr, const Buffers& b, const SolverParams& sp, double* raw_out, cudaStream_t s) {
   using Cfg = ZPlan<NZ>;
   constexpr int G = ZPlan<NZ>::GI;
+  constexpr int MB = (MAXO >= 0) ? ZPlan<NZ>::MBG : ZPlan<NZ>::MBI;
   const int LP = COLS / gr.nv, GL = G * LP;
   const int threads = Cfg::T * G * COLS;
-  const size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
-  auto kern = zinv_residual_kernel<NZ, G, ZPlan<NZ>::MBI>;
+  size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
+  const size_t red = (size_t)(MAX_M + 1) * (threads / 32 + 1) * 2 * sizeof(double);
+  if (shm < red) shm = red;
+  auto kern = zinv_residual_kernel<NZ, G, MB, MAXO>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
+  GramArgs ga{b.gram_part, b.gram_part2, b.tickets, sp.M, sp.restart};
   kern<<<(unsigned)((size_t)gr.n * gr.n / GL), threads, shm, s>>>(b.work, b.tau, b.Z, b.R, raw_out, tws, tw, b.state,
-                                                                   gr.nv, gr.npts, gr.field, sp.b);
+                                                                   gr.nv, gr.npts, gr.field, sp.b, ga);
   return 1;
+}
+
+// raw_out != nullptr: transform only; otherwise the variant compiled for M - 1 stored residuals
+template <int NZ>
+static int launch_zinv_n(const Grid& gr, const Buffers& b, const SolverParams& sp, double* raw_out, cudaStream_t s) {
+  if (raw_out) return launch_zinv_nm<NZ, -1>(gr, b, sp, raw_out, s);
+#define R3D_ZG(MO) case MO + 1: return launch_zinv_nm<NZ, MO>(gr, b, sp, raw_out, s)
+  switch (sp.M) {
+    R3D_ZG(0); R3D_ZG(1); R3D_ZG(2); R3D_ZG(3); R3D_ZG(4); R3D_ZG(5); R3D_ZG(6); R3D_ZG(7);
+    R3D_ZG(8); R3D_ZG(9); R3D_ZG(10); R3D_ZG(11); R3D_ZG(12); R3D_ZG(13); R3D_ZG(14); R3D_ZG(15);
+    default: return 0;
+  }
+#undef R3D_ZG
+}
+
+template <int NZ>
+static int zinv_ctas_n(const Grid& gr) {
+  const int LP = COLS / gr.nv, GL = ZPlan<NZ>::GI * LP;
+  return (int)((size_t)gr.n * gr.n / GL);
+}
+int zinv_ctas(const Grid& g) {
+  switch (g.n / 2) {
+    case 4: return zinv_ctas_n<4>(g);
+    case 8: return zinv_ctas_n<8>(g);
+    case 16: return zinv_ctas_n<16>(g);
+    case 32: return zinv_ctas_n<32>(g);
+    case 64: return zinv_ctas_n<64>(g);
+    case 128: return zinv_ctas_n<128>(g);
+    case 256: return zinv_ctas_n<256>(g);
+    default: return 0;
+  }
 }
 
 int launch_zinv_residual(const Grid& g, const Buffers& b, const SolverParams& sp, double* raw_out, cudaStream_t s) {

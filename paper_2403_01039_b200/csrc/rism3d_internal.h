@@ -27,7 +27,7 @@ struct DevState {
   int m;                       // filled history entries
   int cur;                     // physical history slot that receives the (Z, R) pair of the running iteration
   int upd_m;                   // entries to combine in the update kernel (0: skip)
-  unsigned ticket;             // CTAs of gram_row that have written their partial sums
+  unsigned ticket;             // first-level group adders of the Gram reduction that have finished
   double tol;
   double rms_last;
   double pad_[2];
@@ -65,7 +65,10 @@ struct Buffers {
   double2* phik;         // [n][n][n/2]  phi~(k) exp(+i k.r0) / dV
   double* chi_shell;     // [nshell][nv][nv]   chi_shell[s][g][g'] = chi_{g' g}(k_s)
   double2* tw;           // [2n]         exp(-i pi j / n)
-  double* gram_part;     // [MAX_M+1][gram_blocks][2]  double-double partial sums, one per gram_row CTA
+  double* gram_part;     // [MAX_M+1][gram_blocks][2]  double-double partial sums, one per zinv_residual CTA
+  double* gram_part2;    // [MAX_M+1][groups][2]  first-level sums of groups of 64 partials
+  unsigned* tickets;     // [groups] arrival counters of the partial-sum reduction (zero between launches)
+  size_t n_tickets;
   double* scratch;       // [field] temporary (get_field, setup tables); aliases `work`
   double* qv;            // [nv] solvent charges
   double* rhov;          // [nv]
@@ -93,10 +96,8 @@ int launch_x_inv(const Grid&, const Buffers&, cudaStream_t);
 int launch_kspace_x(const Grid&, const Buffers&, cudaStream_t);
 int launch_y_inv(const Grid&, const Buffers&, bool use_state, cudaStream_t);
 int launch_zinv_residual(const Grid&, const Buffers&, const SolverParams&, double* d_raw_out, cudaStream_t);
+int zinv_ctas(const Grid&);                      // CTAs of zinv_residual (it writes one Gram partial per CTA)
 // mdiis_kernels.cu
-int gram_blocks(const Grid&);
-int gram_blocks_for(int n, int nv);
-int launch_gram_row(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);
 int launch_mdiis_update(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);
 // setup_kernels.cu
 int launch_chi_shell(const Grid&, const Buffers&, const double* d_chi_table, int n_k, double k0, double dk,

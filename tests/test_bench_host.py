@@ -15,13 +15,13 @@ import bench  # noqa: E402
 
 
 def test_kernel_words_add_up_to_the_design_total():
-    # 2M + 13 + 1/n_v words per grid-point*site and iteration
+    # 2M + 12 + 1/n_v words per grid-point*site and iteration
     for n_v, M in [(2, 5), (4, 8), (4, 10)]:
         w = bench.kernel_words(n_v, M)
-        assert abs(sum(w.values()) - (2 * M + 13 + 1.0 / n_v)) < 1e-12
-        assert w["gram_solve"] == M and w["closure_zfwd"] == M + 3
+        assert abs(sum(w.values()) - (2 * M + 12 + 1.0 / n_v)) < 1e-12
+        assert w["zinv_gram_solve"] == M + 3 and w["closure_zfwd"] == M + 3
     names = list(bench.kernel_words(4, 10))
-    assert names == ["closure_zfwd", "y_fwd", "kspace_x", "y_inv", "zinv_residual", "gram_solve"]
+    assert names == ["closure_zfwd", "y_fwd", "kspace_x", "y_inv", "zinv_gram_solve"]
 
 
 def test_loop_kernel_names_match_the_library():
