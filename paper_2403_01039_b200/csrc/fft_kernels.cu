@@ -37,7 +37,11 @@ struct StridedCfg {
   enum { NT = FftCfg<N>::T * FftCfg<N>::G * COLS,                  // threads per CTA
          ITEM = FftCfg<N>::G * N * COLS,                             // complex elements per work item
          SHM = 2 * ITEM * (int)sizeof(cplx),
+#ifdef R3D_STRIDED_MINB
+         MINB = R3D_STRIDED_MINB };
+#else
          MINB = (SHM > 110 * 1024) ? 1 : 2 };      // <= 128 registers per thread: room for the cached twiddles
+#endif
 };
 
 // stage work item `item` (G tiles) into `buf` [G][N][COLS]

@@ -26,7 +26,11 @@ struct KspaceCfg {
          STAGE = ITEM + PHI,
          MIDT = (FftCfg<N>::R3 == 1) ? 0 : (N / FftCfg<N>::R1 / FftCfg<N>::R2) * FftCfg<N>::R2,   // mid-pass twiddle table
          SHM = (2 * STAGE + MIDT) * (int)sizeof(cplx),
+#ifdef R3D_KSPACE_MINB
+         MINB = R3D_KSPACE_MINB };
+#else
          MINB = (SHM > 110 * 1024) ? 1 : ((SHM > 72 * 1024) ? 2 : 3) };
+#endif
 };
 
 template <int N, int NV>

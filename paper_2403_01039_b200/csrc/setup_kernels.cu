@@ -209,8 +209,12 @@ int launch_phi_tilde(const Grid& g, const Buffers& b, const SolverParams& sp, in
                      double2* d_phase, cudaStream_t s) {
   const size_t total = (size_t)3 * n_atoms * g.n;
   const double4* at = reinterpret_cast<const double4*>(d_atoms);
-  phase_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(d_phase, at, n_atoms, g.n, g.h, g.origin[0],
-                                                              g.origin[1], g.origin[2]);
+  int launched = 1;
+  if (total > 0) {                                       // an empty solute has no phase table (phi~ = 0)
+    phase_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(d_phase, at, n_atoms, g.n, g.h, g.origin[0],
+                                                                g.origin[1], g.origin[2]);
+    launched = 2;
+  }
   // charges q_a live in a separate array right after the atom records (set up by the API layer)
   const double* qa = d_atoms + (size_t)4 * n_atoms;
   const int nz = g.n / 2;
@@ -218,7 +222,7 @@ int launch_phi_tilde(const Grid& g, const Buffers& b, const SolverParams& sp, in
   dim3 grid((nz + bx - 1) / bx, g.n / PT_JY, g.n);
   const double pref = 4.0 * 3.14159265358979323846 * sp.beta * COULOMB / (g.h * g.h * g.h);
   phi_tilde_kernel<<<grid, bx, 0, s>>>(b.phik, d_phase, qa, n_atoms, g.n, g.h, sp.kappa, pref);
-  return 2;
+  return launched;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -1,0 +1,160 @@
+"""-m gpu: edge and degenerate cases of the CUDA path against the oracle -- smallest grid, 1 and 8 site types, HNC,
+high PSE order, shifted origin, empty solute, MDIIS restart actually firing, M = 16, divergence reporting, warm
+start, and the split-call / trailing-update logic of rism3d_iterate."""
+import numpy as np
+import pytest
+
+from oracle import rism3d as o3
+from tests._gpu_util import make_pair
+from tests._util import synthetic_chi
+from workloads import Solute, Solvent, make_solute, water
+
+pytestmark = pytest.mark.gpu
+
+
+def _solvent(n_v, seed=0):
+    """made-up neutral solvent of n_v monatomic species (inputs only)"""
+    rng = np.random.default_rng(seed)
+    q = rng.uniform(-0.6, 0.6, n_v)
+    rho = rng.uniform(0.005, 0.02, n_v)
+    if n_v == 1:
+        q[:] = 0.0
+    else:
+        q[-1] = -np.dot(rho[:-1], q[:-1]) / rho[-1]          # sum rho q = 0
+    return Solvent(name=f"syn{n_v}", type_names=[f"S{i}" for i in range(n_v)], q=q, sigma=rng.uniform(2.5, 3.5, n_v),
+                   eps=rng.uniform(0.05, 0.2, n_v), rho=rho, mult=np.ones(n_v, int), site_type=np.arange(n_v),
+                   site_species=np.arange(n_v), species_rho=rho, bond=np.zeros((n_v, n_v)))
+
+
+def _small_solute(seed=1, n=3, charged=True):
+    rng = np.random.default_rng(seed)
+    xyz = rng.uniform(-1.5, 1.5, (n, 3))
+    q = rng.normal(0.0, 0.3, n) if charged else np.zeros(n)
+    return Solute("edge", xyz, q, rng.uniform(2.6, 3.4, n), rng.uniform(0.05, 0.2, n))
+
+
+@pytest.mark.parametrize("n_v,n", [(1, 16), (8, 16), (2, 8), (4, 8)])
+def test_site_counts_and_smallest_grids(n_v, n):
+    sv = _solvent(n_v, seed=n_v)
+    chi = synthetic_chi(n_v, sv.rho, n_k=900, dk=0.02, k0=0.02, seed=n_v, amp=0.5)
+    orc, gpu, _, _ = make_pair(n=n, spacing=0.9, solvent=sv, chi=chi, solute=_small_solute(), M=4)
+    orc.iterate(20, 0.0)
+    nd, rms = gpu.iterate(20, 0.0)
+    assert nd == 20 and abs(rms - orc.rms_history[-1]) <= 1e-9 * orc.rms_history[-1] + 1e-13
+    assert np.max(np.abs(gpu.get_field("G") - orc.get_field("G"))) <= 1e-9
+    mu_o, _ = orc.free_energy()
+    mu_g, _ = gpu.free_energy()
+    assert abs(mu_g - mu_o) <= 1e-9 * max(1.0, abs(mu_o))
+
+
+@pytest.mark.parametrize("closure,order", [("HNC", 1), ("PSE", 3), ("PSE", 7)])
+def test_other_closures(closure, order):
+    sol = _small_solute(seed=3, n=4)
+    sol = Solute("weak", sol.xyz, 0.3 * sol.q, sol.sigma, sol.eps)        # HNC: keep exp() tame
+    orc, gpu, _, _ = make_pair(n=32, spacing=0.5, solvent="water", closure=closure, pse_order=order, solute=sol, M=5)
+    orc.iterate(30, 0.0)
+    gpu.iterate(30, 0.0)
+    g, go = gpu.get_field("G"), orc.get_field("G")
+    assert np.max(np.abs(g - go) / np.maximum(1.0, go)) <= 1e-9
+    mu_o, _ = orc.free_energy()
+    mu_g, _ = gpu.free_energy()
+    assert abs(mu_g - mu_o) <= 1e-8 * max(1.0, abs(mu_o))
+
+
+def test_shifted_origin():
+    """origin not at -(n/2) dr and not a multiple of dr: only R_a - r0 enters (Q13)"""
+    orc, gpu, _, _ = make_pair(n=32, spacing=0.5, solvent="water", solute=_small_solute(seed=5),
+                               origin=(-7.3, -8.1, -8.65))
+    orc.iterate(20, 0.0)
+    gpu.iterate(20, 0.0)
+    assert np.max(np.abs(gpu.get_field("G") - orc.get_field("G"))) <= 1e-9
+    assert np.max(np.abs(gpu.get_field("PHI", 0) - orc.phi)) <= 1e-11 * np.max(np.abs(orc.phi))
+
+
+def test_empty_solute():
+    import paper_2403_01039_b200 as lib
+    from workloads import load_chi
+    sv = water()
+    k0, dk, chi = load_chi("water")
+    s = lib.Solver(16, 0.5, 2)
+    s.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+    s.set_solute(np.zeros((0, 3)), [], [], [])
+    nd, rms = s.iterate(2, 0.0)
+    assert nd == 2 and rms == 0.0 and np.all(s.get_field("G") == 1.0) and s.free_energy()[0] == 0.0
+    assert s.iterate(0, 0.0)[0] == 0                    # zero iterations is a valid request
+
+
+def test_restart_rule_fires_identically():
+    """restart factor 0.95: an iteration that improves on the best residual so far by less than 5 % collapses the
+    history to its best entry (Q8) -- the rule fires in some iterations and not in others, on both sides alike."""
+    sol = make_solute("C2")
+    kw = dict(n=32, spacing=0.5, solvent="water", solute=sol, M=6, b=0.5)
+    orc, gpu, _, _ = make_pair(restart=0.95, **kw)
+    ref, _, _, _ = make_pair(restart=0.0, **kw)
+    orc.iterate(40, 0.0)
+    ref.iterate(40, 0.0)
+    gpu.iterate(40, 0.0)
+    ho, hr = np.array(orc.rms_history), np.array(ref.rms_history)
+    first = int(np.argmax(np.abs(ho - hr) > 1e-12 * hr))
+    assert 2 <= first < 39                               # histories agree until the rule first fires, then part
+    np.testing.assert_allclose(gpu.rms_history(), ho, rtol=1e-7)
+    assert np.max(np.abs(gpu.get_field("G") - orc.get_field("G"))) <= 1e-9
+
+
+def test_mdiis_sixteen_vectors_and_no_restart():
+    orc, gpu, _, _ = make_pair("C1", n_override=32)
+    orc2, gpu2, _, _ = make_pair(n=32, spacing=0.5, solvent="water", solute=make_solute("C1"), M=16, b=0.4, restart=0.0)
+    orc2.iterate(40, 0.0)
+    gpu2.iterate(40, 0.0)
+    np.testing.assert_allclose(gpu2.rms_history(), orc2.rms_history, rtol=1e-5, atol=1e-13)
+    assert np.max(np.abs(gpu2.get_field("G") - orc2.get_field("G"))) <= 1e-9
+
+
+def test_split_calls_equal_one_call():
+    """The MDIIS update of an iteration rides on the next closure pass; the last one of a call is applied by a
+    trailing pass, so tau is current whenever iterate returns."""
+    sol = _small_solute(seed=7)
+    _, a, _, _ = make_pair(n=32, spacing=0.5, solvent="water", solute=sol)
+    _, b, _, _ = make_pair(n=32, spacing=0.5, solvent="water", solute=sol)
+    a.iterate(12, 0.0)
+    for k in (1, 4, 2, 5):
+        b.iterate(k, 0.0)
+    assert np.array_equal(a.rms_history(), b.rms_history())
+    assert np.array_equal(a.get_field("TAU"), b.get_field("TAU"))
+
+
+def test_converged_call_leaves_tau_and_reports_once():
+    orc, gpu, _, _ = make_pair("C1", n_override=32)
+    n1, r1 = gpu.iterate(500, 1e-7)
+    tau = gpu.get_field("TAU")
+    assert r1 < 1e-7 and n1 < 500
+    n2, r2 = gpu.iterate(500, 1e-7)                      # already converged: one more evaluation, nothing moves
+    assert n2 == 1 and r2 < 1e-7
+    assert np.array_equal(gpu.get_field("TAU"), tau)
+    no, ro = orc.iterate(500, 1e-7)
+    assert abs(no - n1) <= 1
+
+
+def test_divergence_is_reported():
+    import paper_2403_01039_b200 as lib
+    sol = Solute("hot", np.array([[0.1, 0.2, -0.1]]), np.array([6.0]), np.array([2.0]), np.array([0.1]))
+    _, gpu, _, _ = make_pair(n=16, spacing=0.5, solvent="water", closure="HNC", solute=sol, M=1, b=1.0, restart=0.0)
+    with pytest.raises(lib.Rism3dError) as e:
+        gpu.iterate(200, 0.0)
+    assert e.value.status == -8
+    assert len(gpu.rms_history()) < 200
+
+
+def test_warm_start_from_device_and_host():
+    sol = _small_solute(seed=9)
+    _, a, _, _ = make_pair(n=16, spacing=0.6, solvent="water", solute=sol)
+    _, b, _, _ = make_pair(n=16, spacing=0.6, solvent="water", solute=sol)
+    a.iterate(7, 0.0)
+    for s in range(2):
+        b.set_tau(s, a.get_field_device("TAU", s))
+    assert np.array_equal(a.get_field("TAU"), b.get_field("TAU"))
+    _, c, _, _ = make_pair(n=16, spacing=0.6, solvent="water", solute=sol)
+    for s in range(2):
+        c.set_tau(s, a.get_field("TAU", s))
+    # same input, empty history on both: the next iterate gives identical residuals
+    assert b.iterate(1, 0.0) == c.iterate(1, 0.0)
