@@ -58,6 +58,10 @@ typedef enum {
 
 typedef enum { RISM3D_KH = 1, RISM3D_PSE = 2, RISM3D_HNC = 3 } rism3d_closure;
 
+/* convergence accelerator: MDIIS with mdiis_nvec stored pairs (Eq. 40), or the paper's modified
+ * Anderson method with two histories (Eq. 34-39; three stored pairs, inner product weighted with 1/rho_g) */
+typedef enum { RISM3D_ACCEL_MDIIS = 0, RISM3D_ACCEL_ANDERSON = 1 } rism3d_accelerator;
+
 /* which-codes of rism3d_get_field */
 typedef enum {
   RISM3D_FIELD_G    = 0,   /* g = closure(w + tau)                                                 */
@@ -83,6 +87,9 @@ typedef struct {
   double kappa;             /* kappa of Eq. 29-30, 1/A (the paper: 1)                              */
   double r_min;             /* distance clamp of the short-range potential, A (Q11)      */
   int    device;            /* CUDA device ordinal                                                 */
+  int    accelerator;       /* rism3d_accelerator; ANDERSON ignores mdiis_nvec / mdiis_restart and uses
+                               mdiis_b as the mixing parameter b of Eq. 39                         */
+  double anderson_s[2];     /* tuning parameters s_1, s_2 of Eq. 34-35 (the paper's GPU code: 0.2, 0)      */
 } rism3d_params;
 
 /* Bytes of DEVICE memory the caller must provide to rism3d_init (0 if the parameters are invalid). */

@@ -278,6 +278,71 @@ class Mdiis:
 
 
 # ----------------------------------------------------------------------------------------------
+# Modified Anderson with two histories  (Eq. 34-39; reading Q17)
+# ----------------------------------------------------------------------------------------------
+def gram_weighted(a: np.ndarray, b: np.ndarray, w: np.ndarray) -> float:
+    """(a, b) = sum_gamma w_gamma sum_r a b  (Eq. 38; a, b are [gamma][...]), extended precision like gram()."""
+    tot = np.longdouble(0.0)
+    for g in range(a.shape[0]):
+        tot += np.longdouble(w[g]) * np.sum(a[g].astype(np.longdouble) * b[g].astype(np.longdouble), dtype=np.longdouble)
+    return float(tot)
+
+
+def anderson_theta(S: np.ndarray) -> np.ndarray:
+    """theta_1, theta_2 of Eq. 36, read as the normal equations of min |R0 - sum_j theta_j dR_j|^2 with
+    dR_j = R^(n-1) - R^(n-j-1):   sum_j (dR_i, dR_j) theta_j = (R0, dR_i),  i = 1, 2.
+    S is the 3x3 weighted Gram matrix of (R0 = newest, R1, R2).  2x2 solve by Cramer's rule on the system scaled by
+    its largest diagonal entry; a singular system gives theta = 0 (plain mixing)."""
+    A = [[0.0, 0.0], [0.0, 0.0]]
+    rhs = [0.0, 0.0]
+    for i in (1, 2):
+        rhs[i - 1] = S[0, 0] - S[0, i]
+        for j in (1, 2):
+            A[i - 1][j - 1] = S[0, 0] - S[0, i] - S[0, j] + S[i, j]
+    amax = max(A[0][0], A[1][1])
+    if not (amax > 0.0):
+        return np.zeros(2)
+    a, b_, c, d = A[0][0] / amax, A[0][1] / amax, A[1][0] / amax, A[1][1] / amax
+    r0, r1 = rhs[0] / amax, rhs[1] / amax
+    det = a * d - b_ * c
+    if det == 0.0:
+        return np.zeros(2)
+    return np.array([(r0 * d - b_ * r1) / det, (a * r1 - r0 * c) / det])
+
+
+class ModifiedAnderson:
+    """Two histories.  With X_k, R_k the inputs and residuals of the newest (k = 0) and the two previous (k = 1, 2)
+    evaluations, Y_k = X_k + R_k:
+        u = X_0 + sum_i (theta_i + s_i)(X_i - X_0)              Eq. 34
+        v = Y_0 + sum_i (theta_i + s_i)(Y_i - Y_0)              Eq. 35
+        X_new = u + b (v - u)                                   Eq. 39
+    Picard steps X + b R until two histories exist."""
+
+    def __init__(self, b: float, s, weights):
+        self.b, self.s, self.w = float(b), (float(s[0]), float(s[1])), np.asarray(weights, float)
+        self.X, self.R = [], []                    # newest first
+
+    def step(self, X: np.ndarray, R: np.ndarray, rms: float) -> np.ndarray:
+        self.X.insert(0, X)
+        self.R.insert(0, R)
+        del self.X[3:], self.R[3:]
+        if len(self.X) < 3:
+            return X + self.b * R
+        S = np.zeros((3, 3))
+        for i in range(3):
+            for j in range(i, 3):
+                S[i, j] = S[j, i] = gram_weighted(self.R[i], self.R[j], self.w)
+        th = anderson_theta(S)
+        u = self.X[0].copy()
+        v = self.X[0] + self.R[0]
+        for i in (1, 2):
+            a = th[i - 1] + self.s[i - 1]
+            u = u + a * (self.X[i] - self.X[0])
+            v = v + a * ((self.X[i] + self.R[i]) - (self.X[0] + self.R[0]))
+        return u + self.b * (v - u)
+
+
+# ----------------------------------------------------------------------------------------------
 # The solver
 # ----------------------------------------------------------------------------------------------
 class Rism3dOracle:
@@ -285,7 +350,8 @@ class Rism3dOracle:
     iterate / free_energy, plus get_field."""
 
     def __init__(self, n, spacing, n_sites, closure="KH", pse_order=1, temperature=298.0,
-                 mdiis_nvec=5, mdiis_b=0.5, mdiis_restart=10.0, kappa=1.0, r_min=1e-3, origin=None):
+                 mdiis_nvec=5, mdiis_b=0.5, mdiis_restart=10.0, kappa=1.0, r_min=1e-3, origin=None,
+                 accelerator="MDIIS", anderson_s=(0.2, 0.0)):
         self.n = (n, n, n) if np.isscalar(n) else tuple(n)
         self.dr = float(spacing)
         self.origin = tuple(-(m // 2) * self.dr for m in self.n) if origin is None else tuple(origin)
@@ -295,6 +361,7 @@ class Rism3dOracle:
         self.kT = K_BOLTZMANN * temperature
         self.M, self.b, self.restart = mdiis_nvec, mdiis_b, mdiis_restart
         self.kappa, self.r_min = float(kappa), float(r_min)
+        self.accelerator, self.anderson_s = accelerator, tuple(anderson_s)
         ax = [r_axis(m, self.dr, o) for m, o in zip(self.n, self.origin)]
         gx, gy, gz = np.meshgrid(*ax, indexing="ij")
         self.points = np.stack([gx.ravel(), gy.ravel(), gz.ravel()], axis=1)
@@ -328,7 +395,10 @@ class Rism3dOracle:
             self.minus_beta_u = -beta_u_at(self.points, xyz, q, sigma, eps, self.q_v, self.sig_v,
                                            self.eps_v, self.beta, self.r_min).reshape(shp)  # Eq. 22
         self.t = self.f.copy()                                                         # step 1
-        self.mdiis = Mdiis(self.M, self.b, self.restart)
+        if self.accelerator == "ANDERSON":          # weight 1/rho_gamma; b is the mixing parameter
+            self.mdiis = ModifiedAnderson(self.b, self.anderson_s, 1.0 / self.rho_v)
+        else:
+            self.mdiis = Mdiis(self.M, self.b, self.restart)
         self.rms_history = []
 
     # -- one pass of steps 2-5 ---------------------------------------------------------------

@@ -6,7 +6,7 @@ There is no CPU fallback: importing works anywhere, but creating a solver withou
 or without a CUDA device raises.
 """
 from .binding import (  # noqa: F401
-    CLOSURES, FIELDS, Rism3dError, Rism3dParams, Solver, library_path, load_library,
+    ACCELERATORS, CLOSURES, FIELDS, Rism3dError, Rism3dParams, Solver, library_path, load_library,
     rism3d_workspace_bytes, rism3d_init, rism3d_set_solvent_chi, rism3d_set_solute, rism3d_iterate,
     rism3d_free_energy, rism3d_get_field, rism3d_set_tau, rism3d_get_rms_history, rism3d_launch_count,
     rism3d_set_profiling, rism3d_get_timings, rism3d_loop_kernel_name, N_LOOP_KERNELS,

@@ -14,6 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = None
 
 CLOSURES = {"KH": 1, "PSE": 2, "HNC": 3}
+ACCELERATORS = {"MDIIS": 0, "ANDERSON": 1}
 FIELDS = {"G": 0, "H": 1, "C_SR": 2, "T": 3, "TAU": 4, "W": 5, "PHI": 6}
 
 EXPORTED_SYMBOLS = [
@@ -46,6 +47,8 @@ class Rism3dParams(C.Structure):
         ("kappa", C.c_double),
         ("r_min", C.c_double),
         ("device", C.c_int),
+        ("accelerator", C.c_int),
+        ("anderson_s", C.c_double * 2),
     ]
 
 
@@ -223,7 +226,8 @@ class Solver:
     """Owns the workspace tensor and the context; each method is one C-ABI call."""
 
     def __init__(self, n, spacing, n_sites, closure="KH", pse_order=1, temperature=298.0, mdiis_nvec=5,
-                 mdiis_b=0.5, mdiis_restart=10.0, kappa=1.0, r_min=1e-3, origin=None, device=0):
+                 mdiis_b=0.5, mdiis_restart=10.0, kappa=1.0, r_min=1e-3, origin=None, device=0,
+                 accelerator="MDIIS", anderson_s=(0.2, 0.0)):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2403_01039_b200 needs a CUDA device (no CPU fallback)")
@@ -244,6 +248,8 @@ class Solver:
         p.kappa = float(kappa)
         p.r_min = float(r_min)
         p.device = int(device)
+        p.accelerator = ACCELERATORS[accelerator]
+        p.anderson_s = (C.c_double * 2)(float(anderson_s[0]), float(anderson_s[1]))
         self.params = p
         nbytes = rism3d_workspace_bytes(p)
         if nbytes == 0:

@@ -22,7 +22,7 @@ struct rism3d_ctx {
   size_t ws_bytes;
   size_t scratch_bytes;      // bytes of the X..work span that set_* may use for uploads
   bool have_solvent, have_solute;
-  double qv[MAX_NV], sigv[MAX_NV], epsv[MAX_NV], rhov[MAX_NV];
+  double qv[MAX_NV], sigv[MAX_NV], epsv[MAX_NV], rhov[MAX_NV], gramw[MAX_NV];
   long long launches;
   bool profiling;            // per-kernel CUDA-event timing of the loop kernels (rism3d_set_profiling)
   std::vector<cudaEvent_t>* ev_pool;
@@ -76,14 +76,18 @@ static bool valid_params(const rism3d_params* p) {
   if (!(p->spacing > 0.0) || !(p->temperature > 0.0) || !(p->kappa > 0.0)) return false;
   if (p->closure != RISM3D_KH && p->closure != RISM3D_PSE && p->closure != RISM3D_HNC) return false;
   if (p->closure == RISM3D_PSE && p->pse_order < 1) return false;
+  if (p->accelerator != RISM3D_ACCEL_MDIIS && p->accelerator != RISM3D_ACCEL_ANDERSON) return false;
   return true;
 }
+
+// stored (input, residual) pairs: mdiis_nvec, or 3 for the modified Anderson method (the newest + two histories)
+static int effective_m(const rism3d_params* p) { return p->accelerator == RISM3D_ACCEL_ANDERSON ? 3 : p->mdiis_nvec; }
 
 static int n_shells(int n) { const int hn = n / 2; return 3 * (hn - 1) * hn / 2 + 1; }
 
 // carve the workspace; with base == nullptr only the total size is computed
 static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_out, size_t* scratch_bytes) {
-  const size_t n = p->nx, nv = p->n_sites, M = p->mdiis_nvec;
+  const size_t n = p->nx, nv = p->n_sites, M = (size_t)effective_m(p);
   const size_t npts = n * n * n, field = npts * nv;
   size_t off = 0;
   auto take = [&](size_t bytes) { char* ptr = base ? base + off : nullptr; off += align256(bytes); return ptr; };
@@ -109,12 +113,13 @@ static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_o
   char* fp = take((size_t)FE_BLOCKS * MAX_NV * 2 * 8);
   char* qv = take(MAX_NV * 8);
   char* rv = take(MAX_NV * 8);
+  char* gw = take(MAX_NV * 8);
   char* out = take(64 * 8);
   if (b) {
     b->state = (DevState*)st;
     b->Z = (double*)Z; b->R = (double*)R; b->tau = (double*)tau; b->w = (double*)w; b->work = (double2*)work;
     b->phi = (double*)phi; b->phik = (double2*)phik; b->chi_shell = (double*)chis; b->tw = (double2*)tw;
-    b->gram_part = (double*)gp; b->gram_part2 = (double*)gp2; b->tickets = (unsigned*)tk; b->n_tickets = ngrp; b->fe_part = (double*)fp; b->qv = (double*)qv; b->rhov = (double*)rv;
+    b->gram_part = (double*)gp; b->gram_part2 = (double*)gp2; b->tickets = (unsigned*)tk; b->n_tickets = ngrp; b->fe_part = (double*)fp; b->qv = (double*)qv; b->rhov = (double*)rv; b->gram_w = (double*)gw;
     b->scratch = (double*)work;
   }
   if (d_out) *d_out = (double*)out;
@@ -171,7 +176,9 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
   SolverParams& sp = ctx->sp;
   sp.closure = p->closure;
   sp.pse_order = p->closure == RISM3D_PSE ? p->pse_order : 1;
-  sp.M = p->mdiis_nvec; sp.b = p->mdiis_b; sp.restart = p->mdiis_restart;
+  sp.M = effective_m(p); sp.b = p->mdiis_b; sp.restart = p->mdiis_restart;
+  sp.accel = p->accelerator; sp.and_s1 = p->anderson_s[0]; sp.and_s2 = p->anderson_s[1];
+  if (sp.accel == RISM3D_ACCEL_ANDERSON) sp.restart = 0.0;   // the paper's method has no restart rule
   sp.kT = K_BOLTZMANN * p->temperature;
   sp.beta = 1.0 / sp.kT;
   sp.kappa = p->kappa; sp.r_min = p->r_min;
@@ -227,6 +234,9 @@ extern "C" int rism3d_set_solvent_chi(rism3d_ctx* ctx, const double* q, const do
   CU(cudaMemcpyAsync(d_table, chi, tbytes, cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaMemcpyAsync(ctx->b.qv, ctx->qv, g.nv * 8, cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaMemcpyAsync(ctx->b.rhov, ctx->rhov, g.nv * 8, cudaMemcpyHostToDevice, ctx->stream));
+  for (int i = 0; i < g.nv; ++i)                   // inner-product weights: 1/rho_g for the modified Anderson method (Eq. 38)
+    ctx->gramw[i] = ctx->sp.accel == RISM3D_ACCEL_ANDERSON ? 1.0 / rho[i] : 1.0;
+  CU(cudaMemcpyAsync(ctx->b.gram_w, ctx->gramw, g.nv * 8, cudaMemcpyHostToDevice, ctx->stream));
   ctx->launches += launch_chi_shell(g, ctx->b, d_table, n_k, k0, dk, ctx->stream);
   CU(cudaGetLastError());
   CU(cudaStreamSynchronize(ctx->stream));

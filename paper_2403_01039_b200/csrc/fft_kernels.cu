@@ -369,8 +369,9 @@ struct GramArgs {
   double* part1;
   double* part2;
   unsigned* tickets;
-  int M;
-  double restart;
+  const double* weight;  // [nv] weights of the inner product (all 1 unless weighted)
+  bool weighted;         // modified Anderson: (a, b) = sum_g (1/rho_g) sum_r a b  (Eq. 38)
+  AccelArgs aa;
 };
 
 template <int NZ, int G, int MINB, int MAXO>
@@ -383,10 +384,10 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
   constexpr int NACC = GRAM ? MAXO + 1 : 1;
   __shared__ int s_other[MAX_M];
   __shared__ int s_nother, s_m, s_flag;
-  __shared__ double s_row[MAX_M + 1];
+  __shared__ double s_row[MAX_M + 2];
   if (GRAM && threadIdx.x == 0) {
     const int m = st->m;
-    const int skip = (m == ga.M) ? 1 : 0;              // a full history drops its oldest entry this iteration
+    const int skip = (m == ga.aa.M) ? 1 : 0;              // a full history drops its oldest entry this iteration
     s_nother = m - skip;
     s_m = m;
     for (int i = 0; i < m - skip; ++i) s_other[i] = st->list[i + skip];
@@ -432,7 +433,7 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
   double* Rc = raw_out ? nullptr : R + (size_t)cur * field;
   double* Zc = raw_out ? nullptr : Z + (size_t)cur * field;
   const int nother = GRAM ? s_nother : 0;              // (written before the barriers of the transform)
-  double acc[NACC];
+  double acc[NACC], acc_u = 0.0;                        // acc_u: unweighted <R, R> of a weighted run (for the rms)
 #pragma unroll
   for (int j = 0; j < NACC; ++j) acc[j] = 0.0;
 
@@ -457,14 +458,18 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
       st2(Zc + off, make_double2(__dadd_rn(xlo.x, __dmul_rn(bdamp, rlo.x)), __dadd_rn(xlo.y, __dmul_rn(bdamp, rlo.y))));
       st2(Zc + off + NZ, make_double2(__dadd_rn(xhi.x, __dmul_rn(bdamp, rhi.x)), __dadd_rn(xhi.y, __dmul_rn(bdamp, rhi.y))));
       if constexpr (GRAM) {
-        acc[MAXO] = fma(rlo.x, rlo.x, fma(rlo.y, rlo.y, fma(rhi.x, rhi.x, fma(rhi.y, rhi.y, acc[MAXO]))));
+        // one side of every product carries the weight of this element's site (exactly 1 in an unweighted run)
+        const double wg = ga.weight[site];
+        const double2 vlo = make_double2(wg * rlo.x, wg * rlo.y), vhi = make_double2(wg * rhi.x, wg * rhi.y);
+        acc[MAXO] = fma(vlo.x, rlo.x, fma(vlo.y, rlo.y, fma(vhi.x, rhi.x, fma(vhi.y, rhi.y, acc[MAXO]))));
+        if (ga.weighted) acc_u = fma(rlo.x, rlo.x, fma(rlo.y, rlo.y, fma(rhi.x, rhi.x, fma(rhi.y, rhi.y, acc_u))));
 #pragma unroll
         for (int j = 0; j < MAXO; ++j)
           if (j < nother) {
             const double* Rj = R + (size_t)s_other[j] * field + off;
             const double2 qlo = __ldcs(reinterpret_cast<const double2*>(Rj));
             const double2 qhi = __ldcs(reinterpret_cast<const double2*>(Rj + NZ));
-            acc[j] = fma(rlo.x, qlo.x, fma(rlo.y, qlo.y, fma(rhi.x, qhi.x, fma(rhi.y, qhi.y, acc[j]))));
+            acc[j] = fma(vlo.x, qlo.x, fma(vlo.y, qlo.y, fma(vhi.x, qhi.x, fma(vhi.y, qhi.y, acc[j]))));
           }
       }
     }
@@ -476,9 +481,9 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
     constexpr int NW = NT / 32;
     const int lane = tid & 31, wid = tid >> 5;
 #pragma unroll
-    for (int j = 0; j <= MAXO; ++j) {
-      if (j < nother || j == MAXO) {
-        double hi = acc[j], lo = 0.0;
+    for (int j = 0; j <= MAXO + 1; ++j) {              // j = MAXO + 1: the unweighted self product
+      if (j < nother || j == MAXO || (j == MAXO + 1 && ga.weighted)) {
+        double hi = (j <= MAXO) ? acc[j < NACC ? j : 0] : acc_u, lo = 0.0;
         for (int o = 16; o > 0; o >>= 1) {
           const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
           dd_add(hi, lo, h2, l2);
@@ -490,15 +495,15 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
       }
     }
     __syncthreads();
-    if (tid <= MAXO && (tid < nother || tid == MAXO)) {
+    if (tid <= MAXO + 1 && (tid < nother || tid == MAXO || (tid == MAXO + 1 && ga.weighted))) {
       double hi = 0.0, lo = 0.0;
       for (int w = 0; w < NW; ++w) dd_add(hi, lo, s_part[(tid * NW + w) * 2], s_part[(tid * NW + w) * 2 + 1]);
       dd_norm(hi, lo);
-      const int j = (tid == MAXO) ? MAX_M : tid;
+      const int j = (tid < MAXO) ? tid : (tid == MAXO ? MAX_M : MAX_M - 1);
       *reinterpret_cast<double2*>(ga.part1 + ((size_t)j * gridDim.x + blockIdx.x) * 2) = make_double2(hi, lo);
       __threadfence();
     }
-    gram_finish<NT>(st, ga.part1, ga.part2, ga.tickets, s_m, nother, ga.M, ga.restart, (double)field, s_row, &s_flag);
+    gram_finish<NT>(st, ga.part1, ga.part2, ga.tickets, s_m, nother, ga.aa, ga.weighted, (double)field, s_row, &s_flag);
   }
 }
 
@@ -510,12 +515,13 @@ static int launch_zinv_nm(const Grid& gr, const Buffers& b, const SolverParams& 
   const int LP = COLS / gr.nv, GL = G * LP;
   const int threads = Cfg::T * G * COLS;
   size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
-  const size_t red = (size_t)(MAX_M + 1) * (threads / 32 + 1) * 2 * sizeof(double);
+  const size_t red = (size_t)(MAX_M + 2) * (threads / 32 + 1) * 2 * sizeof(double);
   if (shm < red) shm = red;
   auto kern = zinv_residual_kernel<NZ, G, MB, MAXO>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
-  GramArgs ga{b.gram_part, b.gram_part2, b.tickets, sp.M, sp.restart};
+  GramArgs ga{b.gram_part, b.gram_part2, b.tickets, b.gram_w, sp.accel == RISM3D_ACCEL_ANDERSON,
+              AccelArgs{sp.M, sp.restart, sp.accel, sp.and_s1, sp.and_s2}};
   kern<<<(unsigned)((size_t)gr.n * gr.n / GL), threads, shm, s>>>(b.work, b.tau, b.Z, b.R, raw_out, tws, tw, b.state,
                                                                    gr.nv, gr.npts, gr.field, sp.b, ga);
   return 1;

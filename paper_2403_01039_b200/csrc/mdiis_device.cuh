@@ -11,11 +11,22 @@ constexpr int GRAM_GROUP = 64;       // CTAs per first-level group of the partia
 
 // History bookkeeping and the small solve, run by ONE thread (the last gram_row CTA) once the Gram row s_row
 // (entries 0..nother-1: <R_new, R_other[j]>, entry nother: <R_new, R_new>) is complete.
-static __device__ __noinline__ void mdiis_bookkeeping_and_solve(DevState* __restrict__ st, const double* s_row, int m_old, int nother,
-                                            int M, double restart, double npts_total) {
+// accelerator settings handed to the kernels that finish a Gram row
+struct AccelArgs {
+  int M;                 // stored pairs (modified Anderson: 3 = the newest + two histories)
+  double restart;        // MDIIS restart factor (<= 0: never)
+  int accel;             // rism3d_accelerator
+  double s1, s2;         // tuning parameters of Eq. 34-35
+};
+
+static __device__ __noinline__ void mdiis_bookkeeping_and_solve(DevState* __restrict__ st, const double* s_row, int m_old,
+                                                                int nother, AccelArgs aa, double self_unweighted,
+                                                                double npts_total) {
+  const int M = aa.M;
+  const double restart = aa.restart;
   const int skip = (m_old == M) ? 1 : 0;
   const double self = s_row[nother];
-  const double rms = sqrt(self / npts_total);          // Eq. 41 (Q9)
+  const double rms = sqrt(self_unweighted / npts_total);   // Eq. 41 (Q9): always the unweighted sum
   st->rms_last = rms;
   st->n_done += 1;
   st->rms_hist[st->hist_n % RMS_HIST_CAP] = rms;
@@ -62,7 +73,33 @@ static __device__ __noinline__ void mdiis_bookkeeping_and_solve(DevState* __rest
   for (int i = 0; i < m; ++i) c[i] = (i == m - 1) ? 1.0 : 0.0;     // fallback: unit vector on the newest entry
   double smax = st->S[0][0];
   for (int i = 1; i < m; ++i) smax = fmax(smax, st->S[i][i]);
-  if (smax > 0.0) {
+  if (aa.accel == RISM3D_ACCEL_ANDERSON) {
+    // Modified Anderson, two histories (Eq. 34-39).  Entries: newest = m-1 (R0), m-2 (R1), m-3 (R2).  theta from the
+    // normal equations of min |R0 - sum_j theta_j dR_j|^2, dR_j = R0 - Rj (Eq. 36); with a_i = theta_i + s_i,
+    //   X_new = u + b (v - u) = (1 - a1 - a2)(X0 + b R0) + a1 (X1 + b R1) + a2 (X2 + b R2) = sum_k c_k Z_k.
+    // Picard steps (unit vector on the newest Z) until two histories exist.
+    if (m == 3) {
+      const double s00 = st->S[2][2], s01 = st->S[2][1], s02 = st->S[2][0], s11 = st->S[1][1], s12 = st->S[1][0],
+                   s22 = st->S[0][0];
+      double a11 = s00 - s01 - s01 + s11, a12 = s00 - s01 - s02 + s12, a22 = s00 - s02 - s02 + s22;
+      double r1 = s00 - s01, r2 = s00 - s02;
+      const double amax = fmax(a11, a22);
+      double th1 = 0.0, th2 = 0.0;
+      if (amax > 0.0) {
+        a11 /= amax; a12 /= amax; a22 /= amax; r1 /= amax; r2 /= amax;
+        // Cramer's rule, products and differences rounded separately (as the oracle's Python expression)
+        const double det = __dsub_rn(__dmul_rn(a11, a22), __dmul_rn(a12, a12));
+        if (det != 0.0) {
+          th1 = __dsub_rn(__dmul_rn(r1, a22), __dmul_rn(a12, r2)) / det;
+          th2 = __dsub_rn(__dmul_rn(a11, r2), __dmul_rn(r1, a12)) / det;
+        }
+      }
+      const double a1 = th1 + aa.s1, a2 = th2 + aa.s2;
+      c[2] = 1.0 - a1 - a2;
+      c[1] = a1;
+      c[0] = a2;
+    }
+  } else if (smax > 0.0) {
     const int n = m + 1;
     double A[MAX_M + 1][MAX_M + 2];
     for (int i = 0; i < n; ++i)
@@ -137,8 +174,14 @@ static __device__ __forceinline__ void warp_sum_partials(const double* part, int
 template <int NT>
 static __device__ __forceinline__ void gram_finish(DevState* __restrict__ st, double* __restrict__ part1,
                                                    double* __restrict__ part2, unsigned* __restrict__ tickets,
-                                                   int m_old, int nother, int M, double restart, double npts_total,
-                                                   double* s_row /* shared, MAX_M + 1 */, int* s_flag /* shared */) {
+                                                   int m_old, int nother, AccelArgs aa, bool weighted,
+                                                   double npts_total, double* s_row /* shared, MAX_M + 2 */,
+                                                   int* s_flag /* shared */) {
+  // entries: jj < nother: <R_new, R_other[jj]> (slot jj); jj = nother: <R_new, R_new> (slot MAX_M); and, when the
+  // inner product is weighted, jj = nother + 1: the unweighted <R_new, R_new> for the rms (slot MAX_M - 1, free
+  // because a weighted run stores at most 3 pairs)
+  const int nent = nother + (weighted ? 2 : 1);
+  auto slot = [&](int jj) { return jj < nother ? jj : (jj == nother ? MAX_M : MAX_M - 1); };
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   constexpr int NW = NT / 32;
   const int nblk = (int)gridDim.x, ngroups = (nblk + GRAM_GROUP - 1) / GRAM_GROUP;
@@ -149,8 +192,8 @@ static __device__ __forceinline__ void gram_finish(DevState* __restrict__ st, do
   __syncthreads();
   if (!*s_flag) return;
   __threadfence();
-  for (int jj = wid; jj <= nother; jj += NW) {         // level 1: this group's partials, one warp per entry
-    const int j = (jj == nother) ? MAX_M : jj;
+  for (int jj = wid; jj < nent; jj += NW) {            // level 1: this group's partials, one warp per entry
+    const int j = slot(jj);
     double hi, lo;
     warp_sum_partials(part1 + ((size_t)j * nblk + (size_t)grp * GRAM_GROUP) * 2, gsize, lane, hi, lo);
     if (lane == 0) {
@@ -167,8 +210,8 @@ static __device__ __forceinline__ void gram_finish(DevState* __restrict__ st, do
   __syncthreads();
   if (!*s_flag) return;
   __threadfence();
-  for (int jj = wid; jj <= nother; jj += NW) {         // level 2: the group sums
-    const int j = (jj == nother) ? MAX_M : jj;
+  for (int jj = wid; jj < nent; jj += NW) {            // level 2: the group sums
+    const int j = slot(jj);
     double hi, lo;
     warp_sum_partials(part2 + (size_t)j * ngroups * 2, ngroups, lane, hi, lo);
     if (lane == 0) s_row[jj] = hi + lo;
@@ -176,7 +219,7 @@ static __device__ __forceinline__ void gram_finish(DevState* __restrict__ st, do
   __syncthreads();
   if (tid != 0) return;
   st->ticket = 0;
-  mdiis_bookkeeping_and_solve(st, s_row, m_old, nother, M, restart, npts_total);
+  mdiis_bookkeeping_and_solve(st, s_row, m_old, nother, aa, weighted ? s_row[nother + 1] : s_row[nother], npts_total);
 }
 
 }  // namespace r3d

@@ -72,6 +72,7 @@ struct Buffers {
   double* scratch;       // [field] temporary (get_field, setup tables); aliases `work`
   double* qv;            // [nv] solvent charges
   double* rhov;          // [nv]
+  double* gram_w;        // [nv] weights of the inner product: 1 (MDIIS) or 1/rho_g (modified Anderson, Eq. 38)
   double* fe_part;       // [FE_BLOCKS][MAX_NV][2]
 };
 
@@ -82,6 +83,8 @@ struct SolverParams {
   double b;
   double restart;
   double beta, kT, kappa, r_min;
+  int accel;             // rism3d_accelerator (ANDERSON: M = 3 stored pairs = the newest + two histories)
+  double and_s1, and_s2; // tuning parameters of Eq. 34-35
 };
 
 // api.cu: per_sm * number of SMs of the device the context lives on (grid size of the persistent kernels)

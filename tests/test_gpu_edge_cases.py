@@ -158,3 +158,34 @@ def test_warm_start_from_device_and_host():
         c.set_tau(s, a.get_field("TAU", s))
     # same input, empty history on both: the next iterate gives identical residuals
     assert b.iterate(1, 0.0) == c.iterate(1, 0.0)
+
+
+# ---- NEXT-1: the paper's modified Anderson accelerator (Eq. 34-39) -------------------------------------------
+@pytest.mark.parametrize("cfg,n,b,s", [("C1", 32, 0.6, (0.2, 0.0)), ("C2", 32, 0.4, (0.2, 0.0)), ("C2", 32, 0.5, (0.1, 0.05))])
+def test_modified_anderson_fifty_iterations(cfg, n, b, s):
+    sol = make_solute(cfg)
+    orc, gpu, _, _ = make_pair(n=n, spacing=0.5, solvent="water", solute=sol, b=b, accelerator="ANDERSON", anderson_s=s)
+    orc.iterate(50, 0.0)
+    nd, rms = gpu.iterate(50, 0.0)
+    assert nd == 50
+    np.testing.assert_allclose(gpu.rms_history(), orc.rms_history, rtol=1e-6, atol=1e-13)
+    assert np.max(np.abs(gpu.get_field("G") - orc.get_field("G"))) <= 1e-9
+
+
+def test_modified_anderson_four_sites_converges_to_the_mdiis_fixed_point():
+    sol = make_solute("C3")
+    keep = np.argsort(np.linalg.norm(sol.xyz, axis=1))[:40]
+    sub = Solute("C3_sub40", sol.xyz[keep], sol.q[keep], sol.sigma[keep], sol.eps[keep])
+    kw = dict(n=32, spacing=0.75, solvent="water_nacl_0.1M", closure="PSE", pse_order=2, solute=sub)
+    orc, gpu, _, _ = make_pair(b=0.5, accelerator="ANDERSON", **kw)
+    _, ref, _, _ = make_pair(M=8, b=0.5, **kw)
+    no, ro = orc.iterate(3000, 1e-9)
+    ng, rg = gpu.iterate(3000, 1e-9)
+    nr, rr = ref.iterate(3000, 1e-9)
+    # (300 iterations amplify rounding differences: the two paths cross the threshold a few iterations apart)
+    assert ro < 1e-9 and rg < 1e-9 and rr < 1e-9 and abs(ng - no) <= 0.1 * no
+    mu_o, mu_g, mu_r = orc.free_energy()[0], gpu.free_energy()[0], ref.free_energy()[0]
+    assert abs(mu_g - mu_o) <= 1e-7 * abs(mu_o)
+    assert abs(mu_g - mu_r) <= 1e-6 * abs(mu_r)          # the fixed point does not depend on the accelerator
+    gg, gr = gpu.get_field("G"), ref.get_field("G")      # (slowly converging case: rms 1e-9 leaves ~1e-6 in g)
+    assert np.max(np.abs(gg - gr) / np.maximum(1.0, gr)) <= 1e-5

@@ -422,3 +422,76 @@ def test_p7_accelerator_independence_and_p11_threshold_protocol():
     # log-linear decay: rms falls by orders of magnitude, monotone on a coarse scale
     h = orc.rms_history
     assert h[-1] < 1e-3 * h[0]
+
+
+# ------------------------------------------------------------------------------------------------
+# Modified Anderson (Eq. 34-39; Q17)
+# ------------------------------------------------------------------------------------------------
+def test_anderson_two_histories_is_exact_on_a_2d_affine_map():
+    """Textbook property: Anderson mixing with m histories solves a linear fixed-point problem of dimension m exactly
+    at step m + 1 (s = 0, b = 1 is the original method)."""
+    rng = np.random.default_rng(0)
+    A = rng.uniform(-0.4, 0.4, (2, 2))
+    y0 = rng.standard_normal(2)
+    exact = np.linalg.solve(np.eye(2) - A, y0)
+    acc = o3.ModifiedAnderson(1.0, (0.0, 0.0), np.ones(1))
+    X = np.zeros((1, 2))
+    errs = []
+    for _ in range(4):
+        R = (A @ X[0] + y0)[None] - X
+        errs.append(np.abs(X[0] - exact).max())
+        X = acc.step(X, R, 0.0)
+    assert errs[2] > 1e-3 and errs[3] < 1e-13
+    # the first two steps are Picard steps X + b R (PAPER.md:298)
+    acc = o3.ModifiedAnderson(0.6, (0.2, 0.0), np.ones(1))
+    X0 = np.array([[0.3, -0.1]])
+    R0 = np.array([[0.5, 0.25]])
+    assert np.allclose(acc.step(X0, R0, 0.0), X0 + 0.6 * R0)
+
+
+def test_anderson_theta_solves_the_least_squares_problem_and_uses_the_weights():
+    rng = np.random.default_rng(3)
+    R = rng.standard_normal((3, 2, 50))                  # R0, R1, R2 as [gamma][r]
+    w = np.array([1.0 / 0.0334, 1.0 / 0.0668])
+    S = np.array([[o3.gram_weighted(R[i], R[j], w) for j in range(3)] for i in range(3)])
+    th = o3.anderson_theta(S)
+    # brute force: minimise sum_g w_g |R0 - th1 (R0 - R1) - th2 (R0 - R2)|^2 with a library least-squares routine
+    sw = np.sqrt(w)[:, None]
+    D = np.stack([((R[0] - R[1]) * sw).ravel(), ((R[0] - R[2]) * sw).ravel()], axis=1)
+    ref = np.linalg.lstsq(D, (R[0] * sw).ravel(), rcond=None)[0]
+    assert np.allclose(th, ref, rtol=1e-10)
+    assert not np.allclose(th, o3.anderson_theta(np.array([[o3.gram(R[i], R[j]) for j in range(3)] for i in range(3)])))
+    assert np.all(o3.anderson_theta(np.zeros((3, 3))) == 0.0)
+
+
+def test_anderson_update_is_the_combination_of_z_entries():
+    """Eq. 34-39 collapse to X_new = (1 - a1 - a2) Z0 + a1 Z1 + a2 Z2 with Z_k = X_k + b R_k, a_i = theta_i + s_i --
+    the form the CUDA path uses."""
+    rng = np.random.default_rng(5)
+    b, s = 0.6, (0.2, 0.05)
+    acc = o3.ModifiedAnderson(b, s, np.array([2.0, 0.5]))
+    Xs = [rng.standard_normal((2, 30)) for _ in range(3)]
+    Rs = [rng.standard_normal((2, 30)) for _ in range(3)]
+    for X, R in zip(Xs[:2], Rs[:2]):
+        acc.step(X, R, 0.0)
+    out = acc.step(Xs[2], Rs[2], 0.0)
+    S = np.array([[o3.gram_weighted(Rs[2 - i], Rs[2 - j], acc.w) for j in range(3)] for i in range(3)])
+    a = o3.anderson_theta(S) + np.array(s)
+    Z = [Xs[2 - k] + b * Rs[2 - k] for k in range(3)]
+    assert np.allclose(out, (1 - a[0] - a[1]) * Z[0] + a[0] * Z[1] + a[1] * Z[2], rtol=1e-12, atol=1e-12)
+
+
+def test_anderson_reaches_the_same_fixed_point_as_mdiis():
+    sv = water()
+    k0, dk, chi = synthetic_chi(2, sv.rho)
+    sol = make_solute("C1")
+    res = []
+    for kw in (dict(mdiis_nvec=5), dict(accelerator="ANDERSON", mdiis_b=0.6, anderson_s=(0.2, 0.0))):
+        orc = o3.Rism3dOracle(16, 0.6, 2, **kw)
+        orc.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+        orc.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps)
+        n, rms = orc.iterate(2000, 1e-10)
+        assert rms < 1e-10
+        res.append((orc.get_field("G"), orc.free_energy()[0]))
+    assert np.max(np.abs(res[0][0] - res[1][0])) < 1e-8
+    assert abs(res[0][1] - res[1][1]) < 1e-8 * abs(res[0][1])
