@@ -128,6 +128,13 @@ int rism3d_iterate(rism3d_ctx* ctx, int max_iter, double tol, int* n_done, doubl
  * kcal/mol.  dmu_site: HOST [n_sites] or NULL. */
 int rism3d_free_energy(rism3d_ctx* ctx, double* dmu_total, double* dmu_site);
 
+/* Partial molar volume of the solute (Eq. 19), A^3:
+ *   V = k_B T chi_T (1 - sum_g rho_g int c_g(r) dr),
+ * chi_t = isothermal compressibility of the pure solvent in A^3 mol/kcal (it comes from the solvent's own RISM
+ * solve, like chi).  Plain grid sum; the long-range part -q_g phi(r) of c_g drops out of the density-weighted sum by
+ * neutrality, so only c_sr enters.  c_int_site (HOST [n_sites] or NULL) receives dV sum_r c_sr,g(r) in A^3. */
+int rism3d_pmv(rism3d_ctx* ctx, double chi_t, double* pmv, double* c_int_site);
+
 /* Copy one field of one site (nx*ny*nz doubles, [ix][iy][iz]) to dst; dst_is_device selects a
  * DEVICE or HOST destination. */
 int rism3d_get_field(rism3d_ctx* ctx, int which, int site, double* dst, int dst_is_device);

@@ -1,7 +1,8 @@
 """O-3D: the 3D-RISM self-consistent loop, step by step, in plain numpy float64.
 
 TEST INFRASTRUCTURE (see oracle/__init__.py).  Follows PAPER.md:222-254 (numerical procedure),
-PAPER.md:300-310 (MDIIS), PAPER.md:374-379 (residual) in the paper's own variable t = h - c, with
+PAPER.md:300-310 (MDIIS), PAPER.md:264-298 (modified Anderson), PAPER.md:374-379 (residual), PAPER.md:148-158 (free
+energy, partial molar volume) in the paper's own variable t = h - c, with
 the readings Q1..Q16 listed in DESIGN.md (the paper prints the KH branches, Eq. 40 and Eq. 41 in
 garbled form).  Nothing here is blocked, fused or reordered: every array op is one line of a
 formula.  Arrays are indexed [gamma][ix][iy][iz].
@@ -458,3 +459,12 @@ class Rism3dOracle:
                              float(np.sum(integrand[gam], dtype=np.longdouble))
                              for gam in range(self.n_v)])
         return float(per_site.sum()), per_site
+
+    def pmv(self, chi_t):
+        """Partial molar volume, Eq. 19:  V = kT chi_T (1 - sum_gamma rho_gamma int c_gamma dr), plain
+        grid sum.  The long-range part -f_gamma of c drops out of the density-weighted sum (sum rho q = 0), as in the
+        free energy (Q10).  Returns (V in A^3, per-site dV sum_r c_sr)."""
+        _, _, c_sr = self.closure_step(self.t)
+        c_int = np.array([self.dr ** 3 * float(np.sum(c_sr[gam], dtype=np.longdouble)) for gam in range(self.n_v)])
+        return float(self.kT * chi_t * (1.0 - np.dot(self.rho_v, c_int))), c_int
+

@@ -19,7 +19,7 @@ FIELDS = {"G": 0, "H": 1, "C_SR": 2, "T": 3, "TAU": 4, "W": 5, "PHI": 6}
 
 EXPORTED_SYMBOLS = [
     "rism3d_workspace_bytes", "rism3d_init", "rism3d_set_solvent_chi", "rism3d_set_solute",
-    "rism3d_iterate", "rism3d_free_energy", "rism3d_get_field", "rism3d_set_tau",
+    "rism3d_iterate", "rism3d_free_energy", "rism3d_pmv", "rism3d_get_field", "rism3d_set_tau",
     "rism3d_get_rms_history", "rism3d_launch_count", "rism3d_set_profiling", "rism3d_get_timings",
     "rism3d_loop_kernel_name", "rism3d_debug_fft_forward",
     "rism3d_debug_fft_inverse", "rism3d_last_error", "rism3d_status_string", "rism3d_destroy",
@@ -79,6 +79,8 @@ def load_library():
     lib.rism3d_iterate.argtypes = [C.c_void_p, C.c_int, C.c_double, ip, dp]
     lib.rism3d_free_energy.restype = C.c_int
     lib.rism3d_free_energy.argtypes = [C.c_void_p, dp, dp]
+    lib.rism3d_pmv.restype = C.c_int
+    lib.rism3d_pmv.argtypes = [C.c_void_p, C.c_double, dp, dp]
     lib.rism3d_get_field.restype = C.c_int
     lib.rism3d_get_field.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]
     lib.rism3d_set_tau.restype = C.c_int
@@ -169,6 +171,14 @@ def rism3d_free_energy(ctx, n_sites: int):
     site = np.zeros(n_sites)
     _check(ctx, load_library().rism3d_free_energy(ctx, C.byref(tot), _dptr(site)))
     return float(tot.value), site
+
+
+def rism3d_pmv(ctx, chi_t: float, n_sites: int):
+    """-> (pmv in A^3, per-site integrals of c_sr in A^3)"""
+    v = C.c_double(0.0)
+    site = np.zeros(n_sites)
+    _check(ctx, load_library().rism3d_pmv(ctx, float(chi_t), C.byref(v), _dptr(site)))
+    return float(v.value), site
 
 
 def rism3d_get_field(ctx, which: int, site: int, dst_ptr: int, dst_is_device: bool):
@@ -281,6 +291,9 @@ class Solver:
 
     def free_energy(self):
         return rism3d_free_energy(self.ctx, self.n_sites)
+
+    def pmv(self, chi_t: float):
+        return rism3d_pmv(self.ctx, chi_t, self.n_sites)
 
     def get_field(self, which: str, site=None) -> np.ndarray:
         """Host copy: [n][n][n] for one site, or [n_sites][n][n][n] when site is None."""

@@ -110,7 +110,7 @@ static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_o
   char* gp = take(nblk * (MAX_M + 1) * 2 * 8);
   char* gp2 = take(ngrp * (MAX_M + 1) * 2 * 8);
   char* tk = take(ngrp * 4);
-  char* fp = take((size_t)FE_BLOCKS * MAX_NV * 2 * 8);
+  char* fp = take((size_t)2 * FE_BLOCKS * MAX_NV * 2 * 8);
   char* qv = take(MAX_NV * 8);
   char* rv = take(MAX_NV * 8);
   char* gw = take(MAX_NV * 8);
@@ -447,6 +447,24 @@ extern "C" int rism3d_free_energy(rism3d_ctx* ctx, double* dmu_total, double* dm
     if (dmu_site) dmu_site[i] = host[i];
   }
   *dmu_total = tot;
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_pmv(rism3d_ctx* ctx, double chi_t, double* pmv, double* c_int_site) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (!pmv) return fail(ctx, RISM3D_ERR_ARG, "pmv is NULL");
+  if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before pmv");
+  ctx->launches += launch_free_energy(ctx->g, ctx->b, ctx->sp, ctx->d_out, ctx->stream);
+  CU(cudaGetLastError());
+  double host[2 * MAX_NV];
+  CU(cudaMemcpyAsync(host, ctx->d_out, 2 * MAX_NV * 8, cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  double sum = 0.0;                                  // sum_g rho_g int c_g dr: the -q_g phi part drops out (sum rho q = 0)
+  for (int i = 0; i < ctx->g.nv; ++i) {
+    sum += ctx->rhov[i] * host[MAX_NV + i];
+    if (c_int_site) c_int_site[i] = host[MAX_NV + i];
+  }
+  *pmv = ctx->sp.kT * chi_t * (1.0 - sum);           // Eq. 19
   return RISM3D_OK;
 }
 

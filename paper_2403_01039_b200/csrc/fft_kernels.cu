@@ -215,7 +215,26 @@ template <int NZ> struct ZPlan : FftCfg<NZ> { enum { GF = FftCfg<NZ>::G, MBF = 1
 #endif
 template <> struct ZPlan<64>  { enum { R1 = 8, R2 = 8, R3 = 1, T = 8, G = 4, GF = 4, MBF = 2, GI = 4, MBI = 2, MBG = 2 }; };
 template <> struct ZPlan<128> { enum { R1 = 4, R2 = 4, R3 = 8, T = 16, G = 2, GF = R3D_ZGF, MBF = R3D_ZMBF, GI = R3D_ZGI, MBI = R3D_ZMBI, MBG = R3D_ZMBG }; };
-template <> struct ZPlan<256> { enum { R1 = 16, R2 = 16, R3 = 1, T = 16, G = 2, GF = 2, MBF = 2, GI = 2, MBI = 2, MBG = 2 }; };
+#ifndef R3D_Z256_PLAN
+#define R3D_Z256_PLAN 0
+#endif
+#ifndef R3D_Z256_GF
+#define R3D_Z256_GF 2
+#endif
+#ifndef R3D_Z256_MBF
+#define R3D_Z256_MBF 2
+#endif
+#ifndef R3D_Z256_GI
+#define R3D_Z256_GI 2
+#endif
+#ifndef R3D_Z256_MBG
+#define R3D_Z256_MBG 2
+#endif
+#if R3D_Z256_PLAN == 0
+template <> struct ZPlan<256> { enum { R1 = 16, R2 = 16, R3 = 1, T = 16, G = 2, GF = R3D_Z256_GF, MBF = R3D_Z256_MBF, GI = R3D_Z256_GI, MBI = 2, MBG = R3D_Z256_MBG }; };
+#else
+template <> struct ZPlan<256> { enum { R1 = 4, R2 = 8, R3 = 8, T = 32, G = 1, GF = R3D_Z256_GF, MBF = R3D_Z256_MBF, GI = R3D_Z256_GI, MBI = 2, MBG = R3D_Z256_MBG }; };
+#endif
 
 __device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
 __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
@@ -369,12 +388,11 @@ struct GramArgs {
   double* part1;
   double* part2;
   unsigned* tickets;
-  const double* weight;  // [nv] weights of the inner product (all 1 unless weighted)
-  bool weighted;         // modified Anderson: (a, b) = sum_g (1/rho_g) sum_r a b  (Eq. 38)
+  const double* weight;  // [nv] weights 1/rho_g of the modified Anderson inner product (Eq. 38); unused otherwise
   AccelArgs aa;
 };
 
-template <int NZ, int G, int MINB, int MAXO>
+template <int NZ, int G, int MINB, int MAXO, bool WEIGHTED>
 __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
     zinv_residual_kernel(const cplx* __restrict__ work, const double* __restrict__ tau_cur, double* __restrict__ Z,
                          double* __restrict__ R, double* __restrict__ raw_out, Twiddle tw_shift, Twiddle tw,
@@ -458,11 +476,16 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
       st2(Zc + off, make_double2(__dadd_rn(xlo.x, __dmul_rn(bdamp, rlo.x)), __dadd_rn(xlo.y, __dmul_rn(bdamp, rlo.y))));
       st2(Zc + off + NZ, make_double2(__dadd_rn(xhi.x, __dmul_rn(bdamp, rhi.x)), __dadd_rn(xhi.y, __dmul_rn(bdamp, rhi.y))));
       if constexpr (GRAM) {
-        // one side of every product carries the weight of this element's site (exactly 1 in an unweighted run)
-        const double wg = ga.weight[site];
-        const double2 vlo = make_double2(wg * rlo.x, wg * rlo.y), vhi = make_double2(wg * rhi.x, wg * rhi.y);
+        // weighted inner product (modified Anderson, Eq. 38): one side of every product carries the weight of this
+        // element's site; the unweighted <R, R> is kept as well, for the rms
+        double2 vlo = rlo, vhi = rhi;
+        if constexpr (WEIGHTED) {
+          const double wg = ga.weight[site];
+          vlo = make_double2(wg * rlo.x, wg * rlo.y);
+          vhi = make_double2(wg * rhi.x, wg * rhi.y);
+          acc_u = fma(rlo.x, rlo.x, fma(rlo.y, rlo.y, fma(rhi.x, rhi.x, fma(rhi.y, rhi.y, acc_u))));
+        }
         acc[MAXO] = fma(vlo.x, rlo.x, fma(vlo.y, rlo.y, fma(vhi.x, rhi.x, fma(vhi.y, rhi.y, acc[MAXO]))));
-        if (ga.weighted) acc_u = fma(rlo.x, rlo.x, fma(rlo.y, rlo.y, fma(rhi.x, rhi.x, fma(rhi.y, rhi.y, acc_u))));
 #pragma unroll
         for (int j = 0; j < MAXO; ++j)
           if (j < nother) {
@@ -482,7 +505,7 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
     const int lane = tid & 31, wid = tid >> 5;
 #pragma unroll
     for (int j = 0; j <= MAXO + 1; ++j) {              // j = MAXO + 1: the unweighted self product
-      if (j < nother || j == MAXO || (j == MAXO + 1 && ga.weighted)) {
+      if (j < nother || j == MAXO || (j == MAXO + 1 && WEIGHTED)) {
         double hi = (j <= MAXO) ? acc[j < NACC ? j : 0] : acc_u, lo = 0.0;
         for (int o = 16; o > 0; o >>= 1) {
           const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
@@ -495,7 +518,7 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
       }
     }
     __syncthreads();
-    if (tid <= MAXO + 1 && (tid < nother || tid == MAXO || (tid == MAXO + 1 && ga.weighted))) {
+    if (tid <= MAXO + 1 && (tid < nother || tid == MAXO || (tid == MAXO + 1 && WEIGHTED))) {
       double hi = 0.0, lo = 0.0;
       for (int w = 0; w < NW; ++w) dd_add(hi, lo, s_part[(tid * NW + w) * 2], s_part[(tid * NW + w) * 2 + 1]);
       dd_norm(hi, lo);
@@ -503,11 +526,11 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
       *reinterpret_cast<double2*>(ga.part1 + ((size_t)j * gridDim.x + blockIdx.x) * 2) = make_double2(hi, lo);
       __threadfence();
     }
-    gram_finish<NT>(st, ga.part1, ga.part2, ga.tickets, s_m, nother, ga.aa, ga.weighted, (double)field, s_row, &s_flag);
+    gram_finish<NT>(st, ga.part1, ga.part2, ga.tickets, s_m, nother, ga.aa, WEIGHTED, (double)field, s_row, &s_flag);
   }
 }
 
-template <int NZ, int MAXO>
+template <int NZ, int MAXO, bool WEIGHTED>
 static int launch_zinv_nm(const Grid& gr, const Buffers& b, const SolverParams& sp, double* raw_out, cudaStream_t s) {
   using Cfg = ZPlan<NZ>;
   constexpr int G = ZPlan<NZ>::GI;
@@ -517,11 +540,10 @@ static int launch_zinv_nm(const Grid& gr, const Buffers& b, const SolverParams& 
   size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
   const size_t red = (size_t)(MAX_M + 2) * (threads / 32 + 1) * 2 * sizeof(double);
   if (shm < red) shm = red;
-  auto kern = zinv_residual_kernel<NZ, G, MB, MAXO>;
+  auto kern = zinv_residual_kernel<NZ, G, MB, MAXO, WEIGHTED>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
-  GramArgs ga{b.gram_part, b.gram_part2, b.tickets, b.gram_w, sp.accel == RISM3D_ACCEL_ANDERSON,
-              AccelArgs{sp.M, sp.restart, sp.accel, sp.and_s1, sp.and_s2}};
+  GramArgs ga{b.gram_part, b.gram_part2, b.tickets, b.gram_w, AccelArgs{sp.M, sp.restart, sp.accel, sp.and_s1, sp.and_s2}};
   kern<<<(unsigned)((size_t)gr.n * gr.n / GL), threads, shm, s>>>(b.work, b.tau, b.Z, b.R, raw_out, tws, tw, b.state,
                                                                    gr.nv, gr.npts, gr.field, sp.b, ga);
   return 1;
@@ -530,8 +552,9 @@ static int launch_zinv_nm(const Grid& gr, const Buffers& b, const SolverParams& 
 // raw_out != nullptr: transform only; otherwise the variant compiled for M - 1 stored residuals
 template <int NZ>
 static int launch_zinv_n(const Grid& gr, const Buffers& b, const SolverParams& sp, double* raw_out, cudaStream_t s) {
-  if (raw_out) return launch_zinv_nm<NZ, -1>(gr, b, sp, raw_out, s);
-#define R3D_ZG(MO) case MO + 1: return launch_zinv_nm<NZ, MO>(gr, b, sp, raw_out, s)
+  if (raw_out) return launch_zinv_nm<NZ, -1, false>(gr, b, sp, raw_out, s);
+  if (sp.accel == RISM3D_ACCEL_ANDERSON) return launch_zinv_nm<NZ, 2, true>(gr, b, sp, raw_out, s);   // 3 stored pairs
+#define R3D_ZG(MO) case MO + 1: return launch_zinv_nm<NZ, MO, false>(gr, b, sp, raw_out, s)
   switch (sp.M) {
     R3D_ZG(0); R3D_ZG(1); R3D_ZG(2); R3D_ZG(3); R3D_ZG(4); R3D_ZG(5); R3D_ZG(6); R3D_ZG(7);
     R3D_ZG(8); R3D_ZG(9); R3D_ZG(10); R3D_ZG(11); R3D_ZG(12); R3D_ZG(13); R3D_ZG(14); R3D_ZG(15);

@@ -268,11 +268,11 @@ __global__ void __launch_bounds__(256)
     free_energy_kernel(double* __restrict__ part, const double* __restrict__ tau, const double* __restrict__ w,
                        const double* __restrict__ phi, const double* __restrict__ qv,
                        const DevState* __restrict__ st, int nv, size_t npts, size_t field, int closure, int order) {
-  __shared__ double s_red[8][2];
+  __shared__ double s_red[8][4];
   double inv_fact = 1.0;
   for (int i = 2; i <= order + 1; ++i) inv_fact /= (double)i;
   for (int g = 0; g < nv; ++g) {
-    double hi = 0.0, lo = 0.0;
+    double hi = 0.0, lo = 0.0, chi_ = 0.0, clo = 0.0;    // integrand of Eq. 17/18; c_sr alone (for Eq. 19)
     const double q = qv[g];
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < npts; i += (size_t)gridDim.x * blockDim.x) {
       const double t = tau[(size_t)g * npts + i];
@@ -286,38 +286,49 @@ __global__ void __launch_bounds__(256)
       else if (closure == RISM3D_PSE) B = d > 0.0 ? pow(d, order + 1) * inv_fact : 0.0;
       const double v = -csr - 0.5 * hh * c + 0.5 * hh * hh - B;
       dd_add(hi, lo, v, 0.0);
+      dd_add(chi_, clo, csr, 0.0);
     }
     for (int o = 16; o > 0; o >>= 1) {
       const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
       dd_add(hi, lo, h2, l2);
+      const double h3 = __shfl_down_sync(0xffffffffu, chi_, o), l3 = __shfl_down_sync(0xffffffffu, clo, o);
+      dd_add(chi_, clo, h3, l3);
     }
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     __syncthreads();
-    if (lane == 0) { s_red[wid][0] = hi; s_red[wid][1] = lo; }
+    if (lane == 0) { s_red[wid][0] = hi; s_red[wid][1] = lo; s_red[wid][2] = chi_; s_red[wid][3] = clo; }
     __syncthreads();
     if (threadIdx.x == 0) {
-      hi = 0.0; lo = 0.0;
-      for (int k = 0; k < 8; ++k) dd_add(hi, lo, s_red[k][0], s_red[k][1]);
+      hi = 0.0; lo = 0.0; chi_ = 0.0; clo = 0.0;
+      for (int k = 0; k < 8; ++k) { dd_add(hi, lo, s_red[k][0], s_red[k][1]); dd_add(chi_, clo, s_red[k][2], s_red[k][3]); }
       part[((size_t)blockIdx.x * MAX_NV + g) * 2 + 0] = hi;
       part[((size_t)blockIdx.x * MAX_NV + g) * 2 + 1] = lo;
+      part[((size_t)(gridDim.x + blockIdx.x) * MAX_NV + g) * 2 + 0] = chi_;
+      part[((size_t)(gridDim.x + blockIdx.x) * MAX_NV + g) * 2 + 1] = clo;
     }
   }
 }
 
 __global__ void free_energy_final_kernel(double* __restrict__ out, const double* __restrict__ part, int nblocks,
-                                         const double* __restrict__ rhov, int nv, double scale) {
+                                         const double* __restrict__ rhov, int nv, double scale, double dv) {
   const int g = threadIdx.x;
   if (g >= nv) return;
   double hi = 0.0, lo = 0.0;
   for (int b = 0; b < nblocks; ++b) dd_add(hi, lo, part[((size_t)b * MAX_NV + g) * 2], part[((size_t)b * MAX_NV + g) * 2 + 1]);
   out[g] = scale * rhov[g] * (hi + lo);
+  // second set: dV sum_r c_sr,g(r)  (A^3), not density weighted
+  hi = 0.0; lo = 0.0;
+  for (int b = 0; b < nblocks; ++b)
+    dd_add(hi, lo, part[((size_t)(nblocks + b) * MAX_NV + g) * 2], part[((size_t)(nblocks + b) * MAX_NV + g) * 2 + 1]);
+  out[MAX_NV + g] = dv * (hi + lo);
 }
 
 int launch_free_energy(const Grid& g, const Buffers& b, const SolverParams& sp, double* d_out, cudaStream_t s) {
   const int blocks = FE_BLOCKS;
   free_energy_kernel<<<blocks, 256, 0, s>>>(b.fe_part, b.tau, b.w, b.phi, b.qv, b.state, g.nv, g.npts, g.field,
                                             sp.closure, sp.pse_order);
-  free_energy_final_kernel<<<1, 32, 0, s>>>(d_out, b.fe_part, blocks, b.rhov, g.nv, sp.kT * g.h * g.h * g.h);
+  free_energy_final_kernel<<<1, 32, 0, s>>>(d_out, b.fe_part, blocks, b.rhov, g.nv, sp.kT * g.h * g.h * g.h,
+                                            g.h * g.h * g.h);
   return 2;
 }
 

@@ -189,3 +189,16 @@ def test_modified_anderson_four_sites_converges_to_the_mdiis_fixed_point():
     assert abs(mu_g - mu_r) <= 1e-6 * abs(mu_r)          # the fixed point does not depend on the accelerator
     gg, gr = gpu.get_field("G"), ref.get_field("G")      # (slowly converging case: rms 1e-9 leaves ~1e-6 in g)
     assert np.max(np.abs(gg - gr) / np.maximum(1.0, gr)) <= 1e-5
+
+
+# ---- NEXT-2 (first item): partial molar volume, Eq. 19 ---------------------------------------------------------
+@pytest.mark.parametrize("cfg,n", [("C1", 32), ("C2", 32)])
+def test_partial_molar_volume_matches_oracle(cfg, n):
+    orc, gpu, _, _ = make_pair(cfg, n_override=n)
+    orc.iterate(400, 1e-9)
+    gpu.iterate(400, 1e-9)
+    chi_t = 0.55                                         # A^3 mol/kcal; any number: it multiplies both sides alike
+    v_o, c_o = orc.pmv(chi_t)
+    v_g, c_g = gpu.pmv(chi_t)
+    assert abs(v_g - v_o) <= 1e-7 * abs(v_o)
+    np.testing.assert_allclose(c_g, c_o, rtol=1e-6, atol=1e-7 * np.max(np.abs(c_o)))

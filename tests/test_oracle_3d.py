@@ -495,3 +495,52 @@ def test_anderson_reaches_the_same_fixed_point_as_mdiis():
         res.append((orc.get_field("G"), orc.free_energy()[0]))
     assert np.max(np.abs(res[0][0] - res[1][0])) < 1e-8
     assert abs(res[0][1] - res[1][1]) < 1e-8 * abs(res[0][1])
+
+
+# ------------------------------------------------------------------------------------------------
+# Partial molar volume, Eq. 19
+# ------------------------------------------------------------------------------------------------
+def test_pmv_ideal_gas_solvent_is_the_second_virial_coefficient():
+    """One-site ideal-gas solvent (chi = 1, rho kT chi_T = 1), HNC, LJ solute: the fixed point is g = exp(-beta u)
+    (pin P3), so Eq. 19 gives V - 1/rho = -int (exp(-beta u) - 1) dr = 2 B_2(T), the textbook second virial
+    coefficient of the pair, here from an independent radial quadrature."""
+    rho, T = 0.02, 298.0
+    kT = o3.K_BOLTZMANN * T
+    sig_v, eps_v, sig_u, eps_u = 3.0, 0.15, 3.4, 0.2
+    n, dr = 64, 0.3
+    orc = o3.Rism3dOracle(n, dr, 1, closure="HNC", mdiis_nvec=3, origin=(-9.45, -9.45, -9.45))   # atom between grid points
+    orc.set_solvent_chi([0.0], [sig_v], [eps_v], [rho], *identity_chi(1, n_k=1300, dk=0.015, k0=0.015))
+    orc.set_solute(np.zeros((1, 3)), [0.0], [sig_u], [eps_u])
+    orc.iterate(3, 0.0)
+    chi_t = 1.0 / (rho * kT)
+    v, c_int = orc.pmv(chi_t)
+    r = np.linspace(1e-4, 9.6 * np.sqrt(3), 400001)
+    s, e = 0.5 * (sig_v + sig_u), np.sqrt(eps_v * eps_u)
+    mayer = np.exp(-4.0 * e * ((s / r) ** 12 - (s / r) ** 6) / kT) - 1.0
+    # the cubic box cuts the integration domain; beyond the inscribed sphere the integrand is ~1e-4 r^2, so compare
+    # with the radial integral over the box's volume-equivalent region by integrating the same function on the grid
+    # of the oracle directly (closed form on the grid) and, loosely, against the radial quadrature to 9.6 A
+    rr = np.sqrt(np.sum(orc.points ** 2, axis=1))
+    on_grid = dr ** 3 * np.sum(np.exp(-4.0 * e * ((s / rr) ** 12 - (s / rr) ** 6) / kT) - 1.0)
+    assert abs(c_int[0] - on_grid) < 1e-9 * abs(on_grid)
+    assert abs(v - (1.0 / rho - on_grid)) < 1e-9 * abs(v)
+    sel = r < 9.6
+    radial = np.trapezoid(4.0 * np.pi * r[sel] ** 2 * mayer[sel], r[sel])
+    shell = dr ** 3 * np.sum((np.exp(-4.0 * e * ((s / rr) ** 12 - (s / rr) ** 6) / kT) - 1.0)[rr < 9.6])
+    assert abs(shell - radial) < 2e-2 * abs(radial)      # 0.3 A grid against the exact radial integral
+
+
+def test_pmv_null_solute_and_sign():
+    sv = water()
+    k0, dk, chi = synthetic_chi(2, sv.rho)
+    orc = o3.Rism3dOracle(16, 0.6, 2)
+    orc.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+    orc.set_solute(np.array([[0.1, 0.0, 0.2]]), [0.0], [3.0], [0.0])
+    orc.iterate(2, 0.0)
+    v, c_int = orc.pmv(0.7)
+    assert np.all(c_int == 0.0) and v == orc.kT * 0.7    # nothing there: the ideal term kT chi_T alone
+    sol = make_solute("C1")
+    orc.set_solute(sol.xyz, 0.0 * sol.q, sol.sigma, sol.eps)
+    orc.iterate(200, 1e-9)
+    v2, c2 = orc.pmv(0.7)
+    assert v2 > v and np.dot(sv.rho, c2) < 0.0           # a repulsive core excludes solvent: c integrates to < 0
