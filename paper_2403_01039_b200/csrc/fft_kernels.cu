@@ -403,6 +403,7 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
   __shared__ int s_other[MAX_M];
   __shared__ int s_nother, s_m, s_flag;
   __shared__ double s_row[MAX_M + 2];
+  __shared__ SolveScratch s_solve;
   if (GRAM && threadIdx.x == 0) {
     const int m = st->m;
     const int skip = (m == ga.aa.M) ? 1 : 0;              // a full history drops its oldest entry this iteration
@@ -526,7 +527,7 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
       *reinterpret_cast<double2*>(ga.part1 + ((size_t)j * gridDim.x + blockIdx.x) * 2) = make_double2(hi, lo);
       __threadfence();
     }
-    gram_finish<NT>(st, ga.part1, ga.part2, ga.tickets, s_m, nother, ga.aa, WEIGHTED, (double)field, s_row, &s_flag);
+    gram_finish<NT>(st, ga.part1, ga.part2, ga.tickets, s_m, nother, ga.aa, WEIGHTED, (double)field, s_row, &s_flag, s_solve);
   }
 }
 
