@@ -266,7 +266,9 @@ class Solver:
             raise Rism3dError(-2, "unsupported grid / site count / MDIIS size")
         self.device = torch.device("cuda", device)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
-        self.stream = torch.cuda.current_stream(self.device)
+        # a stream of its own (not the legacy default stream): the library captures its iteration into CUDA graphs
+        self.stream = torch.cuda.Stream(self.device)
+        self.stream.wait_stream(torch.cuda.current_stream(self.device))     # the workspace allocation above
         self.ctx = rism3d_init(p, self.workspace.data_ptr(), nbytes, self.stream.cuda_stream)
 
     def close(self):
@@ -313,6 +315,7 @@ class Solver:
         import torch
         if isinstance(src, torch.Tensor) and src.is_cuda:
             src = src.contiguous()
+            self.stream.wait_stream(torch.cuda.current_stream(self.device))    # src may still be in flight there
             rism3d_set_tau(self.ctx, site, src.data_ptr(), True)
         else:
             a = _f64(src)
@@ -337,6 +340,7 @@ class Solver:
         import torch
         real_dev = real_dev.contiguous()
         out = torch.empty((self.n, self.n, self.n // 2, self.n_sites), dtype=torch.complex128, device=self.device)
+        self.stream.wait_stream(torch.cuda.current_stream(self.device))
         rism3d_debug_fft_forward(self.ctx, real_dev.data_ptr(), out.data_ptr())
         return out
 
@@ -344,5 +348,6 @@ class Solver:
         import torch
         spec_dev = spec_dev.contiguous()
         out = torch.empty((self.n_sites, self.n, self.n, self.n), dtype=torch.float64, device=self.device)
+        self.stream.wait_stream(torch.cuda.current_stream(self.device))
         rism3d_debug_fft_inverse(self.ctx, spec_dev.data_ptr(), out.data_ptr())
         return out

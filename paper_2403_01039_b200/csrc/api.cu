@@ -29,6 +29,11 @@ struct rism3d_ctx {
   size_t ev_used;
   double prof_ms[RISM3D_N_LOOP_KERNELS];
   long long prof_iters;
+  // CUDA graphs of 1 and of GRAPH_PACK iterations (captured once per context: every launch parameter of an
+  // iteration is fixed, all evolving state lives on the device); not used on the legacy default stream or while profiling
+  cudaGraphExec_t graph1, graph_pack;
+  bool graph_tried;
+  int graph_kernels;         // kernels per captured iteration
   StateHeader* h_hdr;        // pinned
   double* d_out;             // small device array for scalar results (inside workspace)
   char err[512];
@@ -210,6 +215,8 @@ extern "C" void rism3d_destroy(rism3d_ctx* ctx) {
     for (cudaEvent_t e : *ctx->ev_pool) cudaEventDestroy(e);
     delete ctx->ev_pool;
   }
+  if (ctx->graph1) cudaGraphExecDestroy(ctx->graph1);
+  if (ctx->graph_pack) cudaGraphExecDestroy(ctx->graph_pack);
   if (ctx->h_hdr) cudaFreeHost(ctx->h_hdr);
   delete ctx;
 }
@@ -351,6 +358,8 @@ static void prof_collect(rism3d_ctx* ctx) {
   ctx->ev_used = 0;
 }
 
+constexpr int GRAPH_PACK = 8;   // iterations per large graph = iterations between two convergence checks of iterate
+
 static int enqueue_iteration(rism3d_ctx* ctx) {
   const Grid& g = ctx->g;
   const Buffers& b = ctx->b;
@@ -370,6 +379,50 @@ static int enqueue_iteration(rism3d_ctx* ctx) {
                                                            //  closure_zfwd, or by iterate's trailing update pass)
   ctx->launches += k;
   return k;
+}
+
+// capture `iters` iterations into an executable graph; nullptr when capture is not possible on this stream
+static cudaGraphExec_t capture_iterations(rism3d_ctx* ctx, int iters, int* kernels_per_iteration) {
+  if (cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  const long long before = ctx->launches;
+  int k = 0;
+  for (int i = 0; i < iters; ++i) k = enqueue_iteration(ctx);
+  ctx->launches = before;                                  // captured, not launched
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t exec = nullptr;
+  if (cudaStreamEndCapture(ctx->stream, &graph) != cudaSuccess || graph == nullptr) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  if (cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+    cudaGetLastError();
+    exec = nullptr;
+  }
+  cudaGraphDestroy(graph);
+  if (kernels_per_iteration) *kernels_per_iteration = k;
+  return exec;
+}
+
+// enqueue `iters` (1 or GRAPH_PACK) iterations: as a graph launch when possible, else kernel by kernel
+static void enqueue_iterations(rism3d_ctx* ctx, int iters) {
+  if (!ctx->profiling && ctx->stream != nullptr) {
+    if (!ctx->graph_tried) {
+      ctx->graph_tried = true;
+      int k = 0;
+      ctx->graph1 = capture_iterations(ctx, 1, &k);
+      ctx->graph_pack = ctx->graph1 ? capture_iterations(ctx, GRAPH_PACK, &k) : nullptr;
+      ctx->graph_kernels = k;
+    }
+    cudaGraphExec_t exec = (iters == GRAPH_PACK) ? ctx->graph_pack : (iters == 1 ? ctx->graph1 : nullptr);
+    if (exec && cudaGraphLaunch(exec, ctx->stream) == cudaSuccess) {
+      ctx->launches += (long long)ctx->graph_kernels * iters;
+      return;
+    }
+  }
+  for (int i = 0; i < iters; ++i) enqueue_iteration(ctx);
 }
 
 extern "C" int rism3d_set_profiling(rism3d_ctx* ctx, int enable) {
@@ -409,10 +462,14 @@ extern "C" int rism3d_iterate(rism3d_ctx* ctx, int max_iter, double tol, int* n_
   if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before iterate");
   iterate_begin_kernel<<<1, 1, 0, ctx->stream>>>(ctx->b.state, tol);
   ctx->launches += 1;
-  const int check_every = 8;
-  for (int it = 0; it < max_iter; ++it) {
-    enqueue_iteration(ctx);
-    if (tol > 0.0 && ((it + 1) % check_every == 0)) {
+  // packs of GRAPH_PACK iterations (one graph launch each) with a look at the device state in between when a
+  // tolerance is set; once an iteration has converged the remaining kernels of a pack return immediately
+  int it = 0;
+  while (it < max_iter) {
+    const int step = (max_iter - it >= GRAPH_PACK) ? GRAPH_PACK : 1;
+    enqueue_iterations(ctx, step);
+    it += step;
+    if (tol > 0.0 && step == GRAPH_PACK) {
       int rc = read_header(ctx);
       if (rc) return rc;
       if (ctx->h_hdr->done) break;
