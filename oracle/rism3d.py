@@ -395,6 +395,7 @@ class Rism3dOracle:
         else:
             self.minus_beta_u = -beta_u_at(self.points, xyz, q, sigma, eps, self.q_v, self.sig_v,
                                            self.eps_v, self.beta, self.r_min).reshape(shp)  # Eq. 22
+        self._solute = (xyz, q, sigma, eps)
         self.t = self.f.copy()                                                         # step 1
         if self.accelerator == "ANDERSON":          # weight 1/rho_gamma; b is the mixing parameter
             self.mdiis = ModifiedAnderson(self.b, self.anderson_s, 1.0 / self.rho_v)
@@ -467,4 +468,29 @@ class Rism3dOracle:
         _, _, c_sr = self.closure_step(self.t)
         c_int = np.array([self.dr ** 3 * float(np.sum(c_sr[gam], dtype=np.longdouble)) for gam in range(self.n_v)])
         return float(self.kT * chi_t * (1.0 - np.dot(self.rho_v, c_int))), c_int
+
+    def solvation_gradient(self):
+        """d(dmu)/dR_alpha = sum_gamma rho_gamma dV sum_r g_gamma(r) du_gamma(r)/dR_alpha  (the
+        equation after Eq. 23; 'common for both HNC and KH'), kcal/(mol A), all pairs, u of Eq. 22 with the distance
+        clamp of Q11 (inside the clamp the potential is flat: no contribution).  -> [n_atoms][3].
+        d/dR_alpha [1/r] = (r - R_alpha)/r^3 ;  d/dR_alpha [(s/r)^12 - (s/r)^6] = (12 s^12/r^14 - 6 s^6/r^8)(r - R_alpha)."""
+        _, g, _ = self.closure_step(self.t)
+        xyz, q_u, sig_u, eps_u = self._solute
+        out = np.zeros((len(q_u), 3))
+        gw = [self.rho_v[gam] * self.dr ** 3 * g[gam].ravel() for gam in range(self.n_v)]
+        for a in range(len(q_u)):
+            d = self.points - xyz[a]
+            r2 = np.sum(d * d, axis=1)
+            inside = r2 < self.r_min ** 2
+            r2 = np.where(inside, 1.0, r2)
+            coef = np.zeros(len(r2))
+            for gam in range(self.n_v):
+                s = 0.5 * (sig_u[a] + self.sig_v[gam])
+                e = math.sqrt(eps_u[a] * self.eps_v[gam])
+                s6 = (s * s / r2) ** 3
+                du = COULOMB * q_u[a] * self.q_v[gam] / (r2 * np.sqrt(r2)) + 4.0 * e * (12.0 * s6 * s6 - 6.0 * s6) / r2
+                coef += gw[gam] * du
+            coef = np.where(inside, 0.0, coef)
+            out[a] = [float(np.sum(coef * d[:, k], dtype=np.longdouble)) for k in range(3)]
+        return out
 

@@ -19,7 +19,7 @@ FIELDS = {"G": 0, "H": 1, "C_SR": 2, "T": 3, "TAU": 4, "W": 5, "PHI": 6}
 
 EXPORTED_SYMBOLS = [
     "rism3d_workspace_bytes", "rism3d_init", "rism3d_set_solvent_chi", "rism3d_set_solute",
-    "rism3d_iterate", "rism3d_free_energy", "rism3d_pmv", "rism3d_get_field", "rism3d_set_tau",
+    "rism3d_iterate", "rism3d_free_energy", "rism3d_pmv", "rism3d_gradient", "rism3d_get_field", "rism3d_set_tau",
     "rism3d_get_rms_history", "rism3d_launch_count", "rism3d_set_profiling", "rism3d_get_timings",
     "rism3d_loop_kernel_name", "rism3d_debug_fft_forward",
     "rism3d_debug_fft_inverse", "rism3d_last_error", "rism3d_status_string", "rism3d_destroy",
@@ -81,6 +81,8 @@ def load_library():
     lib.rism3d_free_energy.argtypes = [C.c_void_p, dp, dp]
     lib.rism3d_pmv.restype = C.c_int
     lib.rism3d_pmv.argtypes = [C.c_void_p, C.c_double, dp, dp]
+    lib.rism3d_gradient.restype = C.c_int
+    lib.rism3d_gradient.argtypes = [C.c_void_p, dp]
     lib.rism3d_get_field.restype = C.c_int
     lib.rism3d_get_field.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]
     lib.rism3d_set_tau.restype = C.c_int
@@ -179,6 +181,13 @@ def rism3d_pmv(ctx, chi_t: float, n_sites: int):
     site = np.zeros(n_sites)
     _check(ctx, load_library().rism3d_pmv(ctx, float(chi_t), C.byref(v), _dptr(site)))
     return float(v.value), site
+
+
+def rism3d_gradient(ctx, n_atoms: int) -> np.ndarray:
+    """-> d(dmu)/dR [n_atoms][3], kcal/(mol A)"""
+    out = np.zeros((n_atoms, 3))
+    _check(ctx, load_library().rism3d_gradient(ctx, _dptr(out)))
+    return out
 
 
 def rism3d_get_field(ctx, which: int, site: int, dst_ptr: int, dst_is_device: bool):
@@ -286,7 +295,11 @@ class Solver:
         rism3d_set_solvent_chi(self.ctx, q, sigma, eps, rho, k0, dk, chi)
 
     def set_solute(self, xyz, q, sigma, eps, rcut=0.0) -> float:
+        self.n_atoms = len(np.atleast_1d(q))
         return rism3d_set_solute(self.ctx, xyz, q, sigma, eps, rcut)
+
+    def gradient(self) -> np.ndarray:
+        return rism3d_gradient(self.ctx, self.n_atoms)
 
     def iterate(self, max_iter, tol=0.0):
         return rism3d_iterate(self.ctx, max_iter, tol)

@@ -34,6 +34,9 @@ struct rism3d_ctx {
   cudaGraphExec_t graph1, graph_pack;
   bool graph_tried;
   int graph_kernels;         // kernels per captured iteration
+  std::vector<double>* h_atoms;   // host copies of the solute tables (x, y, z, .) and (beta C q q, sigma^2, 4 beta eps)
+  std::vector<double>* h_pair;    //   kept for rism3d_gradient: their device copies live in scratch the loop overwrites
+  int n_atoms;
   StateHeader* h_hdr;        // pinned
   double* d_out;             // small device array for scalar results (inside workspace)
   char err[512];
@@ -215,6 +218,8 @@ extern "C" void rism3d_destroy(rism3d_ctx* ctx) {
     for (cudaEvent_t e : *ctx->ev_pool) cudaEventDestroy(e);
     delete ctx->ev_pool;
   }
+  delete ctx->h_atoms;
+  delete ctx->h_pair;
   if (ctx->graph1) cudaGraphExecDestroy(ctx->graph1);
   if (ctx->graph_pack) cudaGraphExecDestroy(ctx->graph_pack);
   if (ctx->h_hdr) cudaFreeHost(ctx->h_hdr);
@@ -320,6 +325,11 @@ extern "C" int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   if (setup_ms) *setup_ms = ms;
+  if (!ctx->h_atoms) ctx->h_atoms = new std::vector<double>();
+  if (!ctx->h_pair) ctx->h_pair = new std::vector<double>();
+  ctx->h_atoms->assign(atoms.begin(), atoms.begin() + 4 * na);
+  *ctx->h_pair = pair;
+  ctx->n_atoms = n_atoms;
   ctx->have_solute = true;
   return RISM3D_OK;
 }
@@ -522,6 +532,37 @@ extern "C" int rism3d_pmv(rism3d_ctx* ctx, double chi_t, double* pmv, double* c_
     if (c_int_site) c_int_site[i] = host[MAX_NV + i];
   }
   *pmv = ctx->sp.kT * chi_t * (1.0 - sum);           // Eq. 19
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_gradient(rism3d_ctx* ctx, double* grad) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (!grad) return fail(ctx, RISM3D_ERR_ARG, "grad is NULL");
+  if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before gradient");
+  const Grid& g = ctx->g;
+  const int na = ctx->n_atoms;
+  if (na == 0) return RISM3D_OK;
+  // everything lives in the k-space work array, which holds nothing between iterations: tables, partial sums, result
+  const size_t b_atoms = align256((size_t)na * 4 * 8), b_pair = align256((size_t)na * g.nv * 3 * 8);
+  const size_t b_out = align256((size_t)na * 3 * 8);
+  const size_t avail = g.field * 8;
+  if (b_atoms + b_pair + b_out + (size_t)na * 3 * 16 > avail)
+    return fail(ctx, RISM3D_ERR_WORKSPACE, "%d atoms do not fit the scratch array of this grid", na);
+  size_t nchunks = (g.npts + 8191) / 8192;                 // >= 8192 points per block, fewer blocks if memory is short
+  const size_t max_chunks = (avail - b_atoms - b_pair - b_out) / ((size_t)na * 3 * 16);
+  if (nchunks > max_chunks) nchunks = max_chunks;
+  if (nchunks > 4096) nchunks = 4096;
+  char* base = (char*)ctx->b.work;
+  double* d_atoms = (double*)base;
+  double* d_pair = (double*)(base + b_atoms);
+  double* d_out = (double*)(base + b_atoms + b_pair);
+  double* d_part = (double*)(base + b_atoms + b_pair + b_out);
+  CU(cudaMemcpyAsync(d_atoms, ctx->h_atoms->data(), (size_t)na * 4 * 8, cudaMemcpyHostToDevice, ctx->stream));
+  CU(cudaMemcpyAsync(d_pair, ctx->h_pair->data(), (size_t)na * g.nv * 3 * 8, cudaMemcpyHostToDevice, ctx->stream));
+  ctx->launches += launch_gradient(g, ctx->b, ctx->sp, na, d_atoms, d_pair, d_part, (int)nchunks, d_out, ctx->stream);
+  CU(cudaGetLastError());
+  CU(cudaMemcpyAsync(grad, d_out, (size_t)na * 3 * 8, cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
   return RISM3D_OK;
 }
 

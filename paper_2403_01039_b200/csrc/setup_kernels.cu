@@ -363,4 +363,132 @@ int launch_get_field(const Grid& g, const Buffers& b, const SolverParams& sp, in
   return 1;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Solvent-induced gradient on the solute atoms (the equation after Eq. 23):
+//   d(dmu)/dR_a = sum_g rho_g dV sum_r g_g(r) du_g(r)/dR_a,   u of Eq. 22, all pairs, distance clamp of Q11
+//   du_g/dR_a = [C q_a q_g / r^3 + 4 eps_ag (12 s^12/r^14 - 6 s^6/r^8)] (r - R_a)
+// Grid: (point chunks, chunks of GRAD_ATOMS atoms).  A thread walks its points, forms g = closure(w + tau) on the
+// fly and accumulates the 3 components for the block's atoms in registers; the block sum (double-double, fixed
+// order) goes to partial[chunk][atom][3]; gradient_final_kernel adds the chunks in order.  pair carries beta
+// (beta C q_a q_g, sigma_ag^2, 4 beta eps_ag), so the final sum is multiplied by kT.
+// ------------------------------------------------------------------------------------------------
+constexpr int GRAD_ATOMS = 8;
+constexpr int GRAD_THREADS = 256;
+
+template <int NV>
+__global__ void __launch_bounds__(GRAD_THREADS)
+    gradient_kernel(double* __restrict__ partial, const double* __restrict__ tau, const double* __restrict__ w,
+                    const double4* __restrict__ atoms, const double* __restrict__ pair, const double* __restrict__ rhov,
+                    int n_atoms, int n, double h, double ox, double oy, double oz, double r_min, size_t npts,
+                    size_t pts_per_block, int closure, int order) {
+  __shared__ double4 s_atom[GRAD_ATOMS];
+  __shared__ double s_pair[GRAD_ATOMS * NV * 3];
+  __shared__ double s_red[GRAD_THREADS / 32][GRAD_ATOMS * 3][2];
+  const int tid = threadIdx.x;
+  const int a0 = blockIdx.y * GRAD_ATOMS;
+  const int na = min(GRAD_ATOMS, n_atoms - a0);
+  if (tid < na) s_atom[tid] = atoms[a0 + tid];
+  for (int i = tid; i < na * NV * 3; i += GRAD_THREADS) s_pair[i] = pair[(size_t)a0 * NV * 3 + i];
+  __syncthreads();
+  double acc[GRAD_ATOMS][3];
+#pragma unroll
+  for (int a = 0; a < GRAD_ATOMS; ++a) acc[a][0] = acc[a][1] = acc[a][2] = 0.0;
+  const double dv = h * h * h, rmin2 = r_min * r_min;
+  const size_t p0 = (size_t)blockIdx.x * pts_per_block;
+  const size_t p1 = min(npts, p0 + pts_per_block);
+  for (size_t idx = p0 + tid; idx < p1; idx += GRAD_THREADS) {
+    const int iz = (int)(idx % n), iy = (int)((idx / n) % n), ix = (int)(idx / ((size_t)n * n));
+    const double x = __dadd_rn(ox, __dmul_rn(h, (double)ix));
+    const double y = __dadd_rn(oy, __dmul_rn(h, (double)iy));
+    const double z = __dadd_rn(oz, __dmul_rn(h, (double)iz));
+    double gw[NV];
+#pragma unroll
+    for (int g = 0; g < NV; ++g)
+      gw[g] = rhov[g] * dv * closure_g(w[(size_t)g * npts + idx] + tau[(size_t)g * npts + idx], closure, order);
+    // (compiler barrier: re-read the atom tables from shared memory for every point instead of pinning all
+    //  GRAD_ATOMS * (4 + 3 NV) of them in registers across the loop)
+    asm volatile("" ::: "memory");
+#pragma unroll
+    for (int a = 0; a < GRAD_ATOMS; ++a) {
+      if (a < na) {
+        const double4 at = s_atom[a];
+        const double dx = x - at.x, dy = y - at.y, dz = z - at.z;
+        const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+        if (r2 >= rmin2) {                                  // inside the clamp the potential is flat
+          double rinv = (double)rsqrtf((float)r2);
+          rinv = rinv * fma(-0.5 * r2, rinv * rinv, 1.5);
+          rinv = rinv * fma(-0.5 * r2, rinv * rinv, 1.5);
+          const double inv2 = rinv * rinv, inv3 = inv2 * rinv;
+          const double* pp = s_pair + a * NV * 3;
+          double coef = 0.0;
+#pragma unroll
+          for (int g = 0; g < NV; ++g) {
+            const double s2 = pp[g * 3 + 1] * inv2;
+            const double s6 = s2 * s2 * s2;
+            coef += gw[g] * (pp[g * 3 + 0] * inv3 + pp[g * 3 + 2] * (12.0 * s6 * s6 - 6.0 * s6) * inv2);
+          }
+          acc[a][0] = fma(coef, dx, acc[a][0]);
+          acc[a][1] = fma(coef, dy, acc[a][1]);
+          acc[a][2] = fma(coef, dz, acc[a][2]);
+        }
+      }
+    }
+  }
+  // block sum in double-double, fixed order
+  const int lane = tid & 31, wid = tid >> 5;
+#pragma unroll
+  for (int a = 0; a < GRAD_ATOMS; ++a)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      double v = acc[a][k];                                // 32 per-thread sums: plain fp64 tree, then double-double
+      for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+      if (lane == 0) { s_red[wid][a * 3 + k][0] = v; s_red[wid][a * 3 + k][1] = 0.0; }
+    }
+  __syncthreads();
+  if (tid < na * 3) {
+    double hi = 0.0, lo = 0.0;
+    for (int wv = 0; wv < GRAD_THREADS / 32; ++wv) dd_add(hi, lo, s_red[wv][tid][0], s_red[wv][tid][1]);
+    dd_norm(hi, lo);
+    double* dst = partial + (((size_t)blockIdx.x * n_atoms + a0) * 3 + tid) * 2;
+    dst[0] = hi;
+    dst[1] = lo;
+  }
+}
+
+__global__ void gradient_final_kernel(double* __restrict__ out, const double* __restrict__ partial, int nchunks,
+                                      int n_atoms, double kT) {
+  const int e = blockIdx.x * blockDim.x + threadIdx.x;    // atom * 3 + component
+  if (e >= n_atoms * 3) return;
+  double hi = 0.0, lo = 0.0;
+  for (int c = 0; c < nchunks; ++c) {
+    const double* p = partial + ((size_t)c * n_atoms * 3 + e) * 2;
+    dd_add(hi, lo, p[0], p[1]);
+  }
+  out[e] = kT * (hi + lo);
+}
+
+// d_atoms: [n_atoms] double4 (x, y, z, unused); d_pair as in launch_potential; d_partial: nchunks*n_atoms*3*2 doubles;
+// d_out: n_atoms*3 doubles.  Returns the number of kernels launched.
+int launch_gradient(const Grid& g, const Buffers& b, const SolverParams& sp, int n_atoms, const double* d_atoms,
+                    const double* d_pair, double* d_partial, int nchunks, double* d_out, cudaStream_t s) {
+  if (n_atoms == 0) return 0;
+  const size_t per = (g.npts + nchunks - 1) / nchunks;
+  dim3 grid((unsigned)nchunks, (unsigned)((n_atoms + GRAD_ATOMS - 1) / GRAD_ATOMS));
+  const double4* at = reinterpret_cast<const double4*>(d_atoms);
+#define GRD(NV)                                                                                                     \
+  gradient_kernel<NV><<<grid, GRAD_THREADS, 0, s>>>(d_partial, b.tau, b.w, at, d_pair, b.rhov, n_atoms, g.n, g.h,   \
+                                                    g.origin[0], g.origin[1], g.origin[2], sp.r_min, g.npts, per,   \
+                                                    sp.closure, sp.pse_order)
+  switch (g.nv) {
+    case 1: GRD(1); break;
+    case 2: GRD(2); break;
+    case 4: GRD(4); break;
+    case 8: GRD(8); break;
+    default: return 0;
+  }
+#undef GRD
+  gradient_final_kernel<<<(n_atoms * 3 + 127) / 128, 128, 0, s>>>(d_out, d_partial, nchunks, n_atoms, sp.kT);
+  return 2;
+}
+
 }  // namespace r3d

@@ -202,3 +202,27 @@ def test_partial_molar_volume_matches_oracle(cfg, n):
     v_g, c_g = gpu.pmv(chi_t)
     assert abs(v_g - v_o) <= 1e-7 * abs(v_o)
     np.testing.assert_allclose(c_g, c_o, rtol=1e-6, atol=1e-7 * np.max(np.abs(c_o)))
+
+
+# ---- NEXT-2: solvent-induced gradient on the solute atoms --------------------------------------
+@pytest.mark.parametrize("case", ["C2", "sub40", "ion_offcentre"])
+def test_gradient_matches_oracle(case):
+    if case == "C2":
+        orc, gpu, sol, _ = make_pair("C2", n_override=32)
+    elif case == "sub40":
+        full = make_solute("C3")
+        keep = np.argsort(np.linalg.norm(full.xyz, axis=1))[:40]
+        sol = Solute("C3_sub40", full.xyz[keep], full.q[keep], full.sigma[keep], full.eps[keep])
+        orc, gpu, _, _ = make_pair(n=32, spacing=0.75, solvent="water_nacl_0.1M", closure="PSE", pse_order=2, M=8,
+                                   solute=sol)
+    else:
+        sol = Solute("ion", np.array([[0.5, 0.0, 0.0]]), np.array([1.0]), np.array([2.35]), np.array([0.13]))   # on a grid point
+        orc, gpu, _, _ = make_pair(n=32, spacing=0.5, solvent="water", solute=sol)
+    orc.iterate(60, 0.0)
+    gpu.iterate(60, 0.0)
+    go, gg = orc.solvation_gradient(), gpu.gradient()
+    assert gg.shape == (sol.n_atoms, 3)
+    assert np.max(np.abs(gg - go)) <= 1e-8 * max(1.0, np.max(np.abs(go)))
+    gpu.iterate(3, 0.0)                                   # the gradient borrowed the k-space work array: the loop goes on
+    orc.iterate(3, 0.0)
+    assert np.max(np.abs(gpu.get_field("G") - orc.get_field("G"))) <= 5e-9
