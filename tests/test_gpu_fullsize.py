@@ -100,3 +100,49 @@ def test_c4_converges_to_a_fixed_point(c4):
         s.set_tau(k, tau[k])                 # warm start: clears the history, keeps tau
     n2, rms2 = s.iterate(1, 0.0)
     assert n2 == 1 and rms2 < 1.5 * cfg.tol
+
+
+# ---- C5: 512^3 x 4 sites, 20 000 atoms, 54 GB workspace (the single-GPU memory ceiling of BASELINE.json) ----------
+def test_c5_memory_ceiling_setup_and_first_iterations():
+    import time
+    import torch
+    import paper_2403_01039_b200 as lib
+    cfg = get_config("C5")
+    sv = solvent_by_name(cfg.solvent)
+    free, total = torch.cuda.mem_get_info()
+    s = None
+    try:
+        s = lib.Solver(cfg.n, cfg.spacing, sv.n_v, closure=cfg.closure, mdiis_nvec=cfg.mdiis_nvec, mdiis_b=cfg.mdiis_b,
+                       mdiis_restart=cfg.mdiis_restart)
+    except torch.OutOfMemoryError:
+        pytest.skip(f"needs {54} GB of device memory, {free / 1e9:.0f} GB free")
+    assert 50e9 < s.workspace.numel() < 60e9             # (2M + 3) field-sets of 4.29 GB + phi, phi~
+    sol = make_solute("C5")
+    k0, dk, chi = load_chi(sv.name)
+    s.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+    s.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=cfg.rcut)
+    # sampled setup fields against the oracle (64-bit offsets: site 3 starts 3.2e9 bytes into the field-set)
+    rng = np.random.default_rng(55)
+    idx = _sample_points(cfg, sol, rng, 150, 150)
+    pts = (idx - cfg.n // 2) * cfg.spacing
+    beta = 1.0 / (o3.K_BOLTZMANN * cfg.temperature)
+    w_o = o3.w_short_at(pts, sol.xyz, sol.q, sol.sigma, sol.eps, sv.q, sv.sigma, sv.eps, beta, cfg.r_min, cfg.kappa,
+                        cfg.rcut)
+    phi_o = o3.phi_at(pts, sol.xyz, sol.q, beta, cfg.kappa)
+    phi = s.get_field_device("PHI", 0)[idx[:, 0], idx[:, 1], idx[:, 2]].cpu().numpy()
+    assert np.max(np.abs(phi - phi_o)) < 1e-10 * np.max(np.abs(phi_o))
+    for g in (0, 3):
+        w = s.get_field_device("W", g)[idx[:, 0], idx[:, 1], idx[:, 2]].cpu().numpy()
+        finite = np.abs(w_o[g]) < 600.0
+        assert np.max(np.abs(w - w_o[g])[finite]) < 1e-9 * np.maximum(1.0, np.abs(w_o[g][finite])).max()
+    # the loop runs, the residual falls, and G = closure(W + TAU) at sampled points
+    n_done, rms = s.iterate(12, 0.0)
+    hist = s.rms_history()
+    assert n_done == 12 and np.all(np.isfinite(hist)) and hist[-1] < 0.5 * hist[0]
+    for g in (1, 2):
+        w = s.get_field_device("W", g)[idx[:, 0], idx[:, 1], idx[:, 2]].cpu().numpy()
+        t = s.get_field_device("TAU", g)[idx[:, 0], idx[:, 1], idx[:, 2]].cpu().numpy()
+        gg = s.get_field_device("G", g)[idx[:, 0], idx[:, 1], idx[:, 2]].cpu().numpy()
+        expect = o3.closure_g(w + t, cfg.closure, cfg.pse_order)
+        assert np.max(np.abs(gg - expect)) < 1e-12 * max(1.0, expect.max())
+    s.close()
