@@ -213,7 +213,16 @@ template <int NZ> struct ZPlan : FftCfg<NZ> { enum { GF = FftCfg<NZ>::G, MBF = 1
 #ifndef R3D_ZMBG
 #define R3D_ZMBG 5
 #endif
+#ifndef R3D_ZPLAN64
+#define R3D_ZPLAN64 2
+#endif
+#if R3D_ZPLAN64 == 0
 template <> struct ZPlan<64>  { enum { R1 = 8, R2 = 8, R3 = 1, T = 8, G = 4, GF = 4, MBF = 2, GI = 4, MBI = 2, MBG = 2 }; };
+#elif R3D_ZPLAN64 == 1
+template <> struct ZPlan<64>  { enum { R1 = 4, R2 = 4, R3 = 4, T = 16, G = 2, GF = 1, MBF = 4, GI = 1, MBI = 8, MBG = 5 }; };
+#else
+template <> struct ZPlan<64>  { enum { R1 = 8, R2 = 8, R3 = 1, T = 8, G = 4, GF = 2, MBF = 4, GI = 2, MBI = 8, MBG = 5 }; };
+#endif
 template <> struct ZPlan<128> { enum { R1 = 4, R2 = 4, R3 = 8, T = 16, G = 2, GF = R3D_ZGF, MBF = R3D_ZMBF, GI = R3D_ZGI, MBI = R3D_ZMBI, MBG = R3D_ZMBG }; };
 #ifndef R3D_Z256_PLAN
 #define R3D_Z256_PLAN 0
