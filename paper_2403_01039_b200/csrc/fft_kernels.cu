@@ -564,13 +564,14 @@ template <int NZ>
 static int launch_zinv_n(const Grid& gr, const Buffers& b, const SolverParams& sp, double* raw_out, cudaStream_t s) {
   if (raw_out) return launch_zinv_nm<NZ, -1, false>(gr, b, sp, raw_out, s);
   if (sp.accel == RISM3D_ACCEL_ANDERSON) return launch_zinv_nm<NZ, 2, true>(gr, b, sp, raw_out, s);   // 3 stored pairs
-#define R3D_ZG(MO) case MO + 1: return launch_zinv_nm<NZ, MO, false>(gr, b, sp, raw_out, s)
-  switch (sp.M) {
-    R3D_ZG(0); R3D_ZG(1); R3D_ZG(2); R3D_ZG(3); R3D_ZG(4); R3D_ZG(5); R3D_ZG(6); R3D_ZG(7);
-    R3D_ZG(8); R3D_ZG(9); R3D_ZG(10); R3D_ZG(11); R3D_ZG(12); R3D_ZG(13); R3D_ZG(14); R3D_ZG(15);
-    default: return 0;
-  }
-#undef R3D_ZG
+  // compiled for a few history sizes only (each bounds the unrolled Gram loop); M - 1 rounds up to the next one
+  const int mo = sp.M - 1;
+  if (mo <= 0) return launch_zinv_nm<NZ, 0, false>(gr, b, sp, raw_out, s);
+  if (mo <= 2) return launch_zinv_nm<NZ, 2, false>(gr, b, sp, raw_out, s);
+  if (mo <= 4) return launch_zinv_nm<NZ, 4, false>(gr, b, sp, raw_out, s);
+  if (mo <= 7) return launch_zinv_nm<NZ, 7, false>(gr, b, sp, raw_out, s);
+  if (mo <= 9) return launch_zinv_nm<NZ, 9, false>(gr, b, sp, raw_out, s);
+  return launch_zinv_nm<NZ, MAX_M - 1, false>(gr, b, sp, raw_out, s);
 }
 
 template <int NZ>
