@@ -138,7 +138,8 @@ int rism3d_pmv(rism3d_ctx* ctx, double chi_t, double* pmv, double* c_int_site);
 /* Solvent-induced gradient of the free energy on the solute atoms (the equation after Eq. 23;
  * common to HNC and KH):  d(dmu)/dR_a = sum_g rho_g int g_g(r) du_g(r)/dR_a dr,  kcal/(mol A), with u of Eq. 22, all
  * pairs (no cutoff), the distance clamp r_min as in the potential.  grad: HOST [n_atoms][3] of the last set_solute.
- * The force on atom a is minus this.  Uses the k-space work array as scratch (no effect on a later iterate). */
+ * The force on atom a is minus this.  Uses the k-space work array and the history slot the next iteration overwrites
+ * anyway as scratch (no effect on a later iterate). */
 int rism3d_gradient(rism3d_ctx* ctx, double* grad);
 
 /* Copy one field of one site (nx*ny*nz doubles, [ix][iy][iz]) to dst; dst_is_device selects a

@@ -542,24 +542,30 @@ extern "C" int rism3d_gradient(rism3d_ctx* ctx, double* grad) {
   const Grid& g = ctx->g;
   const int na = ctx->n_atoms;
   if (na == 0) return RISM3D_OK;
-  // everything lives in the k-space work array, which holds nothing between iterations: tables, partial sums, result
+  // Scratch: the k-space work array (nothing lives there between iterations) takes rho dV g; the history slot `cur`
+  // that the NEXT (Z, R) pair will overwrite -- an unused slot, or the oldest entry, which the trailing update of
+  // iterate has already consumed and the next Gram row skips -- takes the tables, the partial sums and the result.
+  int rc = read_header(ctx);
+  if (rc) return rc;
+  const int cur = ctx->h_hdr->cur;
   const size_t b_atoms = align256((size_t)na * 4 * 8), b_pair = align256((size_t)na * g.nv * 3 * 8);
   const size_t b_out = align256((size_t)na * 3 * 8);
   const size_t avail = g.field * 8;
   if (b_atoms + b_pair + b_out + (size_t)na * 3 * 16 > avail)
-    return fail(ctx, RISM3D_ERR_WORKSPACE, "%d atoms do not fit the scratch array of this grid", na);
+    return fail(ctx, RISM3D_ERR_WORKSPACE, "%d atoms do not fit one field-set of scratch on this grid", na);
   size_t nchunks = (g.npts + 8191) / 8192;                 // >= 8192 points per block, fewer blocks if memory is short
   const size_t max_chunks = (avail - b_atoms - b_pair - b_out) / ((size_t)na * 3 * 16);
   if (nchunks > max_chunks) nchunks = max_chunks;
-  if (nchunks > 4096) nchunks = 4096;
-  char* base = (char*)ctx->b.work;
+  if (nchunks > 2048) nchunks = 2048;
+  char* base = (char*)(ctx->b.R + (size_t)cur * g.field);
   double* d_atoms = (double*)base;
   double* d_pair = (double*)(base + b_atoms);
   double* d_out = (double*)(base + b_atoms + b_pair);
   double* d_part = (double*)(base + b_atoms + b_pair + b_out);
   CU(cudaMemcpyAsync(d_atoms, ctx->h_atoms->data(), (size_t)na * 4 * 8, cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaMemcpyAsync(d_pair, ctx->h_pair->data(), (size_t)na * g.nv * 3 * 8, cudaMemcpyHostToDevice, ctx->stream));
-  ctx->launches += launch_gradient(g, ctx->b, ctx->sp, na, d_atoms, d_pair, d_part, (int)nchunks, d_out, ctx->stream);
+  ctx->launches += launch_gradient(g, ctx->b, ctx->sp, na, (double*)ctx->b.work, d_atoms, d_pair, d_part, (int)nchunks,
+                                   d_out, ctx->stream);
   CU(cudaGetLastError());
   CU(cudaMemcpyAsync(grad, d_out, (size_t)na * 3 * 8, cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));

@@ -109,7 +109,7 @@ int launch_potential(const Grid&, const Buffers&, const SolverParams&, int n_ato
                      const double* d_pair, double rcut, cudaStream_t);
 int launch_phi_tilde(const Grid&, const Buffers&, const SolverParams&, int n_atoms, const double* d_atoms,
                      double2* d_phase, cudaStream_t);
-int launch_gradient(const Grid&, const Buffers&, const SolverParams&, int n_atoms, const double* d_atoms,
+int launch_gradient(const Grid&, const Buffers&, const SolverParams&, int n_atoms, double* d_gw, const double* d_atoms,
                     const double* d_pair, double* d_partial, int nchunks, double* d_out, cudaStream_t);
 int launch_free_energy(const Grid&, const Buffers&, const SolverParams&, double* d_out, cudaStream_t);
 int launch_get_field(const Grid&, const Buffers&, const SolverParams&, int which, int site, double* d_dst,

@@ -367,20 +367,30 @@ int launch_get_field(const Grid& g, const Buffers& b, const SolverParams& sp, in
 // Solvent-induced gradient on the solute atoms (the equation after Eq. 23):
 //   d(dmu)/dR_a = sum_g rho_g dV sum_r g_g(r) du_g(r)/dR_a,   u of Eq. 22, all pairs, distance clamp of Q11
 //   du_g/dR_a = [C q_a q_g / r^3 + 4 eps_ag (12 s^12/r^14 - 6 s^6/r^8)] (r - R_a)
-// Grid: (point chunks, chunks of GRAD_ATOMS atoms).  A thread walks its points, forms g = closure(w + tau) on the
-// fly and accumulates the 3 components for the block's atoms in registers; the block sum (double-double, fixed
+// Grid: (point chunks, chunks of GRAD_ATOMS atoms).  A thread walks its points, reads rho_g dV g_g(r) (formed once by
+// gradient_weights_kernel) and accumulates the 3 components for the block's atoms in registers; the block sum (double-double, fixed
 // order) goes to partial[chunk][atom][3]; gradient_final_kernel adds the chunks in order.  pair carries beta
 // (beta C q_a q_g, sigma_ag^2, 4 beta eps_ag), so the final sum is multiplied by kT.
 // ------------------------------------------------------------------------------------------------
 constexpr int GRAD_ATOMS = 8;
 constexpr int GRAD_THREADS = 256;
 
+// gw_g(r) = rho_g dV g_g(r), g = closure(w + tau): formed once per call, read by every atom chunk
+__global__ void gradient_weights_kernel(double* __restrict__ gw, const double* __restrict__ tau,
+                                        const double* __restrict__ w, const double* __restrict__ rhov, size_t npts,
+                                        int nv, double dv, int closure, int order) {
+  for (int g = 0; g < nv; ++g) {
+    const double f = rhov[g] * dv;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < npts; i += (size_t)gridDim.x * blockDim.x)
+      gw[(size_t)g * npts + i] = f * closure_g(w[(size_t)g * npts + i] + tau[(size_t)g * npts + i], closure, order);
+  }
+}
+
 template <int NV>
 __global__ void __launch_bounds__(GRAD_THREADS)
-    gradient_kernel(double* __restrict__ partial, const double* __restrict__ tau, const double* __restrict__ w,
-                    const double4* __restrict__ atoms, const double* __restrict__ pair, const double* __restrict__ rhov,
-                    int n_atoms, int n, double h, double ox, double oy, double oz, double r_min, size_t npts,
-                    size_t pts_per_block, int closure, int order) {
+    gradient_kernel(double* __restrict__ partial, const double* __restrict__ gwf, const double4* __restrict__ atoms,
+                    const double* __restrict__ pair, int n_atoms, int n, double h, double ox, double oy, double oz,
+                    double r_min, size_t npts, size_t pts_per_block) {
   __shared__ double4 s_atom[GRAD_ATOMS];
   __shared__ double s_pair[GRAD_ATOMS * NV * 3];
   __shared__ double s_red[GRAD_THREADS / 32][GRAD_ATOMS * 3][2];
@@ -393,7 +403,7 @@ __global__ void __launch_bounds__(GRAD_THREADS)
   double acc[GRAD_ATOMS][3];
 #pragma unroll
   for (int a = 0; a < GRAD_ATOMS; ++a) acc[a][0] = acc[a][1] = acc[a][2] = 0.0;
-  const double dv = h * h * h, rmin2 = r_min * r_min;
+  const double rmin2 = r_min * r_min;
   const size_t p0 = (size_t)blockIdx.x * pts_per_block;
   const size_t p1 = min(npts, p0 + pts_per_block);
   for (size_t idx = p0 + tid; idx < p1; idx += GRAD_THREADS) {
@@ -403,8 +413,7 @@ __global__ void __launch_bounds__(GRAD_THREADS)
     const double z = __dadd_rn(oz, __dmul_rn(h, (double)iz));
     double gw[NV];
 #pragma unroll
-    for (int g = 0; g < NV; ++g)
-      gw[g] = rhov[g] * dv * closure_g(w[(size_t)g * npts + idx] + tau[(size_t)g * npts + idx], closure, order);
+    for (int g = 0; g < NV; ++g) gw[g] = gwf[(size_t)g * npts + idx];
     // (compiler barrier: re-read the atom tables from shared memory for every point instead of pinning all
     //  GRAD_ATOMS * (4 + 3 NV) of them in registers across the loop)
     asm volatile("" ::: "memory");
@@ -467,18 +476,20 @@ __global__ void gradient_final_kernel(double* __restrict__ out, const double* __
   out[e] = kT * (hi + lo);
 }
 
-// d_atoms: [n_atoms] double4 (x, y, z, unused); d_pair as in launch_potential; d_partial: nchunks*n_atoms*3*2 doubles;
-// d_out: n_atoms*3 doubles.  Returns the number of kernels launched.
-int launch_gradient(const Grid& g, const Buffers& b, const SolverParams& sp, int n_atoms, const double* d_atoms,
-                    const double* d_pair, double* d_partial, int nchunks, double* d_out, cudaStream_t s) {
+// d_gw: one field-set of scratch; d_atoms: [n_atoms] double4 (x, y, z, unused); d_pair as in launch_potential;
+// d_partial: nchunks*n_atoms*3*2 doubles; d_out: n_atoms*3 doubles.  Returns the number of kernels launched.
+int launch_gradient(const Grid& g, const Buffers& b, const SolverParams& sp, int n_atoms, double* d_gw,
+                    const double* d_atoms, const double* d_pair, double* d_partial, int nchunks, double* d_out,
+                    cudaStream_t s) {
   if (n_atoms == 0) return 0;
+  gradient_weights_kernel<<<148 * 8, 256, 0, s>>>(d_gw, b.tau, b.w, b.rhov, g.npts, g.nv, g.h * g.h * g.h, sp.closure,
+                                                 sp.pse_order);
   const size_t per = (g.npts + nchunks - 1) / nchunks;
   dim3 grid((unsigned)nchunks, (unsigned)((n_atoms + GRAD_ATOMS - 1) / GRAD_ATOMS));
   const double4* at = reinterpret_cast<const double4*>(d_atoms);
 #define GRD(NV)                                                                                                     \
-  gradient_kernel<NV><<<grid, GRAD_THREADS, 0, s>>>(d_partial, b.tau, b.w, at, d_pair, b.rhov, n_atoms, g.n, g.h,   \
-                                                    g.origin[0], g.origin[1], g.origin[2], sp.r_min, g.npts, per,   \
-                                                    sp.closure, sp.pse_order)
+  gradient_kernel<NV><<<grid, GRAD_THREADS, 0, s>>>(d_partial, d_gw, at, d_pair, n_atoms, g.n, g.h, g.origin[0],   \
+                                                    g.origin[1], g.origin[2], sp.r_min, g.npts, per)
   switch (g.nv) {
     case 1: GRD(1); break;
     case 2: GRD(2); break;
@@ -488,7 +499,7 @@ int launch_gradient(const Grid& g, const Buffers& b, const SolverParams& sp, int
   }
 #undef GRD
   gradient_final_kernel<<<(n_atoms * 3 + 127) / 128, 128, 0, s>>>(d_out, d_partial, nchunks, n_atoms, sp.kT);
-  return 2;
+  return 3;
 }
 
 }  // namespace r3d
