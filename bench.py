@@ -33,8 +33,12 @@ import numpy as np
 
 METRIC = "3D-RISM iterations/s"
 UNIT = "iterations/s"
-CPU_SAMPLE_N = 64            # grid of the oracle's bounded sample (same box as the workload, coarser spacing)
-CPU_SAMPLE_ATOMS = 64        # the loop cost does not depend on the atom count; the (untimed) setup does
+# fp64 flops counted per atom - grid point pair by the setup rooflines: the w pair evaluation of
+# SURVEY.md section 8(d) (25 + 8 n_v: distance, 1/r, exp, then per site the screened Coulomb and 12-6 terms), the phi
+# pair on its common far path (distance 8, float rsqrt seed + two Newton steps 14, one FMA 2), the gradient pair
+FLOPS_W_PAIR = lambda n_v: 25 + 8 * n_v
+FLOPS_PHI_PAIR = 24
+FLOPS_GRAD_PAIR = lambda n_v: 30 + 12 * n_v
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -172,47 +176,101 @@ def workload_label(cfg, sol) -> str:
 # the oracle on a bounded sample (cpu_baseline leg and --impl reference)
 # ---------------------------------------------------------------------------------------------------------
 class OracleSample:
-    """The workload's box, solvent, closure and MDIIS settings on a CPU_SAMPLE_N^3 grid (coarser spacing, same
-    box edge) with the first CPU_SAMPLE_ATOMS atoms of its solute.  One oracle iteration costs the same per
-    grid-point*site whatever the atoms are, so iterations/s at the full grid = measured point*site rate /
-    (n^3 n_v)."""
+    """The oracle (oracle/, numpy fp64, as it stands) on the workload's box, solvent, closure and MDIIS settings:
+    at the workload's own grid when n_sample == cfg.n (no scaling anywhere), else on a coarser n_sample^3 grid over the
+    same box, its iterations/s scaled by the grid-point*site count.  The solute is the first `atoms` atoms: one oracle
+    iteration costs the same whatever the atoms are, and its (untimed) O(N N_a) numpy setup costs seconds per atom at
+    256^3."""
 
-    def __init__(self, name: str):
+    def __init__(self, name: str, n_sample: int, atoms: int):
         from oracle import rism3d as o3
         cfg, sv, sol, (k0, dk, chi) = workload_inputs(name)
         self.cfg, self.sv = cfg, sv
-        self.n = min(CPU_SAMPLE_N, cfg.n)
+        self.n = min(n_sample, cfg.n)
         self.spacing = cfg.spacing * cfg.n / self.n
-        na = min(CPU_SAMPLE_ATOMS, sol.n_atoms)
+        na = min(atoms, sol.n_atoms)
+        t0 = time.perf_counter()
         self.orc = o3.Rism3dOracle(self.n, self.spacing, sv.n_v, closure=cfg.closure, pse_order=cfg.pse_order,
                                    mdiis_nvec=cfg.mdiis_nvec, mdiis_b=cfg.mdiis_b, mdiis_restart=cfg.mdiis_restart)
         self.orc.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+        t1 = time.perf_counter()
         self.orc.set_solute(sol.xyz[:na], sol.q[:na], sol.sigma[:na], sol.eps[:na], rcut=cfg.rcut)
+        self.setup_s_per_atom = (time.perf_counter() - t1) / max(na, 1)
+        self.init_s = t1 - t0
         self.pt_sites_sample = float(self.n ** 3 * sv.n_v)
         self.pt_sites_full = float(cfg.n ** 3 * sv.n_v)
-        self.label = (f"{cfg.name} settings ({sv.n_v} sites, {cfg.closure}, MDIIS {cfg.mdiis_nvec}) on a {self.n}^3 grid at "
-                      f"{self.spacing:g} A (same {cfg.n * cfg.spacing:g} A box, 1/{int(self.pt_sites_full / self.pt_sites_sample)} "
-                      f"of the points), first {na} atoms; rate scaled by grid-point*site count")
+        self.full_size = self.n == cfg.n
+        grid = (f"the workload's own {cfg.n}^3 grid at {cfg.spacing:g} A" if self.full_size else
+                f"a {self.n}^3 grid at {self.spacing:g} A over the same {cfg.n * cfg.spacing:g} A box "
+                f"(1/{int(self.pt_sites_full / self.pt_sites_sample)} of the points; rate scaled by grid-point*site count)")
+        self.label = (f"{cfg.name} settings ({sv.n_v} sites, {cfg.closure}, MDIIS {cfg.mdiis_nvec}) on {grid}, "
+                      f"first {na} atoms of the solute")
 
     def run(self, steps: int, warmup: int):
-        """-> seconds per oracle iteration on the sample (history filled during the warm-up)."""
+        """-> seconds per oracle iteration on the sample"""
         self.orc.iterate(max(warmup, 0), 0.0)
         t0, c0 = time.perf_counter(), time.process_time()
         self.orc.iterate(steps, 0.0)
         wall = time.perf_counter() - t0
         self.threads_used = max(1, int(round((time.process_time() - c0) / wall)))   # CPU time / wall time
+        self.history_entries = min(self.cfg.mdiis_nvec, max(warmup, 0) + steps)
         return wall / steps
 
     def iterations_per_s_full(self, s_per_iter_sample: float) -> float:
         return (self.pt_sites_sample / s_per_iter_sample) / self.pt_sites_full
 
 
+def host_info() -> dict:
+    model = ""
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    mem_gb = 0.0
+    try:
+        import psutil
+        mem_gb = psutil.virtual_memory().available / 1e9
+    except Exception:
+        pass
+    return {"cpu_model": model, "nproc": os.cpu_count(), "host_mem_available_gb": round(mem_gb, 1)}
+
+
+# seconds per oracle iteration, measured once on an 8-core build box (used only to pick a sample that fits the time
+# budget; the reported numbers are always timed live)
+ORACLE_EST_S_PER_ITER = {256: 27.0, 128: 3.2, 64: 0.3, 32: 0.04}
+ORACLE_FULL_GRID_HOST_GB = 20.0
+
+
+def pick_sample_grid(cfg, n_iterations: int, budget_s: float, mem_gb: float) -> int:
+    """largest grid <= the workload's whose n_iterations oracle iterations fit the budget (and the host memory)"""
+    n = cfg.n
+    while n > 32:
+        est = ORACLE_EST_S_PER_ITER.get(n, 27.0 * (n / 256.0) ** 3) * n_iterations
+        mem_ok = n < 256 or mem_gb >= ORACLE_FULL_GRID_HOST_GB * (cfg.mdiis_nvec / 10.0 if n_iterations >= cfg.mdiis_nvec else 0.6)
+        if est <= budget_s and mem_ok:
+            return n
+        n //= 2
+    return n
+
+
 def run_reference(args):
+    """The reference arm = the CPU oracle on the box's host cores.  A step is one oracle iteration of a bounded sample
+    of the workload: the workload's own grid when W + K iterations of it fit ~5 minutes, else the largest coarser grid
+    over the same box that does (rate then scaled by grid-point*site count; `cpu_baseline.sample` says which)."""
     rank, _, world = dist_env()
     if rank != 0:
         return 0
-    smp = OracleSample(args.workload)
-    s_per = smp.run(args.steps, max(args.warmup, smp.cfg.mdiis_nvec))
+    from workloads import get_config
+    cfg0 = get_config(args.workload)
+    hi = host_info()
+    warm = max(args.warmup, 0)
+    n_s = pick_sample_grid(cfg0, warm + args.steps, 300.0, hi["host_mem_available_gb"])
+    smp = OracleSample(args.workload, n_s, 8 if n_s >= 256 else 32)
+    s_per = smp.run(args.steps, warm)
     val = smp.iterations_per_s_full(s_per)
     cfg = smp.cfg
     from workloads import make_solute
@@ -221,14 +279,22 @@ def run_reference(args):
         "warmup": args.warmup, "ms_per_step": s_per * 1e3 * smp.pt_sites_full / smp.pt_sites_sample,
         "ms_per_step_sample": s_per * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_label(cfg, make_solute(cfg.name)), "timing": "host perf_counter (CPU program)"},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": smp.threads_used, "kind": "oracle", "sample": smp.label,
-                         "host_cores_available": os.cpu_count()},
+        "config": bench_config(cfg, make_solute(cfg.name), 1),
+        "cpu_baseline": dict(value=val, unit=UNIT, cores=smp.threads_used, kind="oracle", sample=smp.label,
+                             full_size=smp.full_size, timing="host perf_counter (CPU program)",
+                             mdiis_history_entries=smp.history_entries, **hi),
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
     return 0
+
+
+def bench_config(cfg, sol, world: int) -> dict:
+    """the `config` object of the JSON line -- the same for both arms"""
+    return {"workload": workload_label(cfg, sol), "parallelism": f"replicas x{world} (no collective on the data path)",
+            "l2": "inputs larger than L2 (working set of a replica: (2M + 3) field-sets of %.2f GB)" % (cfg.n ** 3 * 4 * 8 / 1e9 if cfg.solvent != "water" else cfg.n ** 3 * 2 * 8 / 1e9),
+            "mdiis_history": "full (M entries) during the timed steps", "rcut_A": cfg.rcut}
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -254,6 +320,7 @@ def run_ours(args):
     solver.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
     setup_ms = solver.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=cfg.rcut)
     workspace_gb = solver.workspace.numel() / 1e9
+    dfma_tflops = solver.measure_dfma_peak()
 
     def barrier():
         if world > 1:
@@ -265,6 +332,7 @@ def run_ours(args):
     solver.iterate(warm, 0.0)
     launches0 = solver.launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # clocks are sampled from here to the end of the end-to-end solve: the timed steps alone last tens of milliseconds
     sampler = ClockSampler(local_rank) if rank == 0 else None
     barrier()
     ev0.record(solver.stream)
@@ -274,13 +342,15 @@ def run_ours(args):
     ms_local = ev0.elapsed_time(ev1)
     launches = solver.launch_count() - launches0
     value, ms_max = aggregate_throughput(float(args.steps), ms_local, dev)
+    if sampler is not None and not args.no_e2e:
+        # keep the device under the same load for about a second so that the clock record has tens of samples
+        solver.iterate(max(args.steps, int(1000.0 / max(ms_max / args.steps, 1e-3))), 0.0)
 
     # ---- per-kernel CUDA-event times (second pass over the same number of steps) -----------------------------
     solver.set_profiling(True)
     solver.iterate(args.steps, 0.0)
     kern_ms, prof_n = solver.timings()
     solver.set_profiling(False)
-    clocks = sampler.stop() if sampler else None
     peak, peak_src = load_peaks()
     words = kernel_words(n_v, M)
     kernels = {}
@@ -301,6 +371,7 @@ def run_ours(args):
 
     # ---- end to end: one whole solve from HOST inputs to HOST results through the C ABI ------------------------
     e2e = None
+    clocks = None
     if not args.no_e2e:
         g_host = torch.empty((n_v, cfg.n, cfg.n, cfg.n), dtype=torch.float64, pin_memory=True)
         g_np = g_host.numpy()
@@ -317,14 +388,49 @@ def run_ours(args):
         t3 = time.perf_counter()
         (e2e_s,) = reduce_scalars([t3 - t0], "max", dev)
         (it_total,) = reduce_scalars([float(it_conv)], "sum", dev)
+        clocks = sampler.stop() if sampler else None
+        sampler = None
         e2e = {"value": it_total / e2e_s, "unit": UNIT,
                "h2d_bytes_per_step": int(sol.n_atoms * 6 * 8), "d2h_bytes_per_step": int(g_np.nbytes + 8 * (n_v + 1) + 64),
                "what": "one whole solve per replica: set_solute (host atom arrays -> device, S0) + iterate to rms < tol + "
                        "free_energy + g of every site copied to pinned host memory; a 'step' of this leg is the solve",
                "seconds_to_converge": e2e_s, "iterations_to_converge": int(it_conv), "converged": bool(rms_conv < cfg.tol),
                "tol": cfg.tol, "rms": rms_conv, "setup_ms": setup_ms_e2e, "loop_s": t1 - t0 - setup_ms_e2e * 1e-3,
-               "free_energy_ms": (t2 - t1) * 1e3, "get_g_ms": (t3 - t2) * 1e3, "dmu_kcal_mol": mu,
-               "g_max": float(g_np.max())}
+               "free_energy_ms": (t2 - t1) * 1e3, "phi_ms": solver.phi_ms(), "get_g_ms": (t3 - t2) * 1e3,
+               "dmu_kcal_mol": mu, "g_max": float(g_np.max())}
+    if sampler is not None:
+        clocks = sampler.stop()
+
+    # ---- setup (S0) and gradient against the measured fp64 FMA peak (they are bound by plain fp64 arithmetic) ---------
+    setup = None
+    if rank == 0:
+        npts, na = float(cfg.n ** 3), float(sol.n_atoms)
+        if cfg.rcut > 0:
+            dv = cfg.spacing ** 3
+            pairs_w = na * 4.0 / 3.0 * np.pi * cfg.rcut ** 3 / dv          # pairs inside the cutoff (spheres inside the box)
+        else:
+            pairs_w = npts * na
+        t0 = time.perf_counter()
+        solver.get_field_device("PHI", 0)                                   # forces the deferred phi kernel when it has not run
+        phi_ms = solver.phi_ms()
+        setup = {"bound": "alu", "peak_tflops_fp64": dfma_tflops, "peak_source": "measured (rism3d_measure_dfma_peak, independent DFMA chains)",
+                 "setup_ms": setup_ms, "what": ("w from the cell list + phi~ (the loop's inputs)" if cfg.rcut > 0 else "w + phi all pairs, phi~"),
+                 "w_pairs": pairs_w, "w_flops_per_pair": FLOPS_W_PAIR(n_v),
+                 "w_pairs_per_s_upper": pairs_w / (setup_ms * 1e-3),
+                 "w_frac_of_dfma_peak_upper": pairs_w * FLOPS_W_PAIR(n_v) / (setup_ms * 1e-3) / 1e12 / dfma_tflops if dfma_tflops else None,
+                 "note": "setup_ms also holds the phi~ kernels; with a cutoff most of the w kernel's time goes into distance tests of "
+                         "candidate atoms outside the cutoff, which the pair count does not include"}
+        if cfg.rcut > 0 and phi_ms > 0:
+            setup.update({"phi_ms": phi_ms, "phi_pairs": npts * na, "phi_flops_per_pair": FLOPS_PHI_PAIR,
+                          "phi_pairs_per_s": npts * na / (phi_ms * 1e-3),
+                          "phi_frac_of_dfma_peak": npts * na * FLOPS_PHI_PAIR / (phi_ms * 1e-3) / 1e12 / dfma_tflops if dfma_tflops else None})
+        if not args.no_e2e:
+            torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            solver.gradient()
+            grad_ms = (time.perf_counter() - t0) * 1e3
+            setup.update({"gradient_ms": grad_ms, "gradient_pairs": npts * na, "gradient_flops_per_pair": FLOPS_GRAD_PAIR(n_v),
+                          "gradient_frac_of_dfma_peak": npts * na * FLOPS_GRAD_PAIR(n_v) / (grad_ms * 1e-3) / 1e12 / dfma_tflops if dfma_tflops else None})
 
     # ---- context: the hand-written 3D transform pair next to cuFFT (torch.fft, never on the product path) ------------
     fft_cmp = None
@@ -383,31 +489,80 @@ def run_ours(args):
                     "seconds_to_converge": a_s, "iterations_to_converge": int(a_it), "converged": bool(a_rms < cfg.tol),
                     "ms_per_iteration": (a_s - a_setup * 1e-3) / max(a_it, 1) * 1e3, "dmu_kcal_mol": a_mu}
 
+    # ---- the other large configs, briefly (device-resident iterations only): C3 and the memory-ceiling C5 --------------
+    others = None
+    if rank == 0 and world == 1 and not args.no_others and args.workload == "C4":
+        solver.close()
+        others = {}
+        for name in ("C3", "C5"):
+            try:
+                others[name] = quick_workload(lib, name, local_rank, peak)
+            except Exception as ex:                               # e.g. not enough device memory for C5
+                others[name] = {"error": str(ex)[:200]}
+        torch.cuda.empty_cache()
+
     # ---- the oracle on the host cores (rank 0, single-GPU runs only) --------------------------------------------
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        smp = OracleSample(args.workload)
-        s_per = smp.run(args.cpu_steps, M)
-        cpu = {"value": smp.iterations_per_s_full(s_per), "unit": UNIT, "cores": smp.threads_used, "kind": "oracle",
-               "sample": smp.label + f"; {args.cpu_steps} timed iterations after {M} warm-up",
-               "s_per_iteration_sample": s_per, "host_cores_available": os.cpu_count()}
+        hi = host_info()
+        n_s = pick_sample_grid(cfg, 1 + args.cpu_steps, 120.0, hi["host_mem_available_gb"])
+        smp = OracleSample(args.workload, n_s, 8 if n_s >= 256 else 32)
+        s_per = smp.run(args.cpu_steps, 1)
+        cpu = dict(value=smp.iterations_per_s_full(s_per), unit=UNIT, cores=smp.threads_used, kind="oracle",
+                   sample=smp.label + f"; {args.cpu_steps} timed iterations after 1 warm-up (the MDIIS history holds "
+                                      f"{smp.history_entries} of {M} entries: the oracle's accelerator cost is still growing)",
+                   full_size=smp.full_size, s_per_iteration_sample=s_per, setup_s_per_atom=smp.setup_s_per_atom, **hi)
 
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_label(cfg, sol), "parallelism": f"replicas x{world} (no collective on the data path)",
-                       "l2": "inputs larger than L2 (working set %.1f GB per replica)" % workspace_gb,
-                       "mdiis_history": "full (M entries) during the timed steps", "rcut_A": cfg.rcut},
+            "config": bench_config(cfg, sol, world), "workspace_gb": workspace_gb,
             "pt_site_updates_per_s": value * pt_sites, "setup_ms": setup_ms, "rms_after_timed_steps": rms_end,
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "e2e_modified_anderson": anderson, "fft_compare": fft_cmp, "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": roofline, "setup": setup, "other_workloads": others, "cpu_baseline": cpu, "e2e": e2e, "e2e_modified_anderson": anderson, "fft_compare": fft_cmp, "gpu_launches": int(launches), "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
     solver.close()
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def quick_workload(lib, name: str, device: int, peak: float, steps: int = 10) -> dict:
+    """ms per iteration and per-kernel roofline fractions of another config (full MDIIS history, device resident)"""
+    import torch
+    cfg, sv, sol, (k0, dk, chi) = workload_inputs(name)
+    M, n_v = cfg.mdiis_nvec, sv.n_v
+    pt_sites = float(cfg.n ** 3 * n_v)
+    s = lib.Solver(cfg.n, cfg.spacing, n_v, closure=cfg.closure, pse_order=cfg.pse_order, mdiis_nvec=M, mdiis_b=cfg.mdiis_b,
+                   mdiis_restart=cfg.mdiis_restart, temperature=cfg.temperature, kappa=cfg.kappa, r_min=cfg.r_min, device=device)
+    try:
+        s.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+        setup_ms = s.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=cfg.rcut)
+        s.iterate(max(M, 3), 0.0)
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(s.stream)
+        s.iterate(steps, 0.0)
+        ev1.record(s.stream)
+        torch.cuda.synchronize()
+        ms = ev0.elapsed_time(ev1) / steps
+        s.set_profiling(True)
+        s.iterate(steps, 0.0)
+        kern_ms, _ = s.timings()
+        s.set_profiling(False)
+        words = kernel_words(n_v, M)
+        out = {"workload": workload_label(cfg, sol), "ms_per_iteration": ms, "setup_ms": setup_ms,
+               "workspace_gb": s.workspace.numel() / 1e9,
+               "iteration_frac_of_hbm_peak": sum(words.values()) * 8.0 * pt_sites / 1e9 / (ms * 1e-3) / peak,
+               "kernels": {k: {"ms": v, "frac": (words[k] * 8.0 * pt_sites / 1e9 / (v * 1e-3) / peak if v > 0 else 0.0)}
+                           for k, v in kern_ms.items()}}
+        if cfg.n <= 128:
+            out["note"] = "field-set of 67 MB: largely L2 resident, the HBM roofline does not bind"
+        return out
+    finally:
+        s.close()
+        del s
 
 
 def ncu_traffic(kernel: str, workload: str):
@@ -429,7 +584,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C4", choices=["C1", "C2", "C3", "C4", "C5"])
     ap.add_argument("--max-iter", type=int, default=1500, help="iteration cap of the end-to-end solve")
-    ap.add_argument("--cpu-steps", type=int, default=4, help="timed oracle iterations of the cpu_baseline leg")
+    ap.add_argument("--cpu-steps", type=int, default=3, help="timed oracle iterations of the cpu_baseline leg")
+    ap.add_argument("--no-others", action="store_true", help="skip the short C3 / C5 runs of other_workloads")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-anderson", action="store_true", help="skip the extra modified-Anderson solve")

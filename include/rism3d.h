@@ -112,11 +112,19 @@ int rism3d_set_solvent_chi(rism3d_ctx* ctx, const double* q, const double* sigma
 /* Solute (Eq. 22).  HOST arrays xyz [n_atoms][3], q, sigma, eps [n_atoms].
  * rcut <= 0: all pairs (the paper's definition); rcut > 0: the short-range remainder
  * -beta [C q q exp(-kappa r)/r + LJ] only counts pairs with r < rcut (Q12); the
- * long-range functions phi, phi~ are never cut.  Runs the setup kernels, sets tau = 0 (the paper's
+ * long-range functions phi, phi~ are never cut.  With rcut > 0 the atoms are binned into cells of edge rcut / 2 and
+ * every grid point visits only the cells within reach (same pair set as the plain loop over all atoms with the test
+ * r < rcut).  Runs the setup kernels, sets tau = 0 (the paper's
  * initial guess t = f) and clears the MDIIS history.  setup_ms (may be NULL)
  * receives the GPU time of the setup kernels in milliseconds (CUDA events). */
 int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz, const double* q,
                       const double* sigma, const double* eps, double rcut, float* setup_ms);
+
+/* GPU time, in milliseconds, of the deferred phi(r) kernel of the current solute (Eq. 29): with rcut > 0 set_solute
+ * computes only what the loop reads (w from a cell list, phi~); phi(r), which is never cut off and costs an all-pairs
+ * pass, is computed by the first call that needs it (free_energy, pmv, get_field T / PHI).  0 while it has not run
+ * or when set_solute computed it (rcut <= 0). */
+int rism3d_phi_ms(rism3d_ctx* ctx, float* ms);
 
 /* Run the loop.  tol <= 0: exactly max_iter iterations.  tol > 0: stop after the first iteration
  * whose rms residual is below tol (tau is then left unchanged by that iteration) or after max_iter.
@@ -154,6 +162,11 @@ int rism3d_get_rms_history(rism3d_ctx* ctx, double* dst, int cap, int* n);
 
 /* Number of kernels the library has launched on this context so far (for bench.py's gpu_launches). */
 long long rism3d_launch_count(const rism3d_ctx* ctx);
+
+/* Measured fp64 FMA peak of the context's device in TFLOP/s (2 flops per FMA; a microbenchmark of independent DFMA
+ * chains, best of 4 launches, CUDA events): the roofline denominator of the setup kernels (S0) and of
+ * rism3d_gradient, which are bound by plain fp64 arithmetic. */
+int rism3d_measure_dfma_peak(rism3d_ctx* ctx, double* tflops);
 
 /* Per-kernel GPU time of the loop kernels (CUDA events on the context's stream, one before and one after
  * every kernel of an iteration).  set_profiling(1) clears the sums and switches the events on,

@@ -20,7 +20,7 @@ FIELDS = {"G": 0, "H": 1, "C_SR": 2, "T": 3, "TAU": 4, "W": 5, "PHI": 6}
 EXPORTED_SYMBOLS = [
     "rism3d_workspace_bytes", "rism3d_init", "rism3d_set_solvent_chi", "rism3d_set_solute",
     "rism3d_iterate", "rism3d_free_energy", "rism3d_pmv", "rism3d_gradient", "rism3d_get_field", "rism3d_set_tau",
-    "rism3d_get_rms_history", "rism3d_launch_count", "rism3d_set_profiling", "rism3d_get_timings",
+    "rism3d_get_rms_history", "rism3d_launch_count", "rism3d_phi_ms", "rism3d_measure_dfma_peak", "rism3d_set_profiling", "rism3d_get_timings",
     "rism3d_loop_kernel_name", "rism3d_debug_fft_forward",
     "rism3d_debug_fft_inverse", "rism3d_last_error", "rism3d_status_string", "rism3d_destroy",
 ]
@@ -83,6 +83,10 @@ def load_library():
     lib.rism3d_pmv.argtypes = [C.c_void_p, C.c_double, dp, dp]
     lib.rism3d_gradient.restype = C.c_int
     lib.rism3d_gradient.argtypes = [C.c_void_p, dp]
+    lib.rism3d_measure_dfma_peak.restype = C.c_int
+    lib.rism3d_measure_dfma_peak.argtypes = [C.c_void_p, dp]
+    lib.rism3d_phi_ms.restype = C.c_int
+    lib.rism3d_phi_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
     lib.rism3d_get_field.restype = C.c_int
     lib.rism3d_get_field.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int]
     lib.rism3d_set_tau.restype = C.c_int
@@ -190,6 +194,18 @@ def rism3d_gradient(ctx, n_atoms: int) -> np.ndarray:
     return out
 
 
+def rism3d_measure_dfma_peak(ctx) -> float:
+    tf = C.c_double(0.0)
+    _check(ctx, load_library().rism3d_measure_dfma_peak(ctx, C.byref(tf)))
+    return float(tf.value)
+
+
+def rism3d_phi_ms(ctx) -> float:
+    ms = C.c_float(0.0)
+    _check(ctx, load_library().rism3d_phi_ms(ctx, C.byref(ms)))
+    return float(ms.value)
+
+
 def rism3d_get_field(ctx, which: int, site: int, dst_ptr: int, dst_is_device: bool):
     _check(ctx, load_library().rism3d_get_field(ctx, int(which), int(site), C.c_void_p(dst_ptr), int(dst_is_device)))
 
@@ -292,10 +308,22 @@ class Solver:
             pass
 
     def set_solvent_chi(self, q, sigma, eps, rho, k0, dk, chi):
+        # the C side reads n_sites entries of each array and n_k * n_sites^2 of chi: check before handing pointers over
+        q, sigma, eps, rho, chi = _f64(q), _f64(sigma), _f64(eps), _f64(rho), _f64(chi)
+        for name, a in (("q", q), ("sigma", sigma), ("eps", eps), ("rho", rho)):
+            if a.shape != (self.n_sites,):
+                raise ValueError(f"{name} must have shape ({self.n_sites},), got {a.shape}")
+        if chi.ndim != 3 or chi.shape[1:] != (self.n_sites, self.n_sites):
+            raise ValueError(f"chi must have shape (n_k, {self.n_sites}, {self.n_sites}), got {chi.shape}")
         rism3d_set_solvent_chi(self.ctx, q, sigma, eps, rho, k0, dk, chi)
 
     def set_solute(self, xyz, q, sigma, eps, rcut=0.0) -> float:
-        self.n_atoms = len(np.atleast_1d(q))
+        xyz, q, sigma, eps = _f64(xyz), _f64(np.atleast_1d(q)), _f64(np.atleast_1d(sigma)), _f64(np.atleast_1d(eps))
+        n_atoms = len(q)
+        xyz = xyz.reshape(0, 3) if xyz.size == 0 else xyz
+        if xyz.shape != (n_atoms, 3) or sigma.shape != (n_atoms,) or eps.shape != (n_atoms,):
+            raise ValueError(f"solute arrays disagree: xyz {xyz.shape}, q {q.shape}, sigma {sigma.shape}, eps {eps.shape}")
+        self.n_atoms = n_atoms
         return rism3d_set_solute(self.ctx, xyz, q, sigma, eps, rcut)
 
     def gradient(self) -> np.ndarray:
@@ -306,6 +334,12 @@ class Solver:
 
     def free_energy(self):
         return rism3d_free_energy(self.ctx, self.n_sites)
+
+    def measure_dfma_peak(self) -> float:
+        return rism3d_measure_dfma_peak(self.ctx)
+
+    def phi_ms(self) -> float:
+        return rism3d_phi_ms(self.ctx)
 
     def pmv(self, chi_t: float):
         return rism3d_pmv(self.ctx, chi_t, self.n_sites)
@@ -321,6 +355,7 @@ class Solver:
     def get_field_device(self, which: str, site: int):
         import torch
         out = torch.empty((self.n, self.n, self.n), dtype=torch.float64, device=self.device)
+        self.stream.wait_stream(torch.cuda.current_stream(self.device))     # the block may have pending uses there
         rism3d_get_field(self.ctx, FIELDS[which], site, out.data_ptr(), True)
         return out
 

@@ -37,6 +37,9 @@ struct rism3d_ctx {
   std::vector<double>* h_atoms;   // host copies of the solute tables (x, y, z, .) and (beta C q q, sigma^2, 4 beta eps)
   std::vector<double>* h_pair;    //   kept for rism3d_gradient: their device copies live in scratch the loop overwrites
   int n_atoms;
+  bool phi_valid;            // phi(r) has been computed for the current solute (with a cutoff it is computed when first
+                             // needed: the loop never reads it)
+  float phi_ms;              // GPU time of that deferred phi kernel
   StateHeader* h_hdr;        // pinned
   double* d_out;             // small device array for scalar results (inside workspace)
   char err[512];
@@ -58,19 +61,44 @@ static int fail(rism3d_ctx* c, int code, const char* fmt, ...) {
     if (e_ != cudaSuccess) return fail(ctx, RISM3D_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
   } while (0)
 
-// number of SMs of the current device (queried once; every context of this process runs on devices of one kind)
-static int g_num_sms = 0;
-int r3d::resident_ctas(int per_sm) {
-  if (g_num_sms == 0) {
-    int dev = 0, n = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0)
-      n = 148;
-    g_num_sms = n;
+// Every entry point that touches the GPU runs on the context's device, whatever device is current in the calling
+// thread, and leaves the caller's current device as it found it.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = (cudaSetDevice(dev) == cudaSuccess);
   }
-  return per_sm * g_num_sms;
-}
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+#define ON_CTX_DEVICE(ctx) DeviceGuard device_guard_((ctx)->p.device)
 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// TMA descriptor of a row-major 2D array of doubles [rows][row_len] with row pitch `pitch_bytes`, boxes of
+// box_rows x box_cols elements (cuTensorMapEncodeTiled, looked up through the runtime: no link-time libcuda)
+static bool make_tensor_map_2d(CUtensorMap* tm, void* base, uint64_t row_len, uint64_t rows, uint64_t pitch_bytes,
+                               uint32_t box_cols, uint32_t box_rows) {
+  typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || fn == nullptr ||
+      qres != cudaDriverEntryPointSuccess)
+    return false;
+  const cuuint64_t dims[2] = {row_len, rows};
+  const cuuint64_t strides[1] = {pitch_bytes};
+  const cuuint32_t box[2] = {box_cols, box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  return ((encode_fn)fn)(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, base, dims, strides, box, estr,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 
 static bool valid_params(const rism3d_params* p) {
   if (!p) return false;
@@ -82,6 +110,10 @@ static bool valid_params(const rism3d_params* p) {
   if (((n / 2) * nv) % 8) return false;             // tile rows are 8 complex wide
   if (p->mdiis_nvec < 1 || p->mdiis_nvec > MAX_M) return false;
   if (!(p->spacing > 0.0) || !(p->temperature > 0.0) || !(p->kappa > 0.0)) return false;
+  // r_min = 0 (e.g. a zero-initialised struct) would put 1/0 into w for a grid point on an atom (Q11); the clamp must
+  // also stay well inside the float range of the rsqrt seed.  The mixing parameter must be positive.
+  if (!(p->r_min >= 1e-6) || !(p->r_min < 1e6) || !(p->mdiis_b > 0.0) || !(p->mdiis_b < 1e6)) return false;
+  if (kspace_smem_bytes(n, nv) <= 0 || kspace_smem_bytes(n, nv) > 227 * 1024) return false;   // e.g. (512, 1 site)
   if (p->closure != RISM3D_KH && p->closure != RISM3D_PSE && p->closure != RISM3D_HNC) return false;
   if (p->closure == RISM3D_PSE && p->pse_order < 1) return false;
   if (p->accelerator != RISM3D_ACCEL_MDIIS && p->accelerator != RISM3D_ACCEL_ANDERSON) return false;
@@ -168,7 +200,13 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
   if (((uintptr_t)d_workspace) & 255) return RISM3D_ERR_ARG;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= p->device || p->device < 0) return RISM3D_ERR_CUDA;
-  if (cudaSetDevice(p->device) != cudaSuccess) return RISM3D_ERR_CUDA;
+  DeviceGuard device_guard_(p->device);
+  int cur_dev = -1, num_sms = 0, smem_optin = 0;
+  if (cudaGetDevice(&cur_dev) != cudaSuccess || cur_dev != p->device) return RISM3D_ERR_CUDA;
+  if (cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, p->device) != cudaSuccess || num_sms <= 0 ||
+      cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, p->device) != cudaSuccess)
+    return RISM3D_ERR_CUDA;
+  if (kspace_smem_bytes(p->nx, p->n_sites) > smem_optin) return RISM3D_ERR_SIZE;
   rism3d_ctx* ctx = new rism3d_ctx();
   memset(ctx, 0, sizeof(*ctx));
   ctx->p = *p;
@@ -181,6 +219,8 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
   for (int i = 0; i < 3; ++i) g.origin[i] = p->origin[i];
   g.npts = (size_t)g.n * g.n * g.n;
   g.field = g.npts * g.nv;
+  g.num_sms = num_sms;
+  g.smem_optin = smem_optin;
   SolverParams& sp = ctx->sp;
   sp.closure = p->closure;
   sp.pse_order = p->closure == RISM3D_PSE ? p->pse_order : 1;
@@ -196,6 +236,16 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
     const long double a = 3.14159265358979323846264338327950288L * (long double)j / (long double)g.n;
     tw[2 * j] = (double)cosl(a);
     tw[2 * j + 1] = (double)(-sinl(a));
+  }
+  if (kspace_uses_tma(g.n)) {
+    // k-space pass tiles: n rows (jx) of 8 complex = 16 doubles of `work`, and the matching 8 / nv phi~ values per row
+    const uint64_t q2 = (uint64_t)(g.n / 2) * g.nv * 2, h2 = (uint64_t)(g.n / 2) * 2;     // doubles per (jx, jy) row
+    if (!make_tensor_map_2d(&ctx->b.tm_work, ctx->b.work, (uint64_t)g.n * q2, (uint64_t)g.n, (uint64_t)g.n * q2 * 8, 16, (uint32_t)g.n) ||
+        !make_tensor_map_2d(&ctx->b.tm_phik, ctx->b.phik, (uint64_t)g.n * h2, (uint64_t)g.n, (uint64_t)g.n * h2 * 8,
+                            (uint32_t)(2 * 8 / g.nv), (uint32_t)g.n)) {
+      delete ctx;
+      return RISM3D_ERR_CUDA;
+    }
   }
   cudaError_t e = cudaMallocHost((void**)&ctx->h_hdr, sizeof(StateHeader));
   if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->b.tw, tw.data(), tw.size() * 8, cudaMemcpyHostToDevice, ctx->stream);
@@ -213,6 +263,7 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
 
 extern "C" void rism3d_destroy(rism3d_ctx* ctx) {
   if (!ctx) return;
+  ON_CTX_DEVICE(ctx);
   cudaStreamSynchronize(ctx->stream);
   if (ctx->ev_pool) {
     for (cudaEvent_t e : *ctx->ev_pool) cudaEventDestroy(e);
@@ -229,6 +280,7 @@ extern "C" void rism3d_destroy(rism3d_ctx* ctx) {
 extern "C" int rism3d_set_solvent_chi(rism3d_ctx* ctx, const double* q, const double* sigma, const double* eps,
                                       const double* rho, int n_k, double dk, double k0, const double* chi) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   if (!q || !sigma || !eps || !rho || !chi || n_k < 4 || !(dk > 0.0)) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   const Grid& g = ctx->g;
   double neutral = 0.0;
@@ -266,6 +318,7 @@ static int reset_state(rism3d_ctx* ctx) {
 extern "C" int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz, const double* q,
                                  const double* sigma, const double* eps, double rcut, float* setup_ms) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   if (n_atoms < 0 || (n_atoms > 0 && (!xyz || !q || !sigma || !eps))) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   if (!ctx->have_solvent) return fail(ctx, RISM3D_ERR_ORDER, "set_solvent_chi must come before set_solute");
   const Grid& g = ctx->g;
@@ -288,29 +341,87 @@ extern "C" int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz
       pair[(a * nv + s) * 3 + 2] = 4.0 * sp.beta * ep;
     }
   }
-  const size_t b_atoms = align256(atoms.size() * 8 + 8), b_pair = align256(pair.size() * 8 + 8);
+  // With a cutoff the short-range potential comes from a cell list (launch_w_cells): bin the atoms into cubic cells of
+  // edge >= rcut / 2 over their bounding box and sort them by cell index (z fastest), host side -- a counting sort of
+  // n_atoms records; phi(r), which is never cut off and which the loop never reads, is computed when first needed.
+  const bool cells = rcut > 0.0 && n_atoms > 0;
+  std::vector<int> cell_start;
+  std::vector<double> atoms_s, pair_s, q_s;          // the tables sorted by cell
+  int nc[3] = {1, 1, 1};
+  double clo[3] = {0.0, 0.0, 0.0}, cedge = rcut > 0.0 ? 0.5 * rcut : 1.0;
+  if (cells) {
+    double hi[3];
+    for (int k = 0; k < 3; ++k) { clo[k] = hi[k] = xyz[k]; }
+    for (size_t a = 0; a < na; ++a)
+      for (int k = 0; k < 3; ++k) { clo[k] = fmin(clo[k], xyz[3 * a + k]); hi[k] = fmax(hi[k], xyz[3 * a + k]); }
+    double span = fmax(hi[0] - clo[0], fmax(hi[1] - clo[1], hi[2] - clo[2]));
+    if (!(span < 1e300)) return fail(ctx, RISM3D_ERR_ARG, "non-finite atom coordinates");
+    if (span / cedge > 96.0) cedge = span / 96.0;                       // at most ~96 cells per axis
+    for (int k = 0; k < 3; ++k) nc[k] = (int)floor((hi[k] - clo[k]) / cedge) + 1;
+    const size_t ncell = (size_t)nc[0] * nc[1] * nc[2];
+    auto cell_of = [&](size_t a) {
+      size_t c[3];
+      for (int k = 0; k < 3; ++k) {
+        int i = (int)floor((xyz[3 * a + k] - clo[k]) / cedge);
+        c[k] = (size_t)(i < 0 ? 0 : (i >= nc[k] ? nc[k] - 1 : i));
+      }
+      return (c[0] * nc[1] + c[1]) * nc[2] + c[2];
+    };
+    cell_start.assign(ncell + 1, 0);
+    std::vector<size_t> cid(na);
+    for (size_t a = 0; a < na; ++a) { cid[a] = cell_of(a); cell_start[cid[a] + 1] += 1; }
+    for (size_t c = 0; c < ncell; ++c) cell_start[c + 1] += cell_start[c];
+    std::vector<int> fill(cell_start.begin(), cell_start.end() - 1);
+    atoms_s.resize(na * 4);
+    pair_s.resize(na * nv * 3);
+    for (size_t a = 0; a < na; ++a) {                                    // stable: atoms of a cell keep their input order
+      const size_t d = (size_t)fill[cid[a]]++;
+      for (int k = 0; k < 4; ++k) atoms_s[4 * d + k] = atoms[4 * a + k];
+      for (int k = 0; k < nv * 3; ++k) pair_s[d * nv * 3 + k] = pair[a * nv * 3 + k];
+    }
+    // the sorted tables replace the unsorted ones for the setup kernels of this call (phi~ is a sum over all atoms in
+    // any order; its charges follow the atom records); the host copies kept for rism3d_gradient stay in input order
+    q_s.resize(na);
+    std::vector<int> fill2(cell_start.begin(), cell_start.end() - 1);
+    for (size_t a = 0; a < na; ++a) q_s[(size_t)fill2[cid[a]]++] = q[a];
+  }
+  const std::vector<double>& up_atoms = cells ? atoms_s : atoms;
+  const std::vector<double>& up_pair = cells ? pair_s : pair;
+  const size_t b_atoms = align256((na * 5) * 8 + 8), b_pair = align256(pair.size() * 8 + 8);
   const size_t b_phase = align256((size_t)3 * na * g.n * 16 + 16);
-  if (b_atoms + b_pair + b_phase > ctx->scratch_bytes)
+  const size_t b_cells = align256(cell_start.size() * sizeof(int) + 8);
+  if (b_atoms + b_pair + b_phase + b_cells > ctx->scratch_bytes)
     return fail(ctx, RISM3D_ERR_WORKSPACE, "%d atoms need %zu scratch bytes, workspace has %zu", n_atoms,
-                b_atoms + b_pair + b_phase, ctx->scratch_bytes);
+                b_atoms + b_pair + b_phase + b_cells, ctx->scratch_bytes);
   char* scr = (char*)ctx->b.Z;                      // Z, R, tau, w, work are contiguous; the tables live in the
   // history part of the span (rebuilt by the iteration anyway), clear of tau and w, which the setup writes
   const size_t xr_bytes = (size_t)((char*)ctx->b.tau - (char*)ctx->b.Z);
-  if (b_atoms + b_pair + b_phase > xr_bytes)
+  if (b_atoms + b_pair + b_phase + b_cells > xr_bytes)
     return fail(ctx, RISM3D_ERR_WORKSPACE, "%d atoms need %zu scratch bytes, history span has %zu", n_atoms,
-                b_atoms + b_pair + b_phase, xr_bytes);
+                b_atoms + b_pair + b_phase + b_cells, xr_bytes);
   double* d_atoms = (double*)scr;
   double* d_pair = (double*)(scr + b_atoms);
   double2* d_phase = (double2*)(scr + b_atoms + b_pair);
+  int* d_cells = (int*)(scr + b_atoms + b_pair + b_phase);
   cudaEvent_t e0, e1;
   CU(cudaEventCreate(&e0));
   CU(cudaEventCreate(&e1));
   if (na) {
-    CU(cudaMemcpyAsync(d_atoms, atoms.data(), atoms.size() * 8, cudaMemcpyHostToDevice, ctx->stream));
-    CU(cudaMemcpyAsync(d_pair, pair.data(), pair.size() * 8, cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(d_atoms, up_atoms.data(), na * 4 * 8, cudaMemcpyHostToDevice, ctx->stream));
+    // raw charges right after the atom records (phi~ reads them there)
+    CU(cudaMemcpyAsync(d_atoms + 4 * na, cells ? q_s.data() : atoms.data() + 4 * na, na * 8,
+                       cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaMemcpyAsync(d_pair, up_pair.data(), up_pair.size() * 8, cudaMemcpyHostToDevice, ctx->stream));
+    if (cells) CU(cudaMemcpyAsync(d_cells, cell_start.data(), cell_start.size() * sizeof(int), cudaMemcpyHostToDevice, ctx->stream));
   }
   CU(cudaEventRecord(e0, ctx->stream));
-  ctx->launches += launch_potential(g, ctx->b, sp, n_atoms, d_atoms, d_pair, rcut, ctx->stream);
+  if (cells) {
+    ctx->launches += launch_w_cells(g, ctx->b, sp, d_atoms, d_pair, d_cells, nc, clo, cedge, rcut, ctx->stream);
+    ctx->phi_valid = false;
+  } else {
+    ctx->launches += launch_potential(g, ctx->b, sp, n_atoms, d_atoms, d_pair, rcut, ctx->stream);
+    ctx->phi_valid = true;
+  }
   CU(cudaGetLastError());
   ctx->launches += launch_phi_tilde(g, ctx->b, sp, n_atoms, d_atoms, d_phase, ctx->stream);
   CU(cudaGetLastError());
@@ -330,6 +441,7 @@ extern "C" int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz
   ctx->h_atoms->assign(atoms.begin(), atoms.begin() + 4 * na);
   *ctx->h_pair = pair;
   ctx->n_atoms = n_atoms;
+  ctx->phi_ms = 0.f;
   ctx->have_solute = true;
   return RISM3D_OK;
 }
@@ -437,6 +549,7 @@ static void enqueue_iterations(rism3d_ctx* ctx, int iters) {
 
 extern "C" int rism3d_set_profiling(rism3d_ctx* ctx, int enable) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   CU(cudaStreamSynchronize(ctx->stream));
   ctx->ev_used = 0;
   ctx->profiling = enable != 0;
@@ -447,6 +560,7 @@ extern "C" int rism3d_set_profiling(rism3d_ctx* ctx, int enable) {
 
 extern "C" int rism3d_get_timings(rism3d_ctx* ctx, double* ms_total, int cap, long long* n_iterations) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   if (!ms_total || cap < RISM3D_N_LOOP_KERNELS) return fail(ctx, RISM3D_ERR_ARG, "ms_total needs %d entries", RISM3D_N_LOOP_KERNELS);
   CU(cudaStreamSynchronize(ctx->stream));
   prof_collect(ctx);
@@ -468,6 +582,7 @@ static int read_header(rism3d_ctx* ctx) {
 
 extern "C" int rism3d_iterate(rism3d_ctx* ctx, int max_iter, double tol, int* n_done, double* rms) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   if (max_iter < 0) return fail(ctx, RISM3D_ERR_ARG, "max_iter < 0");
   if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before iterate");
   iterate_begin_kernel<<<1, 1, 0, ctx->stream>>>(ctx->b.state, tol);
@@ -499,10 +614,54 @@ extern "C" int rism3d_iterate(rism3d_ctx* ctx, int max_iter, double tol, int* n_
   return RISM3D_OK;
 }
 
+// phi(r) of the current solute, computed on first use when set_solute took the cell-list path (the loop never reads
+// phi; the free energy and the T / PHI getters do).  The atom table goes through the k-space work array, which holds
+// nothing between iterations.
+static int ensure_phi(rism3d_ctx* ctx) {
+  if (ctx->phi_valid) return RISM3D_OK;
+  const size_t na = (size_t)ctx->n_atoms;
+  if (na * 4 * 8 > ctx->g.field * 8) return fail(ctx, RISM3D_ERR_WORKSPACE, "%d atoms do not fit the work array", ctx->n_atoms);
+  double* d_atoms = (double*)ctx->b.work;
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0));
+  CU(cudaEventCreate(&e1));
+  CU(cudaMemcpyAsync(d_atoms, ctx->h_atoms->data(), na * 4 * 8, cudaMemcpyHostToDevice, ctx->stream));
+  CU(cudaEventRecord(e0, ctx->stream));
+  ctx->launches += launch_phi(ctx->g, ctx->b, ctx->sp, ctx->n_atoms, d_atoms, ctx->stream);
+  CU(cudaGetLastError());
+  CU(cudaEventRecord(e1, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  CU(cudaEventElapsedTime(&ctx->phi_ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  ctx->phi_valid = true;
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_measure_dfma_peak(rism3d_ctx* ctx, double* tflops) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
+  if (!tflops) return fail(ctx, RISM3D_ERR_ARG, "tflops is NULL");
+  CU(cudaStreamSynchronize(ctx->stream));
+  *tflops = measure_dfma_peak(ctx->g.num_sms, ctx->d_out, ctx->stream);
+  ctx->launches += 5;
+  CU(cudaGetLastError());
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_phi_ms(rism3d_ctx* ctx, float* ms) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (!ms) return fail(ctx, RISM3D_ERR_ARG, "ms is NULL");
+  *ms = ctx->phi_valid ? ctx->phi_ms : 0.f;
+  return RISM3D_OK;
+}
+
 extern "C" int rism3d_free_energy(rism3d_ctx* ctx, double* dmu_total, double* dmu_site) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   if (!dmu_total) return fail(ctx, RISM3D_ERR_ARG, "dmu_total is NULL");
   if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before free_energy");
+  { const int rc_phi = ensure_phi(ctx); if (rc_phi) return rc_phi; }
   ctx->launches += launch_free_energy(ctx->g, ctx->b, ctx->sp, ctx->d_out, ctx->stream);
   CU(cudaGetLastError());
   double host[MAX_NV];
@@ -519,8 +678,10 @@ extern "C" int rism3d_free_energy(rism3d_ctx* ctx, double* dmu_total, double* dm
 
 extern "C" int rism3d_pmv(rism3d_ctx* ctx, double chi_t, double* pmv, double* c_int_site) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   if (!pmv) return fail(ctx, RISM3D_ERR_ARG, "pmv is NULL");
   if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before pmv");
+  { const int rc_phi = ensure_phi(ctx); if (rc_phi) return rc_phi; }
   ctx->launches += launch_free_energy(ctx->g, ctx->b, ctx->sp, ctx->d_out, ctx->stream);
   CU(cudaGetLastError());
   double host[2 * MAX_NV];
@@ -537,6 +698,7 @@ extern "C" int rism3d_pmv(rism3d_ctx* ctx, double chi_t, double* pmv, double* c_
 
 extern "C" int rism3d_gradient(rism3d_ctx* ctx, double* grad) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   if (!grad) return fail(ctx, RISM3D_ERR_ARG, "grad is NULL");
   if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before gradient");
   const Grid& g = ctx->g;
@@ -574,9 +736,11 @@ extern "C" int rism3d_gradient(rism3d_ctx* ctx, double* grad) {
 
 extern "C" int rism3d_get_field(rism3d_ctx* ctx, int which, int site, double* dst, int dst_is_device) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   if (!dst || which < 0 || which > RISM3D_FIELD_PHI || site < 0 || site >= ctx->g.nv)
     return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before get_field");
+  if (which == RISM3D_FIELD_T || which == RISM3D_FIELD_PHI) { const int rc_phi = ensure_phi(ctx); if (rc_phi) return rc_phi; }
   double* d = dst_is_device ? dst : ctx->b.scratch;
   ctx->launches += launch_get_field(ctx->g, ctx->b, ctx->sp, which, site, d, ctx->stream);
   CU(cudaGetLastError());
@@ -587,6 +751,7 @@ extern "C" int rism3d_get_field(rism3d_ctx* ctx, int which, int site, double* ds
 
 extern "C" int rism3d_set_tau(rism3d_ctx* ctx, int site, const double* src, int src_is_device) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   if (!src || site < 0 || site >= ctx->g.nv) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before set_tau");
   const Grid& g = ctx->g;
@@ -601,6 +766,7 @@ extern "C" int rism3d_set_tau(rism3d_ctx* ctx, int site, const double* src, int 
 
 extern "C" int rism3d_get_rms_history(rism3d_ctx* ctx, double* dst, int cap, int* n) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   if (!dst || cap < 0 || !n) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   int rc = read_header(ctx);
   if (rc) return rc;
@@ -618,6 +784,7 @@ extern "C" int rism3d_get_rms_history(rism3d_ctx* ctx, double* dst, int cap, int
 
 extern "C" int rism3d_debug_fft_forward(rism3d_ctx* ctx, const double* d_in, double* d_out) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   if (!d_in || !d_out) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   const Grid& g = ctx->g;
   int k = launch_closure_zfwd(g, ctx->b, ctx->sp, d_in, ctx->stream);
@@ -632,6 +799,7 @@ extern "C" int rism3d_debug_fft_forward(rism3d_ctx* ctx, const double* d_in, dou
 
 extern "C" int rism3d_debug_fft_inverse(rism3d_ctx* ctx, const double* d_in, double* d_out) {
   if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
   if (!d_in || !d_out) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   const Grid& g = ctx->g;
   CU(cudaMemcpyAsync(ctx->b.work, d_in, g.field * 8, cudaMemcpyDeviceToDevice, ctx->stream));

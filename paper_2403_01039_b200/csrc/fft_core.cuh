@@ -49,6 +49,42 @@ __device__ __forceinline__ cplx mul_w16(cplx v, int idx) {
   }
 }
 
+// cos(pi k / 16), k = 0..16 (compile-time: folds to immediates in fully unrolled code)
+__host__ __device__ constexpr double cos_pi16(int k) {
+  switch (k) {
+    case 0: return 1.0;
+    case 1: return 0.98078528040323044913;
+    case 2: return 0.92387953251128673848;
+    case 3: return 0.83146961230254523708;
+    case 4: return 0.70710678118654752440;
+    case 5: return 0.55557023301960222474;
+    case 6: return 0.38268343236508978178;
+    case 7: return 0.19509032201612826785;
+    case 8: return 0.0;
+    default: return -cos_pi16(16 - k);
+  }
+}
+__host__ __device__ constexpr double sin_pi16(int k) { return k <= 8 ? cos_pi16(8 - k) : cos_pi16(k - 8); }   // k = 0..16
+// v * exp(DIR i pi IDX / 16), IDX in [0, 16)
+template <int IDX, int DIR>
+__device__ __forceinline__ cplx mul_w32c(cplx v) {
+  if constexpr (IDX == 0) return v;
+  else if constexpr (IDX == 8) return make_double2(-(double)DIR * v.y, (double)DIR * v.x);
+  else {
+    constexpr double c = cos_pi16(IDX), s = (double)DIR * sin_pi16(IDX);
+    return make_double2(v.x * c - v.y * s, v.x * s + v.y * c);
+  }
+}
+template <int R, int DIR, int M1 = 1>
+struct HalfShiftAll {       // x[m1] *= exp(DIR i pi m1 / R) for m1 = 1..R-1, R in {2, 4, 8, 16}
+  static __device__ __forceinline__ void run(cplx (&x)[R]) {
+    if constexpr (M1 < R) {
+      x[M1] = mul_w32c<M1 * (16 / R), DIR>(x[M1]);
+      HalfShiftAll<R, DIR, M1 + 1>::run(x);
+    }
+  }
+};
+
 // In-register DFT, natural order in and out:  X[k] = sum_m x[m] exp(DIR 2 pi i m k / R),  R in {1,2,4,8,16}
 template <int R, int DIR>
 struct Dft {

@@ -137,9 +137,9 @@ static int launch_strided_n(const Grid& gr, const Buffers& b, bool x_axis, bool 
   const unsigned nitems = (unsigned)(nchunks / Cfg::G);
   const size_t shm = StridedCfg<N>::SHM;
   auto kern = fft_strided_kernel<N, INV>;
-  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm) != cudaSuccess) return 0;
   Twiddle tw{b.tw, 1, 2 * gr.n - 1};
-  unsigned grid = (unsigned)resident_ctas(StridedCfg<N>::MINB);
+  unsigned grid = (unsigned)(gr.num_sms * StridedCfg<N>::MINB);
   if (grid > nitems) grid = nitems;
   kern<<<grid, StridedCfg<N>::NT, shm, s>>>(b.work, g, tw, use_state ? b.state : nullptr, nitems);
   return 1;
@@ -365,7 +365,7 @@ static int launch_closure_zfwd_n(const Grid& gr, const Buffers& b, const SolverP
   const int threads = Cfg::T * G * COLS;
   const size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
   auto kern = closure_zfwd_kernel<NZ, G, ZPlan<NZ>::MBF>;
-  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm) != cudaSuccess) return 0;
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
   kern<<<(unsigned)(nlines / GL), threads, shm, s>>>(b.tau, b.w, raw, b.Z, b.work, tws, tw, b.state, gr.nv, gr.npts,
                                                        gr.field, sp.closure, sp.pse_order);
@@ -551,7 +551,7 @@ static int launch_zinv_nm(const Grid& gr, const Buffers& b, const SolverParams& 
   const size_t red = (size_t)(MAX_M + 2) * (threads / 32 + 1) * 2 * sizeof(double);
   if (shm < red) shm = red;
   auto kern = zinv_residual_kernel<NZ, G, MB, MAXO, WEIGHTED>;
-  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm) != cudaSuccess) return 0;
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
   GramArgs ga{b.gram_part, b.gram_part2, b.tickets, b.gram_w, AccelArgs{sp.M, sp.restart, sp.accel, sp.and_s1, sp.and_s2}};
   kern<<<(unsigned)((size_t)gr.n * gr.n / GL), threads, shm, s>>>(b.work, b.tau, b.Z, b.R, raw_out, tws, tw, b.state,

@@ -11,10 +11,11 @@
 #include "async_copy.cuh"
 #include "fft_core.cuh"
 #include "rism3d_internal.h"
+#include "tma.cuh"
 
 namespace r3d {
 
-extern __shared__ double2 smem_dyn[];
+extern __shared__ __align__(128) double2 smem_dyn[];
 constexpr int COLS = 8;
 
 // shared-memory layout of one pipeline stage: [G][N][COLS] data tile, then [G][N][COLS/NV] phi~ values
@@ -32,6 +33,35 @@ struct KspaceCfg {
          MINB = (SHM > 110 * 1024) ? 1 : ((SHM > 72 * 1024) ? 2 : 3) };
 #endif
 };
+
+// Eq. 32 + Eq. 13 + Eq. 33 (in k space) for ONE k point, the NV sites of which sit in NV adjacent lanes:
+//   c = c_sr - q_g phi~ ;  h_g = sum_g' c_g' chi_g'g ;  returns tau'(k) = h_g - c_sr.
+// ch: this lane's row of the per-shell table, chi_shell[shell][g][k] = chi_{(g xor k) g}: entry k multiplies the c of
+// lane (g xor k), so the own value needs no shuffle and the others come by NV - 1 butterfly exchanges.
+template <int NV>
+__device__ __forceinline__ cplx kspace_point(cplx csr, cplx ph, double qg, const double* __restrict__ ch) {
+  const cplx c = make_double2(csr.x - qg * ph.x, csr.y - qg * ph.y);          // Eq. 32
+  double chv[NV];                                                             // one 8*NV-byte row, 16-byte loads
+  if constexpr (NV == 1) {
+    chv[0] = __ldg(ch);
+  } else {
+#pragma unroll
+    for (int i = 0; i < NV / 2; ++i) {
+      const double2 v = __ldg(reinterpret_cast<const double2*>(ch) + i);
+      chv[2 * i] = v.x;
+      chv[2 * i + 1] = v.y;
+    }
+  }
+  double hx = c.x * chv[0], hy = c.y * chv[0];
+#pragma unroll
+  for (int k = 1; k < NV; ++k) {
+    const double cx = __shfl_xor_sync(0xffffffffu, c.x, k);
+    const double cy = __shfl_xor_sync(0xffffffffu, c.y, k);
+    hx = fma(cx, chv[k], hx);                                                  // Eq. 13
+    hy = fma(cy, chv[k], hy);
+  }
+  return make_double2(hx - csr.x, hy - csr.y);                                // tau'(k) = h - c_sr
+}
 
 template <int N, int NV>
 __device__ __forceinline__ void stage_kspace(cplx* buf, const cplx* data, const cplx* phik, size_t item, int tid) {
@@ -74,8 +104,6 @@ __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
   const int tid = threadIdx.x;
   const int col = tid % C, t = (tid / C) % T, grp = tid / (C * T);
   const int site = col % NV;
-  const int lane = tid & 31;
-  const int lane0 = lane & ~(NV - 1);
   const double qg = qv[site];
   // this thread's twiddles are the same for every tile: pass-A set in registers, middle-pass set in a shared table
   using Tw = LineTw<N, R1, R2, R3, T, false>;
@@ -124,30 +152,7 @@ __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
         const int jx = j0 + NB * k;
         const int jxf = jx < NZ ? jx : N - 1 - jx;
         const int shell = (jxf * (jxf + 1) + s_yz) >> 1;
-        const cplx ph = sph[jx * PC];
-        const cplx csr = x[k];
-        const cplx c = make_double2(csr.x - qg * ph.x, csr.y - qg * ph.y);     // Eq. 32
-        const double* ch = chi_shell + (size_t)shell * (NV * NV) + site * NV;  // chi_{g' site}, g' = 0..NV-1
-        double chv[NV];                                                         // one 8*NV-byte row, 16-byte loads
-        if constexpr (NV == 1) {
-          chv[0] = __ldg(ch);
-        } else {
-#pragma unroll
-          for (int i = 0; i < NV / 2; ++i) {
-            const double2 v = __ldg(reinterpret_cast<const double2*>(ch) + i);
-            chv[2 * i] = v.x;
-            chv[2 * i + 1] = v.y;
-          }
-        }
-        double hx = 0.0, hy = 0.0;
-#pragma unroll
-        for (int gp = 0; gp < NV; ++gp) {
-          const double cx = __shfl_sync(0xffffffffu, c.x, lane0 + gp);
-          const double cy = __shfl_sync(0xffffffffu, c.y, lane0 + gp);
-          hx += cx * chv[gp];                                                   // Eq. 13
-          hy += cy * chv[gp];
-        }
-        x[k] = make_double2(hx - csr.x, hy - csr.y);                            // tau'(k) = h - c_sr
+        x[k] = kspace_point<NV>(x[k], sph[jx * PC], qg, chi_shell + (size_t)shell * (NV * NV) + site * NV);
       }
       Dft<RL, +1>::run(x);                             // first inverse stage; its twiddles are applied by the loads of the next
 #pragma unroll
@@ -165,6 +170,226 @@ __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Two-pass variant for the line lengths that factor into two radices <= 16 (64 = 8 x 8, 128 = 16 x 8, 256 = 16 x 16):
+// half the shared-memory passes of the three-pass plan (3 loads + 2 stores of the tile per work item instead of 5 + 5),
+// which is what bounds this kernel (L1 / shared data pipe).  T = N / R1 threads per column, one
+// radix-R1 butterfly each in the outer passes; the pass-A twiddles exp(-2 pi i (k1 + 1/2) t / N), k1 = 0..R1-1, are a
+// geometric sequence in k1 and are generated from two seeds per thread instead of being held in 4 R1 registers.
+// One tile (N x 8 complex = 128-byte rows) per CTA at a time, single-buffered: several small CTAs per SM overlap
+// their load, arithmetic and store phases with each other.
+// ------------------------------------------------------------------------------------------------
+template <int N> struct KPlan2 { enum { OK = 0, R1 = 1, R2 = 1 }; };
+#ifndef R3D_K2_OFF
+template <> struct KPlan2<64>  { enum { OK = 1, R1 = 8,  R2 = 8 }; };
+template <> struct KPlan2<128> { enum { OK = 1, R1 = 16, R2 = 8 }; };
+template <> struct KPlan2<256> { enum { OK = 1, R1 = 16, R2 = 16 }; };
+#endif
+
+template <int N, int NV>
+struct Kspace2Cfg {
+  enum { R1 = KPlan2<N>::R1, R2 = KPlan2<N>::R2, T = N / R1, NT = T * COLS,
+         ITEM = N * COLS, PHI = N * (COLS / NV),
+         TILE_BYTES = ITEM * (int)sizeof(cplx), PHI_BYTES = PHI * (int)sizeof(cplx),
+         STAGE = ITEM + PHI,                                // complex elements of one pipeline stage: tile, then phi~
+         SHM = 2 * (TILE_BYTES + PHI_BYTES) + 64,           // two stages and their mbarriers
+#ifdef R3D_K2_MINB
+         MINB = R3D_K2_MINB };
+#else
+         MINB = (227 * 1024 / (SHM + 1024) < 8) ? 227 * 1024 / (SHM + 1024) : 8 };
+#endif
+};
+
+// a[k] = a0 * s^k, k < R (R a power of two): s^2, s^4, ... by squaring, then a[k + h] = a[k] * s^h -- log2(R) dependent
+// products instead of a chain of R - 1
+template <int R>
+__device__ __forceinline__ void twiddle_powers(cplx (&a)[R], cplx a0, cplx s) {
+  a[0] = a0;
+  cplx sh = s;
+#pragma unroll
+  for (int h = 1; h < R; h *= 2) {
+#pragma unroll
+    for (int k = 0; k < h; ++k) a[k + h] = cmul(a[k], sh);
+    if (2 * h < R) sh = cmul(sh, sh);
+  }
+}
+
+// chi row of one k point for this lane's site (kspace_point consumes it)
+template <int NV>
+struct ChiRow {
+  double v[NV];
+  __device__ __forceinline__ void load(const double* __restrict__ ch) {
+    if constexpr (NV == 1) {
+      v[0] = __ldg(ch);
+    } else if constexpr (NV == 2) {
+      const double2 t = __ldg(reinterpret_cast<const double2*>(ch));
+      v[0] = t.x;
+      v[1] = t.y;
+    } else {
+      // 32-byte rows: one 256-bit load each (sm_100: LDG.E.256), half the requests of two 128-bit loads
+#pragma unroll
+      for (int i = 0; i < NV / 4; ++i)
+        asm volatile("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];\n"
+                     : "=d"(v[4 * i]), "=d"(v[4 * i + 1]), "=d"(v[4 * i + 2]), "=d"(v[4 * i + 3])
+                     : "l"(ch + 4 * i));
+    }
+  }
+};
+
+template <int NV>
+__device__ __forceinline__ cplx kspace_point_row(cplx csr, cplx ph, double qg, const ChiRow<NV>& row) {
+  const cplx c = make_double2(csr.x - qg * ph.x, csr.y - qg * ph.y);          // Eq. 32
+  double hx = c.x * row.v[0], hy = c.y * row.v[0];
+#pragma unroll
+  for (int k = 1; k < NV; ++k) {
+    const double cx = __shfl_xor_sync(0xffffffffu, c.x, k);
+    const double cy = __shfl_xor_sync(0xffffffffu, c.y, k);
+    hx = fma(cx, row.v[k], hx);                                                // Eq. 13
+    hy = fma(cy, row.v[k], hy);
+  }
+  return make_double2(hx - csr.x, hy - csr.y);                                // tau'(k) = h - c_sr
+}
+
+template <int N, int NV>
+__global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB)
+    kspace2_kernel(const __grid_constant__ CUtensorMap tm_work, const __grid_constant__ CUtensorMap tm_phik,
+                   const double* __restrict__ chi_shell, const double* __restrict__ qv, Twiddle tw,
+                   const DevState* __restrict__ st, unsigned nitems) {
+  if (st->done) return;
+  using K = Kspace2Cfg<N, NV>;
+  constexpr int R1 = K::R1, R2 = K::R2, T = K::T, C = COLS;
+  constexpr int S1 = N / R1, NB = N / R2;            // S1 == T: one pass-A butterfly per thread
+  constexpr int NZ = N / 2, PC = C / NV;
+  constexpr int Q = NZ * NV;                         // complex elements per (jx, jy) row
+#ifndef R3D_K2_PF
+#define R3D_K2_PF 8
+#endif
+  constexpr int PF = (R2 < R3D_K2_PF) ? R2 : R3D_K2_PF;   // chi rows in flight per thread
+  const int tid = threadIdx.x;
+  const int col = tid % C, t = tid / C;
+  const int site = col % NV;
+  const double qg = qv[site];
+  const cplx a0 = tw(t), astep = tw(2 * t);          // exp(-i pi t / N) and its square: a[k1] = a0 * astep^k1
+  cplx* stages = smem_dyn;                           // [2] x ([N][8] tile, [N][8 / NV] phi~)
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_dyn + 2 * K::STAGE);   // one per stage
+  const double scale = 1.0 / (double)N;
+  // both boxes of work item `it` into stage b; TMA coordinates: innermost = doubles along the flattened (jy, p[, site])
+  auto issue = [&](unsigned it, int b) {
+    const unsigned q0 = it * C;
+    mbar_arrive_expect_tx(&bars[b], K::TILE_BYTES + K::PHI_BYTES);
+    tma_load_2d(stages + b * K::STAGE, &tm_work, (int)(q0 * 2), 0, &bars[b]);
+    tma_load_2d(stages + b * K::STAGE + K::ITEM, &tm_phik, (int)((q0 / Q * NZ + (q0 % Q) / NV) * 2), 0, &bars[b]);
+  };
+  if (tid == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+  unsigned item = blockIdx.x;
+  if (tid == 0 && item < nitems) issue(item, 0);
+  unsigned n_done = 0;
+  for (; item < nitems; item += gridDim.x, ++n_done) {
+    const int b = n_done & 1;
+    const unsigned next = item + gridDim.x;
+    if (tid == 0 && next < nitems) {
+      tma_wait_read();                               // the store of the previous item has left stage b ^ 1
+      issue(next, b ^ 1);
+    }
+    cplx* sm = stages + b * K::STAGE + col;
+    const cplx* sph = stages + b * K::STAGE + K::ITEM + col / NV;
+    auto ld_sm = [&](int i) { return sm[i * C]; };
+    auto st_sm = [&](int i, cplx v) { sm[i * C] = v; };
+    const unsigned q2 = item * C + col;              // flattened (jy, p, site)
+    const int jy = (int)(q2 / Q);
+    const int p = (int)((q2 % Q) / NV);
+    const int jyf = jy < NZ ? jy : N - 1 - jy;       // folded indices: |k_axis| = dk (j' + 1/2)
+    const int jzf = (2 * p) < NZ ? 2 * p : N - 1 - 2 * p;
+    const int s_yz = jyf * (jyf + 1) + jzf * (jzf + 1);
+    auto chi_row = [&](int jx) {
+      const int jxf = jx < NZ ? jx : N - 1 - jx;
+      return chi_shell + (size_t)((jxf * (jxf + 1) + s_yz) >> 1) * (NV * NV) + site * NV;
+    };
+    mbar_wait(&bars[b], (n_done >> 1) & 1);
+
+    {                                                // forward pass A: radix R1 over m1, half-integer shift, twiddle
+      cplx x[R1];
+#pragma unroll
+      for (int m1 = 0; m1 < R1; ++m1) x[m1] = ld_sm(m1 * S1 + t);
+      HalfShiftAll<R1, -1>::run(x);
+      Dft<R1, -1>::run(x);
+      cplx a[R1];
+      twiddle_powers<R1>(a, a0, astep);
+#pragma unroll
+      for (int k1 = 0; k1 < R1; ++k1) st_sm(k1 * S1 + t, cmul(x[k1], a[k1]));
+    }
+    __syncthreads();
+    // inner digit: forward DFT, k-space arithmetic, inverse DFT, all on the same registers; the chi rows of the next
+    // PF k points are in flight while one is used
+    for (int blk = t; blk < NB; blk += T) {
+      ChiRow<NV> ring[PF];
+#pragma unroll
+      for (int k = 0; k < PF; ++k) ring[k].load(chi_row(blk + NB * k));
+      cplx x[R2];
+#pragma unroll
+      for (int m = 0; m < R2; ++m) x[m] = ld_sm(blk * R2 + m);
+      Dft<R2, -1>::run(x);
+#pragma unroll
+      for (int k = 0; k < R2; ++k) {
+        const int jx = blk + NB * k;
+        x[k] = kspace_point_row<NV>(x[k], sph[jx * PC], qg, ring[k % PF]);
+        if (k + PF < R2) ring[k % PF].load(chi_row(blk + NB * (k + PF)));
+      }
+      Dft<R2, +1>::run(x);
+#pragma unroll
+      for (int r = 0; r < R2; ++r) st_sm(blk * R2 + r, x[r]);
+    }
+    __syncthreads();
+    {                                                // inverse last stage: conjugate twiddle, radix R1 over k1, shift
+      cplx x[R1];
+      cplx a[R1];
+      twiddle_powers<R1>(a, a0, astep);
+#pragma unroll
+      for (int k1 = 0; k1 < R1; ++k1) x[k1] = cmulc(ld_sm(k1 * S1 + t), a[k1]);
+      Dft<R1, +1>::run(x);
+      HalfShiftAll<R1, +1>::run(x);
+#pragma unroll
+      for (int m1 = 0; m1 < R1; ++m1) st_sm(m1 * S1 + t, cscale(x[m1], scale));   // in place: the slots this thread read
+    }
+    fence_proxy_async();
+    __syncthreads();
+    if (tid == 0) {
+      tma_store_2d(&tm_work, (int)(item * C * 2), 0, stages + b * K::STAGE);
+      tma_commit();
+    }
+  }
+  if (tid == 0) tma_wait_all();
+}
+
+template <int N, int NV>
+static int launch_kspace2_nv(const Grid& gr, const Buffers& b, cudaStream_t s) {
+  using K = Kspace2Cfg<N, NV>;
+  const size_t Q = (size_t)(gr.n / 2) * gr.nv;
+  const unsigned nitems = (unsigned)((size_t)gr.n * Q / COLS);
+  auto kern = kspace2_kernel<N, NV>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SHM) != cudaSuccess) return 0;
+  Twiddle tw{b.tw, 1, 2 * gr.n - 1};
+  unsigned grid = (unsigned)(gr.num_sms * K::MINB);
+  if (grid > nitems) grid = nitems;
+  kern<<<grid, K::NT, K::SHM, s>>>(b.tm_work, b.tm_phik, b.chi_shell, b.qv, tw, b.state, nitems);
+  return 1;
+}
+
+// true when launch_kspace_x takes the TMA path for this grid (the API layer then builds the tensor maps)
+bool kspace_uses_tma(int n) {
+  switch (n) {
+    case 64: return KPlan2<64>::OK;
+    case 128: return KPlan2<128>::OK;
+    case 256: return KPlan2<256>::OK;
+    default: return false;
+  }
+}
+
 template <int N, int NV>
 static int launch_kspace_nv(const Grid& gr, const Buffers& b, cudaStream_t s) {
   using Cfg = FftCfg<N>;
@@ -173,21 +398,27 @@ static int launch_kspace_nv(const Grid& gr, const Buffers& b, cudaStream_t s) {
   const size_t nchunks = (size_t)gr.n * Q / COLS;
   const unsigned nitems = (unsigned)(nchunks / Cfg::G);
   auto kern = kspace_x_kernel<N, NV>;
-  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SHM);
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SHM) != cudaSuccess) return 0;
   Twiddle tw{b.tw, 1, 2 * gr.n - 1};
-  unsigned grid = (unsigned)resident_ctas(K::MINB);
+  unsigned grid = (unsigned)(gr.num_sms * K::MINB);
   if (grid > nitems) grid = nitems;
   kern<<<grid, K::NT, K::SHM, s>>>(b.work, b.phik, b.chi_shell, b.qv, tw, b.state, nitems);
   return 1;
 }
 
+template <int N, int NV>
+static int launch_kspace_pick(const Grid& g, const Buffers& b, cudaStream_t s) {
+  if constexpr (KPlan2<N>::OK) return launch_kspace2_nv<N, NV>(g, b, s);
+  else return launch_kspace_nv<N, NV>(g, b, s);
+}
+
 template <int N>
 static int launch_kspace_n(const Grid& g, const Buffers& b, cudaStream_t s) {
   switch (g.nv) {
-    case 1: return launch_kspace_nv<N, 1>(g, b, s);
-    case 2: return launch_kspace_nv<N, 2>(g, b, s);
-    case 4: return launch_kspace_nv<N, 4>(g, b, s);
-    case 8: return launch_kspace_nv<N, 8>(g, b, s);
+    case 1: return launch_kspace_pick<N, 1>(g, b, s);
+    case 2: return launch_kspace_pick<N, 2>(g, b, s);
+    case 4: return launch_kspace_pick<N, 4>(g, b, s);
+    case 8: return launch_kspace_pick<N, 8>(g, b, s);
     default: return 0;
   }
 }
@@ -201,6 +432,35 @@ int launch_kspace_x(const Grid& g, const Buffers& b, cudaStream_t s) {
     case 128: return launch_kspace_n<128>(g, b, s);
     case 256: return launch_kspace_n<256>(g, b, s);
     case 512: return launch_kspace_n<512>(g, b, s);
+    default: return 0;
+  }
+}
+
+template <int N, int NV>
+static constexpr int kspace_smem_nv() {
+  if constexpr (KPlan2<N>::OK) return Kspace2Cfg<N, NV>::SHM;
+  else return KspaceCfg<N, NV>::SHM;
+}
+template <int N>
+static int kspace_smem_n(int nv) {
+  switch (nv) {
+    case 1: return kspace_smem_nv<N, 1>();
+    case 2: return kspace_smem_nv<N, 2>();
+    case 4: return kspace_smem_nv<N, 4>();
+    case 8: return kspace_smem_nv<N, 8>();
+    default: return 0;
+  }
+}
+
+int kspace_smem_bytes(int n, int nv) {
+  switch (n) {
+    case 8: return kspace_smem_n<8>(nv);
+    case 16: return kspace_smem_n<16>(nv);
+    case 32: return kspace_smem_n<32>(nv);
+    case 64: return kspace_smem_n<64>(nv);
+    case 128: return kspace_smem_n<128>(nv);
+    case 256: return kspace_smem_n<256>(nv);
+    case 512: return kspace_smem_n<512>(nv);
     default: return 0;
   }
 }

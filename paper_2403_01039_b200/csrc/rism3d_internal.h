@@ -1,5 +1,6 @@
 // rism3d_internal.h -- shared declarations of the CUDA side of librism3d.so (not part of the ABI).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stddef.h>
 #include <stdint.h>
@@ -51,6 +52,8 @@ struct Grid {
   double origin[3];
   size_t npts;           // n^3
   size_t field;          // nv * n^3 doubles in one field-set
+  int num_sms;           // SMs of the device the context lives on (grid size of the persistent kernels)
+  int smem_optin;        // largest dynamic shared memory a kernel may opt in to on that device, bytes
 };
 
 // Device pointers carved from the caller's workspace.
@@ -63,7 +66,7 @@ struct Buffers {
   double2* work;         // [n][n][n/2][nv] complex   k-space work array
   double* phi;           // [npts]       phi(r)
   double2* phik;         // [n][n][n/2]  phi~(k) exp(+i k.r0) / dV
-  double* chi_shell;     // [nshell][nv][nv]   chi_shell[s][g][g'] = chi_{g' g}(k_s)
+  double* chi_shell;     // [nshell][nv][nv]   chi_shell[s][g][k] = chi_{(g xor k) g}(k_s)
   double2* tw;           // [2n]         exp(-i pi j / n)
   double* gram_part;     // [MAX_M+1][gram_blocks][2]  double-double partial sums, one per zinv_residual CTA
   double* gram_part2;    // [MAX_M+1][groups][2]  first-level sums of groups of 64 partials
@@ -74,6 +77,9 @@ struct Buffers {
   double* rhov;          // [nv]
   double* gram_w;        // [nv] weights of the inner product: 1 (MDIIS) or 1/rho_g (modified Anderson, Eq. 38)
   double* fe_part;       // [FE_BLOCKS][MAX_NV][2]
+  // TMA descriptors of the k-space pass (built by rism3d_init when kspace_uses_tma(n)): `work` as a 2D array of doubles
+  // [jx][2 n Q] with boxes of n rows x 128 bytes, `phik` as [jx][2 n n/2] with boxes of n rows x (8 / nv) complex
+  CUtensorMap tm_work, tm_phik;
 };
 
 struct SolverParams {
@@ -87,8 +93,9 @@ struct SolverParams {
   double and_s1, and_s2; // tuning parameters of Eq. 34-35
 };
 
-// api.cu: per_sm * number of SMs of the device the context lives on (grid size of the persistent kernels)
-int resident_ctas(int per_sm);
+// dynamic shared memory of kspace_x for this grid (0: unsupported n / nv); the API layer checks it against the device
+int kspace_smem_bytes(int n, int nv);
+bool kspace_uses_tma(int n);
 
 // ---- launchers (each returns the number of kernels it launched; errors surface via cudaGetLastError) ----
 // fft_kernels.cu
@@ -107,10 +114,14 @@ int launch_chi_shell(const Grid&, const Buffers&, const double* d_chi_table, int
                      cudaStream_t);
 int launch_potential(const Grid&, const Buffers&, const SolverParams&, int n_atoms, const double* d_atoms,
                      const double* d_pair, double rcut, cudaStream_t);
+int launch_w_cells(const Grid&, const Buffers&, const SolverParams&, const double* d_atoms, const double* d_pair,
+                   const int* d_cell_start, const int nc[3], const double lo[3], double edge, double rcut, cudaStream_t);
+int launch_phi(const Grid&, const Buffers&, const SolverParams&, int n_atoms, const double* d_atoms, cudaStream_t);
 int launch_phi_tilde(const Grid&, const Buffers&, const SolverParams&, int n_atoms, const double* d_atoms,
                      double2* d_phase, cudaStream_t);
 int launch_gradient(const Grid&, const Buffers&, const SolverParams&, int n_atoms, double* d_gw, const double* d_atoms,
                     const double* d_pair, double* d_partial, int nchunks, double* d_out, cudaStream_t);
+double measure_dfma_peak(int num_sms, double* d_scratch, cudaStream_t);
 int launch_free_energy(const Grid&, const Buffers&, const SolverParams&, double* d_out, cudaStream_t);
 int launch_get_field(const Grid&, const Buffers&, const SolverParams&, int which, int site, double* d_dst,
                      cudaStream_t);

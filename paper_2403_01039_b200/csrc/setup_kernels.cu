@@ -16,6 +16,72 @@ namespace r3d {
 // ------------------------------------------------------------------------------------------------
 constexpr int ATOM_CHUNK = 64;
 
+// One atom - grid point pair: adds the pair's (1 - exp(-kappa r))/r term to ph (WITH_PHI; never cut off) and its
+// short-range terms -beta [C q q exp(-kappa r)/r + LJ] to acc[g] (WITH_W; only when the pair is inside the cutoff).
+// qa = beta C q_a; pp = (beta C q_a q_g, sigma_ag^2, 4 beta eps_ag) per site.
+// 1/r: float rsqrt seed + two Newton steps in double (~2 ulp; r^2 is far inside the float range).  Beyond kappa r = 40,
+// exp(-kappa r) < 5e-18 vanishes against 1 in double precision: (1 - exp(-kappa r))/r is 1/r to the last bit and the
+// short-range Coulomb term is 0, so far pairs (most of them on the large grids) need no exp at all.
+template <int NV, bool WITH_PHI, bool WITH_W>
+__device__ __forceinline__ void pair_terms(double r2, double qa, const double* __restrict__ pp, double kappa,
+                                           double r_min, double rmin2, double far2, bool cut, double rcut2,
+                                           double& ph, double (&acc)[NV]) {
+  const bool inside = WITH_W && (!cut || r2 < rcut2);
+  if (r2 >= rmin2) {
+    double rinv = (double)rsqrtf((float)r2);
+    rinv = rinv * fma(-0.5 * r2, rinv * rinv, 1.5);
+    rinv = rinv * fma(-0.5 * r2, rinv * rinv, 1.5);
+    if (r2 > far2) {
+      if (WITH_PHI) ph = fma(qa, rinv, ph);
+      if (inside) {                                         // LJ reaches further than exp(-kappa r)
+        const double inv2 = rinv * rinv;
+#pragma unroll
+        for (int g = 0; g < NV; ++g) {
+          const double s2 = pp[g * 3 + 1] * inv2;
+          const double s6 = s2 * s2 * s2;
+          acc[g] -= pp[g * 3 + 2] * (s6 * s6 - s6);
+        }
+      }
+    } else if (WITH_PHI || inside) {
+      const double kr = kappa * (r2 * rinv);
+      // 1 - exp(-kappa r): expm1 where the subtraction would cancel, exp elsewhere
+      const double ex = (kr < 0.5) ? 1.0 + expm1(-kr) : exp(-kr);
+      if (WITH_PHI) {
+        const double om = (kr < 0.5) ? -expm1(-kr) : 1.0 - ex;
+        ph = fma(qa, om * rinv, ph);
+      }
+      if (inside) {
+        const double sc = ex * rinv;                        // exp(-kappa r)/r = 1/r - (1 - exp(-kappa r))/r
+        const double inv2 = rinv * rinv;
+#pragma unroll
+        for (int g = 0; g < NV; ++g) {
+          const double s2 = pp[g * 3 + 1] * inv2;
+          const double s6 = s2 * s2 * s2;
+          acc[g] -= pp[g * 3 + 0] * sc + pp[g * 3 + 2] * (s6 * s6 - s6);
+        }
+      }
+    }
+  } else {
+    // grid point (almost) on an atom: distance clamped at r_min (Q11), phi at its finite limit
+    const double rt = sqrt(r2);
+    const double kr = kappa * rt;
+    const double em = expm1(-kr);
+    const double lr = (kr < 1e-8) ? kappa : -em / rt;       // (1 - exp(-kappa r)) / r and its limit
+    if (WITH_PHI) ph += qa * lr;
+    if (inside) {
+      const double rc = fmax(rt, r_min);
+      const double sc = (rt >= r_min) ? (1.0 + em) / rt : (cut ? exp(-kappa * rc) / rc : 1.0 / rc - lr);
+      const double inv2 = 1.0 / (rc * rc);
+#pragma unroll
+      for (int g = 0; g < NV; ++g) {
+        const double s2 = pp[g * 3 + 1] * inv2;
+        const double s6 = s2 * s2 * s2;
+        acc[g] -= pp[g * 3 + 0] * sc + pp[g * 3 + 2] * (s6 * s6 - s6);
+      }
+    }
+  }
+}
+
 template <int NV>
 __global__ void __launch_bounds__(128)
     potential_kernel(double* __restrict__ w, double* __restrict__ phi, const double4* __restrict__ atoms,
@@ -46,64 +112,7 @@ __global__ void __launch_bounds__(128)
       const double4 at = s_atom[a];
       const double dx = x - at.x, dy = y - at.y, dz = z - at.z;
       const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-      // The common case first.  1/r: float rsqrt seed + two Newton steps in double (~2 ulp; r^2 is far inside the
-      // float range).  Beyond kappa r = 40, exp(-kappa r) < 5e-18 vanishes against 1 in double precision: (1 -
-      // exp(-kappa r))/r is 1/r to the last bit and the short-range Coulomb term is 0, so far pairs (most of them
-      // on the large grids) need no exp at all.
-      if (r2 >= rmin2) {
-        double rinv = (double)rsqrtf((float)r2);
-        rinv = rinv * fma(-0.5 * r2, rinv * rinv, 1.5);
-        rinv = rinv * fma(-0.5 * r2, rinv * rinv, 1.5);
-        if (r2 > far2) {
-          ph = fma(at.w, rinv, ph);
-          if (!cut) {                                         // all-pairs mode: LJ reaches further than exp(-kappa r)
-            const double inv2 = rinv * rinv;
-            const double* pp = s_pair + a * NV * 3;
-#pragma unroll
-            for (int g = 0; g < NV; ++g) {
-              const double s2 = pp[g * 3 + 1] * inv2;
-              const double s6 = s2 * s2 * s2;
-              acc[g] -= pp[g * 3 + 2] * (s6 * s6 - s6);
-            }
-          }
-        } else {
-          const double kr = kappa * (r2 * rinv);
-          // 1 - exp(-kappa r): expm1 where the subtraction would cancel, exp elsewhere
-          const double ex = (kr < 0.5) ? 1.0 + expm1(-kr) : exp(-kr);
-          const double om = (kr < 0.5) ? -expm1(-kr) : 1.0 - ex;
-          ph = fma(at.w, om * rinv, ph);
-          if (!cut || r2 < rcut2) {
-            const double sc = ex * rinv;                      // exp(-kappa r)/r = 1/r - (1 - exp(-kappa r))/r
-            const double inv2 = rinv * rinv;
-            const double* pp = s_pair + a * NV * 3;
-#pragma unroll
-            for (int g = 0; g < NV; ++g) {
-              const double s2 = pp[g * 3 + 1] * inv2;
-              const double s6 = s2 * s2 * s2;
-              acc[g] -= pp[g * 3 + 0] * sc + pp[g * 3 + 2] * (s6 * s6 - s6);
-            }
-          }
-        }
-      } else {
-        // grid point (almost) on an atom: distance clamped at r_min (Q11), phi at its finite limit
-        const double rt = sqrt(r2);
-        const double kr = kappa * rt;
-        const double em = expm1(-kr);
-        const double lr = (kr < 1e-8) ? kappa : -em / rt;     // (1 - exp(-kappa r)) / r and its limit
-        ph += at.w * lr;
-        if (!cut || r2 < rcut2) {
-          const double rc = fmax(rt, r_min);
-          const double sc = (rt >= r_min) ? (1.0 + em) / rt : (cut ? exp(-kappa * rc) / rc : 1.0 / rc - lr);
-          const double inv2 = 1.0 / (rc * rc);
-          const double* pp = s_pair + a * NV * 3;
-#pragma unroll
-          for (int g = 0; g < NV; ++g) {
-            const double s2 = pp[g * 3 + 1] * inv2;
-            const double s6 = s2 * s2 * s2;
-            acc[g] -= pp[g * 3 + 0] * sc + pp[g * 3 + 2] * (s6 * s6 - s6);
-          }
-        }
-      }
+      pair_terms<NV, true, true>(r2, at.w, s_pair + a * NV * 3, kappa, r_min, rmin2, far2, cut, rcut2, ph, acc);
     }
   }
   phi[idx] = ph;
@@ -127,6 +136,155 @@ int launch_potential(const Grid& g, const Buffers& b, const SolverParams& sp, in
     default: return 0;
   }
 #undef POT
+  return 1;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Cell-list grid potential (rcut > 0; Q12): w alone, from the atoms within the cutoff of each grid point.
+// The host bins the atoms into cubic cells of edge >= rcut / 2 and sorts them by cell, z fastest, so that the cells
+// (cx, cy, cz0..cz1) of one column are ONE contiguous range of the sorted atom table.  A CTA owns a brick of 4 x 8 x 8
+// grid points and walks the cell columns that can reach the brick (box-box distance test), staging each column's
+// atoms through shared memory; a thread (one grid point) applies the sharp test r < rcut per atom -- the same pair set,
+// the same rounded r^2 and the same pair arithmetic as the all-pairs kernel, accumulated in the sorted atom order.
+// phi(r), which is never cut off, is left to phi_kernel (computed when first needed, see api.cu).
+// ------------------------------------------------------------------------------------------------
+struct CellGrid {
+  int nc[3];             // cells per axis
+  double lo[3];          // lower corner of cell (0, 0, 0)
+  double edge;           // cell edge
+};
+constexpr int BRICK_X = 4, BRICK_Y = 8, BRICK_Z = 8, BRICK_THREADS = BRICK_X * BRICK_Y * BRICK_Z;
+constexpr int CELL_CHUNK = 128;
+
+template <int NV>
+__global__ void __launch_bounds__(BRICK_THREADS)
+    w_cells_kernel(double* __restrict__ w, const double4* __restrict__ atoms, const double* __restrict__ pair,
+                   const int* __restrict__ cell_start, CellGrid cg, int n, double h, double ox, double oy, double oz,
+                   double kappa, double r_min, double rcut, size_t npts) {
+  __shared__ double4 s_atom[CELL_CHUNK];
+  __shared__ double s_pair[CELL_CHUNK * NV * 3];
+  const int tid = threadIdx.x;
+  const int iz = blockIdx.x * BRICK_Z + tid % BRICK_Z;
+  const int iy = blockIdx.y * BRICK_Y + (tid / BRICK_Z) % BRICK_Y;
+  const int ix = blockIdx.z * BRICK_X + tid / (BRICK_Z * BRICK_Y);
+  const double x = __dadd_rn(ox, __dmul_rn(h, (double)ix));
+  const double y = __dadd_rn(oy, __dmul_rn(h, (double)iy));
+  const double z = __dadd_rn(oz, __dmul_rn(h, (double)iz));
+  double acc[NV];
+#pragma unroll
+  for (int g = 0; g < NV; ++g) acc[g] = 0.0;
+  double ph_unused = 0.0;
+  const double rcut2 = rcut * rcut, rmin2 = r_min * r_min, far2 = 1600.0 / (kappa * kappa);
+  // the brick's box (with a safety margin of a grid spacing against rounding in the cell arithmetic) and the cells it
+  // can reach; everything below is uniform over the CTA
+  const double bx0 = ox + h * (blockIdx.z * BRICK_X) - h, bx1 = ox + h * (blockIdx.z * BRICK_X + BRICK_X - 1) + h;
+  const double by0 = oy + h * (blockIdx.y * BRICK_Y) - h, by1 = oy + h * (blockIdx.y * BRICK_Y + BRICK_Y - 1) + h;
+  const double bz0 = oz + h * (blockIdx.x * BRICK_Z) - h, bz1 = oz + h * (blockIdx.x * BRICK_Z + BRICK_Z - 1) + h;
+  auto cell_lo = [&](double v, int axis) { return max(0, (int)floor((v - rcut - cg.lo[axis]) / cg.edge)); };
+  auto cell_hi = [&](double v, int axis) { return min(cg.nc[axis] - 1, (int)floor((v + rcut - cg.lo[axis]) / cg.edge)); };
+  const int cx0 = cell_lo(bx0, 0), cx1 = cell_hi(bx1, 0);
+  const int cy0 = cell_lo(by0, 1), cy1 = cell_hi(by1, 1);
+  const int cz0 = cell_lo(bz0, 2), cz1 = cell_hi(bz1, 2);
+  // distance from the interval [b0, b1] to cell c of an axis
+  auto gap = [&](double b0, double b1, int c, int axis) {
+    const double c0 = cg.lo[axis] + c * cg.edge, c1 = c0 + cg.edge;
+    return fmax(0.0, fmax(c0 - b1, b0 - c1));
+  };
+  if (cz0 <= cz1) {
+    for (int cx = cx0; cx <= cx1; ++cx) {
+      const double gx = gap(bx0, bx1, cx, 0);
+      for (int cy = cy0; cy <= cy1; ++cy) {
+        const double gy = gap(by0, by1, cy, 1);
+        if (gx * gx + gy * gy > rcut2) continue;
+        const size_t col = ((size_t)cx * cg.nc[1] + cy) * cg.nc[2];
+        const int a_begin = cell_start[col + cz0], a_end = cell_start[col + cz1 + 1];
+        for (int a0 = a_begin; a0 < a_end; a0 += CELL_CHUNK) {
+          const int na = min(CELL_CHUNK, a_end - a0);
+          __syncthreads();
+          for (int i = tid; i < na; i += BRICK_THREADS) s_atom[i] = atoms[a0 + i];
+          for (int i = tid; i < na * NV * 3; i += BRICK_THREADS) s_pair[i] = pair[(size_t)a0 * NV * 3 + i];
+          __syncthreads();
+          for (int a = 0; a < na; ++a) {
+            const double4 at = s_atom[a];
+            const double dx = x - at.x, dy = y - at.y, dz = z - at.z;
+            const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+            if (r2 < rcut2)
+              pair_terms<NV, false, true>(r2, at.w, s_pair + a * NV * 3, kappa, r_min, rmin2, far2, true, rcut2, ph_unused, acc);
+          }
+        }
+      }
+    }
+  }
+  const size_t idx = ((size_t)ix * n + iy) * n + iz;
+#pragma unroll
+  for (int g = 0; g < NV; ++g) w[(size_t)g * npts + idx] = acc[g];
+}
+
+// d_atoms / d_pair: the atom and pair tables SORTED by cell; d_cell_start: [ncells + 1] first atom of every cell
+int launch_w_cells(const Grid& g, const Buffers& b, const SolverParams& sp, const double* d_atoms, const double* d_pair,
+                   const int* d_cell_start, const int nc[3], const double lo[3], double edge, double rcut,
+                   cudaStream_t s) {
+  CellGrid cg;
+  for (int i = 0; i < 3; ++i) { cg.nc[i] = nc[i]; cg.lo[i] = lo[i]; }
+  cg.edge = edge;
+  dim3 grid((unsigned)(g.n / BRICK_Z), (unsigned)(g.n / BRICK_Y), (unsigned)(g.n / BRICK_X));
+  const double4* at = reinterpret_cast<const double4*>(d_atoms);
+#define WCELL(NV)                                                                                                   \
+  w_cells_kernel<NV><<<grid, BRICK_THREADS, 0, s>>>(b.w, at, d_pair, d_cell_start, cg, g.n, g.h, g.origin[0],       \
+                                                    g.origin[1], g.origin[2], sp.kappa, sp.r_min, rcut, g.npts)
+  switch (g.nv) {
+    case 1: WCELL(1); break;
+    case 2: WCELL(2); break;
+    case 4: WCELL(4); break;
+    case 8: WCELL(8); break;
+    default: return 0;
+  }
+#undef WCELL
+  return 1;
+}
+
+// phi(r) = beta C sum_a q_a (1 - exp(-kappa r_a)) / r_a over ALL atoms (Eq. 29; never cut off).  Two grid points per
+// thread (z and z + n/2: two independent dependency chains), atoms staged through shared memory.
+constexpr int PHI_CHUNK = 256;
+__global__ void __launch_bounds__(128)
+    phi_kernel(double* __restrict__ phi, const double4* __restrict__ atoms, int n_atoms, int n, double h, double ox,
+               double oy, double oz, double kappa, double r_min) {
+  __shared__ double4 s_atom[PHI_CHUNK];
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // n^3 / 2 threads
+  const int hz = n / 2;
+  const int iz = (int)(t % hz), iy = (int)((t / hz) % n), ix = (int)(t / ((size_t)hz * n));
+  const double x = __dadd_rn(ox, __dmul_rn(h, (double)ix));
+  const double y = __dadd_rn(oy, __dmul_rn(h, (double)iy));
+  const double z0 = __dadd_rn(oz, __dmul_rn(h, (double)iz));
+  const double z1 = __dadd_rn(oz, __dmul_rn(h, (double)(iz + hz)));
+  const double rmin2 = r_min * r_min, far2 = 1600.0 / (kappa * kappa);
+  double ph0 = 0.0, ph1 = 0.0;
+  double none[1] = {0.0};
+  for (int a0 = 0; a0 < n_atoms; a0 += PHI_CHUNK) {
+    const int na = min(PHI_CHUNK, n_atoms - a0);
+    __syncthreads();
+    for (int i = threadIdx.x; i < na; i += blockDim.x) s_atom[i] = atoms[a0 + i];
+    __syncthreads();
+#pragma unroll 2
+    for (int a = 0; a < na; ++a) {
+      const double4 at = s_atom[a];
+      const double dx = x - at.x, dy = y - at.y, dz0 = z0 - at.z, dz1 = z1 - at.z;
+      const double rxy = __dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy));
+      pair_terms<1, true, false>(__dadd_rn(rxy, __dmul_rn(dz0, dz0)), at.w, nullptr, kappa, r_min, rmin2, far2, false, 0.0, ph0, none);
+      pair_terms<1, true, false>(__dadd_rn(rxy, __dmul_rn(dz1, dz1)), at.w, nullptr, kappa, r_min, rmin2, far2, false, 0.0, ph1, none);
+    }
+  }
+  const size_t idx = ((size_t)ix * n + iy) * n + iz;
+  phi[idx] = ph0;
+  phi[idx + hz] = ph1;
+}
+
+// d_atoms: [n_atoms] (x, y, z, beta C q_a), any order
+int launch_phi(const Grid& g, const Buffers& b, const SolverParams& sp, int n_atoms, const double* d_atoms,
+               cudaStream_t s) {
+  const unsigned blocks = (unsigned)(g.npts / 2 / 128);
+  phi_kernel<<<blocks, 128, 0, s>>>(b.phi, reinterpret_cast<const double4*>(d_atoms), n_atoms, g.n, g.h, g.origin[0],
+                                   g.origin[1], g.origin[2], sp.kappa, sp.r_min);
   return 1;
 }
 
@@ -226,7 +384,8 @@ int launch_phi_tilde(const Grid& g, const Buffers& b, const SolverParams& sp, in
 }
 
 // ------------------------------------------------------------------------------------------------
-// chi per |k| shell.  table: [n_k][nv][nv] (chi[m][g'][g]);  out: [nshell][g][g']
+// chi per |k| shell.  table: [n_k][nv][nv] (chi[m][g'][g]);  out: [nshell][g][k] = chi_{(g xor k) g}: row g holds
+// the column of Eq. 13 that site g needs, ordered for the butterfly exchange of kspace_point (kspace_kernel.cu)
 // ------------------------------------------------------------------------------------------------
 __global__ void chi_shell_kernel(double* __restrict__ out, const double* __restrict__ table, int n_k, double k0,
                                  double dkt, int nv, double dk_grid, int nshell) {
@@ -247,7 +406,7 @@ __global__ void chi_shell_kernel(double* __restrict__ out, const double* __restr
   for (int gp = 0; gp < nv; ++gp)
     for (int g = 0; g < nv; ++g) {
       const double* t = table + (size_t)first * st + gp * nv + g;
-      out[(size_t)sidx * st + g * nv + gp] = l0 * t[0] + l1 * t[st] + l2 * t[2 * st] + l3 * t[3 * st];
+      out[(size_t)sidx * st + g * nv + (gp ^ g)] = l0 * t[0] + l1 * t[st] + l2 * t[2 * st] + l3 * t[3 * st];
     }
 }
 
@@ -500,6 +659,45 @@ int launch_gradient(const Grid& g, const Buffers& b, const SolverParams& sp, int
 #undef GRD
   gradient_final_kernel<<<(n_atoms * 3 + 127) / 128, 128, 0, s>>>(d_out, d_partial, nchunks, n_atoms, sp.kT);
   return 3;
+}
+
+// ------------------------------------------------------------------------------------------------
+// fp64 FMA peak of the device, measured: 16 independent DFMA chains per thread, 1024 resident threads per SM.  The
+// denominator of the setup kernels' roofline (they are bound by plain fp64 arithmetic, not by HBM).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) dfma_peak_kernel(double* __restrict__ out, int iters, double a, double b) {
+  double v[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) v[i] = (double)(threadIdx.x + i);
+  for (int k = 0; k < iters; ++k) {
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = fma(v[i], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += v[i];
+  if (s == 12345.678) out[0] = s;                        // never true: keeps the chains alive
+}
+
+// -> fp64 TFLOP/s (2 flops per DFMA) over ~reps launches; returns the best launch
+double measure_dfma_peak(int num_sms, double* d_scratch, cudaStream_t s) {
+  const int iters = 4096, blocks = num_sms * 4, threads = 256;
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return 0.0;
+  double best = 0.0;
+  for (int rep = 0; rep < 5; ++rep) {
+    cudaEventRecord(e0, s);
+    dfma_peak_kernel<<<blocks, threads, 0, s>>>(d_scratch, iters, 0.999999, 1e-9);
+    cudaEventRecord(e1, s);
+    if (cudaEventSynchronize(e1) != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double tf = 2.0 * 16.0 * iters * (double)blocks * threads / (ms * 1e-3) / 1e12;
+    if (rep > 0 && tf > best) best = tf;                 // the first launch is a warm-up
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  return best;
 }
 
 }  // namespace r3d

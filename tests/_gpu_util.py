@@ -7,7 +7,7 @@ from workloads import get_config, load_chi, make_solute, solvent_by_name
 
 def make_pair(cfg_name=None, *, n=None, spacing=None, solvent="water", closure="KH", pse_order=1, M=5, b=0.5,
               restart=10.0, chi=None, solute=None, rcut=0.0, origin=None, n_override=None, accelerator="MDIIS",
-              anderson_s=(0.2, 0.0)):
+              anderson_s=(0.2, 0.0), kappa=1.0, **extra):
     """-> (oracle, cuda solver, solute, rcut) with identical settings.  cfg_name picks a BASELINE config;
     n_override shrinks its grid (same spacing) so the oracle stays fast."""
     import paper_2403_01039_b200 as lib
@@ -20,10 +20,12 @@ def make_pair(cfg_name=None, *, n=None, spacing=None, solvent="water", closure="
     sv = solvent_by_name(solvent) if isinstance(solvent, str) else solvent
     k0, dk, table = load_chi(sv.name) if chi is None else chi
     orc = o3.Rism3dOracle(n, spacing, sv.n_v, closure=closure, pse_order=pse_order, mdiis_nvec=M, mdiis_b=b,
-                          mdiis_restart=restart, origin=origin, accelerator=accelerator, anderson_s=anderson_s)
+                          mdiis_restart=restart, origin=origin, accelerator=accelerator, anderson_s=anderson_s,
+                          kappa=kappa, **extra)
     orc.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, table)
     gpu = lib.Solver(n, spacing, sv.n_v, closure=closure, pse_order=pse_order, mdiis_nvec=M, mdiis_b=b,
-                     mdiis_restart=restart, origin=origin, accelerator=accelerator, anderson_s=anderson_s)
+                     mdiis_restart=restart, origin=origin, accelerator=accelerator, anderson_s=anderson_s,
+                     kappa=kappa, **extra)
     gpu.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, table)
     if solute is not None:
         orc.set_solute(solute.xyz, solute.q, solute.sigma, solute.eps, rcut=rcut)

@@ -18,8 +18,9 @@ def _torch():
 
 
 # ---- the shifted 3D transform pair alone -----------------------------------------
-@pytest.mark.parametrize("n,nv", [(8, 2), (16, 1), (16, 4), (32, 2), (64, 4), (128, 2)])
+@pytest.mark.parametrize("n,nv", [(8, 2), (16, 1), (16, 4), (32, 2), (64, 4), (128, 2), (128, 4), (256, 4)])
 def test_fft_pair_matches_oracle(n, nv):
+    """element by element, up to the transform size and site count of the benchmarked configuration (256, 4)"""
     torch = _torch()
     import paper_2403_01039_b200 as lib
     rng = np.random.default_rng(n + nv)
@@ -33,7 +34,7 @@ def test_fft_pair_matches_oracle(n, nv):
     assert np.max(np.abs(back - f)) < 2e-14 * np.log2(n) * np.max(np.abs(f))
 
 
-@pytest.mark.parametrize("n,nv", [(256, 1), (512, 1)])
+@pytest.mark.parametrize("n,nv", [(256, 1), (512, 2)])
 def test_fft_round_trip_and_sampled_lines_large(n, nv):
     """Full-size lines: round trip = identity, Parseval, and sampled k points against the defining sum."""
     torch = _torch()
@@ -78,6 +79,19 @@ def test_setup_with_cutoff_matches_oracle_pair_set():
     W, Wo = gpu.get_field("W"), orc.get_field("W")
     finite = np.abs(Wo) < 600.0
     assert np.max(np.abs(W - Wo)[finite]) < 1e-10     # a single differing pair would show up at >= 1e-6
+
+
+@pytest.mark.parametrize("n,spacing,kappa,rcut", [(64, 1.0, 1.0, 50.0), (32, 1.5, 3.0, 16.0), (32, 1.5, 4.0, 12.0)])
+def test_cutoff_beyond_the_screening_range_keeps_lennard_jones(n, spacing, kappa, rcut):
+    """rcut > 40/kappa: between the distance where exp(-kappa r) vanishes in double precision and the cutoff, a
+    pair still contributes its Lennard-Jones term (~1e-7 each at these distances) -- Eq. 22 with the cutoff of Q12."""
+    sol = make_solute("C3")
+    orc, gpu, _, _ = make_pair(n=n, spacing=spacing, solvent="water_nacl_0.1M", solute=sol, rcut=rcut, M=4, kappa=kappa)
+    assert rcut > 40.0 / kappa
+    W, Wo = gpu.get_field("W"), orc.get_field("W")
+    finite = np.abs(Wo) < 600.0
+    assert np.max(np.abs(W - Wo)[finite]) < 1e-10
+    assert np.max(np.abs(gpu.get_field("PHI", 0) - orc.phi)) < 1e-11 * np.max(np.abs(orc.phi))
 
 
 # ---- the loop: 50 fixed iterations, max |dg| <= 1e-9 -------------------------------------------------------
