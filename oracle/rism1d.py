@@ -177,6 +177,40 @@ class Xrism1d:
         Hk, _ = self.h_of_k(c_sr)
         return self.W + self.rho_site[None, :, None] * Hk
 
+    # -- bulk thermodynamics of the solvent -------------------------------------
+    def c_sr_k0(self):
+        """int c_sr,ab(r) dr = 4 pi dr sum_i r_i^2 c_sr,ab(r_i)  -> [a][b]  (the k = 0 value of the short-range part of the
+        site-site direct correlation function of the bulk solvent)."""
+        _, c_sr = self.closure_step(self.tau)
+        g = self.grid
+        return 4.0 * math.pi * g.dr * np.sum(c_sr * g.r ** 2, axis=-1)
+
+    def _rho_rho_c(self):
+        """sum_ab rho_a rho_b int c_ab(r) dr over all solvent sites (rho_a = number density of the species site a
+        belongs to).  c_ab = c_sr,ab - f_ab; the long-range parts sum to (sum_a rho_a q_a)^2 int(...) = 0 for a neutral
+        solvent (the same cancellation as in Eq. 18-19 of the 3D path, Q10), so only c_sr enters."""
+        if abs(float(np.dot(self.rho_site, self.q))) > 1e-12:
+            raise ValueError("solvent not neutral")
+        return float(self.rho_site @ self.c_sr_k0() @ self.rho_site)
+
+    def compressibility(self):
+        """Isothermal compressibility chi_T of the bulk solvent, A^3 mol / kcal, 'obtained by the RISM calculation for a
+        pure solvent system': the compressibility route,
+            1 / (k_B T chi_T) = sum_Gamma rho_Gamma - sum_ab rho_a rho_b int c_ab(r) dr
+        (Gamma: species, a, b: sites).  One species: rho k_B T chi_T = 1 / (1 - rho sum_ab c_ab(k = 0))."""
+        kT = 1.0 / self.beta
+        return 1.0 / (kT * (float(np.sum(self.sv.species_rho)) - self._rho_rho_c()))
+
+    def pressure(self):
+        """Bulk pressure of Eq. 20, kcal / (mol A^3):
+            P = sum_Gamma rho_Gamma (n_Gamma + 1) / (2 beta) - sum_{gamma lambda} (2 pi rho_gamma rho_lambda / beta) int c r^2 dr
+        n_Gamma = number of sites of species Gamma (the paper prints rho_gamma rho_gamma in the second sum: read as
+        rho_gamma rho_lambda).  2 pi int c r^2 dr = (1/2) int c dr."""
+        kT = 1.0 / self.beta
+        n_sites = np.bincount(self.sv.site_species, minlength=len(self.sv.species_rho))
+        ideal = float(np.sum(self.sv.species_rho * (n_sites + 1))) / 2.0
+        return kT * (ideal - 0.5 * self._rho_rho_c())
+
     def chi_types(self):
         """Reduce to site TYPES (Q15): chi_{g'g}(k) = sum_{a in g'} chi^full_ab, b any member of g."""
         sv = self.sv

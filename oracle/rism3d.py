@@ -469,6 +469,13 @@ class Rism3dOracle:
         c_int = np.array([self.dr ** 3 * float(np.sum(c_sr[gam], dtype=np.longdouble)) for gam in range(self.n_v)])
         return float(self.kT * chi_t * (1.0 - np.dot(self.rho_v, c_int))), c_int
 
+    def pressure_correction(self, chi_t, pressure):
+        """PC term of the solvation free energy, Eq. 21:  dmu_PC = -P V, with the partial molar volume of
+        Eq. 19 and the bulk pressure of Eq. 20 (both bulk quantities come from the solvent's own 1D solve).
+        Returns (dmu_PC in kcal/mol, V in A^3)."""
+        v, _ = self.pmv(chi_t)
+        return -pressure * v, v
+
     def solvation_gradient(self):
         """d(dmu)/dR_alpha = sum_gamma rho_gamma dV sum_r g_gamma(r) du_gamma(r)/dR_alpha  (the
         equation after Eq. 23; 'common for both HNC and KH'), kcal/(mol A), all pairs, u of Eq. 22 with the distance

@@ -249,3 +249,74 @@ def test_p10_spherical_ion_3d_matches_radial_1d():
         inside = rr < 1.5
         assert g3[s][inside].max() < 1e-6 and g1[s][grid.r < 1.5].max() < 1e-6      # empty core in both
     assert abs(mu3 - mu1) < 0.01 * abs(mu1)       # measured: -80.44 (3D, 0.5 A grid) vs -80.64 (radial) kcal/mol
+
+
+# ------------------------------------------------------------------------------------------------
+# Bulk thermodynamics of the solvent: compressibility (for Eq. 19) and pressure (Eq. 20)
+# ------------------------------------------------------------------------------------------------
+def _lj_fluid(rho, sigma=3.4, eps=0.24):
+    """one-site Lennard-Jones fluid (inputs only)"""
+    return Solvent(name="lj", type_names=["A"], q=np.zeros(1), sigma=np.array([sigma]), eps=np.array([eps]),
+                   rho=np.array([rho]), mult=np.ones(1, int), site_type=np.zeros(1, int), site_species=np.zeros(1, int),
+                   species_rho=np.array([rho]), bond=np.zeros((1, 1)))
+
+
+def test_compressibility_and_pressure_low_density_limits_and_second_virial_coefficient():
+    """Ideal gas: chi_T = 1/(rho kT), P = rho kT.  To second order in the density (textbook virial expansion, B_2 from an
+    independent radial quadrature of the Mayer function):  P = kT (rho + B_2 rho^2),  1/(kT chi_T) = rho + 2 B_2 rho^2."""
+    T = 298.0
+    kT = o3.K_BOLTZMANN * T
+    sig, eps = 3.4, 0.24
+    r = np.linspace(1e-3, 60.0, 600001)
+    mayer = np.exp(-4.0 * eps * ((sig / r) ** 12 - (sig / r) ** 6) / kT) - 1.0
+    b2 = -2.0 * math.pi * np.trapezoid(mayer * r * r, r)
+    for rho in (1e-7, 2e-5):                               # (third virial term: B_3 rho^3 / |B_2| rho^2 ~ 2e-3 at 2e-5)
+        x = o1.Xrism1d(_lj_fluid(rho, sig, eps), temperature=T, closure="HNC", n_points=4096, dr=0.02)
+        x.solve(tol=1e-12, nvec=5, b=1.0)
+        chi_t, p = x.compressibility(), x.pressure()
+        assert abs(chi_t * rho * kT - 1.0) < 3.0 * abs(2 * b2 * rho) + 1e-9          # -> ideal gas
+        assert abs(p / (rho * kT) - 1.0) < 3.0 * abs(b2 * rho) + 1e-9
+        # second virial level: the remainders are O(rho^2) relative
+        assert abs(p / kT - (rho + b2 * rho * rho)) < 1e-2 * abs(b2) * rho * rho
+        assert abs(1.0 / (kT * chi_t) - (rho + 2.0 * b2 * rho * rho)) < 1e-2 * abs(2.0 * b2) * rho * rho
+
+
+def test_compressibility_equals_structure_factor_at_k_zero():
+    """One-site fluid: rho kT chi_T = S(0) = 1 + rho h(k -> 0) (the textbook compressibility equation) -- h from the
+    converged g(r) by direct integration, against the c-route the oracle uses."""
+    T, rho = 298.0, 0.018
+    kT = o3.K_BOLTZMANN * T
+    x = o1.Xrism1d(_lj_fluid(rho), temperature=T, closure="KH", n_points=8192, dr=0.02)
+    x.solve(tol=1e-12, nvec=8, b=0.7)
+    g = x.g_r()[0, 0]
+    h0 = 4.0 * math.pi * x.grid.dr * np.sum((g - 1.0) * x.grid.r ** 2)
+    assert abs(rho * kT * x.compressibility() - (1.0 + rho * h0)) < 2e-4 * (1.0 + rho * h0)
+
+
+def test_water_thermodynamics_sanity_and_site_sum_convention(coarse_water):
+    """Water (3 sites, one species): rho kT chi_T = 1/(1 - rho sum_ab c_ab(0)) with the sum over ALL NINE site pairs, and
+    Eq. 20 with n_Gamma = 3.  Coarse radial grid (the stored tables use 16384 points): sanity of sign and size only."""
+    sv = water()
+    x = coarse_water
+    kT = 1.0 / x.beta
+    c0 = x.c_sr_k0()
+    assert c0.shape == (3, 3) and np.allclose(c0, c0.T, rtol=1e-9, atol=1e-9)
+    rho = sv.species_rho[0]
+    chi_t = x.compressibility()
+    assert abs(rho * kT * chi_t - 1.0 / (1.0 - rho * c0.sum())) < 1e-12
+    assert 0.0 < rho * kT * chi_t < 1.0                                  # a dense liquid is far less compressible than a gas
+    p = x.pressure()
+    assert abs(p - kT * (rho * (3 + 1) / 2.0 - 0.5 * rho * rho * c0.sum())) < 1e-12 * abs(p)
+
+
+def test_pressure_correction_is_minus_p_v():
+    """Eq. 21 on top of Eq. 19: a null solute has V = kT chi_T and dmu_PC = -P kT chi_T."""
+    sv = water()
+    from tests._util import synthetic_chi
+    k0, dk, chi = synthetic_chi(2, sv.rho)
+    orc = o3.Rism3dOracle(16, 0.6, 2)
+    orc.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+    orc.set_solute(np.array([[0.1, 0.0, 0.2]]), [0.0], [3.0], [0.0])
+    orc.iterate(1, 0.0)
+    pc, v = orc.pressure_correction(0.7, 0.01)
+    assert v == orc.kT * 0.7 and pc == -0.01 * v
