@@ -143,6 +143,11 @@ int rism3d_free_energy(rism3d_ctx* ctx, double* dmu_total, double* dmu_site);
  * neutrality, so only c_sr enters.  c_int_site (HOST [n_sites] or NULL) receives dV sum_r c_sr,g(r) in A^3. */
 int rism3d_pmv(rism3d_ctx* ctx, double chi_t, double* pmv, double* c_int_site);
 
+/* Pressure-correction term of the solvation free energy (Eq. 21), kcal/mol:  dmu_PC = -P V,  V the partial
+ * molar volume of Eq. 19 (returned in *pmv when not NULL, A^3).  chi_t (A^3 mol/kcal) and pressure (the bulk pressure of
+ * Eq. 20, kcal/(mol A^3)) are properties of the bulk solvent and come from its own 1D-RISM solve, like chi. */
+int rism3d_pressure_correction(rism3d_ctx* ctx, double chi_t, double pressure, double* dmu_pc, double* pmv);
+
 /* Solvent-induced gradient of the free energy on the solute atoms (the equation after Eq. 23;
  * common to HNC and KH):  d(dmu)/dR_a = sum_g rho_g int g_g(r) du_g(r)/dR_a dr,  kcal/(mol A), with u of Eq. 22, all
  * pairs (no cutoff), the distance clamp r_min as in the potential.  grad: HOST [n_atoms][3] of the last set_solute.

@@ -1,5 +1,7 @@
 """Writes workloads/chi/<solvent>.npz: the solvent susceptibility chi_{g'g}(k) of the
-three solvents the BASELINE.json configs use, from the 1D XRISM solve of oracle/rism1d.py.
+three solvents the BASELINE.json configs use, from the 1D XRISM solve of oracle/rism1d.py, together with the bulk
+isothermal compressibility chi_T (A^3 mol/kcal; enters Eq. 19) and the bulk pressure P of Eq. 20 (kcal/(mol A^3);
+enters Eq. 21) of the same solve.
 
 TEST INFRASTRUCTURE.  Calls only `oracle/`; the tables are INPUT DATA of the 3D path, read unchanged by
 both the 3D oracle and the CUDA library.
@@ -33,8 +35,10 @@ def make(name: str, n_points: int = 16384, dr: float = 0.025, verbose: bool = Tr
     n_k = int(np.ceil(K_MAX / x.grid.dk)) + 4
     if verbose:
         print(f"{name}: {iters} iterations, n_k = {n_k}, dk = {x.grid.dk:.6f}", flush=True)
+    # bulk thermodynamics of the same converged solve: chi_T for Eq. 19, P of Eq. 20 for Eq. 21
     return dict(k0=x.grid.dk, dk=x.grid.dk, chi=np.ascontiguousarray(chi[:n_k]),
-                names=np.array(sv.type_names), n_points=n_points, dr=dr, iterations=iters)
+                names=np.array(sv.type_names), n_points=n_points, dr=dr, iterations=iters,
+                chi_t=x.compressibility(), pressure=x.pressure())
 
 
 def main(names):

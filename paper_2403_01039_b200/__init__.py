@@ -8,7 +8,7 @@ or without a CUDA device raises.
 from .binding import (  # noqa: F401
     ACCELERATORS, CLOSURES, FIELDS, Rism3dError, Rism3dParams, Solver, library_path, load_library,
     rism3d_workspace_bytes, rism3d_init, rism3d_set_solvent_chi, rism3d_set_solute, rism3d_iterate,
-    rism3d_free_energy, rism3d_pmv, rism3d_gradient, rism3d_get_field, rism3d_set_tau, rism3d_get_rms_history, rism3d_launch_count, rism3d_phi_ms, rism3d_measure_dfma_peak,
+    rism3d_free_energy, rism3d_pmv, rism3d_pressure_correction, rism3d_gradient, rism3d_get_field, rism3d_set_tau, rism3d_get_rms_history, rism3d_launch_count, rism3d_phi_ms, rism3d_measure_dfma_peak,
     rism3d_set_profiling, rism3d_get_timings, rism3d_loop_kernel_name, N_LOOP_KERNELS,
     rism3d_debug_fft_forward, rism3d_debug_fft_inverse, rism3d_last_error, rism3d_status_string,
     rism3d_destroy, EXPORTED_SYMBOLS,

@@ -19,7 +19,7 @@ FIELDS = {"G": 0, "H": 1, "C_SR": 2, "T": 3, "TAU": 4, "W": 5, "PHI": 6}
 
 EXPORTED_SYMBOLS = [
     "rism3d_workspace_bytes", "rism3d_init", "rism3d_set_solvent_chi", "rism3d_set_solute",
-    "rism3d_iterate", "rism3d_free_energy", "rism3d_pmv", "rism3d_gradient", "rism3d_get_field", "rism3d_set_tau",
+    "rism3d_iterate", "rism3d_free_energy", "rism3d_pmv", "rism3d_pressure_correction", "rism3d_gradient", "rism3d_get_field", "rism3d_set_tau",
     "rism3d_get_rms_history", "rism3d_launch_count", "rism3d_phi_ms", "rism3d_measure_dfma_peak", "rism3d_set_profiling", "rism3d_get_timings",
     "rism3d_loop_kernel_name", "rism3d_debug_fft_forward",
     "rism3d_debug_fft_inverse", "rism3d_last_error", "rism3d_status_string", "rism3d_destroy",
@@ -81,6 +81,8 @@ def load_library():
     lib.rism3d_free_energy.argtypes = [C.c_void_p, dp, dp]
     lib.rism3d_pmv.restype = C.c_int
     lib.rism3d_pmv.argtypes = [C.c_void_p, C.c_double, dp, dp]
+    lib.rism3d_pressure_correction.restype = C.c_int
+    lib.rism3d_pressure_correction.argtypes = [C.c_void_p, C.c_double, C.c_double, dp, dp]
     lib.rism3d_gradient.restype = C.c_int
     lib.rism3d_gradient.argtypes = [C.c_void_p, dp]
     lib.rism3d_measure_dfma_peak.restype = C.c_int
@@ -185,6 +187,13 @@ def rism3d_pmv(ctx, chi_t: float, n_sites: int):
     site = np.zeros(n_sites)
     _check(ctx, load_library().rism3d_pmv(ctx, float(chi_t), C.byref(v), _dptr(site)))
     return float(v.value), site
+
+
+def rism3d_pressure_correction(ctx, chi_t: float, pressure: float):
+    """-> (dmu_PC in kcal/mol, pmv in A^3)"""
+    pc, v = C.c_double(0.0), C.c_double(0.0)
+    _check(ctx, load_library().rism3d_pressure_correction(ctx, float(chi_t), float(pressure), C.byref(pc), C.byref(v)))
+    return float(pc.value), float(v.value)
 
 
 def rism3d_gradient(ctx, n_atoms: int) -> np.ndarray:
@@ -337,6 +346,9 @@ class Solver:
 
     def measure_dfma_peak(self) -> float:
         return rism3d_measure_dfma_peak(self.ctx)
+
+    def pressure_correction(self, chi_t: float, pressure: float):
+        return rism3d_pressure_correction(self.ctx, chi_t, pressure)
 
     def phi_ms(self) -> float:
         return rism3d_phi_ms(self.ctx)

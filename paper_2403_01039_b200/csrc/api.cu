@@ -696,6 +696,17 @@ extern "C" int rism3d_pmv(rism3d_ctx* ctx, double chi_t, double* pmv, double* c_
   return RISM3D_OK;
 }
 
+extern "C" int rism3d_pressure_correction(rism3d_ctx* ctx, double chi_t, double pressure, double* dmu_pc, double* pmv) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  if (!dmu_pc) return fail(ctx, RISM3D_ERR_ARG, "dmu_pc is NULL");
+  double v = 0.0;
+  const int rc = rism3d_pmv(ctx, chi_t, &v, nullptr);     // Eq. 19
+  if (rc) return rc;
+  *dmu_pc = -pressure * v;                                 // Eq. 21
+  if (pmv) *pmv = v;
+  return RISM3D_OK;
+}
+
 extern "C" int rism3d_gradient(rism3d_ctx* ctx, double* grad) {
   if (!ctx) return RISM3D_ERR_ARG;
   ON_CTX_DEVICE(ctx);

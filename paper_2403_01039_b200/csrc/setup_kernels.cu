@@ -44,6 +44,12 @@ __device__ __forceinline__ void pair_terms(double r2, double qa, const double* _
       }
     } else if (WITH_PHI || inside) {
       const double kr = kappa * (r2 * rinv);
+      if (WITH_PHI && !WITH_W && kr > 26.0) {
+        // phi alone, 26 < kappa r <= 40: exp(-kappa r) < 5.2e-12, so a single-precision exponential (relative error
+        // < 3e-6 including the rounding of its argument) changes 1 - exp(-kappa r) by < 2e-17, a tenth of its last bit
+        ph = fma(qa, (1.0 - (double)__expf(-(float)kr)) * rinv, ph);
+        return;
+      }
       // 1 - exp(-kappa r): expm1 where the subtraction would cancel, exp elsewhere
       const double ex = (kr < 0.5) ? 1.0 + expm1(-kr) : exp(-kr);
       if (WITH_PHI) {

@@ -237,3 +237,19 @@ def test_gradient_matches_oracle(case):
     gpu.iterate(3, 0.0)
     assert np.array_equal(gpu.rms_history(), twin.rms_history())
     assert np.array_equal(gpu.get_field("G"), twin.get_field("G"))
+
+
+# ---- NEXT-2: pressure correction, Eq. 21, with the bulk chi_T and P stored beside the chi table (Eq. 19-20) --------
+@pytest.mark.parametrize("cfg,n", [("C1", 32), ("C2", 32)])
+def test_pressure_correction_matches_oracle(cfg, n):
+    from workloads import load_solvent_thermo
+    orc, gpu, _, _ = make_pair(cfg, n_override=n)
+    chi_t, pressure = load_solvent_thermo("water")
+    assert chi_t > 0.0 and np.isfinite(pressure)
+    orc.iterate(400, 1e-9)
+    gpu.iterate(400, 1e-9)
+    pc_o, v_o = orc.pressure_correction(chi_t, pressure)
+    pc_g, v_g = gpu.pressure_correction(chi_t, pressure)
+    assert abs(v_g - v_o) <= 1e-7 * abs(v_o)
+    assert abs(pc_g - pc_o) <= 1e-7 * abs(pc_o)
+    assert pc_g == -pressure * v_g

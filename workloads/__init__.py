@@ -12,11 +12,11 @@ its shape (atom count, net charge, 4 solvent site types, 256^3-512^3 grids) and 
 from .solvents import Solvent, water, water_nacl, solvent_by_name
 from .solutes import Solute, make_solute
 from .configs import Config, CONFIGS, get_config
-from .chi_io import load_chi, chi_path
+from .chi_io import load_chi, load_solvent_thermo, chi_path
 
 __all__ = [
     "Solvent", "water", "water_nacl", "solvent_by_name",
     "Solute", "make_solute",
     "Config", "CONFIGS", "get_config",
-    "load_chi", "chi_path",
+    "load_chi", "load_solvent_thermo", "chi_path",
 ]

@@ -6,6 +6,8 @@ unchanged by both the 3D oracle and the CUDA library.  Format: .npz with
   k0, dk   : abscissae k_m = k0 + m*dk  (A^-1)
   chi      : float64 [n_k][n_v][n_v], chi[m][gamma'][gamma]  (gamma' = summed index of Eq. 13)
   names    : site type names
+  chi_t    : isothermal compressibility of the bulk solvent, A^3 mol / kcal   (enters Eq. 19)
+  pressure : bulk pressure of Eq. 20, kcal / (mol A^3)                        (enters Eq. 21)
 """
 from __future__ import annotations
 
@@ -28,3 +30,11 @@ def load_chi(solvent_name: str):
             f"{p} missing: run `python -m oracle.make_chi_tables` (1D solvent solve, CPU oracle)")
     z = np.load(p)
     return float(z["k0"]), float(z["dk"]), np.ascontiguousarray(z["chi"], dtype=np.float64)
+
+
+def load_solvent_thermo(solvent_name: str):
+    """-> (chi_t, pressure) of the bulk solvent, stored beside its chi table by the same 1D solve."""
+    z = np.load(chi_path(solvent_name))
+    if "chi_t" not in z.files:
+        raise KeyError(f"{chi_path(solvent_name)} has no chi_t / pressure: rerun `python -m oracle.make_chi_tables`")
+    return float(z["chi_t"]), float(z["pressure"])
