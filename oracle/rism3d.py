@@ -246,16 +246,28 @@ def gram(a: np.ndarray, b: np.ndarray) -> float:
     return float(np.sum(a.astype(np.longdouble) * b.astype(np.longdouble), dtype=np.longdouble))
 
 
-class Mdiis:
-    """History of (X_i, R_i) pairs, circular over M slots, with the restart rule of Q8."""
+def dynamic_damping(rms: float, b_min: float, b_max: float) -> float:
+    """b = -0.2 log(R), R the rms residual ('when this parameter was changed dynamically ... the 3D-RISM
+    calculation is stable and converges quickly').  The paper gives neither the base of the logarithm nor what happens
+    for R >= 1 (b <= 0) or R < 1e-5 (b > 1): read as the decimal logarithm, clamped to [b_min, b_max] (Q18)."""
+    return min(b_max, max(b_min, -0.2 * math.log10(rms)))
 
-    def __init__(self, nvec: int, b: float, restart: float):
+
+class Mdiis:
+    """History of (X_i, R_i) pairs, circular over M slots, with the restart rule of Q8.
+    dynamic_b = (b_min, b_max): the damping parameter of Eq. 40 follows the residual (dynamic_damping) instead of being
+    the static b; it multiplies the whole sum of Eq. 40, i.e. the CURRENT b applies to every stored residual."""
+
+    def __init__(self, nvec: int, b: float, restart: float, dynamic_b=None):
         self.M, self.b, self.restart = int(nvec), float(b), float(restart)
+        self.dynamic_b = None if dynamic_b is None else (float(dynamic_b[0]), float(dynamic_b[1]))
         self.X, self.R, self.rms = [], [], []      # oldest first
         self.S = np.zeros((0, 0))
 
     def step(self, X: np.ndarray, R: np.ndarray, rms: float) -> np.ndarray:
         """Store (X, R), return the next input X_new = sum_i c_i (X_i + b R_i)."""
+        if self.dynamic_b is not None:
+            self.b = dynamic_damping(rms, *self.dynamic_b)
         if len(self.X) == self.M:                  # overwrite the oldest
             self.X.pop(0); self.R.pop(0); self.rms.pop(0)
             self.S = self.S[1:, 1:]
@@ -352,7 +364,8 @@ class Rism3dOracle:
 
     def __init__(self, n, spacing, n_sites, closure="KH", pse_order=1, temperature=298.0,
                  mdiis_nvec=5, mdiis_b=0.5, mdiis_restart=10.0, kappa=1.0, r_min=1e-3, origin=None,
-                 accelerator="MDIIS", anderson_s=(0.2, 0.0)):
+                 accelerator="MDIIS", anderson_s=(0.2, 0.0), mdiis_dynamic_b=None):
+        self.mdiis_dynamic_b = mdiis_dynamic_b
         self.n = (n, n, n) if np.isscalar(n) else tuple(n)
         self.dr = float(spacing)
         self.origin = tuple(-(m // 2) * self.dr for m in self.n) if origin is None else tuple(origin)
@@ -400,7 +413,7 @@ class Rism3dOracle:
         if self.accelerator == "ANDERSON":          # weight 1/rho_gamma; b is the mixing parameter
             self.mdiis = ModifiedAnderson(self.b, self.anderson_s, 1.0 / self.rho_v)
         else:
-            self.mdiis = Mdiis(self.M, self.b, self.restart)
+            self.mdiis = Mdiis(self.M, self.b, self.restart, self.mdiis_dynamic_b)
         self.rms_history = []
 
     # -- one pass of steps 2-5 ---------------------------------------------------------------

@@ -679,3 +679,43 @@ def test_gradient_of_a_charged_pair_matches_finite_differences_of_the_converged_
         assert abs(fd) > 100.0                                            # Coulomb dominated
         err[n] = abs(grad[0, 0] - fd) / abs(fd)
     assert err[32] < 1e-2 and err[32] < 0.25 * err[16], err
+
+
+# ------------------------------------------------------------------------------------------------
+# Dynamic damping b = -0.2 log R (Q18)
+# ------------------------------------------------------------------------------------------------
+def test_dynamic_damping_values_and_update_formula():
+    assert o3.dynamic_damping(1e-1, 0.1, 1.0) == pytest.approx(0.2, abs=1e-15)
+    assert o3.dynamic_damping(1e-3, 0.1, 1.0) == pytest.approx(0.6, abs=1e-15)
+    assert o3.dynamic_damping(10.0 ** -2.5, 0.1, 1.0) == pytest.approx(0.5, abs=1e-15)
+    assert o3.dynamic_damping(5.0, 0.1, 1.0) == 0.1            # R >= 1 would give b <= 0: clamped from below
+    assert o3.dynamic_damping(1e-9, 0.1, 1.0) == 1.0           # plain DIIS (b = 1) near convergence
+    # the CURRENT b multiplies every stored residual (Eq. 40: b stands in front of the sum)
+    rng = np.random.default_rng(3)
+    md = o3.Mdiis(3, 0.5, 0.0, dynamic_b=(0.1, 1.0))
+    Xs, Rs, rs = [rng.standard_normal(7) for _ in range(3)], [rng.standard_normal(7) for _ in range(3)], [1e-1, 1e-2, 1e-4]
+    for X, R, r in zip(Xs, Rs, rs):
+        out = md.step(X, R, r)
+    S = np.array([[np.dot(a, b) for b in Rs] for a in Rs])
+    c = o3.mdiis_coefficients(S)
+    b_now = 0.8                                                # -0.2 log10(1e-4)
+    assert np.allclose(out, sum(c[i] * (Xs[i] + b_now * Rs[i]) for i in range(3)), rtol=1e-12, atol=1e-12)
+
+
+def test_dynamic_damping_reaches_the_same_fixed_point_faster():
+    """The fixed point does not depend on the damping schedule (invariant P7); on the small ion case the dynamic rule
+    needs fewer iterations than the static b = 0.5 (the paper's claim)."""
+    sv = water()
+    k0, dk, chi = synthetic_chi(2, sv.rho)
+    sol = make_solute("C1")
+    out = []
+    for dyn in (None, (0.1, 1.0)):
+        orc = o3.Rism3dOracle(16, 0.6, 2, mdiis_nvec=5, mdiis_b=0.5, mdiis_dynamic_b=dyn)
+        orc.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+        orc.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps)
+        n, rms = orc.iterate(3000, 1e-10)
+        assert rms < 1e-10
+        out.append((n, orc.get_field("G"), orc.free_energy()[0]))
+    assert np.max(np.abs(out[0][1] - out[1][1])) < 1e-8
+    assert abs(out[0][2] - out[1][2]) < 1e-8 * abs(out[0][2])
+    assert out[1][0] <= out[0][0]
