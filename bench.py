@@ -487,6 +487,40 @@ def run_ours(args):
                     "seconds_to_converge": a_s, "iterations_to_converge": int(a_it), "converged": bool(a_rms < cfg.tol),
                     "ms_per_iteration": (a_s - a_setup * 1e-3) / max(a_it, 1) * 1e3, "dmu_kcal_mol": a_mu}
 
+    # ---- extra (context): the same solve with the dynamic damping b = -0.2 log10(rms) of PAPER.md:308 (opt-in: the
+    # update then reads X_i and R_i, M more words per pt*site and iteration), and the iteration counts on C2 ------------
+    dyn = None
+    if rank == 0 and world == 1 and not args.no_e2e and not args.no_anderson:
+        solver.close()
+        solver = lib.Solver(cfg.n, cfg.spacing, n_v, closure=cfg.closure, pse_order=cfg.pse_order, mdiis_nvec=M,
+                            mdiis_b=cfg.mdiis_b, mdiis_restart=cfg.mdiis_restart, temperature=cfg.temperature,
+                            kappa=cfg.kappa, r_min=cfg.r_min, device=local_rank, mdiis_dynamic_b=(0.1, 1.0))
+        solver.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        d_setup = solver.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=cfg.rcut)
+        d_it, d_rms = solver.iterate(args.max_iter, cfg.tol)
+        d_mu, _ = solver.free_energy()
+        for s_ in range(n_v):
+            lib.rism3d_get_field(solver.ctx, lib.FIELDS["G"], s_, g_np[s_].ctypes.data, False)
+        torch.cuda.synchronize(dev)
+        d_s = time.perf_counter() - t0
+        dyn = {"what": "MDIIS with b = clamp(-0.2 log10(rms), 0.1, 1) (PAPER.md:308, DESIGN.md Q18): (3M + 12 + 1/n_v) words per "
+                       "pt*site and iteration instead of (2M + 12 + 1/n_v)",
+               "seconds_to_converge": d_s, "iterations_to_converge": int(d_it), "converged": bool(d_rms < cfg.tol),
+               "ms_per_iteration": (d_s - d_setup * 1e-3) / max(d_it, 1) * 1e3, "dmu_kcal_mol": d_mu,
+               "static_b_iterations": e2e["iterations_to_converge"] if e2e else None}
+        c2 = {}
+        cfg2, sv2, sol2, (k02, dk2, chi2) = workload_inputs("C2")
+        for label, dynb in (("static", None), ("dynamic", (0.1, 1.0))):
+            s2 = lib.Solver(cfg2.n, cfg2.spacing, sv2.n_v, closure=cfg2.closure, mdiis_nvec=cfg2.mdiis_nvec, mdiis_b=cfg2.mdiis_b,
+                            mdiis_restart=cfg2.mdiis_restart, device=local_rank, mdiis_dynamic_b=dynb)
+            s2.set_solvent_chi(sv2.q, sv2.sigma, sv2.eps, sv2.rho, k02, dk2, chi2)
+            s2.set_solute(sol2.xyz, sol2.q, sol2.sigma, sol2.eps, rcut=cfg2.rcut)
+            c2[label] = int(s2.iterate(3000, cfg2.tol)[0])
+            s2.close()
+        dyn["C2_iterations_to_converge"] = c2
+
     # ---- the other large configs, briefly (device-resident iterations only): C3 and the memory-ceiling C5 --------------
     others = None
     if rank == 0 and world == 1 and not args.no_others and args.workload == "C4":
@@ -518,7 +552,7 @@ def run_ours(args):
             "dtype": "f64", "data": "synthetic",
             "config": bench_config(cfg, sol, world), "workspace_gb": workspace_gb,
             "pt_site_updates_per_s": value * pt_sites, "setup_ms": setup_ms, "rms_after_timed_steps": rms_end,
-            "roofline": roofline, "setup": setup, "other_workloads": others, "cpu_baseline": cpu, "e2e": e2e, "e2e_modified_anderson": anderson, "fft_compare": fft_cmp, "gpu_launches": int(launches), "clocks": clocks,
+            "roofline": roofline, "setup": setup, "other_workloads": others, "cpu_baseline": cpu, "e2e": e2e, "e2e_modified_anderson": anderson, "e2e_dynamic_damping": dyn, "fft_compare": fft_cmp, "gpu_launches": int(launches), "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
     solver.close()

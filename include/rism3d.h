@@ -46,8 +46,9 @@ typedef struct rism3d_ctx rism3d_ctx;   /* opaque; created by rism3d_init, freed
 typedef enum {
   RISM3D_OK            =  0,
   RISM3D_ERR_ARG       = -1,   /* NULL pointer, negative count, unknown enum value                 */
-  RISM3D_ERR_SIZE      = -2,   /* grid not cubic / not a power of two in 8..512, n_sites not 1,2,4,8,
-                                  mdiis_nvec outside 1..16                                         */
+  RISM3D_ERR_SIZE      = -2,   /* grid not cubic / not a power of two in 8..512, n_sites outside 1..8,
+                                  mdiis_nvec outside 1..16, r_min or mdiis_b not positive, or a grid / site
+                                  combination whose k-space tile does not fit shared memory (512^3 with 1 site) */
   RISM3D_ERR_ORDER     = -3,   /* call out of order (set_solute before set_solvent_chi, ...)       */
   RISM3D_ERR_CHI_RANGE = -4,   /* chi table does not cover the 3D |k| range, or is too coarse      */
   RISM3D_ERR_NEUTRAL   = -5,   /* sum_g rho_g q_g != 0 (1e-12)                                     */
@@ -77,7 +78,9 @@ typedef struct {
   int    nx, ny, nz;        /* grid points per axis; this build: nx == ny == nz, power of two, 8..512 */
   double spacing;           /* grid spacing, A                                                     */
   double origin[3];         /* position of grid index (0,0,0), A                                   */
-  int    n_sites;           /* n_v, number of solvent site TYPES: 1, 2, 4 or 8                     */
+  int    n_sites;           /* n_v, number of solvent site TYPES, 1..8 (3, 5, 6, 7 run padded to 4 or 8 with
+                               phantom types of zero charge, LJ, density and chi: same results, the bandwidth
+                               of the padded count)                                                */
   int    closure;           /* rism3d_closure                                                      */
   int    pse_order;         /* n of PSE-n (>= 1; 1 is KH); ignored for KH / HNC                    */
   double temperature;       /* K                                                                   */
@@ -90,6 +93,11 @@ typedef struct {
   int    accelerator;       /* rism3d_accelerator; ANDERSON ignores mdiis_nvec / mdiis_restart and uses
                                mdiis_b as the mixing parameter b of Eq. 39                         */
   double anderson_s[2];     /* tuning parameters s_1, s_2 of Eq. 34-35 (the paper's GPU code: 0.2, 0)      */
+  int    mdiis_dynamic_b;   /* != 0 (MDIIS only): b = -0.2 log10(rms) clamped to [mdiis_b_min, mdiis_b_max] every
+                               iteration instead of the static mdiis_b (Q18).  The
+                               history then keeps X_i and R_i apart and the update reads both: M more words per
+                               grid point, site and iteration                                       */
+  double mdiis_b_min, mdiis_b_max;
 } rism3d_params;
 
 /* Bytes of DEVICE memory the caller must provide to rism3d_init (0 if the parameters are invalid). */
@@ -183,7 +191,8 @@ int rism3d_set_profiling(rism3d_ctx* ctx, int enable);
 int rism3d_get_timings(rism3d_ctx* ctx, double* ms_total, int cap, long long* n_iterations);
 const char* rism3d_loop_kernel_name(int k);             /* static strings; "" when k is out of range */
 
-/* Debug / test hooks: run the shifted 3D transform pair alone on a caller-supplied field.
+/* Debug / test hooks: run the shifted 3D transform pair alone on a caller-supplied field.  n_sites below is the PADDED
+ * site count (n_sites rounded up to 1, 2, 4 or 8).
  * forward: real DEVICE field [n_sites][nx][ny][nz] -> complex DEVICE spectrum
  *   [jx][jy][p][site] (re, im interleaved), p = 0..nz/2-1 standing for jz = 2p, holding
  *   sum_n f(r_n) exp(-i k_j.(r_n - origin)) with k_j = dk (j + 1/2) per axis (no dV factor).

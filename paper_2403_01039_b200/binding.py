@@ -49,6 +49,8 @@ class Rism3dParams(C.Structure):
         ("device", C.c_int),
         ("accelerator", C.c_int),
         ("anderson_s", C.c_double * 2),
+        ("mdiis_dynamic_b", C.c_int),
+        ("mdiis_b_min", C.c_double), ("mdiis_b_max", C.c_double),
     ]
 
 
@@ -271,7 +273,7 @@ class Solver:
 
     def __init__(self, n, spacing, n_sites, closure="KH", pse_order=1, temperature=298.0, mdiis_nvec=5,
                  mdiis_b=0.5, mdiis_restart=10.0, kappa=1.0, r_min=1e-3, origin=None, device=0,
-                 accelerator="MDIIS", anderson_s=(0.2, 0.0)):
+                 accelerator="MDIIS", anderson_s=(0.2, 0.0), mdiis_dynamic_b=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2403_01039_b200 needs a CUDA device (no CPU fallback)")
@@ -294,6 +296,8 @@ class Solver:
         p.device = int(device)
         p.accelerator = ACCELERATORS[accelerator]
         p.anderson_s = (C.c_double * 2)(float(anderson_s[0]), float(anderson_s[1]))
+        p.mdiis_dynamic_b = 0 if mdiis_dynamic_b is None else 1        # (b_min, b_max) of b = -0.2 log10(rms)
+        p.mdiis_b_min, p.mdiis_b_max = (0.0, 0.0) if mdiis_dynamic_b is None else (float(mdiis_dynamic_b[0]), float(mdiis_dynamic_b[1]))
         self.params = p
         nbytes = rism3d_workspace_bytes(p)
         if nbytes == 0:
@@ -395,19 +399,33 @@ class Solver:
         ms, n = rism3d_get_timings(self.ctx)
         return {rism3d_loop_kernel_name(k): (ms[k] / n if n else 0.0) for k in range(N_LOOP_KERNELS)}, n
 
+    @property
+    def _padded_sites(self) -> int:
+        return 1 if self.n_sites <= 1 else (2 if self.n_sites <= 2 else (4 if self.n_sites <= 4 else 8))
+
     def fft_forward(self, real_dev):
         """debug: real device tensor [n_sites][n][n][n] -> complex device tensor [n][n][n/2][n_sites]."""
         import torch
+        nvp = self._padded_sites                     # the library transforms the padded site count (rism3d.h)
+        if nvp != self.n_sites:
+            pad = torch.zeros((nvp, self.n, self.n, self.n), dtype=torch.float64, device=self.device)
+            pad[: self.n_sites] = real_dev
+            real_dev = pad
         real_dev = real_dev.contiguous()
-        out = torch.empty((self.n, self.n, self.n // 2, self.n_sites), dtype=torch.complex128, device=self.device)
+        out = torch.empty((self.n, self.n, self.n // 2, nvp), dtype=torch.complex128, device=self.device)
         self.stream.wait_stream(torch.cuda.current_stream(self.device))
         rism3d_debug_fft_forward(self.ctx, real_dev.data_ptr(), out.data_ptr())
-        return out
+        return out[..., : self.n_sites]
 
     def fft_inverse(self, spec_dev):
         import torch
+        nvp = self._padded_sites
+        if nvp != self.n_sites:
+            pad = torch.zeros((self.n, self.n, self.n // 2, nvp), dtype=torch.complex128, device=self.device)
+            pad[..., : self.n_sites] = spec_dev
+            spec_dev = pad
         spec_dev = spec_dev.contiguous()
-        out = torch.empty((self.n_sites, self.n, self.n, self.n), dtype=torch.float64, device=self.device)
+        out = torch.empty((nvp, self.n, self.n, self.n), dtype=torch.float64, device=self.device)
         self.stream.wait_stream(torch.cuda.current_stream(self.device))
         rism3d_debug_fft_inverse(self.ctx, spec_dev.data_ptr(), out.data_ptr())
-        return out
+        return out[: self.n_sites]

@@ -100,13 +100,17 @@ static bool make_tensor_map_2d(CUtensorMap* tm, void* base, uint64_t row_len, ui
                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// kernels are instantiated for 1, 2, 4 and 8 site types (the sites of a k point share 8 / nv-wide tile rows and are
+// exchanged by butterfly shuffles): other counts run padded with phantom types
+static int padded_sites(int nv) { return nv <= 1 ? 1 : (nv <= 2 ? 2 : (nv <= 4 ? 4 : 8)); }
+
 static bool valid_params(const rism3d_params* p) {
   if (!p) return false;
   const int n = p->nx;
   if (p->ny != n || p->nz != n) return false;
   if (n < 8 || n > 512 || (n & (n - 1))) return false;
-  const int nv = p->n_sites;
-  if (!(nv == 1 || nv == 2 || nv == 4 || nv == 8)) return false;
+  if (p->n_sites < 1 || p->n_sites > MAX_NV) return false;
+  const int nv = padded_sites(p->n_sites);
   if (((n / 2) * nv) % 8) return false;             // tile rows are 8 complex wide
   if (p->mdiis_nvec < 1 || p->mdiis_nvec > MAX_M) return false;
   if (!(p->spacing > 0.0) || !(p->temperature > 0.0) || !(p->kappa > 0.0)) return false;
@@ -117,6 +121,7 @@ static bool valid_params(const rism3d_params* p) {
   if (p->closure != RISM3D_KH && p->closure != RISM3D_PSE && p->closure != RISM3D_HNC) return false;
   if (p->closure == RISM3D_PSE && p->pse_order < 1) return false;
   if (p->accelerator != RISM3D_ACCEL_MDIIS && p->accelerator != RISM3D_ACCEL_ANDERSON) return false;
+  if (p->mdiis_dynamic_b && !(p->mdiis_b_min > 0.0 && p->mdiis_b_max >= p->mdiis_b_min && p->mdiis_b_max < 1e6)) return false;
   return true;
 }
 
@@ -127,7 +132,7 @@ static int n_shells(int n) { const int hn = n / 2; return 3 * (hn - 1) * hn / 2 
 
 // carve the workspace; with base == nullptr only the total size is computed
 static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_out, size_t* scratch_bytes) {
-  const size_t n = p->nx, nv = p->n_sites, M = (size_t)effective_m(p);
+  const size_t n = p->nx, nv = (size_t)padded_sites(p->n_sites), M = (size_t)effective_m(p);
   const size_t npts = n * n * n, field = npts * nv;
   size_t off = 0;
   auto take = [&](size_t bytes) { char* ptr = base ? base + off : nullptr; off += align256(bytes); return ptr; };
@@ -206,7 +211,7 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
   if (cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, p->device) != cudaSuccess || num_sms <= 0 ||
       cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, p->device) != cudaSuccess)
     return RISM3D_ERR_CUDA;
-  if (kspace_smem_bytes(p->nx, p->n_sites) > smem_optin) return RISM3D_ERR_SIZE;
+  if (kspace_smem_bytes(p->nx, padded_sites(p->n_sites)) > smem_optin) return RISM3D_ERR_SIZE;
   rism3d_ctx* ctx = new rism3d_ctx();
   memset(ctx, 0, sizeof(*ctx));
   ctx->p = *p;
@@ -215,7 +220,7 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
   ctx->ws_bytes = bytes;
   carve(p, ctx->ws, &ctx->b, &ctx->d_out, &ctx->scratch_bytes);
   Grid& g = ctx->g;
-  g.n = p->nx; g.nv = p->n_sites; g.h = p->spacing;
+  g.n = p->nx; g.nv = padded_sites(p->n_sites); g.nv_user = p->n_sites; g.h = p->spacing;
   for (int i = 0; i < 3; ++i) g.origin[i] = p->origin[i];
   g.npts = (size_t)g.n * g.n * g.n;
   g.field = g.npts * g.nv;
@@ -227,6 +232,8 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
   sp.M = effective_m(p); sp.b = p->mdiis_b; sp.restart = p->mdiis_restart;
   sp.accel = p->accelerator; sp.and_s1 = p->anderson_s[0]; sp.and_s2 = p->anderson_s[1];
   if (sp.accel == RISM3D_ACCEL_ANDERSON) sp.restart = 0.0;   // the paper's method has no restart rule
+  sp.dyn_b = p->mdiis_dynamic_b != 0 && sp.accel == RISM3D_ACCEL_MDIIS;
+  sp.b_min = p->mdiis_b_min; sp.b_max = p->mdiis_b_max;
   sp.kT = K_BOLTZMANN * p->temperature;
   sp.beta = 1.0 / sp.kT;
   sp.kappa = p->kappa; sp.r_min = p->r_min;
@@ -283,8 +290,9 @@ extern "C" int rism3d_set_solvent_chi(rism3d_ctx* ctx, const double* q, const do
   ON_CTX_DEVICE(ctx);
   if (!q || !sigma || !eps || !rho || !chi || n_k < 4 || !(dk > 0.0)) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   const Grid& g = ctx->g;
+  const int nu = g.nv_user;
   double neutral = 0.0;
-  for (int i = 0; i < g.nv; ++i) neutral += rho[i] * q[i];
+  for (int i = 0; i < nu; ++i) neutral += rho[i] * q[i];
   if (fabs(neutral) > 1e-12) return fail(ctx, RISM3D_ERR_NEUTRAL, "sum rho_g q_g = %.3e", neutral);
   const double dkg = 2.0 * M_PI / (g.n * g.h);
   const double kmin = dkg * sqrt(0.75), kmax = dkg * sqrt(2.0 * (n_shells(g.n) - 1) + 0.75);
@@ -292,18 +300,39 @@ extern "C" int rism3d_set_solvent_chi(rism3d_ctx* ctx, const double* q, const do
     return fail(ctx, RISM3D_ERR_CHI_RANGE, "table covers [%.4f, %.4f], grid needs [%.4f, %.4f]", k0,
                 k0 + (n_k - 1) * dk, kmin, kmax);
   const size_t tbytes = (size_t)n_k * g.nv * g.nv * 8;
-  if (tbytes > ctx->scratch_bytes) return fail(ctx, RISM3D_ERR_WORKSPACE, "chi table larger than the scratch span");
-  for (int i = 0; i < g.nv; ++i) { ctx->qv[i] = q[i]; ctx->sigv[i] = sigma[i]; ctx->epsv[i] = eps[i]; ctx->rhov[i] = rho[i]; }
-  double* d_table = ctx->b.Z;                      // scratch: the history is rebuilt by set_solute anyway
-  CU(cudaMemcpyAsync(d_table, chi, tbytes, cudaMemcpyHostToDevice, ctx->stream));
+  for (int i = 0; i < g.nv; ++i) {                   // phantom types (i >= nu): no charge, no LJ well, no density
+    const bool real = i < nu;
+    ctx->qv[i] = real ? q[i] : 0.0; ctx->sigv[i] = real ? sigma[i] : 1.0; ctx->epsv[i] = real ? eps[i] : 0.0;
+    ctx->rhov[i] = real ? rho[i] : 0.0;
+  }
+  std::vector<double> padded;                        // chi with zero rows and columns for the phantom types
+  const double* table = chi;
+  if (g.nv != nu) {
+    padded.assign((size_t)n_k * g.nv * g.nv, 0.0);
+    for (int m = 0; m < n_k; ++m)
+      for (int a = 0; a < nu; ++a)
+        for (int c = 0; c < nu; ++c) padded[((size_t)m * g.nv + a) * g.nv + c] = chi[((size_t)m * nu + a) * nu + c];
+    table = padded.data();
+  }
+  // the radial table is only needed until chi_shell is built: it goes through the history span (rebuilt by set_solute
+  // anyway) or, on grids too small to hold it, through a temporary allocation of the library's own
+  double* d_table = ctx->b.Z;
+  double* d_tmp = nullptr;
+  if (tbytes > ctx->scratch_bytes) {
+    CU(cudaMalloc((void**)&d_tmp, tbytes));
+    d_table = d_tmp;
+  }
+  CU(cudaMemcpyAsync(d_table, table, tbytes, cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaMemcpyAsync(ctx->b.qv, ctx->qv, g.nv * 8, cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaMemcpyAsync(ctx->b.rhov, ctx->rhov, g.nv * 8, cudaMemcpyHostToDevice, ctx->stream));
   for (int i = 0; i < g.nv; ++i)                   // inner-product weights: 1/rho_g for the modified Anderson method (Eq. 38)
-    ctx->gramw[i] = ctx->sp.accel == RISM3D_ACCEL_ANDERSON ? 1.0 / rho[i] : 1.0;
+    ctx->gramw[i] = (ctx->sp.accel == RISM3D_ACCEL_ANDERSON) ? (i < nu ? 1.0 / rho[i] : 0.0) : 1.0;
   CU(cudaMemcpyAsync(ctx->b.gram_w, ctx->gramw, g.nv * 8, cudaMemcpyHostToDevice, ctx->stream));
   ctx->launches += launch_chi_shell(g, ctx->b, d_table, n_k, k0, dk, ctx->stream);
-  CU(cudaGetLastError());
-  CU(cudaStreamSynchronize(ctx->stream));
+  const cudaError_t e_launch = cudaGetLastError(), e_sync = cudaStreamSynchronize(ctx->stream);
+  if (d_tmp) cudaFree(d_tmp);
+  CU(e_launch);
+  CU(e_sync);
   ctx->have_solvent = true;
   ctx->have_solute = false;
   return RISM3D_OK;
@@ -668,7 +697,7 @@ extern "C" int rism3d_free_energy(rism3d_ctx* ctx, double* dmu_total, double* dm
   CU(cudaMemcpyAsync(host, ctx->d_out, ctx->g.nv * 8, cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   double tot = 0.0;
-  for (int i = 0; i < ctx->g.nv; ++i) {
+  for (int i = 0; i < ctx->g.nv_user; ++i) {
     tot += host[i];
     if (dmu_site) dmu_site[i] = host[i];
   }
@@ -688,7 +717,7 @@ extern "C" int rism3d_pmv(rism3d_ctx* ctx, double chi_t, double* pmv, double* c_
   CU(cudaMemcpyAsync(host, ctx->d_out, 2 * MAX_NV * 8, cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   double sum = 0.0;                                  // sum_g rho_g int c_g dr: the -q_g phi part drops out (sum rho q = 0)
-  for (int i = 0; i < ctx->g.nv; ++i) {
+  for (int i = 0; i < ctx->g.nv_user; ++i) {
     sum += ctx->rhov[i] * host[MAX_NV + i];
     if (c_int_site) c_int_site[i] = host[MAX_NV + i];
   }
@@ -748,7 +777,7 @@ extern "C" int rism3d_gradient(rism3d_ctx* ctx, double* grad) {
 extern "C" int rism3d_get_field(rism3d_ctx* ctx, int which, int site, double* dst, int dst_is_device) {
   if (!ctx) return RISM3D_ERR_ARG;
   ON_CTX_DEVICE(ctx);
-  if (!dst || which < 0 || which > RISM3D_FIELD_PHI || site < 0 || site >= ctx->g.nv)
+  if (!dst || which < 0 || which > RISM3D_FIELD_PHI || site < 0 || site >= ctx->g.nv_user)
     return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before get_field");
   if (which == RISM3D_FIELD_T || which == RISM3D_FIELD_PHI) { const int rc_phi = ensure_phi(ctx); if (rc_phi) return rc_phi; }
@@ -763,7 +792,7 @@ extern "C" int rism3d_get_field(rism3d_ctx* ctx, int which, int site, double* ds
 extern "C" int rism3d_set_tau(rism3d_ctx* ctx, int site, const double* src, int src_is_device) {
   if (!ctx) return RISM3D_ERR_ARG;
   ON_CTX_DEVICE(ctx);
-  if (!src || site < 0 || site >= ctx->g.nv) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
+  if (!src || site < 0 || site >= ctx->g.nv_user) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before set_tau");
   const Grid& g = ctx->g;
   CU(cudaMemcpyAsync(ctx->b.tau + (size_t)site * g.npts, src, g.npts * 8,

@@ -389,28 +389,10 @@ template <> struct FftCfg<8>   { enum { R1 = 4,  R2 = 2,  R3 = 1, T = 2,  G = 8 
 template <> struct FftCfg<16>  { enum { R1 = 4,  R2 = 4,  R3 = 1, T = 4,  G = 8 }; };
 template <> struct FftCfg<32>  { enum { R1 = 8,  R2 = 4,  R3 = 1, T = 4,  G = 8 }; };
 template <> struct FftCfg<64>  { enum { R1 = 8,  R2 = 8,  R3 = 1, T = 8,  G = 4 }; };
-#ifndef R3D_PLAN128
-#define R3D_PLAN128 0
-#endif
-#if R3D_PLAN128 == 0
 template <> struct FftCfg<128> { enum { R1 = 16, R2 = 8,  R3 = 1, T = 8,  G = 2 }; };
-#elif R3D_PLAN128 == 1
-template <> struct FftCfg<128> { enum { R1 = 4,  R2 = 4,  R3 = 8, T = 16, G = 2 }; };
-#else
-template <> struct FftCfg<128> { enum { R1 = 8,  R2 = 4,  R3 = 4, T = 16, G = 2 }; };
-#endif
-#ifndef R3D_PLAN256
-#define R3D_PLAN256 2
-#endif
-#if R3D_PLAN256 == 0
-template <> struct FftCfg<256> { enum { R1 = 16, R2 = 16, R3 = 1, T = 16, G = 1 }; };
-#elif R3D_PLAN256 == 1
-template <> struct FftCfg<256> { enum { R1 = 8, R2 = 8, R3 = 4, T = 32, G = 1 }; };
-#elif R3D_PLAN256 == 2
+// 256: three passes of small radices (4 x 8 x 8, 32 threads per column) beat 16 x 16 in the strided passes, whose
+// register-cached twiddles would not fit beside 16 complex values per thread
 template <> struct FftCfg<256> { enum { R1 = 4, R2 = 8, R3 = 8, T = 32, G = 1 }; };
-#elif R3D_PLAN256 == 3
-template <> struct FftCfg<256> { enum { R1 = 16, R2 = 16, R3 = 1, T = 16, G = 2 }; };
-#endif
 template <> struct FftCfg<512> { enum { R1 = 8,  R2 = 8,  R3 = 8, T = 64, G = 1 }; };
 
 }  // namespace r3d

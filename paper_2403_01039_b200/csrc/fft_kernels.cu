@@ -37,11 +37,7 @@ struct StridedCfg {
   enum { NT = FftCfg<N>::T * FftCfg<N>::G * COLS,                  // threads per CTA
          ITEM = FftCfg<N>::G * N * COLS,                             // complex elements per work item
          SHM = 2 * ITEM * (int)sizeof(cplx),
-#ifdef R3D_STRIDED_MINB
-         MINB = R3D_STRIDED_MINB };
-#else
          MINB = (SHM > 110 * 1024) ? 1 : 2 };      // <= 128 registers per thread: room for the cached twiddles
-#endif
 };
 
 // stage work item `item` (G tiles) into `buf` [G][N][COLS]
@@ -198,52 +194,9 @@ constexpr int ZP = COLS + 1;
 // (GF, MBF) and zinv_residual (GI, MBI).  The large lines run 3-pass plans of small radices: few registers per thread,
 // so that 768-1024 threads per SM hide the latency of the closure's exp() chains and of the streaming loads.
 template <int NZ> struct ZPlan : FftCfg<NZ> { enum { GF = FftCfg<NZ>::G, MBF = 1, GI = FftCfg<NZ>::G, MBI = 1, MBG = 1 }; };
-#ifndef R3D_ZGF
-#define R3D_ZGF 1
-#endif
-#ifndef R3D_ZMBF
-#define R3D_ZMBF 4
-#endif
-#ifndef R3D_ZGI
-#define R3D_ZGI 1
-#endif
-#ifndef R3D_ZMBI
-#define R3D_ZMBI 8
-#endif
-#ifndef R3D_ZMBG
-#define R3D_ZMBG 5
-#endif
-#ifndef R3D_ZPLAN64
-#define R3D_ZPLAN64 2
-#endif
-#if R3D_ZPLAN64 == 0
-template <> struct ZPlan<64>  { enum { R1 = 8, R2 = 8, R3 = 1, T = 8, G = 4, GF = 4, MBF = 2, GI = 4, MBI = 2, MBG = 2 }; };
-#elif R3D_ZPLAN64 == 1
-template <> struct ZPlan<64>  { enum { R1 = 4, R2 = 4, R3 = 4, T = 16, G = 2, GF = 1, MBF = 4, GI = 1, MBI = 8, MBG = 5 }; };
-#else
 template <> struct ZPlan<64>  { enum { R1 = 8, R2 = 8, R3 = 1, T = 8, G = 4, GF = 2, MBF = 4, GI = 2, MBI = 8, MBG = 5 }; };
-#endif
-template <> struct ZPlan<128> { enum { R1 = 4, R2 = 4, R3 = 8, T = 16, G = 2, GF = R3D_ZGF, MBF = R3D_ZMBF, GI = R3D_ZGI, MBI = R3D_ZMBI, MBG = R3D_ZMBG }; };
-#ifndef R3D_Z256_PLAN
-#define R3D_Z256_PLAN 0
-#endif
-#ifndef R3D_Z256_GF
-#define R3D_Z256_GF 2
-#endif
-#ifndef R3D_Z256_MBF
-#define R3D_Z256_MBF 2
-#endif
-#ifndef R3D_Z256_GI
-#define R3D_Z256_GI 2
-#endif
-#ifndef R3D_Z256_MBG
-#define R3D_Z256_MBG 2
-#endif
-#if R3D_Z256_PLAN == 0
-template <> struct ZPlan<256> { enum { R1 = 16, R2 = 16, R3 = 1, T = 16, G = 2, GF = R3D_Z256_GF, MBF = R3D_Z256_MBF, GI = R3D_Z256_GI, MBI = 2, MBG = R3D_Z256_MBG }; };
-#else
-template <> struct ZPlan<256> { enum { R1 = 4, R2 = 8, R3 = 8, T = 32, G = 1, GF = R3D_Z256_GF, MBF = R3D_Z256_MBF, GI = R3D_Z256_GI, MBI = 2, MBG = R3D_Z256_MBG }; };
-#endif
+template <> struct ZPlan<128> { enum { R1 = 4, R2 = 4, R3 = 8, T = 16, G = 2, GF = 1, MBF = 4, GI = 1, MBI = 8, MBG = 5 }; };
+template <> struct ZPlan<256> { enum { R1 = 16, R2 = 16, R3 = 1, T = 16, G = 2, GF = 2, MBF = 2, GI = 2, MBI = 2, MBG = 2 }; };
 
 __device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
 __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
@@ -251,24 +204,29 @@ __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<do
 // closure + forward z.  One tile per CTA.  Stage-in with 16-byte loads (two adjacent z points of both half lines
 // per thread, two such quads in flight), closure, packing u_m = (c_m - i c_{m+n/2}) exp(-i pi m / n) into the
 // shared-memory tile, then the n/2-point complex line FFTs.
-template <int NZ, int G, int MINB>
+// DYN: the damping follows the residual; the Z slots then hold X_i and the update forms X_i + b R_i from both histories
+template <int NZ, int G, int MINB, bool DYN>
 __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
     closure_zfwd_kernel(double* __restrict__ tau_cur, const double* __restrict__ w, const double* __restrict__ raw,
-                        const double* __restrict__ Z, cplx* __restrict__ work, Twiddle tw_shift, Twiddle tw,
-                        const DevState* __restrict__ st, int nv, size_t npts, size_t field, int closure, int order) {
+                        const double* __restrict__ Z, const double* __restrict__ Rh, cplx* __restrict__ work,
+                        Twiddle tw_shift, Twiddle tw, const DevState* __restrict__ st, int nv, size_t npts, size_t field,
+                        int closure, int order) {
   if (raw == nullptr && st->done) return;
   // pending MDIIS update (step 6 of the previous iteration): tau = sum_i c_i Z_i is formed here, on the way in,
   // and written back once, instead of by a separate pass that this kernel would then re-read
   __shared__ int s_ulist[MAX_M];
   __shared__ double s_ucoef[MAX_M];
   __shared__ int s_um;
+  __shared__ double s_bdyn;
   if (threadIdx.x == 0) {
     const int m = raw ? 0 : st->upd_m;
     s_um = m;
+    s_bdyn = st->b_dyn;
     for (int i = 0; i < m; ++i) { s_ulist[i] = st->upd_list[i]; s_ucoef[i] = st->upd_coef[i]; }
   }
   __syncthreads();
   const int um = s_um;
+  const double bdyn = s_bdyn;
   using Cfg = ZPlan<NZ>;
   constexpr int T = Cfg::T, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS, n = 2 * NZ;
   constexpr int NT = T * G * C, HP = NZ / 2, U = 2;
@@ -297,8 +255,15 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
 #pragma unroll 5
           for (int k = 0; k < um; ++k) {
             const double* Zk = Z + (size_t)s_ulist[k] * field + off[u];
-            const double2 z0 = __ldcs(reinterpret_cast<const double2*>(Zk));
-            const double2 z1 = __ldcs(reinterpret_cast<const double2*>(Zk + NZ));
+            double2 z0 = __ldcs(reinterpret_cast<const double2*>(Zk));
+            double2 z1 = __ldcs(reinterpret_cast<const double2*>(Zk + NZ));
+            if constexpr (DYN) {                       // X_i + b R_i with the current b, rounded as the oracle's expression
+              const double* Rk = Rh + (size_t)s_ulist[k] * field + off[u];
+              const double2 r0 = __ldcs(reinterpret_cast<const double2*>(Rk));
+              const double2 r1 = __ldcs(reinterpret_cast<const double2*>(Rk + NZ));
+              z0 = make_double2(__dadd_rn(z0.x, __dmul_rn(bdyn, r0.x)), __dadd_rn(z0.y, __dmul_rn(bdyn, r0.y)));
+              z1 = make_double2(__dadd_rn(z1.x, __dmul_rn(bdyn, r1.x)), __dadd_rn(z1.y, __dmul_rn(bdyn, r1.y)));
+            }
             const double ck = s_ucoef[k];
             a0.x = __dadd_rn(a0.x, __dmul_rn(ck, z0.x));
             a0.y = __dadd_rn(a0.y, __dmul_rn(ck, z0.y));
@@ -364,11 +329,11 @@ static int launch_closure_zfwd_n(const Grid& gr, const Buffers& b, const SolverP
   const size_t nlines = (size_t)gr.n * gr.n;
   const int threads = Cfg::T * G * COLS;
   const size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
-  auto kern = closure_zfwd_kernel<NZ, G, ZPlan<NZ>::MBF>;
+  auto kern = sp.dyn_b ? closure_zfwd_kernel<NZ, G, ZPlan<NZ>::MBF, true> : closure_zfwd_kernel<NZ, G, ZPlan<NZ>::MBF, false>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm) != cudaSuccess) return 0;
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
-  kern<<<(unsigned)(nlines / GL), threads, shm, s>>>(b.tau, b.w, raw, b.Z, b.work, tws, tw, b.state, gr.nv, gr.npts,
-                                                       gr.field, sp.closure, sp.pse_order);
+  kern<<<(unsigned)(nlines / GL), threads, shm, s>>>(b.tau, b.w, raw, b.Z, b.R, b.work, tws, tw, b.state, gr.nv,
+                                                       gr.npts, gr.field, sp.closure, sp.pse_order);
   return 1;
 }
 
@@ -398,6 +363,7 @@ struct GramArgs {
   double* part2;
   unsigned* tickets;
   const double* weight;  // [nv] weights 1/rho_g of the modified Anderson inner product (Eq. 38); unused otherwise
+  double n_values;       // grid points x site types of the caller: the N n_v of Eq. 41 (phantom types do not count)
   AccelArgs aa;
 };
 
@@ -536,7 +502,7 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
       *reinterpret_cast<double2*>(ga.part1 + ((size_t)j * gridDim.x + blockIdx.x) * 2) = make_double2(hi, lo);
       __threadfence();
     }
-    gram_finish<NT>(st, ga.part1, ga.part2, ga.tickets, s_m, nother, ga.aa, WEIGHTED, (double)field, s_row, &s_flag, s_solve);
+    gram_finish<NT>(st, ga.part1, ga.part2, ga.tickets, s_m, nother, ga.aa, WEIGHTED, ga.n_values, s_row, &s_flag, s_solve);
   }
 }
 
@@ -553,9 +519,11 @@ static int launch_zinv_nm(const Grid& gr, const Buffers& b, const SolverParams& 
   auto kern = zinv_residual_kernel<NZ, G, MB, MAXO, WEIGHTED>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm) != cudaSuccess) return 0;
   Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
-  GramArgs ga{b.gram_part, b.gram_part2, b.tickets, b.gram_w, AccelArgs{sp.M, sp.restart, sp.accel, sp.and_s1, sp.and_s2}};
+  GramArgs ga{b.gram_part, b.gram_part2, b.tickets, b.gram_w, (double)gr.npts * gr.nv_user,
+              AccelArgs{sp.M, sp.restart, sp.accel, sp.and_s1, sp.and_s2, sp.b_min, sp.dyn_b ? sp.b_max : 0.0}};
+  // (dynamic damping: the Z slot takes X itself -- X + 0 R is exact -- and the update applies the current b)
   kern<<<(unsigned)((size_t)gr.n * gr.n / GL), threads, shm, s>>>(b.work, b.tau, b.Z, b.R, raw_out, tws, tw, b.state,
-                                                                   gr.nv, gr.npts, gr.field, sp.b, ga);
+                                                                   gr.nv, gr.npts, gr.field, sp.dyn_b ? 0.0 : sp.b, ga);
   return 1;
 }
 

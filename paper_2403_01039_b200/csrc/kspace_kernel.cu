@@ -27,11 +27,7 @@ struct KspaceCfg {
          STAGE = ITEM + PHI,
          MIDT = (FftCfg<N>::R3 == 1) ? 0 : (N / FftCfg<N>::R1 / FftCfg<N>::R2) * FftCfg<N>::R2,   // mid-pass twiddle table
          SHM = (2 * STAGE + MIDT) * (int)sizeof(cplx),
-#ifdef R3D_KSPACE_MINB
-         MINB = R3D_KSPACE_MINB };
-#else
          MINB = (SHM > 110 * 1024) ? 1 : ((SHM > 72 * 1024) ? 2 : 3) };
-#endif
 };
 
 // Eq. 32 + Eq. 13 + Eq. 33 (in k space) for ONE k point, the NV sites of which sit in NV adjacent lanes:
@@ -180,11 +176,9 @@ __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
 // their load, arithmetic and store phases with each other.
 // ------------------------------------------------------------------------------------------------
 template <int N> struct KPlan2 { enum { OK = 0, R1 = 1, R2 = 1 }; };
-#ifndef R3D_K2_OFF
 template <> struct KPlan2<64>  { enum { OK = 1, R1 = 8,  R2 = 8 }; };
 template <> struct KPlan2<128> { enum { OK = 1, R1 = 16, R2 = 8 }; };
 template <> struct KPlan2<256> { enum { OK = 1, R1 = 16, R2 = 16 }; };
-#endif
 
 template <int N, int NV>
 struct Kspace2Cfg {
@@ -193,11 +187,7 @@ struct Kspace2Cfg {
          TILE_BYTES = ITEM * (int)sizeof(cplx), PHI_BYTES = PHI * (int)sizeof(cplx),
          STAGE = ITEM + PHI,                                // complex elements of one pipeline stage: tile, then phi~
          SHM = 2 * (TILE_BYTES + PHI_BYTES) + 64,           // two stages and their mbarriers
-#ifdef R3D_K2_MINB
-         MINB = R3D_K2_MINB };
-#else
          MINB = (227 * 1024 / (SHM + 1024) < 8) ? 227 * 1024 / (SHM + 1024) : 8 };
-#endif
 };
 
 // a[k] = a0 * s^k, k < R (R a power of two): s^2, s^4, ... by squaring, then a[k + h] = a[k] * s^h -- log2(R) dependent
@@ -261,10 +251,7 @@ __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB
   constexpr int S1 = N / R1, NB = N / R2;            // S1 == T: one pass-A butterfly per thread
   constexpr int NZ = N / 2, PC = C / NV;
   constexpr int Q = NZ * NV;                         // complex elements per (jx, jy) row
-#ifndef R3D_K2_PF
-#define R3D_K2_PF 8
-#endif
-  constexpr int PF = (R2 < R3D_K2_PF) ? R2 : R3D_K2_PF;   // chi rows in flight per thread
+  constexpr int PF = (R2 < 8) ? R2 : 8;              // chi rows in flight per thread
   const int tid = threadIdx.x;
   const int col = tid % C, t = tid / C;
   const int site = col % NV;

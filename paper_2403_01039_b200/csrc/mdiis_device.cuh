@@ -17,6 +17,7 @@ struct AccelArgs {
   double restart;        // MDIIS restart factor (<= 0: never)
   int accel;             // rism3d_accelerator
   double s1, s2;         // tuning parameters of Eq. 34-35
+  double b_min, b_max;   // b_max > 0: dynamic damping b = clamp(-0.2 log10 rms, b_min, b_max) (Q18)
 };
 
 // shared-memory scratch of the final step (one per CTA; only the last-arriving CTA uses it)
@@ -54,6 +55,7 @@ static __device__ __noinline__ void mdiis_bookkeeping_and_solve(DevState* __rest
     st->rms_hist[st->hist_n % RMS_HIST_CAP] = rms;
     st->hist_n += 1;
     st->upd_m = 0;
+    if (aa.b_max > 0.0) st->b_dyn = fmin(aa.b_max, fmax(aa.b_min, -0.2 * log10(rms)));
     if (!isfinite(rms)) { st->done = 1; st->status = RISM3D_ERR_DIVERGED; ss.go = 0; }
     else if (st->tol > 0.0 && rms < st->tol) { st->done = 1; ss.go = 0; }   // converged: tau stays as it is
     if (ss.go) {
@@ -183,21 +185,6 @@ static __device__ __noinline__ void mdiis_bookkeeping_and_solve(DevState* __rest
     st->list[lane] = ss.list[lane];
     st->rms[lane] = ss.rms[lane];
     if (lane < m) { st->upd_list[lane] = ss.list[lane]; st->upd_coef[lane] = ss.c[lane]; }
-  }
-}
-
-// Sum of `count` double-double partials part[0..count) by ONE warp, in a fixed order: lane l adds l, l + 32, ...,
-// then the shuffle tree.  Result (hi, lo) in lane 0.
-static __device__ __forceinline__ void warp_sum_partials(const double* part, int count, int lane, double& hi, double& lo) {
-  hi = 0.0;
-  lo = 0.0;
-  for (int i = lane; i < count; i += 32) {
-    const double2 p = __ldcg(reinterpret_cast<const double2*>(part) + i);
-    dd_add(hi, lo, p.x, p.y);
-  }
-  for (int o = 16; o > 0; o >>= 1) {
-    const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
-    dd_add(hi, lo, h2, l2);
   }
 }
 

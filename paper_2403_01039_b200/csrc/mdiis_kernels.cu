@@ -15,9 +15,10 @@ namespace r3d {
 
 // tau = sum_i c_i Z_i over the stored entries, Z_i = X_i + b R_i (Eq. 40 as read in Q7); products and sums are
 // rounded one by one, in the order of the oracle's loop.
+template <bool DYN>
 __global__ void __launch_bounds__(256)
-    mdiis_update_kernel(const DevState* __restrict__ st, const double* __restrict__ Z, double* __restrict__ tau,
-                        size_t field) {
+    mdiis_update_kernel(const DevState* __restrict__ st, const double* __restrict__ Z, const double* __restrict__ Rh,
+                        double* __restrict__ tau, size_t field) {
   if (st->done) return;
   __shared__ int s_list[MAX_M];
   __shared__ double s_c[MAX_M];
@@ -29,13 +30,18 @@ __global__ void __launch_bounds__(256)
   __syncthreads();
   const int m = s_m;
   if (m == 0) return;
+  const double bdyn = st->b_dyn;
   double2* dst = reinterpret_cast<double2*>(tau);
   const size_t n2 = field / 2;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += (size_t)gridDim.x * blockDim.x) {
     double2 acc = make_double2(0.0, 0.0);
 #pragma unroll 4
     for (int k = 0; k < m; ++k) {
-      const double2 zv = __ldcs(reinterpret_cast<const double2*>(Z + (size_t)s_list[k] * field) + i);
+      double2 zv = __ldcs(reinterpret_cast<const double2*>(Z + (size_t)s_list[k] * field) + i);
+      if constexpr (DYN) {                             // X_i + b R_i with the current b (dynamic damping)
+        const double2 rv = __ldcs(reinterpret_cast<const double2*>(Rh + (size_t)s_list[k] * field) + i);
+        zv = make_double2(__dadd_rn(zv.x, __dmul_rn(bdyn, rv.x)), __dadd_rn(zv.y, __dmul_rn(bdyn, rv.y)));
+      }
       const double ck = s_c[k];
       acc.x = __dadd_rn(acc.x, __dmul_rn(ck, zv.x));
       acc.y = __dadd_rn(acc.y, __dmul_rn(ck, zv.y));
@@ -51,7 +57,8 @@ int launch_mdiis_update(const Grid& g, const Buffers& b, const SolverParams& sp,
   size_t blocks = (n2 + 255) / 256;
   const size_t cap = 148 * 8 * 4;
   if (blocks > cap) blocks = cap;
-  mdiis_update_kernel<<<(unsigned)blocks, 256, 0, s>>>(b.state, b.Z, b.tau, g.field);
+  if (sp.dyn_b) mdiis_update_kernel<true><<<(unsigned)blocks, 256, 0, s>>>(b.state, b.Z, b.R, b.tau, g.field);
+  else mdiis_update_kernel<false><<<(unsigned)blocks, 256, 0, s>>>(b.state, b.Z, b.R, b.tau, g.field);
   clear_pending_update_kernel<<<1, 1, 0, s>>>(b.state);
   return 2;
 }

@@ -31,7 +31,8 @@ struct DevState {
   unsigned ticket;             // first-level group adders of the Gram reduction that have finished
   double tol;
   double rms_last;
-  double pad_[2];
+  double b_dyn;                // damping of the pending update when it follows the residual (SolverParams.dyn_b)
+  double pad_[1];
   // ---- MDIIS bookkeeping ----
   int list[MAX_M];             // physical slot of each entry, oldest first
   int upd_list[MAX_M];
@@ -42,12 +43,14 @@ struct DevState {
 };
 struct StateHeader {           // mirrors the first 64 bytes of DevState
   int done, status, n_done, hist_n, m, cur, upd_m; unsigned ticket;
-  double tol, rms_last, pad_[2];
+  double tol, rms_last, b_dyn, pad_[1];
 };
 
 struct Grid {
   int n;                 // points per axis (cubic)
-  int nv;                // site types
+  int nv;                // site types as the kernels see them: nv_user rounded up to a power of two (1, 2, 4, 8); the
+                         // extra "phantom" types have zero charge, LJ, density and chi, stay exactly 0 and cost bandwidth only
+  int nv_user;           // site types of the caller (rism3d_params.n_sites)
   double h;              // spacing
   double origin[3];
   size_t npts;           // n^3
@@ -89,6 +92,8 @@ struct SolverParams {
   double b;
   double restart;
   double beta, kT, kappa, r_min;
+  bool dyn_b;            // damping follows the residual, b = clamp(-0.2 log10 rms, b_min, b_max); the history then holds X_i
+  double b_min, b_max;   //   in the Z slots (stored with b = 0) and the update forms X_i + b R_i from both fields
   int accel;             // rism3d_accelerator (ANDERSON: M = 3 stored pairs = the newest + two histories)
   double and_s1, and_s2; // tuning parameters of Eq. 34-35
 };
@@ -147,6 +152,22 @@ __device__ __forceinline__ void dd_norm(double& hi, double& lo) {
   const double s = hi + lo;
   lo = lo - (s - hi);
   hi = s;
+}
+
+// Sum of `count` double-double partials part[i * stride], i < count, by ONE warp, in a fixed order: lane l adds l, l + 32, ...,
+// then the shuffle tree.  Result (hi, lo) in lane 0.
+__device__ __forceinline__ void warp_sum_partials(const double* part, int count, int lane, double& hi, double& lo,
+                                                  int stride = 1) {
+  hi = 0.0;
+  lo = 0.0;
+  for (int i = lane; i < count; i += 32) {
+    const double2 p = __ldcg(reinterpret_cast<const double2*>(part) + (size_t)i * stride);
+    dd_add(hi, lo, p.x, p.y);
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
+    dd_add(hi, lo, h2, l2);
+  }
 }
 
 // closure g(d) (Q1, Q2): HNC exp(d); KH/PSE-n: exp(d) for d <= 0, sum_{i<=n} d^i/i! for d > 0

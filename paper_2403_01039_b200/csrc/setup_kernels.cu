@@ -474,26 +474,25 @@ __global__ void __launch_bounds__(256)
   }
 }
 
-__global__ void free_energy_final_kernel(double* __restrict__ out, const double* __restrict__ part, int nblocks,
-                                         const double* __restrict__ rhov, int nv, double scale, double dv) {
-  const int g = threadIdx.x;
+// one warp per site type and sum: the per-CTA double-double partials are added in a fixed order (lane l takes l, l + 32,
+// ..., then the shuffle tree).  blockDim = 32 * 2 * MAX_NV; warp = g (free-energy integrand) or MAX_NV + g (c_sr alone).
+__global__ void __launch_bounds__(64 * MAX_NV)
+    free_energy_final_kernel(double* __restrict__ out, const double* __restrict__ part, int nblocks,
+                             const double* __restrict__ rhov, int nv, double scale, double dv) {
+  const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int g = wid % MAX_NV, second = wid / MAX_NV;
   if (g >= nv) return;
-  double hi = 0.0, lo = 0.0;
-  for (int b = 0; b < nblocks; ++b) dd_add(hi, lo, part[((size_t)b * MAX_NV + g) * 2], part[((size_t)b * MAX_NV + g) * 2 + 1]);
-  out[g] = scale * rhov[g] * (hi + lo);
-  // second set: dV sum_r c_sr,g(r)  (A^3), not density weighted
-  hi = 0.0; lo = 0.0;
-  for (int b = 0; b < nblocks; ++b)
-    dd_add(hi, lo, part[((size_t)(nblocks + b) * MAX_NV + g) * 2], part[((size_t)(nblocks + b) * MAX_NV + g) * 2 + 1]);
-  out[MAX_NV + g] = dv * (hi + lo);
+  double hi, lo;
+  warp_sum_partials(part + ((size_t)second * nblocks * MAX_NV + g) * 2, nblocks, lane, hi, lo, MAX_NV);
+  if (lane == 0) out[second * MAX_NV + g] = second ? dv * (hi + lo) : scale * rhov[g] * (hi + lo);
 }
 
 int launch_free_energy(const Grid& g, const Buffers& b, const SolverParams& sp, double* d_out, cudaStream_t s) {
   const int blocks = FE_BLOCKS;
   free_energy_kernel<<<blocks, 256, 0, s>>>(b.fe_part, b.tau, b.w, b.phi, b.qv, b.state, g.nv, g.npts, g.field,
                                             sp.closure, sp.pse_order);
-  free_energy_final_kernel<<<1, 32, 0, s>>>(d_out, b.fe_part, blocks, b.rhov, g.nv, sp.kT * g.h * g.h * g.h,
-                                            g.h * g.h * g.h);
+  free_energy_final_kernel<<<1, 64 * MAX_NV, 0, s>>>(d_out, b.fe_part, blocks, b.rhov, g.nv, sp.kT * g.h * g.h * g.h,
+                                                     g.h * g.h * g.h);
   return 2;
 }
 
@@ -629,16 +628,15 @@ __global__ void __launch_bounds__(GRAD_THREADS)
   }
 }
 
-__global__ void gradient_final_kernel(double* __restrict__ out, const double* __restrict__ partial, int nchunks,
-                                      int n_atoms, double kT) {
-  const int e = blockIdx.x * blockDim.x + threadIdx.x;    // atom * 3 + component
+// one warp per (atom, component): the chunk partials are added in a fixed order (warp_sum_partials)
+__global__ void __launch_bounds__(256)
+    gradient_final_kernel(double* __restrict__ out, const double* __restrict__ partial, int nchunks, int n_atoms,
+                          double kT) {
+  const int e = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);    // atom * 3 + component
   if (e >= n_atoms * 3) return;
-  double hi = 0.0, lo = 0.0;
-  for (int c = 0; c < nchunks; ++c) {
-    const double* p = partial + ((size_t)c * n_atoms * 3 + e) * 2;
-    dd_add(hi, lo, p[0], p[1]);
-  }
-  out[e] = kT * (hi + lo);
+  double hi, lo;
+  warp_sum_partials(partial + (size_t)e * 2, nchunks, threadIdx.x & 31, hi, lo, n_atoms * 3);
+  if ((threadIdx.x & 31) == 0) out[e] = kT * (hi + lo);
 }
 
 // d_gw: one field-set of scratch; d_atoms: [n_atoms] double4 (x, y, z, unused); d_pair as in launch_potential;
@@ -663,7 +661,7 @@ int launch_gradient(const Grid& g, const Buffers& b, const SolverParams& sp, int
     default: return 0;
   }
 #undef GRD
-  gradient_final_kernel<<<(n_atoms * 3 + 127) / 128, 128, 0, s>>>(d_out, d_partial, nchunks, n_atoms, sp.kT);
+  gradient_final_kernel<<<(n_atoms * 3 + 7) / 8, 256, 0, s>>>(d_out, d_partial, nchunks, n_atoms, sp.kT);
   return 3;
 }
 

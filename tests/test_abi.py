@@ -70,9 +70,15 @@ def test_workspace_bytes_and_argument_checks_without_a_device(lib):
     p.nx = 48                                         # not a power of two
     assert handle.rism3d_workspace_bytes(C.byref(p)) == 0
     p.nx = 64
-    p.n_sites = 3
+    p.n_sites = 3                                     # runs padded to 4 site types
+    four = 64 ** 3 * 4 * 8
+    assert (2 * 5 + 3) * four <= handle.rism3d_workspace_bytes(C.byref(p)) <= (2 * 5 + 3 + 1) * four + (8 << 20)
+    p.n_sites = 9
     assert handle.rism3d_workspace_bytes(C.byref(p)) == 0
     p.n_sites = 2
+    p.r_min = 0.0                                     # a zero-initialised clamp is refused
+    assert handle.rism3d_workspace_bytes(C.byref(p)) == 0
+    p.r_min = 1e-3
     p.mdiis_nvec = 17
     assert handle.rism3d_workspace_bytes(C.byref(p)) == 0
     # NULL context: every entry point answers with an error code instead of crashing

@@ -33,8 +33,9 @@ def _small_solute(seed=1, n=3, charged=True):
     return Solute("edge", xyz, q, rng.uniform(2.6, 3.4, n), rng.uniform(0.05, 0.2, n))
 
 
-@pytest.mark.parametrize("n_v,n", [(1, 16), (8, 16), (2, 8), (4, 8)])
+@pytest.mark.parametrize("n_v,n", [(1, 16), (8, 16), (2, 8), (4, 8), (3, 16), (5, 16), (6, 8), (7, 16)])
 def test_site_counts_and_smallest_grids(n_v, n):
+    """every site count 1..8 (3, 5, 6, 7 run padded with phantom types inside the library) on the smallest grids"""
     sv = _solvent(n_v, seed=n_v)
     chi = synthetic_chi(n_v, sv.rho, n_k=900, dk=0.02, k0=0.02, seed=n_v, amp=0.5)
     orc, gpu, _, _ = make_pair(n=n, spacing=0.9, solvent=sv, chi=chi, solute=_small_solute(), M=4)
@@ -42,9 +43,30 @@ def test_site_counts_and_smallest_grids(n_v, n):
     nd, rms = gpu.iterate(20, 0.0)
     assert nd == 20 and abs(rms - orc.rms_history[-1]) <= 1e-9 * orc.rms_history[-1] + 1e-13
     assert np.max(np.abs(gpu.get_field("G") - orc.get_field("G"))) <= 1e-9
-    mu_o, _ = orc.free_energy()
-    mu_g, _ = gpu.free_energy()
+    mu_o, site_o = orc.free_energy()
+    mu_g, site_g = gpu.free_energy()
     assert abs(mu_g - mu_o) <= 1e-9 * max(1.0, abs(mu_o))
+    assert site_g.shape == (n_v,) and np.allclose(site_g, site_o, rtol=1e-8, atol=1e-9 * max(1.0, abs(mu_o)))
+    assert gpu.get_field("TAU").shape == (n_v, n, n, n)
+
+
+def test_three_site_solvent_modified_anderson_and_fft_hooks():
+    """n_v = 3 (padded to 4): the 1/rho-weighted inner product of the modified Anderson method must ignore the phantom
+    type, the rms must be normalised with the caller's site count, and the debug transform hooks pad and unpad."""
+    import torch
+    from tests._gpu_util import oracle_spectrum_in_gpu_layout
+    sv = _solvent(3, seed=3)
+    chi = synthetic_chi(3, sv.rho, n_k=900, dk=0.02, k0=0.02, seed=3, amp=0.5)
+    orc, gpu, _, _ = make_pair(n=16, spacing=0.9, solvent=sv, chi=chi, solute=_small_solute(), b=0.5, accelerator="ANDERSON")
+    orc.iterate(25, 0.0)
+    gpu.iterate(25, 0.0)
+    np.testing.assert_allclose(gpu.rms_history(), orc.rms_history, rtol=1e-7, atol=1e-14)
+    assert np.max(np.abs(gpu.get_field("G") - orc.get_field("G"))) <= 1e-9
+    f = np.random.default_rng(5).standard_normal((3, 16, 16, 16))
+    spec = gpu.fft_forward(torch.from_numpy(f).cuda())
+    ref = oracle_spectrum_in_gpu_layout(f, 0.9)
+    assert spec.shape == ref.shape and np.max(np.abs(spec.cpu().numpy() - ref)) < 1e-12 * np.max(np.abs(ref))
+    assert np.max(np.abs(gpu.fft_inverse(spec).cpu().numpy() - f)) < 1e-12
 
 
 @pytest.mark.parametrize("closure,order", [("HNC", 1), ("PSE", 3), ("PSE", 7)])
@@ -253,3 +275,21 @@ def test_pressure_correction_matches_oracle(cfg, n):
     assert abs(v_g - v_o) <= 1e-7 * abs(v_o)
     assert abs(pc_g - pc_o) <= 1e-7 * abs(pc_o)
     assert pc_g == -pressure * v_g
+
+
+# ---- NEXT-4: dynamic damping b = -0.2 log10(rms) (Q18) -----------------------------------
+@pytest.mark.parametrize("cfg,n,M", [("C1", 32, 5), ("C2", 32, 5), ("C2", 32, 10)])
+def test_dynamic_damping_fifty_iterations(cfg, n, M):
+    sol = make_solute(cfg)
+    orc, gpu, _, _ = make_pair(n=n, spacing=0.5, solvent="water", solute=sol, M=M, mdiis_dynamic_b=(0.1, 1.0))
+    orc.iterate(50, 0.0)
+    nd, rms = gpu.iterate(50, 0.0)
+    assert nd == 50
+    np.testing.assert_allclose(gpu.rms_history(), orc.rms_history, rtol=1e-6, atol=1e-13)
+    assert np.max(np.abs(gpu.get_field("G") - orc.get_field("G"))) <= 1e-9
+    # split calls: the trailing update pass applies the same dynamic b
+    _, twin, _, _ = make_pair(n=n, spacing=0.5, solvent="water", solute=sol, M=M, mdiis_dynamic_b=(0.1, 1.0))
+    for k in (7, 1, 30, 12):
+        twin.iterate(k, 0.0)
+    assert np.array_equal(twin.rms_history(), gpu.rms_history())
+    assert np.array_equal(twin.get_field("TAU"), gpu.get_field("TAU"))

@@ -199,3 +199,13 @@ def test_error_paths():
     assert e.value.status == -5                       # neutrality
     with pytest.raises(lib.Rism3dError):
         lib.Solver(24, 0.5, 2)                        # not a power of two
+    with pytest.raises(lib.Rism3dError):
+        lib.Solver(16, 0.5, 9)                        # more than 8 site types
+    with pytest.raises(lib.Rism3dError):
+        lib.Solver(16, 0.5, 2, r_min=0.0)             # a zero clamp would put 1/0 into w (Q11)
+    with pytest.raises(lib.Rism3dError):
+        lib.Solver(16, 0.5, 2, mdiis_b=0.0)
+    with pytest.raises(ValueError):
+        s.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho[:1], k0, dk, chi)      # array lengths are checked before the C call
+    with pytest.raises(ValueError):
+        s.set_solute(np.zeros((2, 3)), [1.0], [2.0], [0.1])
