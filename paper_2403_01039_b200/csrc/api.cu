@@ -247,9 +247,10 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
   if (kspace_uses_tma(g.n)) {
     // k-space pass tiles: n rows (jx) of 8 complex = 16 doubles of `work`, and the matching 8 / nv phi~ values per row
     const uint64_t q2 = (uint64_t)(g.n / 2) * g.nv * 2, h2 = (uint64_t)(g.n / 2) * 2;     // doubles per (jx, jy) row
-    if (!make_tensor_map_2d(&ctx->b.tm_work, ctx->b.work, (uint64_t)g.n * q2, (uint64_t)g.n, (uint64_t)g.n * q2 * 8, 16, (uint32_t)g.n) ||
+    const uint32_t box_rows = (uint32_t)(g.n < 256 ? g.n : 256);                          // TMA box limit; 512 = two boxes
+    if (!make_tensor_map_2d(&ctx->b.tm_work, ctx->b.work, (uint64_t)g.n * q2, (uint64_t)g.n, (uint64_t)g.n * q2 * 8, 16, box_rows) ||
         !make_tensor_map_2d(&ctx->b.tm_phik, ctx->b.phik, (uint64_t)g.n * h2, (uint64_t)g.n, (uint64_t)g.n * h2 * 8,
-                            (uint32_t)(2 * 8 / g.nv), (uint32_t)g.n)) {
+                            (uint32_t)(2 * 8 / g.nv), box_rows)) {
       delete ctx;
       return RISM3D_ERR_CUDA;
     }

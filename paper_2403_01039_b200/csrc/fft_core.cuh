@@ -1,4 +1,4 @@
-// fft_core.cuh -- fp64 complex FFT building blocks for sm_100a: in-register radix-2/4/8/16 DFTs and
+// fft_core.cuh -- fp64 complex FFT building blocks for sm_100a: in-register radix-2/4/8/16/32 DFTs and
 // the multi-pass Stockham-free (in-place, digit-indexed) line transforms that the 3D passes share.
 //
 // The transform is the SHIFTED DFT of the paper's half-integer k grid:
@@ -75,11 +75,35 @@ __device__ __forceinline__ cplx mul_w32c(cplx v) {
     return make_double2(v.x * c - v.y * s, v.x * s + v.y * c);
   }
 }
+// cos(pi k / 32), k = 0..32
+__host__ __device__ constexpr double cos_pi32(int k) {
+  switch (k) {
+    case 1: return 0.99518472667219688624;
+    case 3: return 0.95694033573220886494;
+    case 5: return 0.88192126434835502971;
+    case 7: return 0.77301045336273696081;
+    case 9: return 0.63439328416364549822;
+    case 11: return 0.47139673682599764856;
+    case 13: return 0.29028467725446236764;
+    case 15: return 0.09801714032956060199;
+    default: return (k & 1) ? -cos_pi32(32 - k) : cos_pi16(k / 2);
+  }
+}
+__host__ __device__ constexpr double sin_pi32(int k) { return k <= 16 ? cos_pi32(16 - k) : cos_pi32(k - 16); }   // k = 0..32
+// v * exp(DIR i pi IDX / 32), IDX in [0, 32)
+template <int IDX, int DIR>
+__device__ __forceinline__ cplx mul_w64c(cplx v) {
+  if constexpr (IDX % 2 == 0) return mul_w32c<IDX / 2, DIR>(v);
+  else {
+    constexpr double c = cos_pi32(IDX), s = (double)DIR * sin_pi32(IDX);
+    return make_double2(v.x * c - v.y * s, v.x * s + v.y * c);
+  }
+}
 template <int R, int DIR, int M1 = 1>
-struct HalfShiftAll {       // x[m1] *= exp(DIR i pi m1 / R) for m1 = 1..R-1, R in {2, 4, 8, 16}
+struct HalfShiftAll {       // x[m1] *= exp(DIR i pi m1 / R) for m1 = 1..R-1, R in {2, 4, 8, 16, 32}
   static __device__ __forceinline__ void run(cplx (&x)[R]) {
     if constexpr (M1 < R) {
-      x[M1] = mul_w32c<M1 * (16 / R), DIR>(x[M1]);
+      x[M1] = mul_w64c<M1 * (32 / R), DIR>(x[M1]);
       HalfShiftAll<R, DIR, M1 + 1>::run(x);
     }
   }
@@ -105,6 +129,29 @@ struct Dft {
 template <int DIR>
 struct Dft<1, DIR> {
   static __device__ __forceinline__ void run(cplx (&)[1]) {}
+};
+// radix 32 (the 512-point k-space lines): two radix-16 halves and the 16 twiddles exp(DIR i pi k / 16) as immediates
+template <int DIR, int K = 0>
+struct Dft32Combine {
+  static __device__ __forceinline__ void run(cplx (&x)[32], const cplx (&e)[16], const cplx (&o)[16]) {
+    if constexpr (K < 16) {
+      const cplx t = mul_w32c<K, DIR>(o[K]);
+      x[K] = cadd(e[K], t);
+      x[K + 16] = csub(e[K], t);
+      Dft32Combine<DIR, K + 1>::run(x, e, o);
+    }
+  }
+};
+template <int DIR>
+struct Dft<32, DIR> {
+  static __device__ __forceinline__ void run(cplx (&x)[32]) {
+    cplx e[16], o[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) { e[k] = x[2 * k]; o[k] = x[2 * k + 1]; }
+    Dft<16, DIR>::run(e);
+    Dft<16, DIR>::run(o);
+    Dft32Combine<DIR>::run(x, e, o);
+  }
 };
 
 // Twiddle table of one grid axis: tab[j] = exp(-i pi j / n), j = 0 .. 2n-1 (device memory, built by the host

@@ -167,7 +167,8 @@ __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
 }
 
 // ------------------------------------------------------------------------------------------------
-// Two-pass variant for the line lengths that factor into two radices <= 16 (64 = 8 x 8, 128 = 16 x 8, 256 = 16 x 16):
+// Two-pass variant for the line lengths that factor into two radices <= 32 (64 = 8 x 8, 128 = 16 x 8, 256 = 16 x 16,
+// 512 = 32 x 16):
 // half the shared-memory passes of the three-pass plan (3 loads + 2 stores of the tile per work item instead of 5 + 5),
 // which is what bounds this kernel (L1 / shared data pipe).  T = N / R1 threads per column, one
 // radix-R1 butterfly each in the outer passes; the pass-A twiddles exp(-2 pi i (k1 + 1/2) t / N), k1 = 0..R1-1, are a
@@ -175,19 +176,26 @@ __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
 // One tile (N x 8 complex = 128-byte rows) per CTA at a time, single-buffered: several small CTAs per SM overlap
 // their load, arithmetic and store phases with each other.
 // ------------------------------------------------------------------------------------------------
-template <int N> struct KPlan2 { enum { OK = 0, R1 = 1, R2 = 1 }; };
-template <> struct KPlan2<64>  { enum { OK = 1, R1 = 8,  R2 = 8 }; };
-template <> struct KPlan2<128> { enum { OK = 1, R1 = 16, R2 = 8 }; };
-template <> struct KPlan2<256> { enum { OK = 1, R1 = 16, R2 = 16 }; };
+template <int N> struct KPlan2 { enum { OK = 0, R1 = 1, R2 = 1, STAGES = 2 }; };
+template <> struct KPlan2<64>  { enum { OK = 1, R1 = 8,  R2 = 8,  STAGES = 2 }; };
+template <> struct KPlan2<128> { enum { OK = 1, R1 = 16, R2 = 8,  STAGES = 2 }; };
+template <> struct KPlan2<256> { enum { OK = 1, R1 = 16, R2 = 16, STAGES = 2 }; };
+// 512 = 32 x 16: the 64 KB tile is single-buffered so that two CTAs fit on an SM and overlap each other's load,
+// arithmetic and store phases
+template <> struct KPlan2<512> { enum { OK = 1, R1 = 32, R2 = 16, STAGES = 1 }; };
+
+constexpr int TMA_BOX_ROWS = 256;                           // a TMA box holds at most 256 elements per dimension
 
 template <int N, int NV>
 struct Kspace2Cfg {
-  enum { R1 = KPlan2<N>::R1, R2 = KPlan2<N>::R2, T = N / R1, NT = T * COLS,
+  enum { R1 = KPlan2<N>::R1, R2 = KPlan2<N>::R2, STAGES = KPlan2<N>::STAGES, T = N / R1, NT = T * COLS,
          ITEM = N * COLS, PHI = N * (COLS / NV),
          TILE_BYTES = ITEM * (int)sizeof(cplx), PHI_BYTES = PHI * (int)sizeof(cplx),
          STAGE = ITEM + PHI,                                // complex elements of one pipeline stage: tile, then phi~
-         SHM = 2 * (TILE_BYTES + PHI_BYTES) + 64,           // two stages and their mbarriers
-         MINB = (227 * 1024 / (SHM + 1024) < 8) ? 227 * 1024 / (SHM + 1024) : 8 };
+         SHM = STAGES * (TILE_BYTES + PHI_BYTES) + 64,      // the stages and their mbarriers
+         BOX_ROWS = N < TMA_BOX_ROWS ? N : TMA_BOX_ROWS, NBOX = N / BOX_ROWS,
+         FIT = 227 * 1024 / (SHM + 1024), CAP = (N >= 256) ? 2 : 8,   // long lines want all 255 registers
+         MINB = FIT < CAP ? FIT : CAP };
 };
 
 // a[k] = a0 * s^k, k < R (R a power of two): s^2, s^4, ... by squaring, then a[k + h] = a[k] * s^h -- log2(R) dependent
@@ -203,6 +211,28 @@ __device__ __forceinline__ void twiddle_powers(cplx (&a)[R], cplx a0, cplx s) {
     if (2 * h < R) sh = cmul(sh, sh);
   }
 }
+// The pass-A twiddles of one thread, a0 * s^k1 for k1 < R1.  Up to R1 = 16 all of them live in registers; for R1 = 32
+// (beside 32 complex data values) only s^0..s^7 and the four chunk bases a0 s^(8c) do, and get() forms the product.
+template <int R1>
+struct PassATw {
+  static constexpr int CH = (R1 > 16) ? 8 : R1, NCH = R1 / CH;
+  cplx p[CH];      // NCH == 1: a0 s^k ;  else s^k, k < CH
+  cplx base[NCH];  // a0 s^(CH c) (unused when NCH == 1)
+  __device__ __forceinline__ PassATw(cplx a0, cplx s) {
+    if constexpr (NCH == 1) {
+      twiddle_powers<CH>(p, a0, s);
+      base[0] = a0;
+    } else {
+      twiddle_powers<CH>(p, make_double2(1.0, 0.0), s);
+      const cplx sc = cmul(p[CH - 1], s);                    // s^CH
+      twiddle_powers<NCH>(base, a0, sc);
+    }
+  }
+  __device__ __forceinline__ cplx get(int k1) const {        // k1 folds at compile time in unrolled loops
+    if constexpr (NCH == 1) return p[k1];
+    else return (k1 % CH == 0) ? base[k1 / CH] : cmul(base[k1 / CH], p[k1 % CH]);
+  }
+};
 
 // chi row of one k point for this lane's site (kspace_point consumes it)
 template <int NV>
@@ -251,37 +281,50 @@ __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB
   constexpr int S1 = N / R1, NB = N / R2;            // S1 == T: one pass-A butterfly per thread
   constexpr int NZ = N / 2, PC = C / NV;
   constexpr int Q = NZ * NV;                         // complex elements per (jx, jy) row
-  constexpr int PF = (R2 < 8) ? R2 : 8;              // chi rows in flight per thread
+  constexpr int PFMAX = (NV > 4) ? 4 : 8;            // chi rows in flight per thread (a row is NV doubles)
+  constexpr int PF = (R2 < PFMAX) ? R2 : PFMAX;
   const int tid = threadIdx.x;
   const int col = tid % C, t = tid / C;
   const int site = col % NV;
   const double qg = qv[site];
   const cplx a0 = tw(t), astep = tw(2 * t);          // exp(-i pi t / N) and its square: a[k1] = a0 * astep^k1
-  cplx* stages = smem_dyn;                           // [2] x ([N][8] tile, [N][8 / NV] phi~)
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_dyn + 2 * K::STAGE);   // one per stage
+  constexpr int STAGES = K::STAGES;
+  cplx* stages = smem_dyn;                           // [STAGES] x ([N][8] tile, [N][8 / NV] phi~)
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_dyn + STAGES * K::STAGE);   // one per stage
   const double scale = 1.0 / (double)N;
-  // both boxes of work item `it` into stage b; TMA coordinates: innermost = doubles along the flattened (jy, p[, site])
+  // the boxes of work item `it` into stage b; TMA coordinates: innermost = doubles along the flattened (jy, p[, site])
   auto issue = [&](unsigned it, int b) {
     const unsigned q0 = it * C;
     mbar_arrive_expect_tx(&bars[b], K::TILE_BYTES + K::PHI_BYTES);
-    tma_load_2d(stages + b * K::STAGE, &tm_work, (int)(q0 * 2), 0, &bars[b]);
-    tma_load_2d(stages + b * K::STAGE + K::ITEM, &tm_phik, (int)((q0 / Q * NZ + (q0 % Q) / NV) * 2), 0, &bars[b]);
+#pragma unroll
+    for (int bx = 0; bx < K::NBOX; ++bx) {
+      tma_load_2d(stages + b * K::STAGE + bx * K::BOX_ROWS * C, &tm_work, (int)(q0 * 2), bx * K::BOX_ROWS, &bars[b]);
+      tma_load_2d(stages + b * K::STAGE + K::ITEM + bx * K::BOX_ROWS * PC, &tm_phik,
+                  (int)((q0 / Q * NZ + (q0 % Q) / NV) * 2), bx * K::BOX_ROWS, &bars[b]);
+    }
   };
   if (tid == 0) {
-    mbar_init(&bars[0], 1);
-    mbar_init(&bars[1], 1);
+#pragma unroll
+    for (int b = 0; b < STAGES; ++b) mbar_init(&bars[b], 1);
     mbar_fence_init();
   }
   __syncthreads();
   unsigned item = blockIdx.x;
-  if (tid == 0 && item < nitems) issue(item, 0);
+  if (STAGES == 2 && tid == 0 && item < nitems) issue(item, 0);
   unsigned n_done = 0;
   for (; item < nitems; item += gridDim.x, ++n_done) {
-    const int b = n_done & 1;
-    const unsigned next = item + gridDim.x;
-    if (tid == 0 && next < nitems) {
-      tma_wait_read();                               // the store of the previous item has left stage b ^ 1
-      issue(next, b ^ 1);
+    const int b = (STAGES == 2) ? (int)(n_done & 1) : 0;
+    if constexpr (STAGES == 2) {
+      const unsigned next = item + gridDim.x;
+      if (tid == 0 && next < nitems) {
+        tma_wait_read();                             // the store of the previous item has left stage b ^ 1
+        issue(next, b ^ 1);
+      }
+    } else {
+      if (tid == 0) {
+        tma_wait_read();                             // the store of the previous item has left the stage
+        issue(item, 0);
+      }
     }
     cplx* sm = stages + b * K::STAGE + col;
     const cplx* sph = stages + b * K::STAGE + K::ITEM + col / NV;
@@ -297,7 +340,7 @@ __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB
       const int jxf = jx < NZ ? jx : N - 1 - jx;
       return chi_shell + (size_t)((jxf * (jxf + 1) + s_yz) >> 1) * (NV * NV) + site * NV;
     };
-    mbar_wait(&bars[b], (n_done >> 1) & 1);
+    mbar_wait(&bars[b], (STAGES == 2) ? ((n_done >> 1) & 1) : (n_done & 1));
 
     {                                                // forward pass A: radix R1 over m1, half-integer shift, twiddle
       cplx x[R1];
@@ -305,10 +348,9 @@ __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB
       for (int m1 = 0; m1 < R1; ++m1) x[m1] = ld_sm(m1 * S1 + t);
       HalfShiftAll<R1, -1>::run(x);
       Dft<R1, -1>::run(x);
-      cplx a[R1];
-      twiddle_powers<R1>(a, a0, astep);
+      const PassATw<R1> a(a0, astep);
 #pragma unroll
-      for (int k1 = 0; k1 < R1; ++k1) st_sm(k1 * S1 + t, cmul(x[k1], a[k1]));
+      for (int k1 = 0; k1 < R1; ++k1) st_sm(k1 * S1 + t, cmul(x[k1], a.get(k1)));
     }
     __syncthreads();
     // inner digit: forward DFT, k-space arithmetic, inverse DFT, all on the same registers; the chi rows of the next
@@ -334,10 +376,9 @@ __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB
     __syncthreads();
     {                                                // inverse last stage: conjugate twiddle, radix R1 over k1, shift
       cplx x[R1];
-      cplx a[R1];
-      twiddle_powers<R1>(a, a0, astep);
+      const PassATw<R1> a(a0, astep);
 #pragma unroll
-      for (int k1 = 0; k1 < R1; ++k1) x[k1] = cmulc(ld_sm(k1 * S1 + t), a[k1]);
+      for (int k1 = 0; k1 < R1; ++k1) x[k1] = cmulc(ld_sm(k1 * S1 + t), a.get(k1));
       Dft<R1, +1>::run(x);
       HalfShiftAll<R1, +1>::run(x);
 #pragma unroll
@@ -346,7 +387,9 @@ __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB
     fence_proxy_async();
     __syncthreads();
     if (tid == 0) {
-      tma_store_2d(&tm_work, (int)(item * C * 2), 0, stages + b * K::STAGE);
+#pragma unroll
+      for (int bx = 0; bx < K::NBOX; ++bx)
+        tma_store_2d(&tm_work, (int)(item * C * 2), bx * K::BOX_ROWS, stages + b * K::STAGE + bx * K::BOX_ROWS * C);
       tma_commit();
     }
   }
@@ -373,6 +416,7 @@ bool kspace_uses_tma(int n) {
     case 64: return KPlan2<64>::OK;
     case 128: return KPlan2<128>::OK;
     case 256: return KPlan2<256>::OK;
+    case 512: return KPlan2<512>::OK;
     default: return false;
   }
 }

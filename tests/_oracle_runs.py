@@ -17,6 +17,9 @@ do not depend on the atom count):
           implementations of the same arithmetic can be apart at that point.
   C4grid  C4: 256^3 at 0.375 A, water + 0.1 M NaCl, KH, MDIIS 10, rcut 16 A; the first 24 atoms of the chain;
           12 iterations (the history of 10 fills and wraps twice)
+  C5grid  C5: 512^3 at 0.5 A, water + 0.15 M NaCl, KH, MDIIS 5, rcut 16 A; the first 3 atoms of the first chain;
+          2 iterations (a 512^3 x 4-site oracle iteration takes more than two minutes): the 512-point instantiations
+          of every loop kernel, whole grid
 """
 from __future__ import annotations
 
@@ -33,6 +36,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 CASES = {
     "C3full": dict(config="C3", atoms=("innermost", 100), iterations=50, checkpoint=25, twin=True, host_gb=5.0),
     "C4grid": dict(config="C4", atoms=("first", 24), iterations=12, host_gb=22.0),
+    "C5grid": dict(config="C5", atoms=("first", 3), iterations=2, host_gb=90.0, disk_gb=16.0, save_phi=False),
 }
 
 
@@ -68,7 +72,8 @@ def run_case(name: str, outdir: str) -> None:
         orc.set_solute(sub.xyz, sub.q, sub.sigma, sub.eps, rcut=cfg.rcut)
         t1 = time.perf_counter()
         np.save(os.path.join(outdir, "W.npy"), orc.get_field("W"))
-        np.save(os.path.join(outdir, "PHI.npy"), orc.phi)
+        if CASES[name].get("save_phi", True):
+            np.save(os.path.join(outdir, "PHI.npy"), orc.phi)
         ckpt = CASES[name].get("checkpoint", 0)
         if ckpt:
             orc.iterate(ckpt, 0.0)

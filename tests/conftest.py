@@ -57,6 +57,11 @@ def pytest_collection_finish(session):
             _BACKGROUND[name] = {"proc": None, "dir": None,
                                  "skip": f"oracle case {name} needs {need:.0f} GB of host memory, {free_gb:.0f} GB available"}
             continue
+        disk = CASES[name].get("disk_gb", 0.0)
+        if disk and shutil.disk_usage(tempfile.gettempdir()).free / 1e9 < disk + 2.0:
+            _BACKGROUND[name] = {"proc": None, "dir": None,
+                                 "skip": f"oracle case {name} writes {disk:.0f} GB of fields to {tempfile.gettempdir()}"}
+            continue
         free_gb -= need
         d = tempfile.mkdtemp(prefix=f"rism3d_oracle_{name}_")
         log = open(os.path.join(d, "worker.log"), "w")
