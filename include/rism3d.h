@@ -30,6 +30,7 @@
  *     synchronise that stream before returning.
  *   - Real 3D fields are laid out [site][ix][iy][iz], iz fastest, n_sites*nx*ny*nz doubles;
  *     grid point (ix,iy,iz) sits at origin + spacing*(ix,iy,iz).
+ *     In a slab-decomposed run (rism3d_params.n_ranks > 1) a context holds nx/n_ranks planes: "Slab decomposition".
  *   - There is no CPU fallback: without a CUDA device rism3d_init fails with RISM3D_ERR_CUDA.
  */
 #ifndef RISM3D_H
@@ -46,9 +47,9 @@ typedef struct rism3d_ctx rism3d_ctx;   /* opaque; created by rism3d_init, freed
 typedef enum {
   RISM3D_OK            =  0,
   RISM3D_ERR_ARG       = -1,   /* NULL pointer, negative count, unknown enum value                 */
-  RISM3D_ERR_SIZE      = -2,   /* grid not cubic / not a power of two in 8..512, n_sites outside 1..8,
-                                  mdiis_nvec outside 1..16, r_min or mdiis_b not positive, or a grid / site
-                                  combination whose k-space tile does not fit shared memory (512^3 with 1 site) */
+  RISM3D_ERR_SIZE      = -2,   /* an axis not a power of two in 8..512, n_sites outside 1..8, mdiis_nvec outside
+                                  1..16, r_min or mdiis_b not positive, (nz/2)*n_sites(padded) not a multiple of 8,
+                                  or a slab decomposition the grid does not divide into (rism3d_params.n_ranks) */
   RISM3D_ERR_ORDER     = -3,   /* call out of order (set_solute before set_solvent_chi, ...)       */
   RISM3D_ERR_CHI_RANGE = -4,   /* chi table does not cover the 3D |k| range, or is too coarse      */
   RISM3D_ERR_NEUTRAL   = -5,   /* sum_g rho_g q_g != 0 (1e-12)                                     */
@@ -75,7 +76,8 @@ typedef enum {
 } rism3d_field;
 
 typedef struct {
-  int    nx, ny, nz;        /* grid points per axis; this build: nx == ny == nz, power of two, 8..512 */
+  int    nx, ny, nz;        /* grid points per axis: each a power of two in 8..512; they may differ (the box
+                               need not be a cube), the spacing is the same on all axes                */
   double spacing;           /* grid spacing, A                                                     */
   double origin[3];         /* position of grid index (0,0,0), A                                   */
   int    n_sites;           /* n_v, number of solvent site TYPES, 1..8 (3, 5, 6, 7 run padded to 4 or 8 with
@@ -98,6 +100,8 @@ typedef struct {
                                history then keeps X_i and R_i apart and the update reads both: M more words per
                                grid point, site and iteration                                       */
   double mdiis_b_min, mdiis_b_max;
+  int    n_ranks, rank;     /* slab decomposition over n_ranks GPUs, one context per GPU and process (0 or 1: the
+                               whole grid on this GPU).  See "Slab decomposition" below.             */
 } rism3d_params;
 
 /* Bytes of DEVICE memory the caller must provide to rism3d_init (0 if the parameters are invalid). */
@@ -134,7 +138,7 @@ int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz, const dou
  * or when set_solute computed it (rcut <= 0). */
 int rism3d_phi_ms(rism3d_ctx* ctx, float* ms);
 
-/* Run the loop.  tol <= 0: exactly max_iter iterations.  tol > 0: stop after the first iteration
+/* Run the loop (single rank, or a slab run in peer mode).  tol <= 0: exactly max_iter iterations.  tol > 0: stop after the first iteration
  * whose rms residual is below tol (tau is then left unchanged by that iteration) or after max_iter.
  * n_done (may be NULL): iterations performed by this call; rms (may be NULL): last residual.
  * Returns RISM3D_ERR_DIVERGED when the residual became non-finite. */
@@ -199,6 +203,70 @@ const char* rism3d_loop_kernel_name(int k);             /* static strings; "" wh
  * inverse: the exact inverse of that map (includes 1/(nx ny nz)). */
 int rism3d_debug_fft_forward(rism3d_ctx* ctx, const double* d_real_in, double* d_spec_out);
 int rism3d_debug_fft_inverse(rism3d_ctx* ctx, const double* d_spec_in, double* d_real_out);
+
+/* ---- Slab decomposition over several GPUs ("2D decomposition 3D-FFT"; one level of it) -----------
+ *
+ * n_ranks = P (a power of two, <= 8; nx/P and ny/P multiples of 8) contexts, one per GPU, share one solve.  Rank r holds
+ * the planes ix in [r nx/P, (r+1) nx/P) of every real field ([site][ix_l][iy][iz]; get_field / set_tau move that slab)
+ * and runs the closure, the z and the y transforms on them.  The x transform, Eq. 32, Eq. 13 and the inverse x transform
+ * need whole x lines: rank r does them for the rows jy in [r ny/P, (r+1) ny/P) of the spectrum, array "K" =
+ * complex [jx][jy_l][p][site].  As in the paper (its steps 6-7, which "can be canceled out") k space is
+ * left in that transposed distribution: one exchange on the way in, one on the way out, both of nx/P x ny/P x (nz/2 n_v)
+ * complex blocks between every pair of ranks, and one exchange of a row of <= 18 double-double Gram sums.
+ *
+ * The exchanges happen INSIDE the transform kernels' loads and stores, through per-rank base pointers:
+ *   forward   the y pass of rank r writes the rows of rank d's slab to   F_d + (ix_l ny/P + jy_l) nz/2 n_v
+ *   backward  the inverse y pass of rank r reads the rows of rank s from B_s + (ix_l ny/P + jy_l) nz/2 n_v
+ * Two ways to provide F and B:
+ *   staged (default)   F_d = stage + d*block, B_s = stage + s*block in this rank's own staging array; the CALLER moves
+ *                      stage -> K of every rank after phase 0 and K -> stage after phase 1 with an all-to-all of equal,
+ *                      contiguous blocks (torch.distributed.all_to_all_single over NCCL), and all-gathers the Gram rows
+ *                      after phase 2.  rism3d_slab_local gives the addresses.
+ *   peer               after rism3d_slab_set_peers (device pointers of every rank's K, Gram and flag arrays, mapped into
+ *                      this process: CUDA IPC / torch symmetric memory over NVLink), F_d = K_d + r*block and
+ *                      B_s = K_s + r*block: the y pass stores straight into the destination GPU's K and the inverse y
+ *                      pass loads straight from the source GPU's K -- the transposes overlap the transforms tile by
+ *                      tile and no staging copy exists.  rism3d_iterate then runs whole iterations with in-stream
+ *                      barriers (a flag per rank, release/acquire at system scope) where the phases meet.
+ * Phases of one iteration (rism3d_slab_phase), every rank the same sequence:
+ *   0  pending MDIIS update, closure, forward z, forward y (-> F)          [exchange: forward blocks]
+ *   1  forward x, Eq. 32, Eq. 13, inverse x on K, in place                 [exchange: backward blocks]
+ *   2  inverse y (<- B), inverse z, residual, Gram row of this slab        [exchange: Gram rows]
+ *   3  sum of the ranks' rows in rank order, rms, restart rule, MDIIS solve (identical on every rank)
+ * set_solvent_chi and set_solute take the same arguments on every rank (each computes its slabs of w, phi, phi~).
+ * free_energy, pmv, pressure_correction and gradient return THIS SLAB'S share of the grid sums: the caller adds the
+ * ranks' numbers (dmu, the site integrals, gradient components).  The debug FFT hooks are single-rank only. */
+
+/* Host-only: the slab of rank params->rank (no context, no GPU needed).  Real fields of the rank: planes ix0 .. ix0+nxl-1;
+ * its k-space slab: rows jy0 .. jy0+nyl-1; row_elems = (nz/2) * n_sites_padded complex numbers per (ix, iy) row of the
+ * spectrum; block_elems = nxl * nyl * row_elems complex numbers per block of the transposes.  Returns RISM3D_ERR_SIZE
+ * when the parameters are invalid.  With n_ranks <= 1 the slab is the whole grid. */
+typedef struct {
+  int nxl, ix0, nyl, jy0;
+  int n_sites_padded;
+  size_t row_elems, block_elems;
+} rism3d_slab_info;
+int rism3d_slab_plan(const rism3d_params* params, rism3d_slab_info* out);
+
+/* Addresses of this rank's exchange arrays (DEVICE pointers inside the workspace) and the block size of the transposes:
+ * K and stage hold n_ranks blocks of block_bytes each (block s <-> rank s); gram holds n_ranks rows of gram_row_bytes;
+ * flags is the barrier array of peer mode.  Any output pointer may be NULL. */
+int rism3d_slab_local(rism3d_ctx* ctx, void** d_K, void** d_stage, void** d_gram, void** d_flags, size_t* block_bytes,
+                      size_t* gram_row_bytes);
+
+/* Switch to peer mode: d_K[r], d_gram[r], d_flags[r] are the arrays rism3d_slab_local returned on rank r, as DEVICE
+ * pointers valid in this process (HOST arrays of n_ranks pointers; entry `rank` is this rank's own). */
+int rism3d_slab_set_peers(rism3d_ctx* ctx, void* const* d_K, void* const* d_gram, void* const* d_flags);
+
+/* Phase calls of a staged run (also usable in peer mode when the caller orders the ranks itself):
+ * begin sets the tolerance of the iterations that follow (as rism3d_iterate's tol) and clears the call's counters;
+ * phase(0..3) enqueues that phase of one iteration; end applies the pending update (tau is then the new input), reads
+ * the state back and reports like rism3d_iterate.  status (rism3d_slab_status): cheap look at the device state between
+ * iterations -- *done != 0 once an iteration has met the tolerance or diverged (further phases return immediately). */
+int rism3d_slab_begin(rism3d_ctx* ctx, double tol);
+int rism3d_slab_phase(rism3d_ctx* ctx, int phase);
+int rism3d_slab_status(rism3d_ctx* ctx, int* done, int* n_done, double* rms);
+int rism3d_slab_end(rism3d_ctx* ctx, int* n_done, double* rms);
 
 const char* rism3d_last_error(const rism3d_ctx* ctx);   /* valid until the next call on ctx */
 const char* rism3d_status_string(int status);           /* static strings                    */

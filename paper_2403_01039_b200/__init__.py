@@ -11,5 +11,6 @@ from .binding import (  # noqa: F401
     rism3d_free_energy, rism3d_pmv, rism3d_pressure_correction, rism3d_gradient, rism3d_get_field, rism3d_set_tau, rism3d_get_rms_history, rism3d_launch_count, rism3d_phi_ms, rism3d_measure_dfma_peak,
     rism3d_set_profiling, rism3d_get_timings, rism3d_loop_kernel_name, N_LOOP_KERNELS,
     rism3d_debug_fft_forward, rism3d_debug_fft_inverse, rism3d_last_error, rism3d_status_string,
-    rism3d_destroy, EXPORTED_SYMBOLS,
+    rism3d_destroy, EXPORTED_SYMBOLS, Rism3dSlabInfo, rism3d_slab_plan, rism3d_slab_local, rism3d_slab_set_peers,
+    rism3d_slab_begin, rism3d_slab_phase, rism3d_slab_status, rism3d_slab_end, SlabSolver, iterate_in_lockstep,
 )

@@ -23,6 +23,8 @@ EXPORTED_SYMBOLS = [
     "rism3d_get_rms_history", "rism3d_launch_count", "rism3d_phi_ms", "rism3d_measure_dfma_peak", "rism3d_set_profiling", "rism3d_get_timings",
     "rism3d_loop_kernel_name", "rism3d_debug_fft_forward",
     "rism3d_debug_fft_inverse", "rism3d_last_error", "rism3d_status_string", "rism3d_destroy",
+    "rism3d_slab_plan", "rism3d_slab_local", "rism3d_slab_set_peers", "rism3d_slab_begin", "rism3d_slab_phase",
+    "rism3d_slab_status", "rism3d_slab_end",
 ]
 
 
@@ -51,7 +53,13 @@ class Rism3dParams(C.Structure):
         ("anderson_s", C.c_double * 2),
         ("mdiis_dynamic_b", C.c_int),
         ("mdiis_b_min", C.c_double), ("mdiis_b_max", C.c_double),
+        ("n_ranks", C.c_int), ("rank", C.c_int),
     ]
+
+
+class Rism3dSlabInfo(C.Structure):
+    _fields_ = [("nxl", C.c_int), ("ix0", C.c_int), ("nyl", C.c_int), ("jy0", C.c_int), ("n_sites_padded", C.c_int),
+                ("row_elems", C.c_size_t), ("block_elems", C.c_size_t)]
 
 
 def library_path() -> str:
@@ -115,6 +123,21 @@ def load_library():
     lib.rism3d_status_string.argtypes = [C.c_int]
     lib.rism3d_destroy.restype = None
     lib.rism3d_destroy.argtypes = [C.c_void_p]
+    vpp, szp = C.POINTER(C.c_void_p), C.POINTER(C.c_size_t)
+    lib.rism3d_slab_plan.restype = C.c_int
+    lib.rism3d_slab_plan.argtypes = [C.POINTER(Rism3dParams), C.POINTER(Rism3dSlabInfo)]
+    lib.rism3d_slab_local.restype = C.c_int
+    lib.rism3d_slab_local.argtypes = [C.c_void_p, vpp, vpp, vpp, vpp, szp, szp]
+    lib.rism3d_slab_set_peers.restype = C.c_int
+    lib.rism3d_slab_set_peers.argtypes = [C.c_void_p, vpp, vpp, vpp]
+    lib.rism3d_slab_begin.restype = C.c_int
+    lib.rism3d_slab_begin.argtypes = [C.c_void_p, C.c_double]
+    lib.rism3d_slab_phase.restype = C.c_int
+    lib.rism3d_slab_phase.argtypes = [C.c_void_p, C.c_int]
+    lib.rism3d_slab_status.restype = C.c_int
+    lib.rism3d_slab_status.argtypes = [C.c_void_p, ip, ip, dp]
+    lib.rism3d_slab_end.restype = C.c_int
+    lib.rism3d_slab_end.argtypes = [C.c_void_p, ip, dp]
     _LIB = lib
     return lib
 
@@ -263,6 +286,49 @@ def rism3d_debug_fft_inverse(ctx, d_in: int, d_out: int):
     _check(ctx, load_library().rism3d_debug_fft_inverse(ctx, C.c_void_p(d_in), C.c_void_p(d_out)))
 
 
+def rism3d_slab_plan(params: Rism3dParams) -> Rism3dSlabInfo:
+    """host-only (no GPU): the slab of rank params.rank"""
+    info = Rism3dSlabInfo()
+    st = load_library().rism3d_slab_plan(C.byref(params), C.byref(info))
+    if st != 0:
+        raise Rism3dError(st, rism3d_status_string(st))
+    return info
+
+
+def rism3d_slab_local(ctx):
+    """-> dict(K, stage, gram, flags: device addresses; block_bytes, gram_row_bytes)"""
+    k, stg, gr, fl = C.c_void_p(), C.c_void_p(), C.c_void_p(), C.c_void_p()
+    bb, gb = C.c_size_t(), C.c_size_t()
+    _check(ctx, load_library().rism3d_slab_local(ctx, C.byref(k), C.byref(stg), C.byref(gr), C.byref(fl), C.byref(bb), C.byref(gb)))
+    return dict(K=k.value, stage=stg.value, gram=gr.value, flags=fl.value, block_bytes=bb.value, gram_row_bytes=gb.value)
+
+
+def rism3d_slab_set_peers(ctx, d_K, d_gram, d_flags):
+    n = len(d_K)
+    arr = lambda v: (C.c_void_p * n)(*[int(x) for x in v])
+    _check(ctx, load_library().rism3d_slab_set_peers(ctx, arr(d_K), arr(d_gram), arr(d_flags)))
+
+
+def rism3d_slab_begin(ctx, tol: float = 0.0):
+    _check(ctx, load_library().rism3d_slab_begin(ctx, float(tol)))
+
+
+def rism3d_slab_phase(ctx, phase: int):
+    _check(ctx, load_library().rism3d_slab_phase(ctx, int(phase)))
+
+
+def rism3d_slab_status(ctx):
+    done, n_done, rms = C.c_int(), C.c_int(), C.c_double()
+    _check(ctx, load_library().rism3d_slab_status(ctx, C.byref(done), C.byref(n_done), C.byref(rms)))
+    return bool(done.value), n_done.value, rms.value
+
+
+def rism3d_slab_end(ctx):
+    n_done, rms = C.c_int(), C.c_double()
+    _check(ctx, load_library().rism3d_slab_end(ctx, C.byref(n_done), C.byref(rms)))
+    return n_done.value, rms.value
+
+
 def rism3d_destroy(ctx):
     load_library().rism3d_destroy(ctx)
 
@@ -273,16 +339,21 @@ class Solver:
 
     def __init__(self, n, spacing, n_sites, closure="KH", pse_order=1, temperature=298.0, mdiis_nvec=5,
                  mdiis_b=0.5, mdiis_restart=10.0, kappa=1.0, r_min=1e-3, origin=None, device=0,
-                 accelerator="MDIIS", anderson_s=(0.2, 0.0), mdiis_dynamic_b=None):
+                 accelerator="MDIIS", anderson_s=(0.2, 0.0), mdiis_dynamic_b=None, n_ranks=1, rank=0, stream=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2403_01039_b200 needs a CUDA device (no CPU fallback)")
         load_library()
-        self.n, self.n_sites, self.spacing = int(n), int(n_sites), float(spacing)
+        # n: points per axis, one number (cube) or (nx, ny, nz); self.n stays the caller's value, self.shape the triple
+        self.shape = (int(n),) * 3 if np.isscalar(n) else tuple(int(m) for m in n)
+        if len(self.shape) != 3:
+            raise ValueError(f"n must be one number or (nx, ny, nz), got {n!r}")
+        self.n = int(n) if np.isscalar(n) else self.shape
+        self.n_sites, self.spacing = int(n_sites), float(spacing)
         p = Rism3dParams()
-        p.nx = p.ny = p.nz = self.n
+        p.nx, p.ny, p.nz = self.shape
         p.spacing = self.spacing
-        org = [-(self.n // 2) * self.spacing] * 3 if origin is None else list(origin)
+        org = [-(m // 2) * self.spacing for m in self.shape] if origin is None else list(origin)
         p.origin = (C.c_double * 3)(*org)
         p.n_sites = self.n_sites
         p.closure = CLOSURES[closure]
@@ -298,6 +369,11 @@ class Solver:
         p.anderson_s = (C.c_double * 2)(float(anderson_s[0]), float(anderson_s[1]))
         p.mdiis_dynamic_b = 0 if mdiis_dynamic_b is None else 1        # (b_min, b_max) of b = -0.2 log10(rms)
         p.mdiis_b_min, p.mdiis_b_max = (0.0, 0.0) if mdiis_dynamic_b is None else (float(mdiis_dynamic_b[0]), float(mdiis_dynamic_b[1]))
+        p.n_ranks, p.rank = int(n_ranks), int(rank)
+        self.n_ranks, self.rank = max(1, int(n_ranks)), int(rank)
+        self.grid_shape = self.shape                 # the whole grid; self.shape = what this context holds (its slab)
+        if self.n_ranks > 1:
+            self.shape = (self.shape[0] // self.n_ranks,) + self.shape[1:]
         self.params = p
         nbytes = rism3d_workspace_bytes(p)
         if nbytes == 0:
@@ -305,7 +381,7 @@ class Solver:
         self.device = torch.device("cuda", device)
         self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
         # a stream of its own (not the legacy default stream): the library captures its iteration into CUDA graphs
-        self.stream = torch.cuda.Stream(self.device)
+        self.stream = torch.cuda.Stream(self.device) if stream is None else stream
         self.stream.wait_stream(torch.cuda.current_stream(self.device))     # the workspace allocation above
         self.ctx = rism3d_init(p, self.workspace.data_ptr(), nbytes, self.stream.cuda_stream)
 
@@ -361,16 +437,16 @@ class Solver:
         return rism3d_pmv(self.ctx, chi_t, self.n_sites)
 
     def get_field(self, which: str, site=None) -> np.ndarray:
-        """Host copy: [n][n][n] for one site, or [n_sites][n][n][n] when site is None."""
+        """Host copy: [nx][ny][nz] for one site, or [n_sites][nx][ny][nz] when site is None."""
         sites = range(self.n_sites) if site is None else [site]
-        out = np.empty((len(sites), self.n, self.n, self.n))
+        out = np.empty((len(sites),) + self.shape)
         for i, s in enumerate(sites):
             rism3d_get_field(self.ctx, FIELDS[which], s, out[i].ctypes.data, False)
         return out if site is None else out[0]
 
     def get_field_device(self, which: str, site: int):
         import torch
-        out = torch.empty((self.n, self.n, self.n), dtype=torch.float64, device=self.device)
+        out = torch.empty(self.shape, dtype=torch.float64, device=self.device)
         self.stream.wait_stream(torch.cuda.current_stream(self.device))     # the block may have pending uses there
         rism3d_get_field(self.ctx, FIELDS[which], site, out.data_ptr(), True)
         return out
@@ -404,15 +480,16 @@ class Solver:
         return 1 if self.n_sites <= 1 else (2 if self.n_sites <= 2 else (4 if self.n_sites <= 4 else 8))
 
     def fft_forward(self, real_dev):
-        """debug: real device tensor [n_sites][n][n][n] -> complex device tensor [n][n][n/2][n_sites]."""
+        """debug: real device tensor [n_sites][nx][ny][nz] -> complex device tensor [nx][ny][nz/2][n_sites]."""
         import torch
         nvp = self._padded_sites                     # the library transforms the padded site count (rism3d.h)
         if nvp != self.n_sites:
-            pad = torch.zeros((nvp, self.n, self.n, self.n), dtype=torch.float64, device=self.device)
+            pad = torch.zeros((nvp,) + self.shape, dtype=torch.float64, device=self.device)
             pad[: self.n_sites] = real_dev
             real_dev = pad
         real_dev = real_dev.contiguous()
-        out = torch.empty((self.n, self.n, self.n // 2, nvp), dtype=torch.complex128, device=self.device)
+        nx, ny, nz = self.shape
+        out = torch.empty((nx, ny, nz // 2, nvp), dtype=torch.complex128, device=self.device)
         self.stream.wait_stream(torch.cuda.current_stream(self.device))
         rism3d_debug_fft_forward(self.ctx, real_dev.data_ptr(), out.data_ptr())
         return out[..., : self.n_sites]
@@ -421,11 +498,150 @@ class Solver:
         import torch
         nvp = self._padded_sites
         if nvp != self.n_sites:
-            pad = torch.zeros((self.n, self.n, self.n // 2, nvp), dtype=torch.complex128, device=self.device)
+            nx, ny, nz = self.shape
+            pad = torch.zeros((nx, ny, nz // 2, nvp), dtype=torch.complex128, device=self.device)
             pad[..., : self.n_sites] = spec_dev
             spec_dev = pad
         spec_dev = spec_dev.contiguous()
-        out = torch.empty((nvp, self.n, self.n, self.n), dtype=torch.float64, device=self.device)
+        out = torch.empty((nvp,) + self.shape, dtype=torch.float64, device=self.device)
         self.stream.wait_stream(torch.cuda.current_stream(self.device))
         rism3d_debug_fft_inverse(self.ctx, spec_dev.data_ptr(), out.data_ptr())
         return out[: self.n_sites]
+
+
+# ---- slab-decomposed runs (include/rism3d.h "Slab decomposition") ----------------------------------------------------
+class SlabSolver(Solver):
+    """One rank of a solve shared by n_ranks GPUs.  Same calls as Solver; fields are this rank's planes
+    [nx / n_ranks][ny][nz]; free_energy / pmv / pressure_correction / gradient return the sums over ALL ranks.
+
+    Two ways to run it:
+      * one process per GPU under torch.distributed (backend nccl): `group` is the process group (None = the default
+        one).  The two transposes are all_to_all_single calls on equal, contiguous blocks that the y passes have
+        already laid out per destination, the Gram rows one all_gather -- issued on the solver's stream between the
+        phase calls.  `connect_peers(addresses)` switches to peer mode (pointers of every rank's arrays mapped into this
+        process, e.g. from torch's symmetric memory): the y passes then store to / load from the other GPUs directly and
+        iterate() is a single C call with in-stream barriers.
+      * several ranks of one process on one GPU, driven phase by phase by `iterate_in_lockstep` (how the tests check
+        the decomposition against the oracle on a single GPU; no rank ever waits for another inside a kernel).
+    Only plumbing lives here: every numerical step is a kernel behind rism3d_slab_phase."""
+
+    def __init__(self, n, spacing, n_sites, n_ranks, rank, group=None, **kw):
+        super().__init__(n, spacing, n_sites, n_ranks=n_ranks, rank=rank, **kw)
+        import torch
+        self.group = group
+        loc = rism3d_slab_local(self.ctx)
+        self.local = loc
+        base = self.workspace.data_ptr()
+
+        def view(addr, nbytes):
+            return self.workspace[addr - base: addr - base + nbytes].view(torch.float64)
+
+        nb = loc["block_bytes"] * self.n_ranks
+        self.K = view(loc["K"], nb)                     # [n_ranks][block]: block s came from rank s
+        self.stage = view(loc["stage"], nb)             # [n_ranks][block]: block d goes to rank d / came back from it
+        self.gram = view(loc["gram"], loc["gram_row_bytes"] * self.n_ranks)
+        self.peer_mode = False
+
+    # -- phase calls ---------------------------------------------------------------------------------------------
+    def begin(self, tol=0.0):
+        rism3d_slab_begin(self.ctx, tol)
+
+    def phase(self, k):
+        rism3d_slab_phase(self.ctx, k)
+
+    def status(self):
+        return rism3d_slab_status(self.ctx)
+
+    def end(self):
+        return rism3d_slab_end(self.ctx)
+
+    def connect_peers(self, d_K, d_gram, d_flags):
+        rism3d_slab_set_peers(self.ctx, d_K, d_gram, d_flags)
+        self.peer_mode = True
+
+    # -- one process per GPU -------------------------------------------------------------------------------------
+    def iterate(self, max_iter, tol=0.0, check_every=8):
+        if self.peer_mode:
+            return rism3d_iterate(self.ctx, max_iter, tol)
+        import torch
+        import torch.distributed as dist
+        row = self.gram.numel() // self.n_ranks
+        self.begin(tol)
+        with torch.cuda.stream(self.stream):
+            for it in range(max_iter):
+                self.phase(0)
+                dist.all_to_all_single(self.K, self.stage, group=self.group)          # forward transpose
+                self.phase(1)
+                dist.all_to_all_single(self.stage, self.K, group=self.group)          # backward transpose
+                self.phase(2)
+                dist.all_gather_into_tensor(self.gram, self.gram[self.rank * row:(self.rank + 1) * row], group=self.group)
+                self.phase(3)
+                if tol > 0.0 and (it + 1) % check_every == 0 and self.status()[0]:
+                    break
+        return self.end()
+
+    def _sum_over_ranks(self, values):
+        import torch
+        import torch.distributed as dist
+        t = torch.as_tensor(np.asarray(values, dtype=np.float64), device=self.device)
+        dist.all_reduce(t, group=self.group)
+        return t.cpu().numpy()
+
+    def free_energy(self):
+        mu, site = rism3d_free_energy(self.ctx, self.n_sites)
+        tot = self._sum_over_ranks(np.concatenate([[mu], site]))
+        return float(tot[0]), tot[1:]
+
+    def pmv(self, chi_t: float):
+        v, c_int = rism3d_pmv(self.ctx, chi_t, self.n_sites)
+        tot = self._sum_over_ranks(np.concatenate([[v], c_int]))
+        return float(tot[0]), tot[1:]
+
+    def pressure_correction(self, chi_t: float, pressure: float):
+        v, _ = self.pmv(chi_t)
+        return -pressure * v, v
+
+    def gradient(self) -> np.ndarray:
+        return self._sum_over_ranks(rism3d_gradient(self.ctx, self.n_atoms))
+
+
+def iterate_in_lockstep(ranks, max_iter, tol=0.0):
+    """Drive all ranks of a slab run that live in ONE process on ONE GPU (SlabSolver objects created with the same
+    `stream`), phase by phase.  Staged mode: the blocks move by device copies that stand in for the all-to-all; peer
+    mode (after connect_peers with each other's addresses): nothing to move.  -> (n_done, rms) of rank 0."""
+    import torch
+    P = len(ranks)
+    stream = ranks[0].stream
+    assert all(r.stream is stream for r in ranks), "lockstep ranks share one stream"
+    peer = ranks[0].peer_mode
+    blk = ranks[0].K.numel() // P
+    row = ranks[0].gram.numel() // P
+    for r in ranks:
+        r.begin(tol)
+    with torch.cuda.stream(stream):
+        for it in range(max_iter):
+            for r in ranks:
+                r.phase(0)
+            if not peer:
+                for d in range(P):
+                    for s in range(P):
+                        ranks[d].K[s * blk:(s + 1) * blk].copy_(ranks[s].stage[d * blk:(d + 1) * blk])
+            for r in ranks:
+                r.phase(1)
+            if not peer:
+                for d in range(P):
+                    for s in range(P):
+                        ranks[d].stage[s * blk:(s + 1) * blk].copy_(ranks[s].K[d * blk:(d + 1) * blk])
+            for r in ranks:
+                r.phase(2)
+            if not peer:
+                for d in range(P):
+                    for s in range(P):
+                        if s != d:
+                            ranks[d].gram[s * row:(s + 1) * row].copy_(ranks[s].gram[s * row:(s + 1) * row])
+            for r in ranks:
+                r.phase(3)
+            if tol > 0.0 and (it + 1) % 8 == 0 and ranks[0].status()[0]:
+                break
+    out = [r.end() for r in ranks]
+    return out[0]

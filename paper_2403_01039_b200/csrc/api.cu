@@ -104,36 +104,65 @@ static bool make_tensor_map_2d(CUtensorMap* tm, void* base, uint64_t row_len, ui
 // exchanged by butterfly shuffles): other counts run padded with phantom types
 static int padded_sites(int nv) { return nv <= 1 ? 1 : (nv <= 2 ? 2 : (nv <= 4 ? 4 : 8)); }
 
+static bool pow2_in(int n, int lo, int hi) { return n >= lo && n <= hi && (n & (n - 1)) == 0; }
+
 static bool valid_params(const rism3d_params* p) {
   if (!p) return false;
-  const int n = p->nx;
-  if (p->ny != n || p->nz != n) return false;
-  if (n < 8 || n > 512 || (n & (n - 1))) return false;
+  // every axis a power of two in 8..512, one spacing: the three lengths may differ (a box is rarely a cube)
+  if (!pow2_in(p->nx, 8, 512) || !pow2_in(p->ny, 8, 512) || !pow2_in(p->nz, 8, 512)) return false;
   if (p->n_sites < 1 || p->n_sites > MAX_NV) return false;
   const int nv = padded_sites(p->n_sites);
-  if (((n / 2) * nv) % 8) return false;             // tile rows are 8 complex wide
+  if (((p->nz / 2) * nv) % 8) return false;         // tile rows are 8 complex wide
   if (p->mdiis_nvec < 1 || p->mdiis_nvec > MAX_M) return false;
   if (!(p->spacing > 0.0) || !(p->temperature > 0.0) || !(p->kappa > 0.0)) return false;
   // r_min = 0 (e.g. a zero-initialised struct) would put 1/0 into w for a grid point on an atom (Q11); the clamp must
   // also stay well inside the float range of the rsqrt seed.  The mixing parameter must be positive.
   if (!(p->r_min >= 1e-6) || !(p->r_min < 1e6) || !(p->mdiis_b > 0.0) || !(p->mdiis_b < 1e6)) return false;
-  if (kspace_smem_bytes(n, nv) <= 0 || kspace_smem_bytes(n, nv) > 227 * 1024) return false;   // e.g. (512, 1 site)
+  if (kspace_smem_bytes(p->nx, nv) <= 0 || kspace_smem_bytes(p->nx, nv) > 227 * 1024) return false;
   if (p->closure != RISM3D_KH && p->closure != RISM3D_PSE && p->closure != RISM3D_HNC) return false;
   if (p->closure == RISM3D_PSE && p->pse_order < 1) return false;
   if (p->accelerator != RISM3D_ACCEL_MDIIS && p->accelerator != RISM3D_ACCEL_ANDERSON) return false;
   if (p->mdiis_dynamic_b && !(p->mdiis_b_min > 0.0 && p->mdiis_b_max >= p->mdiis_b_min && p->mdiis_b_max < 1e6)) return false;
+  if (p->n_ranks > 1) {                              // slab decomposition: whole bricks / tiles per rank
+    const int P = p->n_ranks;
+    if (P > MAX_RANKS || (P & (P - 1)) || p->rank < 0 || p->rank >= P) return false;
+    if (p->nx % P || p->ny % P || (p->nx / P) % 8 || (p->ny / P) % 8) return false;
+  } else if (p->n_ranks < 0 || (p->n_ranks <= 1 && p->rank != 0)) {
+    return false;
+  }
   return true;
+}
+
+// geometry of the context's grid from the caller's parameters (device attributes are filled in by rism3d_init)
+static Grid make_grid(const rism3d_params* p) {
+  Grid g{};
+  g.nx = p->nx; g.ny = p->ny; g.nz = p->nz;
+  g.nmax = g.nx > g.ny ? (g.nx > g.nz ? g.nx : g.nz) : (g.ny > g.nz ? g.ny : g.nz);
+  const int ex = g.nmax / g.nx, ey = g.nmax / g.ny, ez = g.nmax / g.nz;
+  g.wx = ex * ex; g.wy = ey * ey; g.wz = ez * ez;
+  // largest shell index: every folded index at its maximum n_axis / 2 - 1
+  auto top = [](int n, int w) { const long long hn = n / 2; return (long long)w * (hn - 1) * hn; };
+  g.nshell = (int)((top(g.nx, g.wx) + top(g.ny, g.wy) + top(g.nz, g.wz)) / 2 + 1);
+  g.nv = padded_sites(p->n_sites); g.nv_user = p->n_sites; g.h = p->spacing;
+  for (int i = 0; i < 3; ++i) g.origin[i] = p->origin[i];
+  g.n_ranks = p->n_ranks > 1 ? p->n_ranks : 1;
+  g.rank = p->n_ranks > 1 ? p->rank : 0;
+  g.nxl = g.nx / g.n_ranks; g.ix0 = g.rank * g.nxl;
+  g.nyl = g.ny / g.n_ranks; g.jy0 = g.rank * g.nyl;
+  g.npts = (size_t)g.nxl * g.ny * g.nz;
+  g.npts_global = (size_t)g.nx * g.ny * g.nz;
+  g.field = g.npts * g.nv;
+  return g;
 }
 
 // stored (input, residual) pairs: mdiis_nvec, or 3 for the modified Anderson method (the newest + two histories)
 static int effective_m(const rism3d_params* p) { return p->accelerator == RISM3D_ACCEL_ANDERSON ? 3 : p->mdiis_nvec; }
 
-static int n_shells(int n) { const int hn = n / 2; return 3 * (hn - 1) * hn / 2 + 1; }
-
 // carve the workspace; with base == nullptr only the total size is computed
 static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_out, size_t* scratch_bytes) {
-  const size_t n = p->nx, nv = (size_t)padded_sites(p->n_sites), M = (size_t)effective_m(p);
-  const size_t npts = n * n * n, field = npts * nv;
+  const Grid gq = make_grid(p);
+  const size_t nv = (size_t)gq.nv, M = (size_t)effective_m(p);
+  const size_t npts = gq.npts, field = gq.field;
   size_t off = 0;
   auto take = [&](size_t bytes) { char* ptr = base ? base + off : nullptr; off += align256(bytes); return ptr; };
   char* st = take(sizeof(DevState));
@@ -146,10 +175,8 @@ static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_o
   const size_t scr = off - off_x;
   char* phi = take(npts * 8);
   char* phik = take(npts * 8);
-  char* chis = take((size_t)n_shells((int)n) * nv * nv * 8);
-  char* tw = take(2 * n * 16);
-  Grid gq{};
-  gq.n = (int)n; gq.nv = (int)nv; gq.npts = npts; gq.field = field;
+  char* chis = take((size_t)gq.nshell * nv * nv * 8);
+  char* tw = take(2 * (size_t)gq.nmax * 16);
   const size_t nblk = (size_t)zinv_ctas(gq);          // one Gram partial per zinv_residual CTA
   const size_t ngrp = (nblk + 63) / 64;
   char* gp = take(nblk * (MAX_M + 1) * 2 * 8);
@@ -160,7 +187,15 @@ static size_t carve(const rism3d_params* p, char* base, Buffers* b, double** d_o
   char* rv = take(MAX_NV * 8);
   char* gw = take(MAX_NV * 8);
   char* out = take(64 * 8);
+  char *kb = work, *stg = nullptr, *gx = nullptr, *xf = nullptr;
+  if (gq.n_ranks > 1) {                             // slab run: the k-space slab, the staging array, the exchange rows
+    kb = take(field * 8);
+    stg = take(field * 8);
+    gx = take((size_t)MAX_RANKS * GRAM_SLOT * 2 * 8);
+    xf = take((MAX_RANKS + 1) * sizeof(unsigned long long));
+  }
   if (b) {
+    b->kbuf = (double2*)kb; b->stage = (double2*)stg; b->gram_x = (double*)gx; b->xflags = (unsigned long long*)xf;
     b->state = (DevState*)st;
     b->Z = (double*)Z; b->R = (double*)R; b->tau = (double*)tau; b->w = (double*)w; b->work = (double2*)work;
     b->phi = (double*)phi; b->phik = (double2*)phik; b->chi_shell = (double*)chis; b->tw = (double2*)tw;
@@ -220,10 +255,7 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
   ctx->ws_bytes = bytes;
   carve(p, ctx->ws, &ctx->b, &ctx->d_out, &ctx->scratch_bytes);
   Grid& g = ctx->g;
-  g.n = p->nx; g.nv = padded_sites(p->n_sites); g.nv_user = p->n_sites; g.h = p->spacing;
-  for (int i = 0; i < 3; ++i) g.origin[i] = p->origin[i];
-  g.npts = (size_t)g.n * g.n * g.n;
-  g.field = g.npts * g.nv;
+  g = make_grid(p);
   g.num_sms = num_sms;
   g.smem_optin = smem_optin;
   SolverParams& sp = ctx->sp;
@@ -237,25 +269,38 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
   sp.kT = K_BOLTZMANN * p->temperature;
   sp.beta = 1.0 / sp.kT;
   sp.kappa = p->kappa; sp.r_min = p->r_min;
-  // twiddle table exp(-i pi j / n), j < 2n, from long double
-  std::vector<double> tw(4 * (size_t)g.n);
-  for (int j = 0; j < 2 * g.n; ++j) {
-    const long double a = 3.14159265358979323846264338327950288L * (long double)j / (long double)g.n;
+  // twiddle table exp(-i pi j / nmax), j < 2 nmax, from long double (an axis of length n reads every (nmax/n)-th entry)
+  std::vector<double> tw(4 * (size_t)g.nmax);
+  for (int j = 0; j < 2 * g.nmax; ++j) {
+    const long double a = 3.14159265358979323846264338327950288L * (long double)j / (long double)g.nmax;
     tw[2 * j] = (double)cosl(a);
     tw[2 * j + 1] = (double)(-sinl(a));
   }
-  if (kspace_uses_tma(g.n)) {
-    // k-space pass tiles: n rows (jx) of 8 complex = 16 doubles of `work`, and the matching 8 / nv phi~ values per row
-    const uint64_t q2 = (uint64_t)(g.n / 2) * g.nv * 2, h2 = (uint64_t)(g.n / 2) * 2;     // doubles per (jx, jy) row
-    const uint32_t box_rows = (uint32_t)(g.n < 256 ? g.n : 256);                          // TMA box limit; 512 = two boxes
-    if (!make_tensor_map_2d(&ctx->b.tm_work, ctx->b.work, (uint64_t)g.n * q2, (uint64_t)g.n, (uint64_t)g.n * q2 * 8, 16, box_rows) ||
-        !make_tensor_map_2d(&ctx->b.tm_phik, ctx->b.phik, (uint64_t)g.n * h2, (uint64_t)g.n, (uint64_t)g.n * h2 * 8,
-                            (uint32_t)(2 * 8 / g.nv), box_rows)) {
+  if (kspace_uses_tma(g.nx)) {
+    // k-space pass tiles: nx rows (jx) of 8 complex = 16 doubles of `work`, and the matching 8 / nv phi~ values per row
+    const uint64_t row_w = (uint64_t)g.nyl * g.q() * 2, row_p = (uint64_t)g.nyl * (g.nz / 2) * 2;   // doubles per jx row
+    const uint32_t box_rows = (uint32_t)(g.nx < 256 ? g.nx : 256);                         // TMA box limit; 512 = two boxes
+    if (!make_tensor_map_2d(&ctx->b.tm_work, ctx->b.kbuf, row_w, (uint64_t)g.nx, row_w * 8, 16, box_rows) ||
+        !make_tensor_map_2d(&ctx->b.tm_phik, ctx->b.phik, row_p, (uint64_t)g.nx, row_p * 8, (uint32_t)(2 * 8 / g.nv), box_rows)) {
       delete ctx;
       return RISM3D_ERR_CUDA;
     }
   }
+  if (g.n_ranks > 1) {
+    // staged exchange until rism3d_slab_set_peers: block d of the staging array takes the rows of rank d's slab on the
+    // way in and holds the rows that came back from rank d on the way out; the Gram row goes into this rank's own array
+    const size_t blk = (size_t)g.nxl * g.nyl * g.q();
+    for (int r = 0; r < g.n_ranks; ++r) {
+      ctx->b.fwd_dst[r] = ctx->b.stage + (size_t)r * blk;
+      ctx->b.bwd_src[r] = ctx->b.stage + (size_t)r * blk;
+    }
+    ctx->b.gram_dst[0] = ctx->b.gram_x;
+    ctx->b.n_gram_dst = 1;
+    ctx->b.peer_mode = false;
+  }
   cudaError_t e = cudaMallocHost((void**)&ctx->h_hdr, sizeof(StateHeader));
+  if (e == cudaSuccess && g.n_ranks > 1) e = cudaMemsetAsync(ctx->b.gram_x, 0, (size_t)MAX_RANKS * GRAM_SLOT * 16, ctx->stream);
+  if (e == cudaSuccess && g.n_ranks > 1) e = cudaMemsetAsync(ctx->b.xflags, 0, (MAX_RANKS + 1) * sizeof(unsigned long long), ctx->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->b.tw, tw.data(), tw.size() * 8, cudaMemcpyHostToDevice, ctx->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(ctx->b.state, 0, sizeof(DevState), ctx->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(ctx->b.tickets, 0, ctx->b.n_tickets * sizeof(unsigned), ctx->stream);
@@ -295,8 +340,8 @@ extern "C" int rism3d_set_solvent_chi(rism3d_ctx* ctx, const double* q, const do
   double neutral = 0.0;
   for (int i = 0; i < nu; ++i) neutral += rho[i] * q[i];
   if (fabs(neutral) > 1e-12) return fail(ctx, RISM3D_ERR_NEUTRAL, "sum rho_g q_g = %.3e", neutral);
-  const double dkg = 2.0 * M_PI / (g.n * g.h);
-  const double kmin = dkg * sqrt(0.75), kmax = dkg * sqrt(2.0 * (n_shells(g.n) - 1) + 0.75);
+  const double dkg = 2.0 * M_PI / (g.nmax * g.h), quarter_w = 0.25 * (g.wx + g.wy + g.wz);
+  const double kmin = dkg * sqrt(quarter_w), kmax = dkg * sqrt(2.0 * (g.nshell - 1) + quarter_w);
   if ((kmin - k0) / dk < 0.0 || (kmax - k0) / dk > (double)(n_k - 1))
     return fail(ctx, RISM3D_ERR_CHI_RANGE, "table covers [%.4f, %.4f], grid needs [%.4f, %.4f]", k0,
                 k0 + (n_k - 1) * dk, kmin, kmax);
@@ -418,7 +463,7 @@ extern "C" int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz
   const std::vector<double>& up_atoms = cells ? atoms_s : atoms;
   const std::vector<double>& up_pair = cells ? pair_s : pair;
   const size_t b_atoms = align256((na * 5) * 8 + 8), b_pair = align256(pair.size() * 8 + 8);
-  const size_t b_phase = align256((size_t)3 * na * g.n * 16 + 16);
+  const size_t b_phase = align256((size_t)3 * na * g.nmax * 16 + 16);
   const size_t b_cells = align256(cell_start.size() * sizeof(int) + 8);
   if (b_atoms + b_pair + b_phase + b_cells > ctx->scratch_bytes)
     return fail(ctx, RISM3D_ERR_WORKSPACE, "%d atoms need %zu scratch bytes, workspace has %zu", n_atoms,
@@ -516,17 +561,24 @@ static int enqueue_iteration(rism3d_ctx* ctx) {
   const Grid& g = ctx->g;
   const Buffers& b = ctx->b;
   cudaStream_t s = ctx->stream;
+  const bool peers = g.n_ranks > 1;                        // (rism3d_iterate only gets here in peer mode)
   int k = 0;
   prof_mark(ctx);
   k += launch_closure_zfwd(g, b, ctx->sp, nullptr, s);     // step 2 + z of step 3
   prof_mark(ctx);
-  k += launch_y_fwd(g, b, true, s);                        // step 3
+  k += launch_y_fwd(g, b, true, s);                        // step 3 (slab run: stores into the peers' k-space slabs)
+  if (peers) k += launch_xbarrier(g, b, s);
   prof_mark(ctx);
   k += launch_kspace_x(g, b, s);                           // step 3 (x), Eq. 32, step 4, x of step 5
+  if (peers) k += launch_xbarrier(g, b, s);
   prof_mark(ctx);
-  k += launch_y_inv(g, b, true, s);                        // step 5
+  k += launch_y_inv(g, b, true, s);                        // step 5 (slab run: loads from the peers' k-space slabs)
   prof_mark(ctx);
   k += launch_zinv_residual(g, b, ctx->sp, nullptr, s);    // step 5 (z), Eq. 33, steps 6-7: Gram row, rms test, MDIIS solve
+  if (peers) {
+    k += launch_xbarrier(g, b, s);                         // every rank's Gram row has arrived; nobody reads K any more
+    k += launch_gram_solve(g, b, ctx->sp, s);
+  }
   prof_mark(ctx);                                          // (the update tau = sum c_i Z_i is applied by the next
                                                            //  closure_zfwd, or by iterate's trailing update pass)
   ctx->launches += k;
@@ -615,6 +667,8 @@ extern "C" int rism3d_iterate(rism3d_ctx* ctx, int max_iter, double tol, int* n_
   ON_CTX_DEVICE(ctx);
   if (max_iter < 0) return fail(ctx, RISM3D_ERR_ARG, "max_iter < 0");
   if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before iterate");
+  if (ctx->g.n_ranks > 1 && !ctx->b.peer_mode)
+    return fail(ctx, RISM3D_ERR_ORDER, "a staged slab run is driven by rism3d_slab_phase (or call rism3d_slab_set_peers)");
   iterate_begin_kernel<<<1, 1, 0, ctx->stream>>>(ctx->b.state, tol);
   ctx->launches += 1;
   // packs of GRAPH_PACK iterations (one graph launch each) with a look at the device state in between when a
@@ -722,7 +776,7 @@ extern "C" int rism3d_pmv(rism3d_ctx* ctx, double chi_t, double* pmv, double* c_
     sum += ctx->rhov[i] * host[MAX_NV + i];
     if (c_int_site) c_int_site[i] = host[MAX_NV + i];
   }
-  *pmv = ctx->sp.kT * chi_t * (1.0 - sum);           // Eq. 19
+  *pmv = ctx->sp.kT * chi_t * ((ctx->g.rank == 0 ? 1.0 : 0.0) - sum);   // Eq. 19 (slab run: this slab's share)
   return RISM3D_OK;
 }
 
@@ -823,11 +877,129 @@ extern "C" int rism3d_get_rms_history(rism3d_ctx* ctx, double* dst, int cap, int
   return RISM3D_OK;
 }
 
+extern "C" int rism3d_slab_plan(const rism3d_params* p, rism3d_slab_info* out) {
+  if (!p || !out) return RISM3D_ERR_ARG;
+  if (!valid_params(p)) return RISM3D_ERR_SIZE;
+  const Grid g = make_grid(p);
+  out->nxl = g.nxl; out->ix0 = g.ix0; out->nyl = g.nyl; out->jy0 = g.jy0;
+  out->n_sites_padded = g.nv;
+  out->row_elems = g.q();
+  out->block_elems = (size_t)g.nxl * g.nyl * g.q();
+  return RISM3D_OK;
+}
+
+// ---- slab decomposition: exchange addresses, peer tables, phase calls (include/rism3d.h "Slab decomposition") ----
+extern "C" int rism3d_slab_local(rism3d_ctx* ctx, void** d_K, void** d_stage, void** d_gram, void** d_flags,
+                                 size_t* block_bytes, size_t* gram_row_bytes) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  const Grid& g = ctx->g;
+  if (g.n_ranks <= 1) return fail(ctx, RISM3D_ERR_ORDER, "not a slab run (rism3d_params.n_ranks <= 1)");
+  if (d_K) *d_K = ctx->b.kbuf;
+  if (d_stage) *d_stage = ctx->b.stage;
+  if (d_gram) *d_gram = ctx->b.gram_x;
+  if (d_flags) *d_flags = ctx->b.xflags;
+  if (block_bytes) *block_bytes = (size_t)g.nxl * g.nyl * g.q() * sizeof(double2);
+  if (gram_row_bytes) *gram_row_bytes = (size_t)GRAM_SLOT * 2 * sizeof(double);
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_slab_set_peers(rism3d_ctx* ctx, void* const* d_K, void* const* d_gram, void* const* d_flags) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
+  Grid& g = ctx->g;
+  if (g.n_ranks <= 1) return fail(ctx, RISM3D_ERR_ORDER, "not a slab run (rism3d_params.n_ranks <= 1)");
+  if (!d_K || !d_gram || !d_flags) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
+  for (int r = 0; r < g.n_ranks; ++r)
+    if (!d_K[r] || !d_gram[r] || !d_flags[r]) return fail(ctx, RISM3D_ERR_ARG, "peer %d: NULL pointer", r);
+  if (d_K[g.rank] != (void*)ctx->b.kbuf || d_gram[g.rank] != (void*)ctx->b.gram_x || d_flags[g.rank] != (void*)ctx->b.xflags)
+    return fail(ctx, RISM3D_ERR_ARG, "entry %d must be this rank's own arrays (rism3d_slab_local)", g.rank);
+  CU(cudaStreamSynchronize(ctx->stream));
+  // rank r's rows of the spectrum sit in block `rank` of rank r's K: stores on the way in, loads on the way out
+  const size_t blk = (size_t)g.nxl * g.nyl * g.q();
+  for (int r = 0; r < g.n_ranks; ++r) {
+    ctx->b.fwd_dst[r] = (double2*)d_K[r] + (size_t)g.rank * blk;
+    ctx->b.bwd_src[r] = (const double2*)d_K[r] + (size_t)g.rank * blk;
+    ctx->b.gram_dst[r] = (double*)d_gram[r];
+    ctx->b.flag_dst[r] = (unsigned long long*)d_flags[r];
+  }
+  ctx->b.n_gram_dst = g.n_ranks;
+  ctx->b.peer_mode = true;
+  // graphs captured before the switch hold the old tables
+  if (ctx->graph1) { cudaGraphExecDestroy(ctx->graph1); ctx->graph1 = nullptr; }
+  if (ctx->graph_pack) { cudaGraphExecDestroy(ctx->graph_pack); ctx->graph_pack = nullptr; }
+  ctx->graph_tried = false;
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_slab_begin(rism3d_ctx* ctx, double tol) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
+  if (ctx->g.n_ranks <= 1) return fail(ctx, RISM3D_ERR_ORDER, "not a slab run (rism3d_params.n_ranks <= 1)");
+  if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before the iteration");
+  iterate_begin_kernel<<<1, 1, 0, ctx->stream>>>(ctx->b.state, tol);
+  ctx->launches += 1;
+  CU(cudaGetLastError());
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_slab_phase(rism3d_ctx* ctx, int phase) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
+  const Grid& g = ctx->g;
+  if (g.n_ranks <= 1) return fail(ctx, RISM3D_ERR_ORDER, "not a slab run (rism3d_params.n_ranks <= 1)");
+  if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before the iteration");
+  cudaStream_t s = ctx->stream;
+  int k = 0;
+  switch (phase) {
+    case 0:
+      k += launch_closure_zfwd(g, ctx->b, ctx->sp, nullptr, s);
+      k += launch_y_fwd(g, ctx->b, true, s);
+      break;
+    case 1: k += launch_kspace_x(g, ctx->b, s); break;
+    case 2:
+      k += launch_y_inv(g, ctx->b, true, s);
+      k += launch_zinv_residual(g, ctx->b, ctx->sp, nullptr, s);
+      break;
+    case 3: k += launch_gram_solve(g, ctx->b, ctx->sp, s); break;
+    default: return fail(ctx, RISM3D_ERR_ARG, "phase %d (0..3)", phase);
+  }
+  ctx->launches += k;
+  CU(cudaGetLastError());
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_slab_status(rism3d_ctx* ctx, int* done, int* n_done, double* rms) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
+  int rc = read_header(ctx);
+  if (rc) return rc;
+  if (done) *done = ctx->h_hdr->done;
+  if (n_done) *n_done = ctx->h_hdr->n_done;
+  if (rms) *rms = ctx->h_hdr->rms_last;
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_slab_end(rism3d_ctx* ctx, int* n_done, double* rms) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
+  if (ctx->g.n_ranks <= 1) return fail(ctx, RISM3D_ERR_ORDER, "not a slab run (rism3d_params.n_ranks <= 1)");
+  ctx->launches += launch_mdiis_update(ctx->g, ctx->b, ctx->sp, ctx->stream);   // no-op when nothing is pending
+  CU(cudaGetLastError());
+  int rc = read_header(ctx);
+  if (rc) return rc;
+  if (n_done) *n_done = ctx->h_hdr->n_done;
+  if (rms) *rms = ctx->h_hdr->rms_last;
+  if (ctx->h_hdr->status == RISM3D_ERR_DIVERGED)
+    return fail(ctx, RISM3D_ERR_DIVERGED, "non-finite residual after %d iterations", ctx->h_hdr->n_done);
+  return RISM3D_OK;
+}
+
 extern "C" int rism3d_debug_fft_forward(rism3d_ctx* ctx, const double* d_in, double* d_out) {
   if (!ctx) return RISM3D_ERR_ARG;
   ON_CTX_DEVICE(ctx);
   if (!d_in || !d_out) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   const Grid& g = ctx->g;
+  if (g.n_ranks > 1) return fail(ctx, RISM3D_ERR_ORDER, "the debug transforms are single-rank only");
   int k = launch_closure_zfwd(g, ctx->b, ctx->sp, d_in, ctx->stream);
   k += launch_y_fwd(g, ctx->b, false, ctx->stream);
   k += launch_x_fwd(g, ctx->b, ctx->stream);
@@ -843,6 +1015,7 @@ extern "C" int rism3d_debug_fft_inverse(rism3d_ctx* ctx, const double* d_in, dou
   ON_CTX_DEVICE(ctx);
   if (!d_in || !d_out) return fail(ctx, RISM3D_ERR_ARG, "bad argument");
   const Grid& g = ctx->g;
+  if (g.n_ranks > 1) return fail(ctx, RISM3D_ERR_ORDER, "the debug transforms are single-rank only");
   CU(cudaMemcpyAsync(ctx->b.work, d_in, g.field * 8, cudaMemcpyDeviceToDevice, ctx->stream));
   int k = launch_x_inv(g, ctx->b, ctx->stream);
   k += launch_y_inv(g, ctx->b, false, ctx->stream);

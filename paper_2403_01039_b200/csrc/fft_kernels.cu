@@ -40,10 +40,21 @@ struct StridedCfg {
          MINB = (SHM > 110 * 1024) ? 1 : 2 };      // <= 128 registers per thread: room for the cached twiddles
 };
 
+// Slab-decomposed runs (Grid::n_ranks > 1): the y lines of one x plane are complete in r space, but the rows j_y of the
+// spectrum belong to the rank that transforms them along x.  Row j of plane ix_l lives at
+//   base[j >> shift] + (ix_l * nyl + (j & mask)) * es          (+ the column offset inside the row)
+// -- the forward pass WRITES its rows there (the transpose of PAPER.md:318-322 happens in its stores: a staging block
+// per destination rank, or the destination's own array over NVLink), the inverse pass READS them from there.
+struct RowMap {
+  cplx* base[MAX_RANKS];
+  int shift, mask, nyl;
+};
+
 // stage work item `item` (G tiles) into `buf` [G][N][COLS]
-// (INV: row j goes to the slot the first inverse stage reads it from in place)
-template <int N, bool INV>
-__device__ __forceinline__ void stage_strided(cplx* buf, const cplx* data, const LineGeom& g, size_t item, int tid) {
+// (INV: row j goes to the slot the first inverse stage reads it from in place; SLAB: rows come through the row map)
+template <int N, bool INV, bool SLAB>
+__device__ __forceinline__ void stage_strided(cplx* buf, const cplx* data, const LineGeom& g, const RowMap& rm,
+                                              size_t item, int tid) {
   using Cfg = FftCfg<N>;
   constexpr int NT = StridedCfg<N>::NT, C = COLS;
 #pragma unroll
@@ -51,17 +62,22 @@ __device__ __forceinline__ void stage_strided(cplx* buf, const cplx* data, const
     const int idx = tid + k * NT;
     const int grp = idx / (N * C), rem = idx % (N * C), row = rem / C, col = rem % C;
     const size_t chunk = item * Cfg::G + grp;
-    const cplx* src = data + (chunk / g.chunks_per_outer) * g.outer_stride + (chunk % g.chunks_per_outer) * C +
-                      (size_t)row * g.es + col;
+    const cplx* src;
+    if constexpr (SLAB && INV)
+      src = rm.base[row >> rm.shift] + ((chunk / g.chunks_per_outer) * rm.nyl + (size_t)(row & rm.mask)) * g.es +
+            (chunk % g.chunks_per_outer) * C + col;
+    else
+      src = data + (chunk / g.chunks_per_outer) * g.outer_stride + (chunk % g.chunks_per_outer) * C +
+            (size_t)row * g.es + col;
     constexpr int RL = (Cfg::R3 == 1) ? Cfg::R2 : Cfg::R3;
     const int slot = INV ? inv_first_slot<N, RL, Cfg::R1>(row) : row;
     cp_async16(buf + (grp * N + slot) * C + col, src);
   }
 }
 
-template <int N, bool INV>
+template <int N, bool INV, bool SLAB>
 __global__ void __launch_bounds__(StridedCfg<N>::NT, StridedCfg<N>::MINB)
-    fft_strided_kernel(cplx* __restrict__ data, LineGeom g, Twiddle tw, const DevState* __restrict__ st,
+    fft_strided_kernel(cplx* __restrict__ data, LineGeom g, RowMap rm, Twiddle tw, const DevState* __restrict__ st,
                        unsigned nitems) {
   if (st != nullptr && st->done) return;
   using Cfg = FftCfg<N>;
@@ -75,23 +91,27 @@ __global__ void __launch_bounds__(StridedCfg<N>::NT, StridedCfg<N>::MINB)
   w.init(t, tw);
   int b = 0;
   size_t item = blockIdx.x;
-  if (item < nitems) stage_strided<N, INV>(smem_dyn, data, g, item, tid);
+  if (item < nitems) stage_strided<N, INV, SLAB>(smem_dyn, data, g, rm, item, tid);
   cp_async_commit();
   for (; item < nitems; item += gridDim.x) {
     const size_t next = item + gridDim.x;
-    if (next < nitems) stage_strided<N, INV>(smem_dyn + (b ^ 1) * ITEM, data, g, next, tid);
+    if (next < nitems) stage_strided<N, INV, SLAB>(smem_dyn + (b ^ 1) * ITEM, data, g, rm, next, tid);
     cp_async_commit();
     cp_async_wait<1>();
     __syncthreads();
     cplx* sm = smem_dyn + b * ITEM + grp * (N * C) + col;
     const size_t chunk = item * Cfg::G + grp;
-    cplx* base = data + (chunk / g.chunks_per_outer) * g.outer_stride + (chunk % g.chunks_per_outer) * C + col;
+    const size_t plane = chunk / g.chunks_per_outer, inrow = (chunk % g.chunks_per_outer) * C + col;
+    cplx* base = data + plane * g.outer_stride + inrow;
     auto ld_sm = [&](int i) { return sm[i * C]; };
     auto st_sm = [&](int i, cplx v) { sm[i * C] = v; };
     if (!INV) {
       fwd_a_c(t, w, tw, ld_sm, st_sm);
       __syncthreads();
-      auto out = [&](int j, cplx v) { base[j * es] = v; };
+      auto out = [&](int j, cplx v) {
+        if constexpr (SLAB) rm.base[j >> rm.shift][(plane * rm.nyl + (size_t)(j & rm.mask)) * es + inrow] = v;
+        else base[j * es] = v;
+      };
       if constexpr (R3 != 1) {
         fwd_mid_c(t, w, ld_sm, st_sm);
         __syncthreads();
@@ -116,28 +136,37 @@ __global__ void __launch_bounds__(StridedCfg<N>::NT, StridedCfg<N>::MINB)
 template <int N, bool INV>
 static int launch_strided_n(const Grid& gr, const Buffers& b, bool x_axis, bool use_state, cudaStream_t s) {
   using Cfg = FftCfg<N>;
-  const size_t Q = (size_t)(gr.n / 2) * gr.nv;
+  const size_t Q = gr.q();
   LineGeom g;
   size_t nchunks;
-  if (x_axis) {
+  if (x_axis) {                                          // lines along x of [nx][nyl][Q] (N = nx)
     g.outer_stride = 0;
-    g.es = (size_t)gr.n * Q;
-    g.chunks_per_outer = (unsigned)((size_t)gr.n * Q / COLS);
+    g.es = (size_t)gr.nyl * Q;
+    g.chunks_per_outer = (unsigned)((size_t)gr.nyl * Q / COLS);
     nchunks = g.chunks_per_outer;
-  } else {
-    g.outer_stride = (size_t)gr.n * Q;
+  } else {                                               // lines along y of [nxl][ny][Q] (N = ny)
+    g.outer_stride = (size_t)gr.ny * Q;
     g.es = Q;
     g.chunks_per_outer = (unsigned)(Q / COLS);
-    nchunks = (size_t)gr.n * g.chunks_per_outer;
+    nchunks = (size_t)gr.nxl * g.chunks_per_outer;
   }
   const unsigned nitems = (unsigned)(nchunks / Cfg::G);
   const size_t shm = StridedCfg<N>::SHM;
-  auto kern = fft_strided_kernel<N, INV>;
+  const bool slab = gr.n_ranks > 1 && !x_axis;
+  RowMap rm{};
+  if (slab) {
+    rm.nyl = gr.nyl;
+    rm.mask = gr.nyl - 1;
+    rm.shift = 0;
+    while ((1 << rm.shift) < gr.nyl) ++rm.shift;
+    for (int r = 0; r < gr.n_ranks; ++r) rm.base[r] = INV ? const_cast<cplx*>(b.bwd_src[r]) : b.fwd_dst[r];
+  }
+  auto kern = slab ? fft_strided_kernel<N, INV, true> : fft_strided_kernel<N, INV, false>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm) != cudaSuccess) return 0;
-  Twiddle tw{b.tw, 1, 2 * gr.n - 1};
+  Twiddle tw{b.tw, gr.nmax / N, 2 * gr.nmax - 1};
   unsigned grid = (unsigned)(gr.num_sms * StridedCfg<N>::MINB);
   if (grid > nitems) grid = nitems;
-  kern<<<grid, StridedCfg<N>::NT, shm, s>>>(b.work, g, tw, use_state ? b.state : nullptr, nitems);
+  kern<<<grid, StridedCfg<N>::NT, shm, s>>>(b.work, g, rm, tw, use_state ? b.state : nullptr, nitems);
   return 1;
 }
 
@@ -156,28 +185,28 @@ static int launch_strided_n(const Grid& gr, const Buffers& b, bool x_axis, bool 
 int launch_y_fwd(const Grid& g, const Buffers& b, bool use_state, cudaStream_t s) {
   int k = 0;
 #define CALL(N) k = launch_strided_n<N, false>(g, b, false, use_state, s)
-  R3D_DISPATCH_N(g.n, CALL)
+  R3D_DISPATCH_N(g.ny, CALL)
 #undef CALL
   return k;
 }
 int launch_y_inv(const Grid& g, const Buffers& b, bool use_state, cudaStream_t s) {
   int k = 0;
 #define CALL(N) k = launch_strided_n<N, true>(g, b, false, use_state, s)
-  R3D_DISPATCH_N(g.n, CALL)
+  R3D_DISPATCH_N(g.ny, CALL)
 #undef CALL
   return k;
 }
 int launch_x_fwd(const Grid& g, const Buffers& b, cudaStream_t s) {
   int k = 0;
 #define CALL(N) k = launch_strided_n<N, false>(g, b, true, false, s)
-  R3D_DISPATCH_N(g.n, CALL)
+  R3D_DISPATCH_N(g.nx, CALL)
 #undef CALL
   return k;
 }
 int launch_x_inv(const Grid& g, const Buffers& b, cudaStream_t s) {
   int k = 0;
 #define CALL(N) k = launch_strided_n<N, true>(g, b, true, false, s)
-  R3D_DISPATCH_N(g.n, CALL)
+  R3D_DISPATCH_N(g.nx, CALL)
 #undef CALL
   return k;
 }
@@ -326,12 +355,13 @@ static int launch_closure_zfwd_n(const Grid& gr, const Buffers& b, const SolverP
   using Cfg = ZPlan<NZ>;
   constexpr int G = ZPlan<NZ>::GF;
   const int LP = COLS / gr.nv, GL = G * LP;
-  const size_t nlines = (size_t)gr.n * gr.n;
+  const size_t nlines = (size_t)gr.nxl * gr.ny;
   const int threads = Cfg::T * G * COLS;
   const size_t shm = (size_t)G * NZ * ZP * sizeof(cplx);
   auto kern = sp.dyn_b ? closure_zfwd_kernel<NZ, G, ZPlan<NZ>::MBF, true> : closure_zfwd_kernel<NZ, G, ZPlan<NZ>::MBF, false>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm) != cudaSuccess) return 0;
-  Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
+  const int ez = gr.nmax / gr.nz;
+  Twiddle tws{b.tw, ez, 2 * gr.nmax - 1}, tw{b.tw, 2 * ez, 2 * gr.nmax - 1};
   kern<<<(unsigned)(nlines / GL), threads, shm, s>>>(b.tau, b.w, raw, b.Z, b.R, b.work, tws, tw, b.state, gr.nv,
                                                        gr.npts, gr.field, sp.closure, sp.pse_order);
   return 1;
@@ -339,7 +369,7 @@ static int launch_closure_zfwd_n(const Grid& gr, const Buffers& b, const SolverP
 
 int launch_closure_zfwd(const Grid& g, const Buffers& b, const SolverParams& sp, const double* raw, cudaStream_t s) {
   int k = 0;
-  switch (g.n / 2) {
+  switch (g.nz / 2) {
     case 4: k = launch_closure_zfwd_n<4>(g, b, sp, raw, s); break;
     case 8: k = launch_closure_zfwd_n<8>(g, b, sp, raw, s); break;
     case 16: k = launch_closure_zfwd_n<16>(g, b, sp, raw, s); break;
@@ -365,6 +395,7 @@ struct GramArgs {
   const double* weight;  // [nv] weights 1/rho_g of the modified Anderson inner product (Eq. 38); unused otherwise
   double n_values;       // grid points x site types of the caller: the N n_v of Eq. 41 (phantom types do not count)
   AccelArgs aa;
+  GramExchange xr;       // slab runs: where this rank's row goes (mdiis_device.cuh)
 };
 
 template <int NZ, int G, int MINB, int MAXO, bool WEIGHTED>
@@ -502,8 +533,20 @@ __global__ void __launch_bounds__(ZPlan<NZ>::T* G* COLS, MINB)
       *reinterpret_cast<double2*>(ga.part1 + ((size_t)j * gridDim.x + blockIdx.x) * 2) = make_double2(hi, lo);
       __threadfence();
     }
-    gram_finish<NT>(st, ga.part1, ga.part2, ga.tickets, s_m, nother, ga.aa, WEIGHTED, ga.n_values, s_row, &s_flag, s_solve);
+    gram_finish<NT>(st, ga.part1, ga.part2, ga.tickets, s_m, nother, ga.aa, WEIGHTED, ga.n_values, s_row, &s_flag, s_solve,
+                    ga.xr);
   }
+}
+
+static AccelArgs accel_args(const SolverParams& sp) {
+  return AccelArgs{sp.M, sp.restart, sp.accel, sp.and_s1, sp.and_s2, sp.b_min, sp.dyn_b ? sp.b_max : 0.0};
+}
+static GramExchange gram_exchange(const Grid& gr, const Buffers& b) {
+  GramExchange xr{};
+  xr.rank = gr.rank;
+  xr.n_dst = gr.n_ranks > 1 ? b.n_gram_dst : 0;
+  for (int d = 0; d < xr.n_dst; ++d) xr.dst[d] = b.gram_dst[d];
+  return xr;
 }
 
 template <int NZ, int MAXO, bool WEIGHTED>
@@ -518,11 +561,12 @@ static int launch_zinv_nm(const Grid& gr, const Buffers& b, const SolverParams& 
   if (shm < red) shm = red;
   auto kern = zinv_residual_kernel<NZ, G, MB, MAXO, WEIGHTED>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm) != cudaSuccess) return 0;
-  Twiddle tws{b.tw, 1, 2 * gr.n - 1}, tw{b.tw, 2, 2 * gr.n - 1};
-  GramArgs ga{b.gram_part, b.gram_part2, b.tickets, b.gram_w, (double)gr.npts * gr.nv_user,
-              AccelArgs{sp.M, sp.restart, sp.accel, sp.and_s1, sp.and_s2, sp.b_min, sp.dyn_b ? sp.b_max : 0.0}};
+  const int ez = gr.nmax / gr.nz;
+  Twiddle tws{b.tw, ez, 2 * gr.nmax - 1}, tw{b.tw, 2 * ez, 2 * gr.nmax - 1};
+  GramArgs ga{b.gram_part, b.gram_part2, b.tickets, b.gram_w, (double)gr.npts_global * gr.nv_user, accel_args(sp),
+              gram_exchange(gr, b)};
   // (dynamic damping: the Z slot takes X itself -- X + 0 R is exact -- and the update applies the current b)
-  kern<<<(unsigned)((size_t)gr.n * gr.n / GL), threads, shm, s>>>(b.work, b.tau, b.Z, b.R, raw_out, tws, tw, b.state,
+  kern<<<(unsigned)((size_t)gr.nxl * gr.ny / GL), threads, shm, s>>>(b.work, b.tau, b.Z, b.R, raw_out, tws, tw, b.state,
                                                                    gr.nv, gr.npts, gr.field, sp.dyn_b ? 0.0 : sp.b, ga);
   return 1;
 }
@@ -545,10 +589,10 @@ static int launch_zinv_n(const Grid& gr, const Buffers& b, const SolverParams& s
 template <int NZ>
 static int zinv_ctas_n(const Grid& gr) {
   const int LP = COLS / gr.nv, GL = ZPlan<NZ>::GI * LP;
-  return (int)((size_t)gr.n * gr.n / GL);
+  return (int)((size_t)gr.nxl * gr.ny / GL);
 }
 int zinv_ctas(const Grid& g) {
-  switch (g.n / 2) {
+  switch (g.nz / 2) {
     case 4: return zinv_ctas_n<4>(g);
     case 8: return zinv_ctas_n<8>(g);
     case 16: return zinv_ctas_n<16>(g);
@@ -562,7 +606,7 @@ int zinv_ctas(const Grid& g) {
 
 int launch_zinv_residual(const Grid& g, const Buffers& b, const SolverParams& sp, double* raw_out, cudaStream_t s) {
   int k = 0;
-  switch (g.n / 2) {
+  switch (g.nz / 2) {
     case 4: k = launch_zinv_n<4>(g, b, sp, raw_out, s); break;
     case 8: k = launch_zinv_n<8>(g, b, sp, raw_out, s); break;
     case 16: k = launch_zinv_n<16>(g, b, sp, raw_out, s); break;
@@ -573,6 +617,71 @@ int launch_zinv_residual(const Grid& g, const Buffers& b, const SolverParams& sp
     default: break;
   }
   return k;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Slab-decomposed runs: the second half of the MDIIS step.  gram_x holds one row of double-double totals per rank
+// (written by the last-arriving CTA of every rank's zinv_residual, moved by the caller's all-gather or stored straight
+// into the peers' arrays); one warp adds them in rank order and runs the same bookkeeping and solve as a single rank.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(32)
+    gram_solve_kernel(DevState* __restrict__ st, const double* __restrict__ gram_x, int n_ranks, AccelArgs aa,
+                      int weighted, double n_values) {
+  if (st->done) return;
+  __shared__ SolveScratch s_solve;
+  __shared__ double s_row[MAX_M + 2];
+  const int lane = threadIdx.x;
+  const int m = st->m;
+  const int nother = m - ((m == aa.M) ? 1 : 0);          // as zinv_residual saw it: a full history drops its oldest entry
+  const int nent = nother + (weighted ? 2 : 1);
+  if (lane < nent) {
+    double hi = 0.0, lo = 0.0;
+    for (int r = 0; r < n_ranks; ++r) {
+      const double2 p = __ldcg(reinterpret_cast<const double2*>(gram_x) + (size_t)r * GRAM_SLOT + lane);
+      dd_add(hi, lo, p.x, p.y);
+    }
+    s_row[lane] = hi + lo;
+  }
+  __syncwarp();
+  mdiis_bookkeeping_and_solve(st, s_solve, s_row, m, nother, aa, weighted ? s_row[nother + 1] : s_row[nother], n_values);
+}
+
+int launch_gram_solve(const Grid& gr, const Buffers& b, const SolverParams& sp, cudaStream_t s) {
+  gram_solve_kernel<<<1, 32, 0, s>>>(b.state, b.gram_x, gr.n_ranks, accel_args(sp), sp.accel == RISM3D_ACCEL_ANDERSON ? 1 : 0,
+                                     (double)gr.npts_global * gr.nv_user);
+  return 1;
+}
+
+// In-stream barrier across the ranks of a peer-mapped slab run: every rank stores its next epoch into slot `rank` of
+// every rank's flag array (release, system scope: the stores of the kernels before it in the stream are visible to
+// whoever sees the flag) and waits until all slots of its own array have reached that epoch.  All ranks enqueue the same
+// sequence of kernels, so epochs agree without any host involvement; the kernel is graph-capturable.
+struct FlagPtrs { unsigned long long* p[MAX_RANKS]; };
+__global__ void __launch_bounds__(32)
+    xbarrier_kernel(unsigned long long* __restrict__ mine, FlagPtrs peers, int n_ranks, int rank) {
+  __shared__ unsigned long long s_epoch;
+  const int lane = threadIdx.x;
+  if (lane == 0) {
+    s_epoch = mine[MAX_RANKS] + 1;
+    mine[MAX_RANKS] = s_epoch;
+  }
+  __syncwarp();
+  const unsigned long long epoch = s_epoch;
+  __threadfence_system();
+  if (lane < n_ranks) {
+    asm volatile("st.release.sys.global.u64 [%0], %1;\n" ::"l"(peers.p[lane] + rank), "l"(epoch) : "memory");
+    unsigned long long seen;
+    do {
+      asm volatile("ld.acquire.sys.global.u64 %0, [%1];\n" : "=l"(seen) : "l"(mine + lane) : "memory");
+    } while (seen < epoch);
+  }
+}
+
+int launch_xbarrier(const Grid& gr, const Buffers& b, cudaStream_t s) {
+  FlagPtrs fp{};
+  for (int r = 0; r < gr.n_ranks; ++r) fp.p[r] = b.flag_dst[r];
+  xbarrier_kernel<<<1, 32, 0, s>>>(b.xflags, fp, gr.n_ranks, gr.rank);
+  return 1;
 }
 
 }  // namespace r3d

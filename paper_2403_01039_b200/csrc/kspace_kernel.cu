@@ -18,6 +18,22 @@ namespace r3d {
 extern __shared__ __align__(128) double2 smem_dyn[];
 constexpr int COLS = 8;
 
+// geometry of the k-space slab this context transforms along x: work is [nx][nyl][nzh][nv] complex, row jy_l stands for
+// j_y = jy0 + jy_l of the whole grid (nyl = ny, jy0 = 0 without a slab decomposition)
+struct KGeom {
+  int nzh;               // nz / 2 stored j_z = 2p
+  int nyl, jy0;
+  int ny, nz;            // whole-grid lengths: folded index j' = j < n/2 ? j : n - 1 - j
+  int wx, wy, wz;        // weights of the shell index (Grid)
+  __device__ __forceinline__ int s_yz(int jy_l, int p) const {
+    const int jy = jy0 + jy_l;
+    const int jyf = 2 * jy < ny ? jy : ny - 1 - jy;
+    const int jzf = 4 * p < nz ? 2 * p : nz - 1 - 2 * p;
+    return wy * jyf * (jyf + 1) + wz * jzf * (jzf + 1);
+  }
+};
+static KGeom make_kgeom(const Grid& g) { return KGeom{g.nz / 2, g.nyl, g.jy0, g.ny, g.nz, g.wx, g.wy, g.wz}; }
+
 // shared-memory layout of one pipeline stage: [G][N][COLS] data tile, then [G][N][COLS/NV] phi~ values
 template <int N, int NV>
 struct KspaceCfg {
@@ -60,11 +76,12 @@ __device__ __forceinline__ cplx kspace_point(cplx csr, cplx ph, double qg, const
 }
 
 template <int N, int NV>
-__device__ __forceinline__ void stage_kspace(cplx* buf, const cplx* data, const cplx* phik, size_t item, int tid) {
+__device__ __forceinline__ void stage_kspace(cplx* buf, const cplx* data, const cplx* phik, const KGeom& kg, size_t item,
+                                             int tid) {
   using Cfg = FftCfg<N>;
   using K = KspaceCfg<N, NV>;
-  constexpr int C = COLS, NZ = N / 2, PC = C / NV;
-  constexpr size_t Q = (size_t)NZ * NV, ES = (size_t)N * Q;
+  constexpr int C = COLS, PC = C / NV;
+  const size_t Q = (size_t)kg.nzh * NV, ES = (size_t)kg.nyl * Q;
 #pragma unroll
   for (int k = 0; k < K::ITEM / K::NT; ++k) {
     const int idx = tid + k * K::NT;
@@ -77,9 +94,9 @@ __device__ __forceinline__ void stage_kspace(cplx* buf, const cplx* data, const 
     const int idx = tid + k * K::NT;
     if (idx < K::PHI) {
       const int grp = idx / (N * PC), rem = idx % (N * PC), row = rem / PC, c = rem % PC;
-      const size_t q2 = (item * Cfg::G + grp) * C;       // flattened (jy, p, site) of the tile's first column
+      const size_t q2 = (item * Cfg::G + grp) * C;       // flattened (jy_l, p, site) of the tile's first column
       const size_t jy = q2 / Q, p0 = (q2 % Q) / NV;
-      cp_async16(buf + K::ITEM + idx, phik + (size_t)row * N * NZ + jy * NZ + p0 + c);
+      cp_async16(buf + K::ITEM + idx, phik + ((size_t)row * kg.nyl + jy) * kg.nzh + p0 + c);
     }
   }
 }
@@ -87,16 +104,16 @@ __device__ __forceinline__ void stage_kspace(cplx* buf, const cplx* data, const 
 template <int N, int NV>
 __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
     kspace_x_kernel(cplx* __restrict__ data, const cplx* __restrict__ phik, const double* __restrict__ chi_shell,
-                    const double* __restrict__ qv, Twiddle tw, const DevState* __restrict__ st, unsigned nitems) {
+                    const double* __restrict__ qv, Twiddle tw, const DevState* __restrict__ st, KGeom kg, unsigned nitems) {
   if (st->done) return;
   using Cfg = FftCfg<N>;
   using K = KspaceCfg<N, NV>;
   constexpr int T = Cfg::T, R1 = Cfg::R1, R2 = Cfg::R2, R3 = Cfg::R3, C = COLS;
   constexpr int RL = (R3 == 1) ? R2 : R3;            // radix of the innermost digit
   constexpr int NB = N / RL, RMID = NB / R1;
-  constexpr int NZ = N / 2, PC = C / NV;
-  constexpr size_t Q = (size_t)NZ * NV;              // complex elements per (jx, jy) row
-  constexpr size_t ES = (size_t)N * Q;               // stride of the x axis
+  constexpr int NZ = N / 2, PC = C / NV;             // NZ: folding point of the x index
+  const size_t Q = (size_t)kg.nzh * NV;              // complex elements per (jx, jy) row
+  const size_t ES = (size_t)kg.nyl * Q;              // stride of the x axis
   const int tid = threadIdx.x;
   const int col = tid % C, t = (tid / C) % T, grp = tid / (C * T);
   const int site = col % NV;
@@ -109,11 +126,11 @@ __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
   w.init(t, tw, mid_table);
   int b = 0;
   size_t item = blockIdx.x;
-  if (item < nitems) stage_kspace<N, NV>(smem_dyn, data, phik, item, tid);
+  if (item < nitems) stage_kspace<N, NV>(smem_dyn, data, phik, kg, item, tid);
   cp_async_commit();
   for (; item < nitems; item += gridDim.x) {
     const size_t next = item + gridDim.x;
-    if (next < nitems) stage_kspace<N, NV>(smem_dyn + (b ^ 1) * K::STAGE, data, phik, next, tid);
+    if (next < nitems) stage_kspace<N, NV>(smem_dyn + (b ^ 1) * K::STAGE, data, phik, kg, next, tid);
     cp_async_commit();
     cp_async_wait<1>();
     __syncthreads();
@@ -121,11 +138,7 @@ __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
     const cplx* sph = smem_dyn + b * K::STAGE + K::ITEM + grp * (N * PC) + col / NV;
     const size_t q2 = (item * Cfg::G + grp) * C + col;   // flattened (jy, p, site)
     cplx* base = data + q2;
-    const int jy = (int)(q2 / Q);
-    const int p = (int)((q2 % Q) / NV);
-    const int jyf = jy < NZ ? jy : N - 1 - jy;         // folded indices: |k_axis| = dk (j' + 1/2)
-    const int jzf = (2 * p) < NZ ? 2 * p : N - 1 - 2 * p;
-    const int s_yz = jyf * (jyf + 1) + jzf * (jzf + 1);
+    const int s_yz = kg.s_yz((int)(q2 / Q), (int)((q2 % Q) / NV));   // folded indices: |k_axis| = dk (j' + 1/2)
     auto ld_sm = [&](int i) { return sm[i * C]; };
     auto st_sm = [&](int i, cplx v) { sm[i * C] = v; };
 
@@ -147,7 +160,7 @@ __global__ void __launch_bounds__(KspaceCfg<N, NV>::NT, KspaceCfg<N, NV>::MINB)
       for (int k = 0; k < RL; ++k) {
         const int jx = j0 + NB * k;
         const int jxf = jx < NZ ? jx : N - 1 - jx;
-        const int shell = (jxf * (jxf + 1) + s_yz) >> 1;
+        const int shell = (kg.wx * jxf * (jxf + 1) + s_yz) >> 1;
         x[k] = kspace_point<NV>(x[k], sph[jx * PC], qg, chi_shell + (size_t)shell * (NV * NV) + site * NV);
       }
       Dft<RL, +1>::run(x);                             // first inverse stage; its twiddles are applied by the loads of the next
@@ -274,13 +287,13 @@ template <int N, int NV>
 __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB)
     kspace2_kernel(const __grid_constant__ CUtensorMap tm_work, const __grid_constant__ CUtensorMap tm_phik,
                    const double* __restrict__ chi_shell, const double* __restrict__ qv, Twiddle tw,
-                   const DevState* __restrict__ st, unsigned nitems) {
+                   const DevState* __restrict__ st, KGeom kg, unsigned nitems) {
   if (st->done) return;
   using K = Kspace2Cfg<N, NV>;
   constexpr int R1 = K::R1, R2 = K::R2, T = K::T, C = COLS;
   constexpr int S1 = N / R1, NB = N / R2;            // S1 == T: one pass-A butterfly per thread
-  constexpr int NZ = N / 2, PC = C / NV;
-  constexpr int Q = NZ * NV;                         // complex elements per (jx, jy) row
+  constexpr int NZ = N / 2, PC = C / NV;             // NZ: folding point of the x index
+  const unsigned Q = (unsigned)kg.nzh * NV;          // complex elements per (jx, jy) row
   constexpr int PFMAX = (NV > 4) ? 4 : 8;            // chi rows in flight per thread (a row is NV doubles)
   constexpr int PF = (R2 < PFMAX) ? R2 : PFMAX;
   const int tid = threadIdx.x;
@@ -300,7 +313,7 @@ __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB
     for (int bx = 0; bx < K::NBOX; ++bx) {
       tma_load_2d(stages + b * K::STAGE + bx * K::BOX_ROWS * C, &tm_work, (int)(q0 * 2), bx * K::BOX_ROWS, &bars[b]);
       tma_load_2d(stages + b * K::STAGE + K::ITEM + bx * K::BOX_ROWS * PC, &tm_phik,
-                  (int)((q0 / Q * NZ + (q0 % Q) / NV) * 2), bx * K::BOX_ROWS, &bars[b]);
+                  (int)((q0 / Q * kg.nzh + (q0 % Q) / NV) * 2), bx * K::BOX_ROWS, &bars[b]);
     }
   };
   if (tid == 0) {
@@ -331,14 +344,10 @@ __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB
     auto ld_sm = [&](int i) { return sm[i * C]; };
     auto st_sm = [&](int i, cplx v) { sm[i * C] = v; };
     const unsigned q2 = item * C + col;              // flattened (jy, p, site)
-    const int jy = (int)(q2 / Q);
-    const int p = (int)((q2 % Q) / NV);
-    const int jyf = jy < NZ ? jy : N - 1 - jy;       // folded indices: |k_axis| = dk (j' + 1/2)
-    const int jzf = (2 * p) < NZ ? 2 * p : N - 1 - 2 * p;
-    const int s_yz = jyf * (jyf + 1) + jzf * (jzf + 1);
+    const int s_yz = kg.s_yz((int)(q2 / Q), (int)((q2 % Q) / NV));   // folded indices: |k_axis| = dk (j' + 1/2)
     auto chi_row = [&](int jx) {
       const int jxf = jx < NZ ? jx : N - 1 - jx;
-      return chi_shell + (size_t)((jxf * (jxf + 1) + s_yz) >> 1) * (NV * NV) + site * NV;
+      return chi_shell + (size_t)((kg.wx * jxf * (jxf + 1) + s_yz) >> 1) * (NV * NV) + site * NV;
     };
     mbar_wait(&bars[b], (STAGES == 2) ? ((n_done >> 1) & 1) : (n_done & 1));
 
@@ -399,14 +408,13 @@ __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB
 template <int N, int NV>
 static int launch_kspace2_nv(const Grid& gr, const Buffers& b, cudaStream_t s) {
   using K = Kspace2Cfg<N, NV>;
-  const size_t Q = (size_t)(gr.n / 2) * gr.nv;
-  const unsigned nitems = (unsigned)((size_t)gr.n * Q / COLS);
+  const unsigned nitems = (unsigned)((size_t)gr.nyl * gr.q() / COLS);
   auto kern = kspace2_kernel<N, NV>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SHM) != cudaSuccess) return 0;
-  Twiddle tw{b.tw, 1, 2 * gr.n - 1};
+  Twiddle tw{b.tw, gr.nmax / N, 2 * gr.nmax - 1};
   unsigned grid = (unsigned)(gr.num_sms * K::MINB);
   if (grid > nitems) grid = nitems;
-  kern<<<grid, K::NT, K::SHM, s>>>(b.tm_work, b.tm_phik, b.chi_shell, b.qv, tw, b.state, nitems);
+  kern<<<grid, K::NT, K::SHM, s>>>(b.tm_work, b.tm_phik, b.chi_shell, b.qv, tw, b.state, make_kgeom(gr), nitems);
   return 1;
 }
 
@@ -425,15 +433,14 @@ template <int N, int NV>
 static int launch_kspace_nv(const Grid& gr, const Buffers& b, cudaStream_t s) {
   using Cfg = FftCfg<N>;
   using K = KspaceCfg<N, NV>;
-  const size_t Q = (size_t)(gr.n / 2) * gr.nv;
-  const size_t nchunks = (size_t)gr.n * Q / COLS;
+  const size_t nchunks = (size_t)gr.nyl * gr.q() / COLS;
   const unsigned nitems = (unsigned)(nchunks / Cfg::G);
   auto kern = kspace_x_kernel<N, NV>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SHM) != cudaSuccess) return 0;
-  Twiddle tw{b.tw, 1, 2 * gr.n - 1};
+  Twiddle tw{b.tw, gr.nmax / N, 2 * gr.nmax - 1};
   unsigned grid = (unsigned)(gr.num_sms * K::MINB);
   if (grid > nitems) grid = nitems;
-  kern<<<grid, K::NT, K::SHM, s>>>(b.work, b.phik, b.chi_shell, b.qv, tw, b.state, nitems);
+  kern<<<grid, K::NT, K::SHM, s>>>(b.kbuf, b.phik, b.chi_shell, b.qv, tw, b.state, make_kgeom(gr), nitems);
   return 1;
 }
 
@@ -455,7 +462,7 @@ static int launch_kspace_n(const Grid& g, const Buffers& b, cudaStream_t s) {
 }
 
 int launch_kspace_x(const Grid& g, const Buffers& b, cudaStream_t s) {
-  switch (g.n) {
+  switch (g.nx) {
     case 8: return launch_kspace_n<8>(g, b, s);
     case 16: return launch_kspace_n<16>(g, b, s);
     case 32: return launch_kspace_n<32>(g, b, s);

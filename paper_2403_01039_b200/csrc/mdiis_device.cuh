@@ -194,12 +194,23 @@ static __device__ __noinline__ void mdiis_bookkeeping_and_solve(DevState* __rest
 // the group's partials into part2[(j * ngroups + group)].  Level 2: the last such group adder adds the group sums,
 // then one thread runs the bookkeeping and the small solve.  Every sum runs in a fixed order, so the result does not
 // depend on which CTA arrives last.  tickets: [ngroups] counters, zero on entry, zero again on exit.
+// Slab-decomposed runs (xr.n_dst > 0): this rank's sums cover its own planes only.  The last arriver then writes its
+// row of double-double totals into slot `rank` of every destination's exchange array and stops; gram_solve_kernel,
+// launched once all ranks' rows are there, adds them in rank order and runs the bookkeeping and the solve -- on every
+// rank, from identical numbers, so all ranks take identical decisions.
+struct GramExchange {
+  double* dst[MAX_RANKS];   // [n_ranks][GRAM_SLOT][2] arrays: this rank's own, and its peers' when they are mapped
+  int n_dst;                // 0: single rank, solve right away
+  int rank;
+};
+
 template <int NT>
 static __device__ __forceinline__ void gram_finish(DevState* __restrict__ st, double* __restrict__ part1,
                                                    double* __restrict__ part2, unsigned* __restrict__ tickets,
                                                    int m_old, int nother, AccelArgs aa, bool weighted,
                                                    double npts_total, double* s_row /* shared, MAX_M + 2 */,
-                                                   int* s_flag /* shared */, SolveScratch& ss /* shared */) {
+                                                   int* s_flag /* shared */, SolveScratch& ss /* shared */,
+                                                   const GramExchange& xr) {
   // entries: jj < nother: <R_new, R_other[jj]> (slot jj); jj = nother: <R_new, R_new> (slot MAX_M); and, when the
   // inner product is weighted, jj = nother + 1: the unweighted <R_new, R_new> for the rms (slot MAX_M - 1, free
   // because a weighted run stores at most 3 pairs)
@@ -237,11 +248,23 @@ static __device__ __forceinline__ void gram_finish(DevState* __restrict__ st, do
     const int j = slot(jj);
     double hi, lo;
     warp_sum_partials(part2 + (size_t)j * ngroups * 2, ngroups, lane, hi, lo);
-    if (lane == 0) s_row[jj] = hi + lo;
+    if (lane == 0) {
+      if (xr.n_dst > 0) {
+        dd_norm(hi, lo);
+        for (int d = 0; d < xr.n_dst; ++d)
+          *reinterpret_cast<double2*>(xr.dst[d] + ((size_t)xr.rank * GRAM_SLOT + jj) * 2) = make_double2(hi, lo);
+      } else {
+        s_row[jj] = hi + lo;
+      }
+    }
   }
   __syncthreads();
   if (wid != 0) return;
   if (lane == 0) st->ticket = 0;
+  if (xr.n_dst > 0) {
+    __threadfence_system();                            // peers read the row after the in-stream barrier
+    return;
+  }
   mdiis_bookkeeping_and_solve(st, ss, s_row, m_old, nother, aa, weighted ? s_row[nother + 1] : s_row[nother], npts_total);
 }
 

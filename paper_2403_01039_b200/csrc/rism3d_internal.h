@@ -13,6 +13,8 @@ constexpr int MAX_M = 16;            // MDIIS history slots (rism3d_params.mdiis
 constexpr int MAX_NV = 8;            // solvent site types
 constexpr int RMS_HIST_CAP = 65536;
 constexpr int FE_BLOCKS = 148 * 4;        // CTAs of the free-energy reduction
+constexpr int MAX_RANKS = 8;              // processes of a slab-decomposed run (rism3d_params.n_ranks)
+constexpr int GRAM_SLOT = MAX_M + 2;      // double-double Gram entries one rank hands to the others per iteration
 
 constexpr double K_BOLTZMANN = 0.001987204259;   // kcal/(mol K)     (Q3)
 constexpr double COULOMB = 332.06371;            // kcal A/(mol e^2) (Q3)
@@ -47,16 +49,27 @@ struct StateHeader {           // mirrors the first 64 bytes of DevState
 };
 
 struct Grid {
-  int n;                 // points per axis (cubic)
+  int nx, ny, nz;        // points per axis of the WHOLE grid: powers of two, one spacing (the box need not be cubic)
+  int nmax;              // the largest of the three: the twiddle table and the |k| shell table are built for it
+  int wx, wy, wz;        // (nmax / n_axis)^2: with dk0 = 2 pi / (nmax h), |k|^2 = dk0^2 (s + (wx + wy + wz) / 4),
+                         // s = sum_axis w_axis j'(j' + 1) an even integer (j' the folded index): shell index s / 2
+  int nshell;            // entries of the shell table: largest s / 2, plus one
   int nv;                // site types as the kernels see them: nv_user rounded up to a power of two (1, 2, 4, 8); the
                          // extra "phantom" types have zero charge, LJ, density and chi, stay exactly 0 and cost bandwidth only
   int nv_user;           // site types of the caller (rism3d_params.n_sites)
   double h;              // spacing
-  double origin[3];
-  size_t npts;           // n^3
-  size_t field;          // nv * n^3 doubles in one field-set
+  double origin[3];      // position of grid point (0, 0, 0) of the whole grid
+  // slab decomposition over n_ranks processes (n_ranks = 1: this context holds the whole grid).  r space and the z / y
+  // passes: planes ix0 .. ix0 + nxl - 1;  the k-space pass (x lines): rows jy0 .. jy0 + nyl - 1.
+  int n_ranks, rank;
+  int nxl, ix0;
+  int nyl, jy0;
+  size_t npts;           // r-space points of THIS context: nxl * ny * nz
+  size_t field;          // nv * npts doubles in one field-set
+  size_t npts_global;    // nx * ny * nz
   int num_sms;           // SMs of the device the context lives on (grid size of the persistent kernels)
   int smem_optin;        // largest dynamic shared memory a kernel may opt in to on that device, bytes
+  __host__ __device__ size_t q() const { return (size_t)(nz / 2) * nv; }   // complex elements per (ix, iy) row of `work`
 };
 
 // Device pointers carved from the caller's workspace.
@@ -66,11 +79,11 @@ struct Buffers {
   double* R;             // [M][field]   MDIIS residuals R_i = Y_i - X_i
   double* tau;           // [field]      current input X (tau = t - f)
   double* w;             // [field]      -beta u + f
-  double2* work;         // [n][n][n/2][nv] complex   k-space work array
+  double2* work;         // [nxl][ny][nz/2][nv] complex   k-space work array (x lines: [nx][nyl][nz/2][nv])
   double* phi;           // [npts]       phi(r)
-  double2* phik;         // [n][n][n/2]  phi~(k) exp(+i k.r0) / dV
+  double2* phik;         // [nx][nyl][nz/2]  phi~(k) exp(+i k.r0) / dV
   double* chi_shell;     // [nshell][nv][nv]   chi_shell[s][g][k] = chi_{(g xor k) g}(k_s)
-  double2* tw;           // [2n]         exp(-i pi j / n)
+  double2* tw;           // [2 nmax]     exp(-i pi j / nmax)
   double* gram_part;     // [MAX_M+1][gram_blocks][2]  double-double partial sums, one per zinv_residual CTA
   double* gram_part2;    // [MAX_M+1][groups][2]  first-level sums of groups of 64 partials
   unsigned* tickets;     // [groups] arrival counters of the partial-sum reduction (zero between launches)
@@ -80,6 +93,18 @@ struct Buffers {
   double* rhov;          // [nv]
   double* gram_w;        // [nv] weights of the inner product: 1 (MDIIS) or 1/rho_g (modified Anderson, Eq. 38)
   double* fe_part;       // [FE_BLOCKS][MAX_NV][2]
+  // ---- slab decomposition (n_ranks > 1; with one rank kbuf == work and the tables are unused) ----
+  double2* kbuf;         // [nx][nyl][nz/2][nv] complex   this rank's k-space slab: x lines complete
+  double2* stage;        // [n_ranks][nxl][nyl][nz/2][nv] staging buffer of the two transposes when a library collective
+                         // moves the blocks (rism3d_slab_local); unused once rism3d_slab_set_peers has been called
+  double* gram_x;        // [n_ranks][GRAM_SLOT][2]  every rank's double-double Gram row, summed in rank order by the solve
+  unsigned long long* xflags;   // [MAX_RANKS + 1] arrival epochs of the in-stream barrier (peer mode) + this rank's epoch counter
+  double2* fwd_dst[MAX_RANKS];        // y_fwd writes the rows j_y of rank d's slab of plane ix_l to fwd_dst[d] + (ix_l nyl + jy_l) Q
+  const double2* bwd_src[MAX_RANKS];  // y_inv reads them back from bwd_src[s] + (ix_l nyl + jy_l) Q
+  double* gram_dst[MAX_RANKS];        // copies of gram_x this rank writes its slot into (itself; every peer in peer mode)
+  unsigned long long* flag_dst[MAX_RANKS];   // peer mode: xflags of every rank
+  int n_gram_dst;
+  bool peer_mode;
   // TMA descriptors of the k-space pass (built by rism3d_init when kspace_uses_tma(n)): `work` as a 2D array of doubles
   // [jx][2 n Q] with boxes of n rows x 128 bytes, `phik` as [jx][2 n n/2] with boxes of n rows x (8 / nv) complex
   CUtensorMap tm_work, tm_phik;
@@ -99,17 +124,19 @@ struct SolverParams {
 };
 
 // dynamic shared memory of kspace_x for this grid (0: unsupported n / nv); the API layer checks it against the device
-int kspace_smem_bytes(int n, int nv);
-bool kspace_uses_tma(int n);
+int kspace_smem_bytes(int nx, int nv);
+bool kspace_uses_tma(int nx);
 
 // ---- launchers (each returns the number of kernels it launched; errors surface via cudaGetLastError) ----
 // fft_kernels.cu
 int launch_closure_zfwd(const Grid&, const Buffers&, const SolverParams&, const double* d_raw_in, cudaStream_t);
-int launch_y_fwd(const Grid&, const Buffers&, bool use_state, cudaStream_t);
+int launch_y_fwd(const Grid&, const Buffers&, bool use_state, cudaStream_t);   // slab runs: writes through fwd_dst
 int launch_x_fwd(const Grid&, const Buffers&, cudaStream_t);
 int launch_x_inv(const Grid&, const Buffers&, cudaStream_t);
 int launch_kspace_x(const Grid&, const Buffers&, cudaStream_t);
-int launch_y_inv(const Grid&, const Buffers&, bool use_state, cudaStream_t);
+int launch_y_inv(const Grid&, const Buffers&, bool use_state, cudaStream_t);   // slab runs: reads through bwd_src
+int launch_gram_solve(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);   // slab runs: sum the ranks' rows, solve
+int launch_xbarrier(const Grid&, const Buffers&, cudaStream_t);                // peer mode: all ranks have reached this point
 int launch_zinv_residual(const Grid&, const Buffers&, const SolverParams&, double* d_raw_out, cudaStream_t);
 int zinv_ctas(const Grid&);                      // CTAs of zinv_residual (it writes one Gram partial per CTA)
 // mdiis_kernels.cu

@@ -91,12 +91,12 @@ __device__ __forceinline__ void pair_terms(double r2, double qa, const double* _
 template <int NV>
 __global__ void __launch_bounds__(128)
     potential_kernel(double* __restrict__ w, double* __restrict__ phi, const double4* __restrict__ atoms,
-                     const double* __restrict__ pair, int n_atoms, int n, double h, double ox, double oy, double oz,
-                     double kappa, double r_min, double rcut2, size_t npts) {
+                     const double* __restrict__ pair, int n_atoms, int ny, int nz, int ix0, double h, double ox,
+                     double oy, double oz, double kappa, double r_min, double rcut2, size_t npts) {
   __shared__ double4 s_atom[ATOM_CHUNK];
   __shared__ double s_pair[ATOM_CHUNK * NV * 3];
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;   // npts is a multiple of blockDim
-  const int iz = (int)(idx % n), iy = (int)((idx / n) % n), ix = (int)(idx / ((size_t)n * n));
+  const int iz = (int)(idx % nz), iy = (int)((idx / nz) % ny), ix = ix0 + (int)(idx / ((size_t)nz * ny));
   // r_n = origin + spacing * index, each operation rounded separately (the pair set of a cutoff must not depend
   // on contraction)
   const double x = __dadd_rn(ox, __dmul_rn(h, (double)ix));
@@ -132,8 +132,8 @@ int launch_potential(const Grid& g, const Buffers& b, const SolverParams& sp, in
   const double rcut2 = rcut > 0.0 ? rcut * rcut : 0.0;
   const double4* at = reinterpret_cast<const double4*>(d_atoms);
 #define POT(NV)                                                                                                   \
-  potential_kernel<NV><<<blocks, 128, 0, s>>>(b.w, b.phi, at, d_pair, n_atoms, g.n, g.h, g.origin[0], g.origin[1], \
-                                              g.origin[2], sp.kappa, sp.r_min, rcut2, g.npts)
+  potential_kernel<NV><<<blocks, 128, 0, s>>>(b.w, b.phi, at, d_pair, n_atoms, g.ny, g.nz, g.ix0, g.h, g.origin[0], \
+                                              g.origin[1], g.origin[2], sp.kappa, sp.r_min, rcut2, g.npts)
   switch (g.nv) {
     case 1: POT(1); break;
     case 2: POT(2); break;
@@ -165,14 +165,15 @@ constexpr int CELL_CHUNK = 128;
 template <int NV>
 __global__ void __launch_bounds__(BRICK_THREADS)
     w_cells_kernel(double* __restrict__ w, const double4* __restrict__ atoms, const double* __restrict__ pair,
-                   const int* __restrict__ cell_start, CellGrid cg, int n, double h, double ox, double oy, double oz,
-                   double kappa, double r_min, double rcut, size_t npts) {
+                   const int* __restrict__ cell_start, CellGrid cg, int ny, int nz, int ix0, double h, double ox,
+                   double oy, double oz, double kappa, double r_min, double rcut, size_t npts) {
   __shared__ double4 s_atom[CELL_CHUNK];
   __shared__ double s_pair[CELL_CHUNK * NV * 3];
   const int tid = threadIdx.x;
   const int iz = blockIdx.x * BRICK_Z + tid % BRICK_Z;
   const int iy = blockIdx.y * BRICK_Y + (tid / BRICK_Z) % BRICK_Y;
-  const int ix = blockIdx.z * BRICK_X + tid / (BRICK_Z * BRICK_Y);
+  const int ixl = blockIdx.z * BRICK_X + tid / (BRICK_Z * BRICK_Y);   // plane of this context's slab
+  const int ix = ix0 + ixl;
   const double x = __dadd_rn(ox, __dmul_rn(h, (double)ix));
   const double y = __dadd_rn(oy, __dmul_rn(h, (double)iy));
   const double z = __dadd_rn(oz, __dmul_rn(h, (double)iz));
@@ -183,7 +184,7 @@ __global__ void __launch_bounds__(BRICK_THREADS)
   const double rcut2 = rcut * rcut, rmin2 = r_min * r_min, far2 = 1600.0 / (kappa * kappa);
   // the brick's box (with a safety margin of a grid spacing against rounding in the cell arithmetic) and the cells it
   // can reach; everything below is uniform over the CTA
-  const double bx0 = ox + h * (blockIdx.z * BRICK_X) - h, bx1 = ox + h * (blockIdx.z * BRICK_X + BRICK_X - 1) + h;
+  const double bx0 = ox + h * (ix0 + blockIdx.z * BRICK_X) - h, bx1 = ox + h * (ix0 + blockIdx.z * BRICK_X + BRICK_X - 1) + h;
   const double by0 = oy + h * (blockIdx.y * BRICK_Y) - h, by1 = oy + h * (blockIdx.y * BRICK_Y + BRICK_Y - 1) + h;
   const double bz0 = oz + h * (blockIdx.x * BRICK_Z) - h, bz1 = oz + h * (blockIdx.x * BRICK_Z + BRICK_Z - 1) + h;
   auto cell_lo = [&](double v, int axis) { return max(0, (int)floor((v - rcut - cg.lo[axis]) / cg.edge)); };
@@ -221,7 +222,7 @@ __global__ void __launch_bounds__(BRICK_THREADS)
       }
     }
   }
-  const size_t idx = ((size_t)ix * n + iy) * n + iz;
+  const size_t idx = ((size_t)ixl * ny + iy) * nz + iz;
 #pragma unroll
   for (int g = 0; g < NV; ++g) w[(size_t)g * npts + idx] = acc[g];
 }
@@ -233,11 +234,12 @@ int launch_w_cells(const Grid& g, const Buffers& b, const SolverParams& sp, cons
   CellGrid cg;
   for (int i = 0; i < 3; ++i) { cg.nc[i] = nc[i]; cg.lo[i] = lo[i]; }
   cg.edge = edge;
-  dim3 grid((unsigned)(g.n / BRICK_Z), (unsigned)(g.n / BRICK_Y), (unsigned)(g.n / BRICK_X));
+  dim3 grid((unsigned)(g.nz / BRICK_Z), (unsigned)(g.ny / BRICK_Y), (unsigned)(g.nxl / BRICK_X));
   const double4* at = reinterpret_cast<const double4*>(d_atoms);
 #define WCELL(NV)                                                                                                   \
-  w_cells_kernel<NV><<<grid, BRICK_THREADS, 0, s>>>(b.w, at, d_pair, d_cell_start, cg, g.n, g.h, g.origin[0],       \
-                                                    g.origin[1], g.origin[2], sp.kappa, sp.r_min, rcut, g.npts)
+  w_cells_kernel<NV><<<grid, BRICK_THREADS, 0, s>>>(b.w, at, d_pair, d_cell_start, cg, g.ny, g.nz, g.ix0, g.h,      \
+                                                    g.origin[0], g.origin[1], g.origin[2], sp.kappa, sp.r_min, rcut, \
+                                                    g.npts)
   switch (g.nv) {
     case 1: WCELL(1); break;
     case 2: WCELL(2); break;
@@ -253,13 +255,13 @@ int launch_w_cells(const Grid& g, const Buffers& b, const SolverParams& sp, cons
 // thread (z and z + n/2: two independent dependency chains), atoms staged through shared memory.
 constexpr int PHI_CHUNK = 256;
 __global__ void __launch_bounds__(128)
-    phi_kernel(double* __restrict__ phi, const double4* __restrict__ atoms, int n_atoms, int n, double h, double ox,
-               double oy, double oz, double kappa, double r_min) {
+    phi_kernel(double* __restrict__ phi, const double4* __restrict__ atoms, int n_atoms, int ny, int nz, int ix0,
+               double h, double ox, double oy, double oz, double kappa, double r_min) {
   __shared__ double4 s_atom[PHI_CHUNK];
-  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // n^3 / 2 threads
-  const int hz = n / 2;
-  const int iz = (int)(t % hz), iy = (int)((t / hz) % n), ix = (int)(t / ((size_t)hz * n));
-  const double x = __dadd_rn(ox, __dmul_rn(h, (double)ix));
+  const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;      // npts / 2 threads
+  const int hz = nz / 2;
+  const int iz = (int)(t % hz), iy = (int)((t / hz) % ny), ixl = (int)(t / ((size_t)hz * ny));
+  const double x = __dadd_rn(ox, __dmul_rn(h, (double)(ix0 + ixl)));
   const double y = __dadd_rn(oy, __dmul_rn(h, (double)iy));
   const double z0 = __dadd_rn(oz, __dmul_rn(h, (double)iz));
   const double z1 = __dadd_rn(oz, __dmul_rn(h, (double)(iz + hz)));
@@ -280,7 +282,7 @@ __global__ void __launch_bounds__(128)
       pair_terms<1, true, false>(__dadd_rn(rxy, __dmul_rn(dz1, dz1)), at.w, nullptr, kappa, r_min, rmin2, far2, false, 0.0, ph1, none);
     }
   }
-  const size_t idx = ((size_t)ix * n + iy) * n + iz;
+  const size_t idx = ((size_t)ixl * ny + iy) * nz + iz;
   phi[idx] = ph0;
   phi[idx + hz] = ph1;
 }
@@ -289,28 +291,33 @@ __global__ void __launch_bounds__(128)
 int launch_phi(const Grid& g, const Buffers& b, const SolverParams& sp, int n_atoms, const double* d_atoms,
                cudaStream_t s) {
   const unsigned blocks = (unsigned)(g.npts / 2 / 128);
-  phi_kernel<<<blocks, 128, 0, s>>>(b.phi, reinterpret_cast<const double4*>(d_atoms), n_atoms, g.n, g.h, g.origin[0],
-                                   g.origin[1], g.origin[2], sp.kappa, sp.r_min);
+  phi_kernel<<<blocks, 128, 0, s>>>(b.phi, reinterpret_cast<const double4*>(d_atoms), n_atoms, g.ny, g.nz, g.ix0, g.h,
+                                   g.origin[0], g.origin[1], g.origin[2], sp.kappa, sp.r_min);
   return 1;
 }
 
 // ------------------------------------------------------------------------------------------------
 // phi~(k): separable phase tables E_axis[a][j] = exp(-i k_j (R_a,axis - r0,axis)), then
-//   phik[jx][jy][p] = (4 pi beta C / dV) kappa^2 / (k^2 (k^2 + kappa^2)) sum_a q_a Ex[a][jx] Ey[a][jy] Ez[a][2p]
-// d_phase: [3][n_atoms][n] complex (z table holds only the even j at index p, n/2 entries used)
+//   phik[jx][jy_l][p] = (4 pi beta C / dV) kappa^2 / (k^2 (k^2 + kappa^2)) sum_a q_a Ex[a][jx] Ey[a][jy0 + jy_l] Ez[a][2p]
+// d_phase: [3][n_atoms][nmax] complex (axis a uses its first n_a entries; the z table holds only the even j at index p,
+// nz/2 entries used)
 // ------------------------------------------------------------------------------------------------
-__global__ void phase_kernel(double2* __restrict__ phase, const double4* __restrict__ atoms, int n_atoms, int n,
-                             double h, double ox, double oy, double oz) {
+struct AxisLen { int n[3]; };
+
+__global__ void phase_kernel(double2* __restrict__ phase, const double4* __restrict__ atoms, int n_atoms, AxisLen al,
+                             int nmax, double h, double ox, double oy, double oz) {
   const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const size_t total = (size_t)3 * n_atoms * n;
+  const size_t total = (size_t)3 * n_atoms * nmax;
   if (idx >= total) return;
-  const int j = (int)(idx % n);
-  const int a = (int)((idx / n) % n_atoms);
-  const int axis = (int)(idx / ((size_t)n * n_atoms));
+  const int j = (int)(idx % nmax);
+  const int a = (int)((idx / nmax) % n_atoms);
+  const int axis = (int)(idx / ((size_t)nmax * n_atoms));
+  const int n = al.n[axis];
   const double4 at = atoms[a];
   const double d = axis == 0 ? at.x - ox : (axis == 1 ? at.y - oy : at.z - oz);
   int jj = j;
-  if (axis == 2) { if (j >= n / 2) { phase[idx] = make_double2(0.0, 0.0); return; } jj = 2 * j; }
+  if (axis == 2) jj = 2 * j;
+  if (jj >= n) { phase[idx] = make_double2(0.0, 0.0); return; }
   const double f = (jj < n / 2) ? (jj + 0.5) : (jj + 0.5 - n);          // k = dk * f, dk = 2 pi / (n h)
   double sn, cs;
   sincospi(2.0 * f * (d / (n * h)), &sn, &cs);
@@ -322,15 +329,15 @@ constexpr int PT_AC = 32;     // atoms per shared-memory chunk
 
 __global__ void __launch_bounds__(64)
     phi_tilde_kernel(double2* __restrict__ phik, const double2* __restrict__ phase, const double* __restrict__ qa,
-                     int n_atoms, int n, double h, double kappa, double pref) {
+                     int n_atoms, AxisLen al, int nmax, int nyl, int jy0g, double h, double kappa, double pref) {
   __shared__ double2 s_a[PT_AC][PT_JY];
-  const int nz = n / 2;
+  const int nzh = al.n[2] / 2;
   const int p = blockIdx.x * blockDim.x + threadIdx.x;
-  const int jy0 = blockIdx.y * PT_JY;
+  const int jyl0 = blockIdx.y * PT_JY;                   // first row of this CTA inside the context's k-space slab
   const int jx = blockIdx.z;
   const double2* Ex = phase;
-  const double2* Ey = phase + (size_t)n_atoms * n;
-  const double2* Ez = phase + (size_t)2 * n_atoms * n;
+  const double2* Ey = phase + (size_t)n_atoms * nmax;
+  const double2* Ez = phase + (size_t)2 * n_atoms * nmax;
   double2 acc[PT_JY];
 #pragma unroll
   for (int i = 0; i < PT_JY; ++i) acc[i] = make_double2(0.0, 0.0);
@@ -338,15 +345,15 @@ __global__ void __launch_bounds__(64)
     const int na = min(PT_AC, n_atoms - a0);
     __syncthreads();
     for (int i = threadIdx.x; i < na * PT_JY; i += blockDim.x) {
-      const int a = a0 + i / PT_JY, jy = jy0 + i % PT_JY;
-      const double2 ex = Ex[(size_t)a * n + jx], ey = Ey[(size_t)a * n + jy];
+      const int a = a0 + i / PT_JY, jy = jy0g + jyl0 + i % PT_JY;
+      const double2 ex = Ex[(size_t)a * nmax + jx], ey = Ey[(size_t)a * nmax + jy];
       const double q = qa[a];
       s_a[i / PT_JY][i % PT_JY] = make_double2(q * (ex.x * ey.x - ex.y * ey.y), q * (ex.x * ey.y + ex.y * ey.x));
     }
     __syncthreads();
-    if (p < nz) {
+    if (p < nzh) {
       for (int a = 0; a < na; ++a) {
-        const double2 ez = Ez[(size_t)(a0 + a) * n + p];
+        const double2 ez = Ez[(size_t)(a0 + a) * nmax + p];
 #pragma unroll
         for (int i = 0; i < PT_JY; ++i) {
           const double2 v = s_a[a][i];
@@ -356,36 +363,40 @@ __global__ void __launch_bounds__(64)
       }
     }
   }
-  if (p >= nz) return;
-  const double dk = 2.0 * 3.14159265358979323846 / (n * h);
-  auto kof = [&](int j) { return dk * ((j < nz) ? (j + 0.5) : (j + 0.5 - n)); };
-  const double kx = kof(jx), kz = kof(2 * p);
+  if (p >= nzh) return;
+  auto kof = [&](int j, int axis) {
+    const int n = al.n[axis];
+    const double dk = 2.0 * 3.14159265358979323846 / (n * h);
+    return dk * ((j < n / 2) ? (j + 0.5) : (j + 0.5 - n));
+  };
+  const double kx = kof(jx, 0), kz = kof(2 * p, 2);
 #pragma unroll
   for (int i = 0; i < PT_JY; ++i) {
-    const double ky = kof(jy0 + i);
+    const double ky = kof(jy0g + jyl0 + i, 1);
     const double k2 = kx * kx + ky * ky + kz * kz;
     const double f = pref * kappa * kappa / (k2 * (k2 + kappa * kappa));
-    phik[((size_t)jx * n + (jy0 + i)) * nz + p] = make_double2(f * acc[i].x, f * acc[i].y);
+    phik[((size_t)jx * nyl + (jyl0 + i)) * nzh + p] = make_double2(f * acc[i].x, f * acc[i].y);
   }
 }
 
 int launch_phi_tilde(const Grid& g, const Buffers& b, const SolverParams& sp, int n_atoms, const double* d_atoms,
                      double2* d_phase, cudaStream_t s) {
-  const size_t total = (size_t)3 * n_atoms * g.n;
+  const size_t total = (size_t)3 * n_atoms * g.nmax;
   const double4* at = reinterpret_cast<const double4*>(d_atoms);
+  const AxisLen al{{g.nx, g.ny, g.nz}};
   int launched = 1;
   if (total > 0) {                                       // an empty solute has no phase table (phi~ = 0)
-    phase_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(d_phase, at, n_atoms, g.n, g.h, g.origin[0],
+    phase_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(d_phase, at, n_atoms, al, g.nmax, g.h, g.origin[0],
                                                                 g.origin[1], g.origin[2]);
     launched = 2;
   }
   // charges q_a live in a separate array right after the atom records (set up by the API layer)
   const double* qa = d_atoms + (size_t)4 * n_atoms;
-  const int nz = g.n / 2;
-  const int bx = nz < 64 ? nz : 64;
-  dim3 grid((nz + bx - 1) / bx, g.n / PT_JY, g.n);
+  const int nzh = g.nz / 2;
+  const int bx = nzh < 64 ? nzh : 64;
+  dim3 grid((nzh + bx - 1) / bx, g.nyl / PT_JY, g.nx);
   const double pref = 4.0 * 3.14159265358979323846 * sp.beta * COULOMB / (g.h * g.h * g.h);
-  phi_tilde_kernel<<<grid, bx, 0, s>>>(b.phik, d_phase, qa, n_atoms, g.n, g.h, sp.kappa, pref);
+  phi_tilde_kernel<<<grid, bx, 0, s>>>(b.phik, d_phase, qa, n_atoms, al, g.nmax, g.nyl, g.jy0, g.h, sp.kappa, pref);
   return launched;
 }
 
@@ -394,10 +405,10 @@ int launch_phi_tilde(const Grid& g, const Buffers& b, const SolverParams& sp, in
 // the column of Eq. 13 that site g needs, ordered for the butterfly exchange of kspace_point (kspace_kernel.cu)
 // ------------------------------------------------------------------------------------------------
 __global__ void chi_shell_kernel(double* __restrict__ out, const double* __restrict__ table, int n_k, double k0,
-                                 double dkt, int nv, double dk_grid, int nshell) {
+                                 double dkt, int nv, double dk_grid, double quarter_w, int nshell) {
   const int sidx = blockIdx.x * blockDim.x + threadIdx.x;
   if (sidx >= nshell) return;
-  const double kmag = dk_grid * sqrt(2.0 * sidx + 0.75);
+  const double kmag = dk_grid * sqrt(2.0 * sidx + quarter_w);   // |k|^2 = dk0^2 (s + (wx + wy + wz) / 4), s = 2 sidx
   const double xk = (kmag - k0) / dkt;
   int m = (int)floor(xk);
   int first = m - 1;
@@ -418,10 +429,9 @@ __global__ void chi_shell_kernel(double* __restrict__ out, const double* __restr
 
 int launch_chi_shell(const Grid& g, const Buffers& b, const double* d_table, int n_k, double k0, double dk,
                      cudaStream_t s) {
-  const int hn = g.n / 2;
-  const int nshell = 3 * (hn - 1) * hn / 2 + 1;
-  const double dk_grid = 2.0 * 3.14159265358979323846 / (g.n * g.h);
-  chi_shell_kernel<<<(nshell + 127) / 128, 128, 0, s>>>(b.chi_shell, d_table, n_k, k0, dk, g.nv, dk_grid, nshell);
+  const double dk_grid = 2.0 * 3.14159265358979323846 / (g.nmax * g.h);
+  chi_shell_kernel<<<(g.nshell + 127) / 128, 128, 0, s>>>(b.chi_shell, d_table, n_k, k0, dk, g.nv, dk_grid,
+                                                          0.25 * (g.wx + g.wy + g.wz), g.nshell);
   return 1;
 }
 
@@ -553,8 +563,8 @@ __global__ void gradient_weights_kernel(double* __restrict__ gw, const double* _
 template <int NV>
 __global__ void __launch_bounds__(GRAD_THREADS)
     gradient_kernel(double* __restrict__ partial, const double* __restrict__ gwf, const double4* __restrict__ atoms,
-                    const double* __restrict__ pair, int n_atoms, int n, double h, double ox, double oy, double oz,
-                    double r_min, size_t npts, size_t pts_per_block) {
+                    const double* __restrict__ pair, int n_atoms, int ny, int nz, int ix0, double h, double ox,
+                    double oy, double oz, double r_min, size_t npts, size_t pts_per_block) {
   __shared__ double4 s_atom[GRAD_ATOMS];
   __shared__ double s_pair[GRAD_ATOMS * NV * 3];
   __shared__ double s_red[GRAD_THREADS / 32][GRAD_ATOMS * 3][2];
@@ -571,7 +581,7 @@ __global__ void __launch_bounds__(GRAD_THREADS)
   const size_t p0 = (size_t)blockIdx.x * pts_per_block;
   const size_t p1 = min(npts, p0 + pts_per_block);
   for (size_t idx = p0 + tid; idx < p1; idx += GRAD_THREADS) {
-    const int iz = (int)(idx % n), iy = (int)((idx / n) % n), ix = (int)(idx / ((size_t)n * n));
+    const int iz = (int)(idx % nz), iy = (int)((idx / nz) % ny), ix = ix0 + (int)(idx / ((size_t)nz * ny));
     const double x = __dadd_rn(ox, __dmul_rn(h, (double)ix));
     const double y = __dadd_rn(oy, __dmul_rn(h, (double)iy));
     const double z = __dadd_rn(oz, __dmul_rn(h, (double)iz));
@@ -651,8 +661,8 @@ int launch_gradient(const Grid& g, const Buffers& b, const SolverParams& sp, int
   dim3 grid((unsigned)nchunks, (unsigned)((n_atoms + GRAD_ATOMS - 1) / GRAD_ATOMS));
   const double4* at = reinterpret_cast<const double4*>(d_atoms);
 #define GRD(NV)                                                                                                     \
-  gradient_kernel<NV><<<grid, GRAD_THREADS, 0, s>>>(d_partial, d_gw, at, d_pair, n_atoms, g.n, g.h, g.origin[0],   \
-                                                    g.origin[1], g.origin[2], sp.r_min, g.npts, per)
+  gradient_kernel<NV><<<grid, GRAD_THREADS, 0, s>>>(d_partial, d_gw, at, d_pair, n_atoms, g.ny, g.nz, g.ix0, g.h,   \
+                                                    g.origin[0], g.origin[1], g.origin[2], sp.r_min, g.npts, per)
   switch (g.nv) {
     case 1: GRD(1); break;
     case 2: GRD(2); break;

@@ -293,3 +293,64 @@ def test_dynamic_damping_fifty_iterations(cfg, n, M):
         twin.iterate(k, 0.0)
     assert np.array_equal(twin.rms_history(), gpu.rms_history())
     assert np.array_equal(twin.get_field("TAU"), gpu.get_field("TAU"))
+
+
+# ---- boxes that are not cubes: (nx, ny, nz) powers of two with one spacing (rism3d.h "grid") ------------------
+@pytest.mark.parametrize("shape,nv", [((8, 16, 32), 2), ((32, 16, 8), 4), ((64, 32, 16), 1), ((16, 64, 128), 4),
+                                      ((128, 32, 64), 2), ((256, 16, 16), 4)])
+def test_fft_pair_on_non_cubic_grids(shape, nv):
+    import torch
+    import paper_2403_01039_b200 as lib
+    from tests._gpu_util import oracle_spectrum_in_gpu_layout
+    rng = np.random.default_rng(sum(shape) + nv)
+    f = rng.standard_normal((nv,) + shape)
+    s = lib.Solver(shape, 0.5, nv)
+    spec = s.fft_forward(torch.from_numpy(f).cuda()).cpu().numpy()
+    ref = oracle_spectrum_in_gpu_layout(f, 0.5)
+    assert spec.shape == ref.shape == (shape[0], shape[1], shape[2] // 2, nv)
+    tol = 2e-14 * np.log2(max(shape))
+    assert np.max(np.abs(spec - ref)) < tol * np.max(np.abs(ref))
+    back = s.fft_inverse(torch.from_numpy(ref).cuda()).cpu().numpy()
+    assert np.max(np.abs(back - f)) < tol * np.max(np.abs(f))
+    s.close()
+
+
+@pytest.mark.parametrize("shape,rcut", [((32, 64, 16), 0.0), ((16, 32, 64), 7.0), ((64, 16, 32), 0.0)])
+def test_fifty_iterations_on_a_non_cubic_grid(shape, rcut):
+    """A small charged solute in water in a box that is not a cube (the |k| shells of the three axes then differ by factors of
+    4 in the shell index): setup fields, 50 fixed iterations, free energy, gradient."""
+    sol = _small_solute(seed=sum(shape), n=4)                # fits the shortest axis (8 A)
+    orc, gpu, _, _ = make_pair(n=shape, spacing=0.5, solvent="water", M=5, solute=sol, rcut=rcut)
+    W, Wo = gpu.get_field("W"), orc.get_field("W")
+    assert W.shape == (2,) + shape
+    finite = np.abs(Wo) < 600.0
+    assert np.max(np.abs(W - Wo)[finite]) < 1e-10
+    assert np.max(np.abs(gpu.get_field("PHI", 0) - orc.phi)) < 1e-11 * np.max(np.abs(orc.phi))
+    orc.iterate(50, 0.0)
+    nd, rms = gpu.iterate(50, 0.0)
+    assert nd == 50
+    np.testing.assert_allclose(gpu.rms_history(), orc.rms_history, rtol=1e-6, atol=1e-12)
+    assert np.max(np.abs(gpu.get_field("G") - orc.get_field("G"))) <= 1e-9
+    assert np.max(np.abs(gpu.get_field("TAU") - orc.get_field("TAU"))) <= 1e-9
+    mu, _ = gpu.free_energy()
+    mu_o, _ = orc.free_energy()
+    assert abs(mu - mu_o) <= 1e-7 * abs(mu_o)
+    if rcut == 0.0:
+        go = orc.solvation_gradient()
+        assert np.max(np.abs(gpu.gradient() - go)) <= 1e-8 * max(1.0, np.max(np.abs(go)))
+    gpu.close()
+
+
+def test_non_cubic_four_sites_pse2():
+    """4 site types, PSE-2, M = 8 on (64, 32, 32) with a 40-atom subset of C3's solute."""
+    from workloads import Solute, make_solute
+    sol = make_solute("C3")
+    keep = np.argsort(np.linalg.norm(sol.xyz, axis=1))[:40]
+    sub = Solute("C3_sub40", sol.xyz[keep], sol.q[keep], sol.sigma[keep], sol.eps[keep])
+    orc, gpu, _, _ = make_pair(n=(64, 32, 32), spacing=0.75, solvent="water_nacl_0.1M", closure="PSE", pse_order=2,
+                               M=8, solute=sub)
+    orc.iterate(30, 0.0)
+    gpu.iterate(30, 0.0)
+    np.testing.assert_allclose(gpu.rms_history(), orc.rms_history, rtol=1e-6, atol=1e-12)
+    assert np.max(np.abs(gpu.get_field("G") - orc.get_field("G"))) <= 1e-9
+    gpu.close()

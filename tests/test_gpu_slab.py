@@ -1,0 +1,141 @@
+"""-m gpu: the slab decomposition (include/rism3d.h "Slab decomposition") against the oracle.
+
+One GPU is what the test box has, so the n_ranks contexts of a run live in ONE process on ONE device and are driven
+phase by phase on one stream (`iterate_in_lockstep`): every kernel of every rank is the kernel a multi-GPU run launches,
+with that rank's slab geometry, base-pointer tables and Gram exchange; no kernel ever waits for another rank.  Staged
+mode moves the blocks with device copies that stand in for the all-to-all; peer mode hands every rank the addresses of
+the other ranks' arrays (here: plain device pointers of the same GPU), so the y passes write into / read from the other
+ranks' k-space slabs directly, as they do over NVLink."""
+import numpy as np
+import pytest
+
+from oracle import rism3d as o3
+from workloads import Solute, load_chi, make_solute, solvent_by_name
+
+pytestmark = pytest.mark.gpu
+
+
+def _solute(seed, n, spread):
+    rng = np.random.default_rng(seed)
+    xyz = rng.uniform(-spread, spread, (n, 3))
+    q = rng.normal(0.0, 0.3, n)
+    return Solute("slab", xyz, q, rng.uniform(2.6, 3.4, n), rng.uniform(0.05, 0.2, n))
+
+
+def _make(shape, spacing, solvent, P, sol, rcut, peer, **kw):
+    import torch
+    import paper_2403_01039_b200 as lib
+    sv = solvent_by_name(solvent)
+    k0, dk, chi = load_chi(sv.name)
+    orc = o3.Rism3dOracle(shape, spacing, sv.n_v, **kw)
+    orc.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+    orc.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=rcut)
+    stream = torch.cuda.Stream()
+    ranks = [lib.SlabSolver(shape, spacing, sv.n_v, P, r, stream=stream, **kw) for r in range(P)]
+    for r in ranks:
+        r.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+        r.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=rcut)
+    if peer:
+        loc = [r.local for r in ranks]
+        for r in ranks:
+            r.connect_peers([l["K"] for l in loc], [l["gram"] for l in loc], [l["flags"] for l in loc])
+    return orc, ranks, sv
+
+
+def _gather(ranks, which):
+    """whole-grid field [n_sites][nx][ny][nz] from the ranks' slabs"""
+    return np.concatenate([r.get_field(which) for r in ranks], axis=1)
+
+
+@pytest.mark.parametrize("P,shape,solvent,rcut,peer", [
+    (2, (32, 32, 32), "water", 0.0, False),
+    (2, (32, 32, 32), "water", 0.0, True),
+    (4, (32, 64, 16), "water", 7.0, False),
+    (4, (64, 32, 32), "water_nacl_0.1M", 0.0, True),
+    (8, (64, 64, 16), "water", 0.0, True),
+])
+def test_slab_ranks_match_oracle(P, shape, solvent, rcut, peer):
+    import paper_2403_01039_b200 as lib
+    sol = _solute(sum(shape) + P, 4, 1.5)
+    kw = dict(closure="KH", mdiis_nvec=5, mdiis_b=0.5, mdiis_restart=10.0)
+    orc, ranks, sv = _make(shape, 0.5, solvent, P, sol, rcut, peer, **kw)
+    # S0 on every slab
+    Wo = orc.get_field("W")
+    W = _gather(ranks, "W")
+    assert W.shape == Wo.shape
+    finite = np.abs(Wo) < 600.0
+    assert np.max(np.abs(W - Wo)[finite]) < 1e-10
+    phi = np.concatenate([r.get_field("PHI", 0) for r in ranks], axis=0)
+    assert np.max(np.abs(phi - orc.phi)) < 1e-11 * np.max(np.abs(orc.phi))
+    # the loop
+    iters = 30
+    orc.iterate(iters, 0.0)
+    nd, rms = lib.iterate_in_lockstep(ranks, iters, 0.0)
+    assert nd == iters
+    hist = ranks[0].rms_history()
+    np.testing.assert_allclose(hist, orc.rms_history, rtol=1e-6, atol=1e-12)
+    for r in ranks[1:]:
+        assert np.array_equal(r.rms_history(), hist)         # every rank solved the same small system
+    assert np.max(np.abs(_gather(ranks, "G") - orc.get_field("G"))) <= 1e-9
+    assert np.max(np.abs(_gather(ranks, "TAU") - orc.get_field("TAU"))) <= 1e-9
+    # grid sums: every rank returns its slab's share
+    mu = sum(lib.rism3d_free_energy(r.ctx, sv.n_v)[0] for r in ranks)
+    mu_o, _ = orc.free_energy()
+    assert abs(mu - mu_o) <= 1e-7 * abs(mu_o)
+    v = sum(lib.rism3d_pmv(r.ctx, 0.05, sv.n_v)[0] for r in ranks)
+    v_o, _ = orc.pmv(0.05)
+    assert abs(v - v_o) <= 1e-7 * abs(v_o)
+    grad = sum(lib.rism3d_gradient(r.ctx, sol.n_atoms) for r in ranks)
+    go = orc.solvation_gradient()
+    assert np.max(np.abs(grad - go)) <= 1e-8 * max(1.0, np.max(np.abs(go)))
+    for r in ranks:
+        r.close()
+
+
+def test_staged_and_peer_mode_agree_bit_for_bit_and_with_one_rank():
+    """same kernels, same arithmetic: only where the rows travel differs.  Against a single rank the Gram sums are
+    added in a different order (per slab, then over ranks), so that comparison is to rounding, not to the bit."""
+    import paper_2403_01039_b200 as lib
+    shape, P = (32, 32, 32), 2
+    sol = _solute(5, 5, 2.0)
+    kw = dict(closure="PSE", pse_order=2, mdiis_nvec=4)
+    _, staged, sv = _make(shape, 0.5, "water", P, sol, 0.0, False, **kw)
+    _, peers, _ = _make(shape, 0.5, "water", P, sol, 0.0, True, **kw)
+    lib.iterate_in_lockstep(staged, 20, 0.0)
+    lib.iterate_in_lockstep(peers, 20, 0.0)
+    assert np.array_equal(_gather(staged, "TAU"), _gather(peers, "TAU"))
+    assert np.array_equal(staged[0].rms_history(), peers[1].rms_history())
+    k0, dk, chi = load_chi(sv.name)
+    one = lib.Solver(shape, 0.5, sv.n_v, **kw)
+    one.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+    one.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps)
+    one.iterate(20, 0.0)
+    np.testing.assert_allclose(staged[0].rms_history(), one.rms_history(), rtol=1e-9)
+    assert np.max(np.abs(_gather(staged, "TAU") - one.get_field("TAU"))) <= 1e-10
+
+
+def test_slab_convergence_stops_all_ranks_together():
+    import paper_2403_01039_b200 as lib
+    sol = Solute("ion", np.array([[0.0, 0.0, 0.0]]), np.array([1.0]), np.array([2.35]), np.array([0.13]))
+    orc, ranks, sv = _make((32, 32, 32), 0.5, "water", 2, sol, 0.0, False, closure="KH", mdiis_nvec=5)
+    n_o, rms_o = orc.iterate(400, 1e-6)
+    nd, rms = lib.iterate_in_lockstep(ranks, 400, 1e-6)
+    assert nd == n_o and rms < 1e-6 and abs(rms - rms_o) <= 1e-6 * rms_o
+    assert np.max(np.abs(_gather(ranks, "G") - orc.get_field("G"))) <= 1e-9
+
+
+def test_slab_argument_checks():
+    import paper_2403_01039_b200 as lib
+    p = lib.Rism3dParams()
+    p.nx = p.ny = p.nz = 32
+    p.spacing, p.n_sites, p.closure, p.pse_order, p.temperature = 0.5, 2, 1, 1, 298.0
+    p.mdiis_nvec, p.mdiis_b, p.mdiis_restart, p.kappa, p.r_min = 5, 0.5, 10.0, 1.0, 1e-3
+    p.n_ranks, p.rank = 2, 0
+    assert lib.rism3d_workspace_bytes(p) > 0
+    for bad_ranks, bad_rank in [(3, 0), (2, 2), (8, 0), (16, 0), (2, -1)]:      # 32 / 8 = 4 planes: not whole bricks
+        p.n_ranks, p.rank = bad_ranks, bad_rank
+        assert lib.rism3d_workspace_bytes(p) == 0
+    one = lib.Solver(32, 0.5, 2)
+    with pytest.raises(lib.Rism3dError):
+        lib.rism3d_slab_phase(one.ctx, 0)                    # not a slab run
+    one.close()
