@@ -560,21 +560,48 @@ class SlabSolver(Solver):
         self.peer_mode = True
 
     # -- one process per GPU -------------------------------------------------------------------------------------
+    def _device_collectives(self) -> bool:
+        """True when the process group moves device tensors itself (nccl); any other backend (gloo, in the CPU-side
+        tests and on boxes without NVLink) gets the blocks through host memory."""
+        import torch.distributed as dist
+        return dist.get_backend(self.group) == "nccl"
+
+    def _all_to_all(self, dst, src):
+        import torch
+        import torch.distributed as dist
+        if self._device_collectives():
+            dist.all_to_all_single(dst, src, group=self.group)
+        else:
+            h_src = src.cpu()                            # synchronises the solver's stream (the current one here)
+            h_dst = torch.empty_like(h_src)
+            dist.all_to_all_single(h_dst, h_src, group=self.group)
+            dst.copy_(h_dst)
+
+    def _all_gather_rows(self):
+        import torch
+        import torch.distributed as dist
+        row = self.gram.numel() // self.n_ranks
+        mine = self.gram[self.rank * row:(self.rank + 1) * row]
+        if self._device_collectives():
+            dist.all_gather_into_tensor(self.gram, mine, group=self.group)
+        else:
+            h = torch.empty(self.gram.numel(), dtype=torch.float64)
+            dist.all_gather_into_tensor(h, mine.cpu(), group=self.group)
+            self.gram.copy_(h)
+
     def iterate(self, max_iter, tol=0.0, check_every=8):
         if self.peer_mode:
             return rism3d_iterate(self.ctx, max_iter, tol)
         import torch
-        import torch.distributed as dist
-        row = self.gram.numel() // self.n_ranks
         self.begin(tol)
         with torch.cuda.stream(self.stream):
             for it in range(max_iter):
                 self.phase(0)
-                dist.all_to_all_single(self.K, self.stage, group=self.group)          # forward transpose
+                self._all_to_all(self.K, self.stage)                                  # forward transpose
                 self.phase(1)
-                dist.all_to_all_single(self.stage, self.K, group=self.group)          # backward transpose
+                self._all_to_all(self.stage, self.K)                                  # backward transpose
                 self.phase(2)
-                dist.all_gather_into_tensor(self.gram, self.gram[self.rank * row:(self.rank + 1) * row], group=self.group)
+                self._all_gather_rows()
                 self.phase(3)
                 if tol > 0.0 and (it + 1) % check_every == 0 and self.status()[0]:
                     break
@@ -583,7 +610,9 @@ class SlabSolver(Solver):
     def _sum_over_ranks(self, values):
         import torch
         import torch.distributed as dist
-        t = torch.as_tensor(np.asarray(values, dtype=np.float64), device=self.device)
+        t = torch.as_tensor(np.asarray(values, dtype=np.float64))
+        if self._device_collectives():
+            t = t.to(self.device)
         dist.all_reduce(t, group=self.group)
         return t.cpu().numpy()
 

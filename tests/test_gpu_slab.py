@@ -139,3 +139,69 @@ def test_slab_argument_checks():
     with pytest.raises(lib.Rism3dError):
         lib.rism3d_slab_phase(one.ctx, 0)                    # not a slab run
     one.close()
+
+
+# ---- the multi-process driver (SlabSolver.iterate under torch.distributed) ------------------------------------------
+MP_WORKER = r"""
+import os, sys
+sys.path.insert(0, {root!r})
+import numpy as np
+import torch
+import torch.distributed as dist
+import paper_2403_01039_b200 as lib
+from workloads import Solute, load_chi, solvent_by_name
+
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo", rank=rank, world_size=world)       # one GPU on this box: the blocks travel through the host
+sv = solvent_by_name("water")
+k0, dk, chi = load_chi(sv.name)
+d = np.load({inputs!r})
+s = lib.SlabSolver((32, 32, 32), 0.5, sv.n_v, world, rank, closure="KH", mdiis_nvec=5)
+s.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+s.set_solute(d["xyz"], d["q"], d["sigma"], d["eps"])
+nd, rms = s.iterate(25, 0.0)
+mu, _ = s.free_energy()
+grad = s.gradient()
+np.savez(os.path.join({out!r}, f"rank{{rank}}.npz"), G=s.get_field("G"), TAU=s.get_field("TAU"), hist=s.rms_history(),
+         nd=nd, mu=mu, grad=grad)
+dist.barrier()
+dist.destroy_process_group()
+"""
+
+
+def test_two_processes_share_one_solve(tmp_path):
+    """SlabSolver.iterate as a multi-GPU job runs it: one process per rank, collectives between the phase calls.  Both
+    processes use this box's one GPU and a gloo group (host-side waits only; no kernel waits for another process)."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sol = _solute(21, 4, 1.5)
+    inputs = str(tmp_path / "solute.npz")
+    np.savez(inputs, xyz=sol.xyz, q=sol.q, sigma=sol.sigma, eps=sol.eps)
+    script = tmp_path / "mp_worker.py"
+    script.write_text(MP_WORKER.format(root=root, inputs=inputs, out=str(tmp_path)))
+    port = 29700 + (os.getpid() % 200)
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.PIPE, text=True))
+    for p in procs:
+        out, err = p.communicate(timeout=600)
+        assert p.returncode == 0, err[-3000:]
+    sv = solvent_by_name("water")
+    k0, dk, chi = load_chi(sv.name)
+    orc = o3.Rism3dOracle((32, 32, 32), 0.5, sv.n_v, closure="KH", mdiis_nvec=5)
+    orc.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+    orc.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps)
+    orc.iterate(25, 0.0)
+    r = [np.load(tmp_path / f"rank{k}.npz") for k in range(2)]
+    assert int(r[0]["nd"]) == 25
+    np.testing.assert_allclose(r[0]["hist"], orc.rms_history, rtol=1e-6, atol=1e-12)
+    assert np.array_equal(r[0]["hist"], r[1]["hist"])
+    assert np.max(np.abs(np.concatenate([r[0]["G"], r[1]["G"]], axis=1) - orc.get_field("G"))) <= 1e-9
+    mu_o, _ = orc.free_energy()
+    assert abs(float(r[0]["mu"]) - mu_o) <= 1e-7 * abs(mu_o) and float(r[0]["mu"]) == float(r[1]["mu"])
+    go = orc.solvation_gradient()
+    assert np.max(np.abs(r[1]["grad"] - go)) <= 1e-8 * max(1.0, np.max(np.abs(go)))
