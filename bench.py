@@ -532,6 +532,14 @@ def run_ours(args):
             except Exception as ex:                               # e.g. not enough device memory for C5
                 others[name] = {"error": str(ex)[:200]}
         torch.cuda.empty_cache()
+        slab = {}
+        for n_ranks in (2, 8):
+            try:
+                slab[f"x{n_ranks}"] = slab_lockstep(lib, args.workload, local_rank, n_ranks)
+            except Exception as ex:
+                slab[f"x{n_ranks}"] = {"error": str(ex)[:200]}
+            torch.cuda.empty_cache()
+        others["slab_decomposition"] = slab
 
     # ---- the oracle on the host cores (rank 0, single-GPU runs only) --------------------------------------------
     cpu = None
@@ -558,6 +566,125 @@ def run_ours(args):
     solver.close()
     if world > 1:
         dist.destroy_process_group()
+    return 0
+
+
+NVLINK_GBS_PER_DIRECTION = 900.0      # NVLink 5 per GPU and direction (nominal; no second GPU here to measure it)
+
+
+def slab_lockstep(lib, name: str, device: int, n_ranks: int, steps: int = 10) -> dict:
+    """The slab decomposition (include/rism3d.h "Slab decomposition") measured on ONE GPU: the n_ranks contexts of one
+    solve live in this process, peer tables point at each other's arrays, and the phases run rank after rank on one
+    stream.  What this times is every rank's own kernel work (CUDA events per rank and phase); what it cannot time is
+    the NVLink traffic (here the 'remote' rows land in the same HBM) and the overlap between ranks."""
+    import torch
+    cfg, sv, sol, (k0, dk, chi) = workload_inputs(name)
+    M, n_v = cfg.mdiis_nvec, sv.n_v
+    stream = torch.cuda.Stream(torch.device("cuda", device))
+    ranks = [lib.SlabSolver(cfg.n, cfg.spacing, n_v, n_ranks, r, closure=cfg.closure, pse_order=cfg.pse_order, mdiis_nvec=M,
+                            mdiis_b=cfg.mdiis_b, mdiis_restart=cfg.mdiis_restart, temperature=cfg.temperature,
+                            kappa=cfg.kappa, r_min=cfg.r_min, device=device, stream=stream) for r in range(n_ranks)]
+    try:
+        setup_ms = []
+        for r in ranks:
+            r.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+            setup_ms.append(r.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=cfg.rcut))
+        loc = [r.local for r in ranks]
+        for r in ranks:
+            r.connect_peers([l["K"] for l in loc], [l["gram"] for l in loc], [l["flags"] for l in loc])
+        lib.iterate_in_lockstep(ranks, max(M, 3), 0.0)                   # fill the history
+        ms = np.zeros((n_ranks, 4))
+        for r in ranks:
+            r.begin(0.0)
+        with torch.cuda.stream(stream):
+            for _ in range(steps):
+                for ph in range(4):
+                    for k, r in enumerate(ranks):
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        e0.record(stream)
+                        r.phase(ph)
+                        e1.record(stream)
+                        e1.synchronize()
+                        ms[k, ph] += e0.elapsed_time(e1)
+        for r in ranks:
+            r.end()
+        ms /= steps
+        per_rank = ms.sum(axis=1)
+        block = loc[0]["block_bytes"]
+        out_bytes = (n_ranks - 1) * block                                # leaves a rank per transposition
+        nvlink_ms = 2.0 * out_bytes / (NVLINK_GBS_PER_DIRECTION * 1e9) * 1e3
+        return {"workload": workload_label(cfg, sol), "n_ranks": n_ranks,
+                "how": "all ranks in one process on one GPU, peer tables, phases in lockstep (sequential)",
+                "phase_ms_slowest_rank": {"closure_zfwd+y_fwd": float(ms[:, 0].max()), "kspace_x": float(ms[:, 1].max()),
+                                          "y_inv+zinv_gram": float(ms[:, 2].max()), "gram_solve": float(ms[:, 3].max())},
+                "ms_per_iteration_slowest_rank": float(per_rank.max()), "ms_per_iteration_all_ranks": float(per_rank.sum()),
+                "setup_ms_slowest_rank": float(max(setup_ms)),
+                "bytes_leaving_a_rank_per_iteration": int(2 * out_bytes),
+                "nvlink_ms_per_iteration_at_nominal_900_GBs": nvlink_ms,
+                "note": "per-rank kernel time only: on n_ranks GPUs the ranks run side by side and the rows cross NVLink "
+                        "inside the y passes' stores / loads; neither is measurable on one GPU"}
+    finally:
+        for r in ranks:
+            r.close()
+
+
+def run_slab(args):
+    """--decompose slab: ONE solve shared by all ranks (strong scaling), one process per GPU, SlabSolver.iterate with
+    the process group's all-to-all between the phases.  Prints the contract line with "scaling": "strong"."""
+    import torch
+    import paper_2403_01039_b200 as lib
+    rank, local_rank, world = dist_env()
+    if world < 2:
+        raise RuntimeError("--decompose slab needs at least 2 ranks (torchrun --nproc-per-node N)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist_init("nccl")
+    import torch.distributed as dist
+    cfg, sv, sol, (k0, dk, chi) = workload_inputs(args.workload, 0)      # every rank the same solute
+    M, n_v = cfg.mdiis_nvec, sv.n_v
+    s = lib.SlabSolver(cfg.n, cfg.spacing, n_v, world, rank, closure=cfg.closure, pse_order=cfg.pse_order, mdiis_nvec=M,
+                       mdiis_b=cfg.mdiis_b, mdiis_restart=cfg.mdiis_restart, temperature=cfg.temperature, kappa=cfg.kappa,
+                       r_min=cfg.r_min, device=local_rank)
+    s.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
+    setup_ms = s.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=cfg.rcut)
+    warm = max(args.warmup, M, 3)
+    s.iterate(warm, 0.0)
+    launches0 = s.launch_count()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dist.barrier(); torch.cuda.synchronize(dev)
+    ev0.record(s.stream)
+    s.iterate(args.steps, 0.0)
+    ev1.record(s.stream)
+    dist.barrier(); torch.cuda.synchronize(dev)
+    (ms_max,) = reduce_scalars([ev0.elapsed_time(ev1)], "max", dev)
+    launches = s.launch_count() - launches0
+    # end to end: host atoms -> converged solve -> host g slabs
+    g_host = torch.empty((n_v,) + s.shape, dtype=torch.float64, pin_memory=True)
+    g_np = g_host.numpy()
+    dist.barrier(); torch.cuda.synchronize(dev)
+    t0 = time.perf_counter()
+    s.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=cfg.rcut)
+    it_conv, rms_conv = s.iterate(args.max_iter, cfg.tol)
+    mu, _ = s.free_energy()
+    for g in range(n_v):
+        lib.rism3d_get_field(s.ctx, lib.FIELDS["G"], g, g_np[g].ctypes.data, False)
+    torch.cuda.synchronize(dev)
+    (e2e_s,) = reduce_scalars([time.perf_counter() - t0], "max", dev)
+    clocks = sampler.stop() if sampler else None
+    if rank == 0:
+        cfgd = bench_config(cfg, sol, world)
+        cfgd["parallelism"] = f"slab x{world}: one solve, x planes in r space, y rows in k space, two all-to-all transposes per iteration"
+        print(json.dumps({
+            "metric": METRIC, "value": args.steps / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": warm, "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfgd, "setup_ms": setup_ms,
+            "e2e": {"value": it_conv / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(sol.n_atoms * 6 * 8),
+                    "d2h_bytes_per_step": int(g_np.nbytes + 64), "seconds_to_converge": e2e_s,
+                    "iterations_to_converge": int(it_conv), "converged": bool(rms_conv < cfg.tol), "dmu_kcal_mol": mu},
+            "gpu_launches": int(launches), "clocks": clocks}), flush=True)
+    s.close()
+    dist.destroy_process_group()
     return 0
 
 
@@ -622,10 +749,14 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-anderson", action="store_true", help="skip the extra modified-Anderson solve")
     ap.add_argument("--no-fft-compare", action="store_true", help="skip the cuFFT comparison")
+    ap.add_argument("--decompose", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: N independent solves (default, weak scaling) or ONE solve in x / y slabs (strong scaling)")
     args = ap.parse_args()
     if args.steps < 1:
         ap.error("--steps must be >= 1")
-    return run_reference(args) if args.impl == "reference" else run_ours(args)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_slab(args) if args.decompose == "slab" else run_ours(args)
 
 
 if __name__ == "__main__":
