@@ -26,6 +26,10 @@ EXPORTED_SYMBOLS = [
     "rism3d_slab_plan", "rism3d_slab_local", "rism3d_slab_set_peers", "rism3d_slab_begin", "rism3d_slab_phase",
     "rism3d_slab_status", "rism3d_slab_end",
 ]
+EXPORTED_SYMBOLS_1D = [
+    "rism1d_workspace_bytes", "rism1d_init", "rism1d_set_solvent", "rism1d_solve", "rism1d_get_pair", "rism1d_get_chi",
+    "rism1d_get_chi_types", "rism1d_thermo", "rism1d_launch_count", "rism1d_last_error", "rism1d_destroy",
+]
 
 
 class Rism3dError(RuntimeError):
@@ -55,6 +59,12 @@ class Rism3dParams(C.Structure):
         ("mdiis_b_min", C.c_double), ("mdiis_b_max", C.c_double),
         ("n_ranks", C.c_int), ("rank", C.c_int),
     ]
+
+
+class Rism1dParams(C.Structure):
+    _fields_ = [("n_sites", C.c_int), ("n_points", C.c_int), ("dr", C.c_double), ("temperature", C.c_double),
+                ("kappa", C.c_double), ("closure", C.c_int), ("pse_order", C.c_int), ("mdiis_nvec", C.c_int),
+                ("mdiis_b", C.c_double), ("mdiis_restart", C.c_double), ("device", C.c_int)]
 
 
 class Rism3dSlabInfo(C.Structure):
@@ -138,6 +148,29 @@ def load_library():
     lib.rism3d_slab_status.argtypes = [C.c_void_p, ip, ip, dp]
     lib.rism3d_slab_end.restype = C.c_int
     lib.rism3d_slab_end.argtypes = [C.c_void_p, ip, dp]
+    # ---- include/rism1d.h ----
+    lib.rism1d_workspace_bytes.restype = C.c_size_t
+    lib.rism1d_workspace_bytes.argtypes = [C.POINTER(Rism1dParams)]
+    lib.rism1d_init.restype = C.c_int
+    lib.rism1d_init.argtypes = [C.POINTER(C.c_void_p), C.POINTER(Rism1dParams), C.c_void_p, C.c_size_t, C.c_void_p]
+    lib.rism1d_set_solvent.restype = C.c_int
+    lib.rism1d_set_solvent.argtypes = [C.c_void_p, dp, dp, dp, dp, ip, dp]
+    lib.rism1d_solve.restype = C.c_int
+    lib.rism1d_solve.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_double, ip, dp]
+    lib.rism1d_get_pair.restype = C.c_int
+    lib.rism1d_get_pair.argtypes = [C.c_void_p, C.c_int, dp]
+    lib.rism1d_get_chi.restype = C.c_int
+    lib.rism1d_get_chi.argtypes = [C.c_void_p, dp]
+    lib.rism1d_get_chi_types.restype = C.c_int
+    lib.rism1d_get_chi_types.argtypes = [C.c_void_p, C.c_int, ip, dp]
+    lib.rism1d_thermo.restype = C.c_int
+    lib.rism1d_thermo.argtypes = [C.c_void_p, dp, dp, dp]
+    lib.rism1d_launch_count.restype = C.c_longlong
+    lib.rism1d_launch_count.argtypes = [C.c_void_p]
+    lib.rism1d_last_error.restype = C.c_char_p
+    lib.rism1d_last_error.argtypes = [C.c_void_p]
+    lib.rism1d_destroy.restype = None
+    lib.rism1d_destroy.argtypes = [C.c_void_p]
     _LIB = lib
     return lib
 
@@ -674,3 +707,149 @@ def iterate_in_lockstep(ranks, max_iter, tol=0.0):
                 break
     out = [r.end() for r in ranks]
     return out[0]
+
+
+# ---- the 1D solvent solve (include/rism1d.h) ---------------------------------------------------------------------------
+def _check1(ctx, status: int):
+    if status != 0:
+        lib = load_library()
+        msg = lib.rism1d_last_error(ctx).decode() if ctx else ""
+        raise Rism3dError(status, msg or lib.rism3d_status_string(status).decode())
+
+
+def rism1d_workspace_bytes(params: Rism1dParams) -> int:
+    return int(load_library().rism1d_workspace_bytes(C.byref(params)))
+
+
+def rism1d_init(params: Rism1dParams, d_workspace: int, nbytes: int, cuda_stream: int):
+    ctx = C.c_void_p()
+    st = load_library().rism1d_init(C.byref(ctx), C.byref(params), C.c_void_p(d_workspace), nbytes, C.c_void_p(cuda_stream))
+    if st != 0:
+        raise Rism3dError(st, rism3d_status_string(st))
+    return ctx
+
+
+def rism1d_set_solvent(ctx, q, sigma, eps, rho_site, species, bond):
+    q, sigma, eps, rho_site, bond = _f64(q), _f64(sigma), _f64(eps), _f64(rho_site), _f64(bond)
+    species = np.ascontiguousarray(np.asarray(species, dtype=np.int32))
+    _check1(ctx, load_library().rism1d_set_solvent(ctx, _dptr(q), _dptr(sigma), _dptr(eps), _dptr(rho_site),
+                                                   species.ctypes.data_as(C.POINTER(C.c_int)), _dptr(bond)))
+
+
+def rism1d_solve(ctx, charge_scale: float, max_iter: int, tol: float):
+    n_done, rms = C.c_int(), C.c_double()
+    _check1(ctx, load_library().rism1d_solve(ctx, float(charge_scale), int(max_iter), float(tol), C.byref(n_done), C.byref(rms)))
+    return n_done.value, rms.value
+
+
+def rism1d_get_pair(ctx, which: int, n_sites: int, n_points: int) -> np.ndarray:
+    out = np.empty((n_sites, n_sites, n_points - 1))
+    _check1(ctx, load_library().rism1d_get_pair(ctx, int(which), _dptr(out)))
+    return out
+
+
+def rism1d_get_chi(ctx, n_sites: int, n_points: int) -> np.ndarray:
+    out = np.empty((n_points - 1, n_sites, n_sites))
+    _check1(ctx, load_library().rism1d_get_chi(ctx, _dptr(out)))
+    return out
+
+
+def rism1d_get_chi_types(ctx, site_type, n_points: int) -> np.ndarray:
+    st = np.ascontiguousarray(np.asarray(site_type, dtype=np.int32))
+    n_types = int(st.max()) + 1
+    out = np.empty((n_points - 1, n_types, n_types))
+    _check1(ctx, load_library().rism1d_get_chi_types(ctx, n_types, st.ctypes.data_as(C.POINTER(C.c_int)), _dptr(out)))
+    return out
+
+
+def rism1d_thermo(ctx, n_sites: int):
+    chi_t, pr = C.c_double(), C.c_double()
+    c0 = np.empty((n_sites, n_sites))
+    _check1(ctx, load_library().rism1d_thermo(ctx, C.byref(chi_t), C.byref(pr), _dptr(c0)))
+    return chi_t.value, pr.value, c0
+
+
+def rism1d_launch_count(ctx) -> int:
+    return int(load_library().rism1d_launch_count(ctx))
+
+
+def rism1d_last_error(ctx) -> str:
+    return load_library().rism1d_last_error(ctx).decode()
+
+
+def rism1d_destroy(ctx):
+    load_library().rism1d_destroy(ctx)
+
+
+class Solver1d:
+    """Solvent-solvent 1D-RISM on the GPU: owns the workspace and the context; each method is one C-ABI call (the
+    charge ramp is a loop of solve calls).  Produces chi for rism3d_set_solvent_chi, chi_T and P."""
+
+    PAIRS = {"G": 0, "TAU": 1, "C_SR": 2}
+
+    def __init__(self, n_sites, n_points=16384, dr=0.025, temperature=298.0, kappa=1.0, closure="KH", pse_order=1,
+                 mdiis_nvec=10, mdiis_b=0.5, mdiis_restart=10.0, device=0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2403_01039_b200 needs a CUDA device (no CPU fallback)")
+        load_library()
+        p = Rism1dParams()
+        p.n_sites, p.n_points, p.dr, p.temperature, p.kappa = int(n_sites), int(n_points), float(dr), float(temperature), float(kappa)
+        p.closure, p.pse_order = CLOSURES[closure], int(pse_order)
+        p.mdiis_nvec, p.mdiis_b, p.mdiis_restart, p.device = int(mdiis_nvec), float(mdiis_b), float(mdiis_restart), int(device)
+        self.params, self.n_sites, self.n_points, self.dr = p, int(n_sites), int(n_points), float(dr)
+        nbytes = rism1d_workspace_bytes(p)
+        if nbytes == 0:
+            raise Rism3dError(-2, "unsupported site count / radial grid / MDIIS size")
+        self.device = torch.device("cuda", device)
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.stream = torch.cuda.Stream(self.device)
+        self.stream.wait_stream(torch.cuda.current_stream(self.device))
+        self.ctx = rism1d_init(p, self.workspace.data_ptr(), nbytes, self.stream.cuda_stream)
+
+    @property
+    def k(self) -> np.ndarray:
+        return np.arange(1, self.n_points) * (np.pi / (self.n_points * self.dr))
+
+    @property
+    def r(self) -> np.ndarray:
+        return np.arange(1, self.n_points) * self.dr
+
+    def close(self):
+        if getattr(self, "ctx", None) is not None:
+            rism1d_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_solvent(self, q, sigma, eps, rho_site, species, bond):
+        n = self.n_sites
+        for name, a in (("q", q), ("sigma", sigma), ("eps", eps), ("rho_site", rho_site), ("species", species)):
+            if np.shape(a) != (n,):
+                raise ValueError(f"{name} must have shape ({n},), got {np.shape(a)}")
+        if np.shape(bond) != (n, n):
+            raise ValueError(f"bond must have shape ({n}, {n}), got {np.shape(bond)}")
+        rism1d_set_solvent(self.ctx, q, sigma, eps, rho_site, species, bond)
+
+    def solve(self, charge_scale=1.0, max_iter=5000, tol=1e-10):
+        return rism1d_solve(self.ctx, charge_scale, max_iter, tol)
+
+    def pair(self, which="G") -> np.ndarray:
+        return rism1d_get_pair(self.ctx, self.PAIRS[which], self.n_sites, self.n_points)
+
+    def chi(self) -> np.ndarray:
+        return rism1d_get_chi(self.ctx, self.n_sites, self.n_points)
+
+    def chi_types(self, site_type) -> np.ndarray:
+        return rism1d_get_chi_types(self.ctx, site_type, self.n_points)
+
+    def thermo(self):
+        """-> (chi_T [A^3 mol/kcal], P [kcal/(mol A^3)], int c_sr,ab dr [n][n])"""
+        return rism1d_thermo(self.ctx, self.n_sites)
+
+    def launch_count(self) -> int:
+        return rism1d_launch_count(self.ctx)

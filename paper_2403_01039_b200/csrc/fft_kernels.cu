@@ -646,6 +646,13 @@ __global__ void __launch_bounds__(32)
   mdiis_bookkeeping_and_solve(st, s_solve, s_row, m, nother, aa, weighted ? s_row[nother + 1] : s_row[nother], n_values);
 }
 
+// the same for any array of double-double rows [n_rows][GRAM_SLOT][2] (the 1D solver's per-CTA partial sums)
+int launch_gram_solve_rows(DevState* st, const double* rows, int n_rows, const SolverParams& sp, double n_values,
+                           cudaStream_t s) {
+  gram_solve_kernel<<<1, 32, 0, s>>>(st, rows, n_rows, accel_args(sp), sp.accel == RISM3D_ACCEL_ANDERSON ? 1 : 0, n_values);
+  return 1;
+}
+
 int launch_gram_solve(const Grid& gr, const Buffers& b, const SolverParams& sp, cudaStream_t s) {
   gram_solve_kernel<<<1, 32, 0, s>>>(b.state, b.gram_x, gr.n_ranks, accel_args(sp), sp.accel == RISM3D_ACCEL_ANDERSON ? 1 : 0,
                                      (double)gr.npts_global * gr.nv_user);

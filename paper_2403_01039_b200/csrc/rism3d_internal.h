@@ -136,6 +136,7 @@ int launch_x_inv(const Grid&, const Buffers&, cudaStream_t);
 int launch_kspace_x(const Grid&, const Buffers&, cudaStream_t);
 int launch_y_inv(const Grid&, const Buffers&, bool use_state, cudaStream_t);   // slab runs: reads through bwd_src
 int launch_gram_solve(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);   // slab runs: sum the ranks' rows, solve
+int launch_gram_solve_rows(DevState*, const double* rows, int n_rows, const SolverParams&, double n_values, cudaStream_t);
 int launch_xbarrier(const Grid&, const Buffers&, cudaStream_t);                // peer mode: all ranks have reached this point
 int launch_zinv_residual(const Grid&, const Buffers&, const SolverParams&, double* d_raw_out, cudaStream_t);
 int zinv_ctas(const Grid&);                      // CTAs of zinv_residual (it writes one Gram partial per CTA)

@@ -8,13 +8,14 @@ import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 HEADER = os.path.join(ROOT, "include", "rism3d.h")
+HEADER_1D = os.path.join(ROOT, "include", "rism1d.h")
 
 
-def declared_functions():
-    """Names of the functions declared in include/rism3d.h (prototype = `name(` at the start of a declaration)."""
-    src = open(HEADER).read()
+def declared_functions(header=HEADER, prefix="rism3d_"):
+    """Names of the functions declared in a header of include/ (prototype = `name(` at the start of a declaration)."""
+    src = open(header).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)          # drop comments
-    names = re.findall(r"\b(rism3d_[a-z0-9_]+)\s*\(", src)
+    names = re.findall(r"\b(" + prefix + r"[a-z0-9_]+)\s*\(", src)
     return sorted(set(names))
 
 
@@ -42,11 +43,31 @@ def test_library_exports_every_declared_symbol(lib):
         assert callable(getattr(lib, name)), f"binding has no function {name}"
 
 
+def test_library_exports_every_symbol_of_the_1d_header(lib):
+    handle = lib.load_library()
+    names = declared_functions(HEADER_1D, "rism1d_")
+    assert "rism1d_solve" in names and "rism1d_get_chi" in names
+    for name in names:
+        assert hasattr(handle, name), f"librism3d.so does not export {name}"
+        assert callable(getattr(lib, name)), f"binding has no function {name}"
+    assert sorted(lib.EXPORTED_SYMBOLS_1D) == names
+    p = lib.Rism1dParams()
+    p.n_sites, p.n_points, p.dr, p.temperature, p.kappa, p.closure, p.pse_order = 3, 2048, 0.025, 298.0, 1.0, 1, 1
+    p.mdiis_nvec, p.mdiis_b, p.mdiis_restart = 10, 0.5, 10.0
+    assert lib.rism1d_workspace_bytes(p) > 0
+    for field, bad in [("n_sites", 9), ("n_points", 1000), ("n_points", 32768), ("dr", 0.0), ("mdiis_nvec", 17)]:
+        keep = getattr(p, field)
+        setattr(p, field, bad)
+        assert lib.rism1d_workspace_bytes(p) == 0
+        setattr(p, field, keep)
+
+
 def test_no_torch_types_in_the_abi():
-    src = open(HEADER).read()
-    code = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    assert "torch" not in code.lower() and "at::" not in code and "#include <cuda" not in code
-    assert 'extern "C"' in src
+    for header in (HEADER, HEADER_1D):
+        src = open(header).read()
+        code = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+        assert "torch" not in code.lower() and "at::" not in code and "#include <cuda" not in code
+        assert 'extern "C"' in src
 
 
 def test_workspace_bytes_and_argument_checks_without_a_device(lib):
