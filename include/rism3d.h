@@ -258,6 +258,17 @@ int rism3d_slab_local(rism3d_ctx* ctx, void** d_K, void** d_stage, void** d_gram
  * pointers valid in this process (HOST arrays of n_ranks pointers; entry `rank` is this rank's own). */
 int rism3d_slab_set_peers(rism3d_ctx* ctx, void* const* d_K, void* const* d_gram, void* const* d_flags);
 
+/* Mapping the peers' arrays into this process (CUDA IPC; one GPU per process on one node).  A workspace that is to
+ * be exported must be an allocation of its own: peer_alloc is a plain cudaMalloc on `device` (a sub-block of a caching
+ * allocator cannot be exported).  peer_export fills a 64-byte handle that another process turns into a DEVICE pointer
+ * valid in ITS address space with peer_open (which also enables peer access from `device` to the owner's GPU); the
+ * arrays of rism3d_slab_local sit at the same offsets in every rank's workspace. */
+int rism3d_peer_alloc(int device, size_t bytes, void** d_ptr);
+int rism3d_peer_free(int device, void* d_ptr);
+int rism3d_peer_export(int device, void* d_ptr, unsigned char handle[64]);
+int rism3d_peer_open(int device, const unsigned char handle[64], void** d_ptr);
+int rism3d_peer_close(int device, void* d_ptr);
+
 /* Phase calls of a staged run (also usable in peer mode when the caller orders the ranks itself):
  * begin sets the tolerance of the iterations that follow (as rism3d_iterate's tol) and clears the call's counters;
  * phase(0..3) enqueues that phase of one iteration; end applies the pending update (tau is then the new input), reads

@@ -25,6 +25,7 @@ EXPORTED_SYMBOLS = [
     "rism3d_debug_fft_inverse", "rism3d_last_error", "rism3d_status_string", "rism3d_destroy",
     "rism3d_slab_plan", "rism3d_slab_local", "rism3d_slab_set_peers", "rism3d_slab_begin", "rism3d_slab_phase",
     "rism3d_slab_status", "rism3d_slab_end",
+    "rism3d_peer_alloc", "rism3d_peer_free", "rism3d_peer_export", "rism3d_peer_open", "rism3d_peer_close",
 ]
 EXPORTED_SYMBOLS_1D = [
     "rism1d_workspace_bytes", "rism1d_init", "rism1d_set_solvent", "rism1d_solve", "rism1d_get_pair", "rism1d_get_chi",
@@ -148,6 +149,16 @@ def load_library():
     lib.rism3d_slab_status.argtypes = [C.c_void_p, ip, ip, dp]
     lib.rism3d_slab_end.restype = C.c_int
     lib.rism3d_slab_end.argtypes = [C.c_void_p, ip, dp]
+    lib.rism3d_peer_alloc.restype = C.c_int
+    lib.rism3d_peer_alloc.argtypes = [C.c_int, C.c_size_t, vpp]
+    lib.rism3d_peer_free.restype = C.c_int
+    lib.rism3d_peer_free.argtypes = [C.c_int, C.c_void_p]
+    lib.rism3d_peer_export.restype = C.c_int
+    lib.rism3d_peer_export.argtypes = [C.c_int, C.c_void_p, C.POINTER(C.c_ubyte)]
+    lib.rism3d_peer_open.restype = C.c_int
+    lib.rism3d_peer_open.argtypes = [C.c_int, C.POINTER(C.c_ubyte), vpp]
+    lib.rism3d_peer_close.restype = C.c_int
+    lib.rism3d_peer_close.argtypes = [C.c_int, C.c_void_p]
     # ---- include/rism1d.h ----
     lib.rism1d_workspace_bytes.restype = C.c_size_t
     lib.rism1d_workspace_bytes.argtypes = [C.POINTER(Rism1dParams)]
@@ -342,6 +353,39 @@ def rism3d_slab_set_peers(ctx, d_K, d_gram, d_flags):
     _check(ctx, load_library().rism3d_slab_set_peers(ctx, arr(d_K), arr(d_gram), arr(d_flags)))
 
 
+def rism3d_peer_alloc(device: int, nbytes: int) -> int:
+    ptr = C.c_void_p()
+    st = load_library().rism3d_peer_alloc(int(device), int(nbytes), C.byref(ptr))
+    if st != 0:
+        raise Rism3dError(st, f"cudaMalloc of {nbytes} bytes failed")
+    return ptr.value
+
+
+def rism3d_peer_free(device: int, ptr: int):
+    load_library().rism3d_peer_free(int(device), C.c_void_p(ptr))
+
+
+def rism3d_peer_export(device: int, ptr: int) -> bytes:
+    h = (C.c_ubyte * 64)()
+    st = load_library().rism3d_peer_export(int(device), C.c_void_p(ptr), h)
+    if st != 0:
+        raise Rism3dError(st, "cudaIpcGetMemHandle failed")
+    return bytes(h)
+
+
+def rism3d_peer_open(device: int, handle: bytes) -> int:
+    h = (C.c_ubyte * 64).from_buffer_copy(handle)
+    ptr = C.c_void_p()
+    st = load_library().rism3d_peer_open(int(device), h, C.byref(ptr))
+    if st != 0:
+        raise Rism3dError(st, "cudaIpcOpenMemHandle failed")
+    return ptr.value
+
+
+def rism3d_peer_close(device: int, ptr: int):
+    load_library().rism3d_peer_close(int(device), C.c_void_p(ptr))
+
+
 def rism3d_slab_begin(ctx, tol: float = 0.0):
     _check(ctx, load_library().rism3d_slab_begin(ctx, float(tol)))
 
@@ -372,7 +416,8 @@ class Solver:
 
     def __init__(self, n, spacing, n_sites, closure="KH", pse_order=1, temperature=298.0, mdiis_nvec=5,
                  mdiis_b=0.5, mdiis_restart=10.0, kappa=1.0, r_min=1e-3, origin=None, device=0,
-                 accelerator="MDIIS", anderson_s=(0.2, 0.0), mdiis_dynamic_b=None, n_ranks=1, rank=0, stream=None):
+                 accelerator="MDIIS", anderson_s=(0.2, 0.0), mdiis_dynamic_b=None, n_ranks=1, rank=0, stream=None,
+                 exportable=False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2403_01039_b200 needs a CUDA device (no CPU fallback)")
@@ -412,16 +457,27 @@ class Solver:
         if nbytes == 0:
             raise Rism3dError(-2, "unsupported grid / site count / MDIIS size")
         self.device = torch.device("cuda", device)
-        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self._raw_workspace = None
+        if exportable:
+            # an allocation of its own (plain cudaMalloc) that other processes can map: rism3d_peer_export
+            self._raw_workspace = rism3d_peer_alloc(device, nbytes)
+            self.workspace = None
+            self.workspace_ptr, self.workspace_bytes = self._raw_workspace, nbytes
+        else:
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.workspace_ptr, self.workspace_bytes = self.workspace.data_ptr(), nbytes
         # a stream of its own (not the legacy default stream): the library captures its iteration into CUDA graphs
         self.stream = torch.cuda.Stream(self.device) if stream is None else stream
         self.stream.wait_stream(torch.cuda.current_stream(self.device))     # the workspace allocation above
-        self.ctx = rism3d_init(p, self.workspace.data_ptr(), nbytes, self.stream.cuda_stream)
+        self.ctx = rism3d_init(p, self.workspace_ptr, nbytes, self.stream.cuda_stream)
 
     def close(self):
         if getattr(self, "ctx", None) is not None:
             rism3d_destroy(self.ctx)
             self.ctx = None
+        if getattr(self, "_raw_workspace", None) is not None:
+            rism3d_peer_free(self.device.index, self._raw_workspace)
+            self._raw_workspace = None
 
     def __del__(self):
         try:
@@ -564,16 +620,18 @@ class SlabSolver(Solver):
         self.group = group
         loc = rism3d_slab_local(self.ctx)
         self.local = loc
-        base = self.workspace.data_ptr()
+        base = self.workspace_ptr
+        self.K = self.stage = self.gram = None
+        if self.workspace is not None:                  # (an exportable workspace is for peer mode: nothing is staged)
+            def view(addr, nbytes):
+                return self.workspace[addr - base: addr - base + nbytes].view(torch.float64)
 
-        def view(addr, nbytes):
-            return self.workspace[addr - base: addr - base + nbytes].view(torch.float64)
-
-        nb = loc["block_bytes"] * self.n_ranks
-        self.K = view(loc["K"], nb)                     # [n_ranks][block]: block s came from rank s
-        self.stage = view(loc["stage"], nb)             # [n_ranks][block]: block d goes to rank d / came back from it
-        self.gram = view(loc["gram"], loc["gram_row_bytes"] * self.n_ranks)
+            nb = loc["block_bytes"] * self.n_ranks
+            self.K = view(loc["K"], nb)                 # [n_ranks][block]: block s came from rank s
+            self.stage = view(loc["stage"], nb)         # [n_ranks][block]: block d goes to rank d / came back from it
+            self.gram = view(loc["gram"], loc["gram_row_bytes"] * self.n_ranks)
         self.peer_mode = False
+        self._opened = []
 
     # -- phase calls ---------------------------------------------------------------------------------------------
     def begin(self, tol=0.0):
@@ -591,6 +649,56 @@ class SlabSolver(Solver):
     def connect_peers(self, d_K, d_gram, d_flags):
         rism3d_slab_set_peers(self.ctx, d_K, d_gram, d_flags)
         self.peer_mode = True
+
+    def connect_peers_ipc(self):
+        """Peer mode across processes (one GPU each, one node): every rank exports its workspace (created with
+        exportable=True), the handles travel through the process group, every rank maps the others' workspaces (CUDA
+        IPC; the arrays sit at the same offsets everywhere) and hands the addresses to rism3d_slab_set_peers."""
+        import torch.distributed as dist
+        if self._raw_workspace is None:
+            raise RuntimeError("connect_peers_ipc needs SlabSolver(..., exportable=True)")
+        handles = [None] * self.n_ranks
+        dist.all_gather_object(handles, rism3d_peer_export(self.device.index, self._raw_workspace), group=self.group)
+        off = {k: self.local[k] - self.workspace_ptr for k in ("K", "gram", "flags")}
+        bases = []
+        for r in range(self.n_ranks):
+            if r == self.rank:
+                bases.append(self.workspace_ptr)
+            else:
+                bases.append(rism3d_peer_open(self.device.index, handles[r]))
+                self._opened.append(bases[-1])
+        self.connect_peers([b + off["K"] for b in bases], [b + off["gram"] for b in bases], [b + off["flags"] for b in bases])
+        dist.barrier(group=self.group)
+
+    def iterate_host_ordered(self, max_iter, tol=0.0, check_every=8):
+        """Peer mode with the ranks kept in step by the HOST (stream synchronise + process-group barrier where the
+        phases meet) instead of the in-stream barrier kernel: for ranks whose kernels cannot be relied on to run at the
+        same time (several ranks time-slicing one GPU, as in the tests)."""
+        import torch.distributed as dist
+        if not self.peer_mode:
+            raise RuntimeError("iterate_host_ordered is for peer mode (connect_peers / connect_peers_ipc)")
+
+        def meet():
+            self.stream.synchronize()
+            dist.barrier(group=self.group)
+
+        self.begin(tol)
+        for it in range(max_iter):
+            self.phase(0); meet()
+            self.phase(1); meet()
+            self.phase(2); meet()
+            self.phase(3)
+            if tol > 0.0 and (it + 1) % check_every == 0 and self.status()[0]:
+                break
+        out = self.end()
+        meet()
+        return out
+
+    def close(self):
+        for ptr in getattr(self, "_opened", []):
+            rism3d_peer_close(self.device.index, ptr)
+        self._opened = []
+        super().close()
 
     # -- one process per GPU -------------------------------------------------------------------------------------
     def _device_collectives(self) -> bool:
@@ -676,8 +784,8 @@ def iterate_in_lockstep(ranks, max_iter, tol=0.0):
     stream = ranks[0].stream
     assert all(r.stream is stream for r in ranks), "lockstep ranks share one stream"
     peer = ranks[0].peer_mode
-    blk = ranks[0].K.numel() // P
-    row = ranks[0].gram.numel() // P
+    blk = ranks[0].local["block_bytes"] // 8
+    row = ranks[0].local["gram_row_bytes"] // 8
     for r in ranks:
         r.begin(tol)
     with torch.cuda.stream(stream):

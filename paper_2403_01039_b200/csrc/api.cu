@@ -931,6 +931,42 @@ extern "C" int rism3d_slab_set_peers(rism3d_ctx* ctx, void* const* d_K, void* co
   return RISM3D_OK;
 }
 
+// ---- CUDA IPC helpers for peer mode ----
+static_assert(sizeof(cudaIpcMemHandle_t) == 64, "the ABI passes IPC handles as 64 bytes");
+
+extern "C" int rism3d_peer_alloc(int device, size_t bytes, void** d_ptr) {
+  if (!d_ptr || bytes == 0) return RISM3D_ERR_ARG;
+  DeviceGuard guard(device);
+  return cudaMalloc(d_ptr, bytes) == cudaSuccess ? RISM3D_OK : RISM3D_ERR_CUDA;
+}
+
+extern "C" int rism3d_peer_free(int device, void* d_ptr) {
+  DeviceGuard guard(device);
+  return cudaFree(d_ptr) == cudaSuccess ? RISM3D_OK : RISM3D_ERR_CUDA;
+}
+
+extern "C" int rism3d_peer_export(int device, void* d_ptr, unsigned char handle[64]) {
+  if (!d_ptr || !handle) return RISM3D_ERR_ARG;
+  DeviceGuard guard(device);
+  cudaIpcMemHandle_t h;
+  if (cudaIpcGetMemHandle(&h, d_ptr) != cudaSuccess) return RISM3D_ERR_CUDA;
+  memcpy(handle, &h, 64);
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_peer_open(int device, const unsigned char handle[64], void** d_ptr) {
+  if (!d_ptr || !handle) return RISM3D_ERR_ARG;
+  DeviceGuard guard(device);
+  cudaIpcMemHandle_t h;
+  memcpy(&h, handle, 64);
+  return cudaIpcOpenMemHandle(d_ptr, h, cudaIpcMemLazyEnablePeerAccess) == cudaSuccess ? RISM3D_OK : RISM3D_ERR_CUDA;
+}
+
+extern "C" int rism3d_peer_close(int device, void* d_ptr) {
+  DeviceGuard guard(device);
+  return cudaIpcCloseMemHandle(d_ptr) == cudaSuccess ? RISM3D_OK : RISM3D_ERR_CUDA;
+}
+
 extern "C" int rism3d_slab_begin(rism3d_ctx* ctx, double tol) {
   if (!ctx) return RISM3D_ERR_ARG;
   ON_CTX_DEVICE(ctx);

@@ -156,10 +156,17 @@ dist.init_process_group("gloo", rank=rank, world_size=world)       # one GPU on 
 sv = solvent_by_name("water")
 k0, dk, chi = load_chi(sv.name)
 d = np.load({inputs!r})
-s = lib.SlabSolver((32, 32, 32), 0.5, sv.n_v, world, rank, closure="KH", mdiis_nvec=5)
+peer = {peer!r}
+s = lib.SlabSolver((32, 32, 32), 0.5, sv.n_v, world, rank, closure="KH", mdiis_nvec=5, exportable=peer)
 s.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
 s.set_solute(d["xyz"], d["q"], d["sigma"], d["eps"])
-nd, rms = s.iterate(25, 0.0)
+if peer:
+    # the other process's arrays mapped through CUDA IPC: this rank's y pass stores into THAT process's memory; the
+    # host keeps the ranks in step (both time-slice one GPU: no kernel may wait for the other)
+    s.connect_peers_ipc()
+    nd, rms = s.iterate_host_ordered(25, 0.0)
+else:
+    nd, rms = s.iterate(25, 0.0)
 mu, _ = s.free_energy()
 grad = s.gradient()
 np.savez(os.path.join({out!r}, f"rank{{rank}}.npz"), G=s.get_field("G"), TAU=s.get_field("TAU"), hist=s.rms_history(),
@@ -169,9 +176,12 @@ dist.destroy_process_group()
 """
 
 
-def test_two_processes_share_one_solve(tmp_path):
-    """SlabSolver.iterate as a multi-GPU job runs it: one process per rank, collectives between the phase calls.  Both
-    processes use this box's one GPU and a gloo group (host-side waits only; no kernel waits for another process)."""
+@pytest.mark.parametrize("peer", [False, True])
+def test_two_processes_share_one_solve(tmp_path, peer):
+    """SlabSolver as a multi-GPU job runs it: one process per rank.  Both processes use this box's one GPU and a gloo
+    group (host-side waits only; no kernel waits for another process).  peer = False: staged blocks and collectives
+    between the phase calls; peer = True: each process maps the other's workspace (CUDA IPC) and the transposes are
+    stores into / loads from the other process's memory."""
     import os
     import subprocess
     import sys
@@ -180,7 +190,7 @@ def test_two_processes_share_one_solve(tmp_path):
     inputs = str(tmp_path / "solute.npz")
     np.savez(inputs, xyz=sol.xyz, q=sol.q, sigma=sol.sigma, eps=sol.eps)
     script = tmp_path / "mp_worker.py"
-    script.write_text(MP_WORKER.format(root=root, inputs=inputs, out=str(tmp_path)))
+    script.write_text(MP_WORKER.format(root=root, inputs=inputs, out=str(tmp_path), peer=peer))
     port = 29700 + (os.getpid() % 200)
     procs = []
     for rank in range(2):
