@@ -540,6 +540,10 @@ def run_ours(args):
                 slab[f"x{n_ranks}"] = {"error": str(ex)[:200]}
             torch.cuda.empty_cache()
         others["slab_decomposition"] = slab
+        try:
+            others["rism1d"] = rism1d_block(lib, cfg.solvent, local_rank)
+        except Exception as ex:
+            others["rism1d"] = {"error": str(ex)[:200]}
 
     # ---- the oracle on the host cores (rank 0, single-GPU runs only) --------------------------------------------
     cpu = None
@@ -626,6 +630,37 @@ def slab_lockstep(lib, name: str, device: int, n_ranks: int, steps: int = 10) ->
     finally:
         for r in ranks:
             r.close()
+
+
+def rism1d_block(lib, solvent_name: str, device: int) -> dict:
+    """The GPU 1D solvent solve (include/rism1d.h) that makes the chi table of the workload's solvent: the production
+    settings of oracle/make_chi_tables.py (16 384 radial points at 0.025 A, seven-step charge ramp, MDIIS 10, b = 0.3,
+    tol 1e-10), wall time with the host in the loop, and how far the result is from the stored table."""
+    import torch
+    from workloads import load_chi, solvent_by_name
+    sv = solvent_by_name(solvent_name)
+    ramp = (0.0, 0.25, 0.5, 0.75, 0.85, 0.95, 1.0)
+    one = lib.Solver1d(sv.n_s, n_points=16384, dr=0.025, mdiis_nvec=10, mdiis_b=0.3, mdiis_restart=0.0, device=device)
+    try:
+        one.set_solvent(sv.q[sv.site_type], sv.sigma[sv.site_type], sv.eps[sv.site_type], sv.species_rho[sv.site_species],
+                        sv.site_species, sv.bond)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        iters, rms = 0, 0.0
+        for lam in ramp:
+            n, rms = one.solve(lam, 3000, 1e-10)
+            iters += n
+        chi = one.chi_types(sv.site_type)
+        chi_t, pressure, _ = one.thermo()
+        secs = time.perf_counter() - t0
+        k0, dk, table = load_chi(sv.name)
+        return {"solvent": sv.name, "full_sites": int(sv.n_s), "radial_points": 16384, "charge_ramp": list(ramp),
+                "iterations": int(iters), "seconds": secs, "ms_per_iteration": secs / max(iters, 1) * 1e3,
+                "kernel_launches": int(one.launch_count()), "rms_last": rms, "chi_T_A3_mol_per_kcal": chi_t,
+                "pressure_kcal_per_mol_A3": pressure,
+                "max_rel_diff_to_stored_oracle_table": float(np.max(np.abs(chi[:table.shape[0]] - table)) / np.max(np.abs(table)))}
+    finally:
+        one.close()
 
 
 def run_slab(args):
