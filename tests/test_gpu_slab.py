@@ -114,15 +114,15 @@ def test_staged_and_peer_mode_agree_bit_for_bit_and_with_one_rank():
     assert np.max(np.abs(_gather(staged, "TAU") - one.get_field("TAU"))) <= 1e-10
 
 
-@pytest.mark.parametrize("variant", ["anderson", "dynamic_b", "hnc_m1"])
+@pytest.mark.parametrize("variant", ["anderson", "dynamic_b", "pse3_m1"])
 def test_slab_ranks_with_the_other_accelerators(variant):
     """the modified Anderson method (weighted Gram row + the unweighted one for the rms travel together), the dynamic
-    damping (the update reads both histories) and damped Picard iteration (M = 1) under the slab decomposition"""
+    damping (the update reads both histories) and damped Picard iteration (M = 1, PSE-3) under the slab decomposition"""
     import paper_2403_01039_b200 as lib
     sol = _solute(9, 3, 1.2)
     kw = {"anderson": dict(closure="KH", accelerator="ANDERSON", mdiis_b=0.6, anderson_s=(0.2, 0.0)),
           "dynamic_b": dict(closure="KH", mdiis_nvec=4, mdiis_dynamic_b=(0.1, 1.0)),
-          "hnc_m1": dict(closure="HNC", mdiis_nvec=1, mdiis_b=0.3)}[variant]
+          "pse3_m1": dict(closure="PSE", pse_order=3, mdiis_nvec=1, mdiis_b=0.2)}[variant]
     orc, ranks, sv = _make((32, 32, 32), 0.5, "water", 4, sol, 0.0, True, **kw)
     orc.iterate(25, 0.0)
     lib.iterate_in_lockstep(ranks, 25, 0.0)
