@@ -294,7 +294,7 @@ __device__ __forceinline__ cplx kspace_point_row(cplx csr, cplx ph, double qg, c
 template <int N, int NV>
 __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB)
     kspace2_kernel(const __grid_constant__ CUtensorMap tm_work, const __grid_constant__ CUtensorMap tm_phik,
-                   const double* __restrict__ chi_shell, const double* __restrict__ qv, Twiddle tw,
+                   cplx* __restrict__ work, const double* __restrict__ chi_shell, const double* __restrict__ qv, Twiddle tw,
                    const DevState* __restrict__ st, KGeom kg, unsigned nitems) {
   if (st->done) return;
   using K = Kspace2Cfg<N, NV>;
@@ -332,22 +332,17 @@ __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB
   }
   __syncthreads();
   unsigned item = blockIdx.x;
-  if (STAGES == 2 && tid == 0 && item < nitems) issue(item, 0);
+  if (tid == 0 && item < nitems) issue(item, 0);
   unsigned n_done = 0;
   for (; item < nitems; item += gridDim.x, ++n_done) {
     const int b = (STAGES == 2) ? (int)(n_done & 1) : 0;
+    const unsigned next = item + gridDim.x;
     if constexpr (STAGES == 2) {
-      const unsigned next = item + gridDim.x;
       if (tid == 0 && next < nitems) {
         tma_wait_read();                             // the store of the previous item has left stage b ^ 1
         issue(next, b ^ 1);
       }
-    } else {
-      if (tid == 0) {
-        tma_wait_read();                             // the store of the previous item has left the stage
-        issue(item, 0);
-      }
-    }
+    }                                                // (one stage: the next tile is requested inside the last pass)
     cplx* sm = stages + b * K::STAGE + col;
     const cplx* sph = stages + b * K::STAGE + K::ITEM + col / NV;
     auto ld_sm = [&](int i) { return sm[i * C]; };
@@ -397,21 +392,36 @@ __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB
       const PassATw<R1> a(a0, astep);
 #pragma unroll
       for (int k1 = 0; k1 < R1; ++k1) x[k1] = cmulc(ld_sm(k1 * S1 + t), a.get(k1));
+      if constexpr (STAGES == 1) {
+        // single-buffered tiles (n = 512): once every thread holds its values the stage is free -- the next tile is
+        // requested now and lands under this pass's arithmetic; the results leave from registers (128-byte rows)
+        __syncthreads();
+        if (tid == 0 && next < nitems) issue(next, 0);
+      }
       Dft<R1, +1>::run(x);
       HalfShiftAll<R1, +1>::run(x);
+      if constexpr (STAGES == 1) {
+        cplx* dst = work + (size_t)item * C + col;
+        const size_t ES = (size_t)kg.nyl * Q;          // stride of the x axis
 #pragma unroll
-      for (int m1 = 0; m1 < R1; ++m1) st_sm(m1 * S1 + t, cscale(x[m1], scale));   // in place: the slots this thread read
+        for (int m1 = 0; m1 < R1; ++m1) dst[(size_t)(m1 * S1 + t) * ES] = cscale(x[m1], scale);
+      } else {
+#pragma unroll
+        for (int m1 = 0; m1 < R1; ++m1) st_sm(m1 * S1 + t, cscale(x[m1], scale));   // in place: the slots this thread read
+      }
     }
-    fence_proxy_async();
-    __syncthreads();
-    if (tid == 0) {
+    if constexpr (STAGES == 2) {
+      fence_proxy_async();
+      __syncthreads();
+      if (tid == 0) {
 #pragma unroll
-      for (int bx = 0; bx < K::NBOX; ++bx)
-        tma_store_2d(&tm_work, (int)(item * C * 2), bx * K::BOX_ROWS, stages + b * K::STAGE + bx * K::BOX_ROWS * C);
-      tma_commit();
+        for (int bx = 0; bx < K::NBOX; ++bx)
+          tma_store_2d(&tm_work, (int)(item * C * 2), bx * K::BOX_ROWS, stages + b * K::STAGE + bx * K::BOX_ROWS * C);
+        tma_commit();
+      }
     }
   }
-  if (tid == 0) tma_wait_all();
+  if (STAGES == 2 && tid == 0) tma_wait_all();
 }
 
 template <int N, int NV>
@@ -423,7 +433,7 @@ static int launch_kspace2_nv(const Grid& gr, const Buffers& b, cudaStream_t s) {
   Twiddle tw{b.tw, gr.nmax / N, 2 * gr.nmax - 1};
   unsigned grid = (unsigned)(gr.num_sms * K::MINB);
   if (grid > nitems) grid = nitems;
-  kern<<<grid, K::NT, K::SHM, s>>>(b.tm_work, b.tm_phik, b.chi_shell, b.qv, tw, b.state, make_kgeom(gr), nitems);
+  kern<<<grid, K::NT, K::SHM, s>>>(b.tm_work, b.tm_phik, b.kbuf, b.chi_shell, b.qv, tw, b.state, make_kgeom(gr), nitems);
   return 1;
 }
 
