@@ -298,6 +298,13 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
     ctx->b.n_gram_dst = 1;
     ctx->b.peer_mode = false;
   }
+  if (y_uses_tma(g.ny, g.n_ranks)) {
+    const uint64_t row = (uint64_t)g.q() * 2;                                                // doubles per (ix, iy) row
+    if (!make_tensor_map_2d(&ctx->b.tm_ywork, ctx->b.work, row, (uint64_t)g.nxl * g.ny, row * 8, 16, (uint32_t)g.ny)) {
+      delete ctx;
+      return RISM3D_ERR_CUDA;
+    }
+  }
   cudaError_t e = cudaMallocHost((void**)&ctx->h_hdr, sizeof(StateHeader));
   if (e == cudaSuccess && g.n_ranks > 1) e = cudaMemsetAsync(ctx->b.gram_x, 0, (size_t)MAX_RANKS * GRAM_SLOT * 16, ctx->stream);
   if (e == cudaSuccess && g.n_ranks > 1) e = cudaMemsetAsync(ctx->b.xflags, 0, (MAX_RANKS + 1) * sizeof(unsigned long long), ctx->stream);

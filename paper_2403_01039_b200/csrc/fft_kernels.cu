@@ -14,10 +14,11 @@
 #include "fft_core.cuh"
 #include "mdiis_device.cuh"
 #include "rism3d_internal.h"
+#include "tma.cuh"
 
 namespace r3d {
 
-extern __shared__ double2 smem_dyn[];
+extern __shared__ __align__(128) double2 smem_dyn[];
 
 constexpr int COLS = 8;   // complex columns per tile row = 128-byte runs in global memory
 
@@ -170,6 +171,134 @@ static int launch_strided_n(const Grid& gr, const Buffers& b, bool x_axis, bool 
   return 1;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Two-pass y transform for the long lines (64 = 8 x 8, 128 = 16 x 8, 256 = 16 x 16), single-rank runs: the scheme of the
+// k-space pass (kspace_kernel.cu) without its arithmetic.  Tiles of N rows x 128 bytes arrive by TMA (one request per
+// tile, two stages, no LDGSTS issue slots and no staging registers), each thread does one radix-R1 butterfly per outer
+// pass with twiddles generated from two seeds, the other pass runs on registers and the results leave from registers as
+// 128-byte rows: 2 loads + 1 store of the tile in shared memory per work item instead of 3 + 3 (cp.async staging
+// included) in the three-pass kernel above.
+// ------------------------------------------------------------------------------------------------
+template <int N> struct YPlan2 { enum { OK = 0, R1 = 1, R2 = 1 }; };
+template <> struct YPlan2<64>  { enum { OK = 1, R1 = 8,  R2 = 8 }; };
+template <> struct YPlan2<128> { enum { OK = 1, R1 = 16, R2 = 8 }; };
+template <> struct YPlan2<256> { enum { OK = 1, R1 = 16, R2 = 16 }; };
+
+template <int N>
+struct Y2Cfg {
+  enum { R1 = YPlan2<N>::R1, R2 = YPlan2<N>::R2, T = N / R1, NT = T * COLS, NB = N / R2, IB = NB / T,
+         ITEM = N * COLS, TILE_BYTES = ITEM * (int)sizeof(cplx), SHM = 2 * TILE_BYTES + 64,
+         FIT = 227 * 1024 / (SHM + 1024), CAP = (N >= 256) ? 2 : 4, MINB = FIT < CAP ? FIT : CAP };
+};
+
+template <int N, bool INV>
+__global__ void __launch_bounds__(Y2Cfg<N>::NT, Y2Cfg<N>::MINB)
+    fft_y2_kernel(const __grid_constant__ CUtensorMap tm, cplx* __restrict__ data, Twiddle tw,
+                  const DevState* __restrict__ st, unsigned chunks_per_plane, size_t plane_stride, size_t es,
+                  unsigned nitems) {
+  if (st != nullptr && st->done) return;
+  using K = Y2Cfg<N>;
+  constexpr int R1 = K::R1, R2 = K::R2, T = K::T, C = COLS, S1 = N / R1, NB = K::NB, IB = K::IB;
+  const int tid = threadIdx.x;
+  const int col = tid % C, t = tid / C;
+  const cplx a0 = tw(t), astep = tw(2 * t);          // exp(-i pi t / N) and its square: a[k1] = a0 * astep^k1
+  cplx* stages = smem_dyn;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem_dyn + 2 * K::ITEM);
+  auto issue = [&](unsigned it, int b) {
+    mbar_arrive_expect_tx(&bars[b], K::TILE_BYTES);
+    tma_load_2d(stages + b * K::ITEM, &tm, (int)((it % chunks_per_plane) * C * 2), (int)((it / chunks_per_plane) * N), &bars[b]);
+  };
+  if (tid == 0) {
+    mbar_init(&bars[0], 1);
+    mbar_init(&bars[1], 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+  unsigned item = blockIdx.x;
+  if (tid == 0 && item < nitems) issue(item, 0);
+  unsigned n_done = 0;
+  for (; item < nitems; item += gridDim.x, ++n_done) {
+    const int b = n_done & 1;
+    const unsigned next = item + gridDim.x;
+    if (tid == 0 && next < nitems) issue(next, b ^ 1);   // (every thread left stage b ^ 1 before the barrier that ended the last item)
+    cplx* sm = stages + b * K::ITEM + col;
+    auto ld_sm = [&](int i) { return sm[i * C]; };
+    auto st_sm = [&](int i, cplx v) { sm[i * C] = v; };
+    cplx* base = data + (size_t)(item / chunks_per_plane) * plane_stride + (size_t)(item % chunks_per_plane) * C + col;
+    mbar_wait(&bars[b], (n_done >> 1) & 1);
+    if constexpr (!INV) {
+      {                                              // pass A: half-integer shift, radix R1 over m1, twiddle
+        cplx x[R1];
+#pragma unroll
+        for (int m1 = 0; m1 < R1; ++m1) x[m1] = ld_sm(m1 * S1 + t);
+        HalfShiftAll<R1, -1>::run(x);
+        Dft<R1, -1>::run(x);
+        const PassATw<R1> a(a0, astep);
+#pragma unroll
+        for (int k1 = 0; k1 < R1; ++k1) st_sm(k1 * S1 + t, cmul(x[k1], a.get(k1)));
+      }
+      __syncthreads();
+#pragma unroll
+      for (int i = 0; i < IB; ++i) {                 // pass B on registers, rows out in natural order
+        const int blk = t + i * T;
+        cplx x[R2];
+#pragma unroll
+        for (int m = 0; m < R2; ++m) x[m] = ld_sm(blk * R2 + m);
+        Dft<R2, -1>::run(x);
+#pragma unroll
+        for (int k = 0; k < R2; ++k) base[(size_t)(blk + NB * k) * es] = x[k];
+      }
+    } else {
+      cplx y[IB][R2];                                // first inverse stage: rows blk + NB k, natural order in the tile
+#pragma unroll
+      for (int i = 0; i < IB; ++i)
+#pragma unroll
+        for (int k = 0; k < R2; ++k) y[i][k] = ld_sm((t + i * T) + NB * k);
+      __syncthreads();                               // every row has been read before any slot is rewritten
+#pragma unroll
+      for (int i = 0; i < IB; ++i) {
+        Dft<R2, +1>::run(y[i]);
+#pragma unroll
+        for (int r = 0; r < R2; ++r) st_sm((t + i * T) * R2 + r, y[i][r]);
+      }
+      __syncthreads();
+      {                                              // last stage: conjugate twiddle, radix R1 over k1, shift, 1/N
+        cplx x[R1];
+        const PassATw<R1> a(a0, astep);
+#pragma unroll
+        for (int k1 = 0; k1 < R1; ++k1) x[k1] = cmulc(ld_sm(k1 * S1 + t), a.get(k1));
+        Dft<R1, +1>::run(x);
+        HalfShiftAll<R1, +1>::run(x);
+        const double scale = 1.0 / (double)N;
+#pragma unroll
+        for (int m1 = 0; m1 < R1; ++m1) base[(size_t)(m1 * S1 + t) * es] = cscale(x[m1], scale);
+      }
+    }
+    __syncthreads();                                 // stage b is free again
+  }
+}
+
+template <int N, bool INV>
+static int launch_y2_n(const Grid& gr, const Buffers& b, bool use_state, cudaStream_t s) {
+  if constexpr (YPlan2<N>::OK) {
+    using K = Y2Cfg<N>;
+    const size_t Q = gr.q();
+    const unsigned cpp = (unsigned)(Q / COLS), nitems = (unsigned)gr.nxl * cpp;
+    auto kern = fft_y2_kernel<N, INV>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SHM) != cudaSuccess) return 0;
+    Twiddle tw{b.tw, gr.nmax / N, 2 * gr.nmax - 1};
+    unsigned grid = (unsigned)(gr.num_sms * K::MINB);
+    if (grid > nitems) grid = nitems;
+    kern<<<grid, K::NT, K::SHM, s>>>(b.tm_ywork, b.work, tw, use_state ? b.state : nullptr, cpp, (size_t)gr.ny * Q, Q, nitems);
+    return 1;
+  } else {
+    return 0;
+  }
+}
+
+// true when the y passes of this grid take the two-pass TMA kernel (the API layer then builds its tensor map)
+bool y_uses_tma(int ny, int n_ranks) { return n_ranks == 1 && (ny == 64 || ny == 128 || ny == 256); }
+
 #define R3D_DISPATCH_N(n, CALL)                    \
   switch (n) {                                     \
     case 8: CALL(8); break;                        \
@@ -184,6 +313,13 @@ static int launch_strided_n(const Grid& gr, const Buffers& b, bool x_axis, bool 
 
 int launch_y_fwd(const Grid& g, const Buffers& b, bool use_state, cudaStream_t s) {
   int k = 0;
+  if (y_uses_tma(g.ny, g.n_ranks)) {
+    switch (g.ny) {
+      case 64: return launch_y2_n<64, false>(g, b, use_state, s);
+      case 128: return launch_y2_n<128, false>(g, b, use_state, s);
+      default: return launch_y2_n<256, false>(g, b, use_state, s);
+    }
+  }
 #define CALL(N) k = launch_strided_n<N, false>(g, b, false, use_state, s)
   R3D_DISPATCH_N(g.ny, CALL)
 #undef CALL
@@ -191,6 +327,13 @@ int launch_y_fwd(const Grid& g, const Buffers& b, bool use_state, cudaStream_t s
 }
 int launch_y_inv(const Grid& g, const Buffers& b, bool use_state, cudaStream_t s) {
   int k = 0;
+  if (y_uses_tma(g.ny, g.n_ranks)) {
+    switch (g.ny) {
+      case 64: return launch_y2_n<64, true>(g, b, use_state, s);
+      case 128: return launch_y2_n<128, true>(g, b, use_state, s);
+      default: return launch_y2_n<256, true>(g, b, use_state, s);
+    }
+  }
 #define CALL(N) k = launch_strided_n<N, true>(g, b, false, use_state, s)
   R3D_DISPATCH_N(g.ny, CALL)
 #undef CALL

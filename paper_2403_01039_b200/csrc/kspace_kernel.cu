@@ -211,43 +211,6 @@ struct Kspace2Cfg {
          MINB = FIT < CAP ? FIT : CAP };
 };
 
-// a[k] = a0 * s^k, k < R (R a power of two): s^2, s^4, ... by squaring, then a[k + h] = a[k] * s^h -- log2(R) dependent
-// products instead of a chain of R - 1
-template <int R>
-__device__ __forceinline__ void twiddle_powers(cplx (&a)[R], cplx a0, cplx s) {
-  a[0] = a0;
-  cplx sh = s;
-#pragma unroll
-  for (int h = 1; h < R; h *= 2) {
-#pragma unroll
-    for (int k = 0; k < h; ++k) a[k + h] = cmul(a[k], sh);
-    if (2 * h < R) sh = cmul(sh, sh);
-  }
-}
-// The pass-A twiddles of one thread, a0 * s^k1 for k1 < R1.  Up to R1 = 16 all of them live in registers; for R1 = 32
-// (beside 32 complex data values) only s^0..s^7 and the four chunk bases a0 s^(8c) do, and get() forms the product.
-template <int R1>
-struct PassATw {
-  static constexpr int CH = (R1 > 16) ? 8 : R1, NCH = R1 / CH;
-  cplx p[CH];      // NCH == 1: a0 s^k ;  else s^k, k < CH
-  cplx base[NCH];  // a0 s^(CH c) (unused when NCH == 1)
-  __device__ __forceinline__ PassATw(cplx a0, cplx s) {
-    if constexpr (NCH == 1) {
-      twiddle_powers<CH>(p, a0, s);
-      base[0] = a0;
-    } else {
-      twiddle_powers<CH>(p, make_double2(1.0, 0.0), s);
-      const cplx sc = cmul(p[CH - 1], s);                    // s^CH
-      twiddle_powers<NCH>(base, a0, sc);
-    }
-  }
-  __device__ __forceinline__ cplx get(int k1) const {        // k1 folds at compile time in unrolled loops
-    if constexpr (NCH == 1) return p[k1];
-    else return (k1 % CH == 0) ? base[k1 / CH] : cmul(base[k1 / CH], p[k1 % CH]);
-  }
-};
-
-// chi row of one k point for this lane's site (kspace_point consumes it)
 // L2 policy of the chi gathers: keep the shell table resident (evict_last) under the streaming tiles -- at 512^3 the
 // table is 12.5 MB and, without the hint, a tenth of the pass's DRAM reads were table rows coming back
 __device__ __forceinline__ uint64_t l2_keep_policy() {

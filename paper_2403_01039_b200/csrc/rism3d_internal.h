@@ -108,6 +108,8 @@ struct Buffers {
   // TMA descriptors of the k-space pass (built by rism3d_init when kspace_uses_tma(n)): `work` as a 2D array of doubles
   // [jx][2 n Q] with boxes of n rows x 128 bytes, `phik` as [jx][2 n n/2] with boxes of n rows x (8 / nv) complex
   CUtensorMap tm_work, tm_phik;
+  // the y passes (single-rank runs, ny = 64, 128, 256): `work` as [nxl * ny][2 Q] doubles, boxes of ny rows x 128 bytes
+  CUtensorMap tm_ywork;
 };
 
 struct SolverParams {
@@ -126,6 +128,7 @@ struct SolverParams {
 // dynamic shared memory of kspace_x for this grid (0: unsupported n / nv); the API layer checks it against the device
 int kspace_smem_bytes(int nx, int nv);
 bool kspace_uses_tma(int nx);
+bool y_uses_tma(int ny, int n_ranks);
 
 // ---- launchers (each returns the number of kernels it launched; errors surface via cudaGetLastError) ----
 // fft_kernels.cu
