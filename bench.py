@@ -671,10 +671,13 @@ def run_slab(args):
     rank, local_rank, world = dist_env()
     if world < 2:
         raise RuntimeError("--decompose slab needs at least 2 ranks (torchrun --nproc-per-node N)")
+    local_rank = local_rank % torch.cuda.device_count()                   # (--backend gloo: ranks may share a GPU)
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    dist_init("nccl")
+    dist_init(args.backend)
     import torch.distributed as dist
+    if args.backend != "nccl":
+        dev = None                                                        # scalars of the timing reductions stay on the host
     cfg, sv, sol, (k0, dk, chi) = workload_inputs(args.workload, 0)      # every rank the same solute
     M, n_v = cfg.mdiis_nvec, sv.n_v
     s = lib.SlabSolver(cfg.n, cfg.spacing, n_v, world, rank, closure=cfg.closure, pse_order=cfg.pse_order, mdiis_nvec=M,
@@ -687,29 +690,30 @@ def run_slab(args):
     launches0 = s.launch_count()
     sampler = ClockSampler(local_rank) if rank == 0 else None
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    dist.barrier(); torch.cuda.synchronize(dev)
+    dist.barrier(); torch.cuda.synchronize()
     ev0.record(s.stream)
     s.iterate(args.steps, 0.0)
     ev1.record(s.stream)
-    dist.barrier(); torch.cuda.synchronize(dev)
+    dist.barrier(); torch.cuda.synchronize()
     (ms_max,) = reduce_scalars([ev0.elapsed_time(ev1)], "max", dev)
     launches = s.launch_count() - launches0
     # end to end: host atoms -> converged solve -> host g slabs
     g_host = torch.empty((n_v,) + s.shape, dtype=torch.float64, pin_memory=True)
     g_np = g_host.numpy()
-    dist.barrier(); torch.cuda.synchronize(dev)
+    dist.barrier(); torch.cuda.synchronize()
     t0 = time.perf_counter()
     s.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=cfg.rcut)
     it_conv, rms_conv = s.iterate(args.max_iter, cfg.tol)
     mu, _ = s.free_energy()
     for g in range(n_v):
         lib.rism3d_get_field(s.ctx, lib.FIELDS["G"], g, g_np[g].ctypes.data, False)
-    torch.cuda.synchronize(dev)
+    torch.cuda.synchronize()
     (e2e_s,) = reduce_scalars([time.perf_counter() - t0], "max", dev)
     clocks = sampler.stop() if sampler else None
     if rank == 0:
         cfgd = bench_config(cfg, sol, world)
-        cfgd["parallelism"] = f"slab x{world}: one solve, x planes in r space, y rows in k space, two all-to-all transposes per iteration"
+        cfgd["parallelism"] = (f"slab x{world}: one solve, x planes in r space, y rows in k space, two all-to-all transposes "
+                               f"per iteration ({args.backend})")
         print(json.dumps({
             "metric": METRIC, "value": args.steps / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": warm, "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "strong",
@@ -784,6 +788,9 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-anderson", action="store_true", help="skip the extra modified-Anderson solve")
     ap.add_argument("--no-fft-compare", action="store_true", help="skip the cuFFT comparison")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="process group of --decompose slab (gloo: the blocks travel through host memory; lets several "
+                         "ranks share one GPU, for testing)")
     ap.add_argument("--decompose", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: N independent solves (default, weak scaling) or ONE solve in x / y slabs (strong scaling)")
     args = ap.parse_args()

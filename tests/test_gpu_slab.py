@@ -234,3 +234,30 @@ def test_two_processes_share_one_solve(tmp_path, peer):
     assert abs(float(r[0]["mu"]) - mu_o) <= 1e-7 * abs(mu_o) and float(r[0]["mu"]) == float(r[1]["mu"])
     go = orc.solvation_gradient()
     assert np.max(np.abs(r[1]["grad"] - go)) <= 1e-8 * max(1.0, np.max(np.abs(go)))
+
+
+def test_bench_decompose_slab_two_processes(tmp_path):
+    """bench.py --decompose slab end to end (one solve over two ranks, strong scaling line), both ranks on this box's one
+    GPU with a gloo group"""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    port = 29400 + (os.getpid() % 200)
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT=str(port))
+        procs.append(subprocess.Popen([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--decompose", "slab",
+                                       "--backend", "gloo", "--workload", "C2", "--steps", "4", "--warmup", "5",
+                                       "--max-iter", "600"], env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True))
+    outs = []
+    for p in procs:
+        out, err = p.communicate(timeout=900)
+        assert p.returncode == 0, err[-3000:]
+        outs.append(out)
+    line = json.loads(outs[0].strip().splitlines()[-1])
+    assert outs[1].strip() == ""
+    assert line["scaling"] == "strong" and line["n_gpus"] == 2 and line["value"] > 0 and line["gpu_launches"] > 0
+    assert line["e2e"]["converged"] and 300 < line["e2e"]["iterations_to_converge"] < 450      # a single rank needs 359
