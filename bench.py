@@ -682,7 +682,14 @@ def run_slab(args):
     M, n_v = cfg.mdiis_nvec, sv.n_v
     s = lib.SlabSolver(cfg.n, cfg.spacing, n_v, world, rank, closure=cfg.closure, pse_order=cfg.pse_order, mdiis_nvec=M,
                        mdiis_b=cfg.mdiis_b, mdiis_restart=cfg.mdiis_restart, temperature=cfg.temperature, kappa=cfg.kappa,
-                       r_min=cfg.r_min, device=local_rank)
+                       r_min=cfg.r_min, device=local_rank, exportable=args.peer)
+    if args.peer:
+        # every rank maps the others' workspaces (CUDA IPC): the y passes store to / load from the other GPUs directly and
+        # rism3d_iterate runs whole iterations with in-stream barriers.  One GPU per rank only: the barrier kernels of
+        # the ranks wait for one another.
+        if torch.cuda.device_count() < world:
+            raise RuntimeError("--peer needs one GPU per rank")
+        s.connect_peers_ipc()
     s.set_solvent_chi(sv.q, sv.sigma, sv.eps, sv.rho, k0, dk, chi)
     setup_ms = s.set_solute(sol.xyz, sol.q, sol.sigma, sol.eps, rcut=cfg.rcut)
     warm = max(args.warmup, M, 3)
@@ -713,7 +720,7 @@ def run_slab(args):
     if rank == 0:
         cfgd = bench_config(cfg, sol, world)
         cfgd["parallelism"] = (f"slab x{world}: one solve, x planes in r space, y rows in k space, two all-to-all transposes "
-                               f"per iteration ({args.backend})")
+                               f"per iteration ({'peer stores over NVLink' if args.peer else args.backend})")
         print(json.dumps({
             "metric": METRIC, "value": args.steps / (ms_max * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": warm, "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "strong",
@@ -791,6 +798,8 @@ def main():
     ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
                     help="process group of --decompose slab (gloo: the blocks travel through host memory; lets several "
                          "ranks share one GPU, for testing)")
+    ap.add_argument("--peer", action="store_true",
+                    help="--decompose slab in peer mode: CUDA IPC mappings, transposes inside the y passes' stores and loads")
     ap.add_argument("--decompose", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: N independent solves (default, weak scaling) or ONE solve in x / y slabs (strong scaling)")
     args = ap.parse_args()
