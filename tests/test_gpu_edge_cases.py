@@ -354,3 +354,23 @@ def test_non_cubic_four_sites_pse2():
     np.testing.assert_allclose(gpu.rms_history(), orc.rms_history, rtol=1e-6, atol=1e-12)
     assert np.max(np.abs(gpu.get_field("G") - orc.get_field("G"))) <= 1e-9
     gpu.close()
+
+
+@pytest.mark.parametrize("shape,nv,M", [((512, 8, 16), 2, 3), ((8, 512, 16), 4, 3), ((16, 8, 512), 2, 3), ((512, 16, 8), 8, 2),
+                                        ((256, 8, 8), 2, 5), ((8, 256, 8), 2, 4), ((8, 8, 256), 4, 4), ((128, 64, 8), 3, 6)])
+def test_longest_lines_on_thin_grids(shape, nv, M):
+    """the 256- and 512-point instantiations of every pass (two-pass k-space kernels, the TMA y pass, the strided y pass
+    at 512, the 256-point z lines) on grids that are thin in the other directions, whole grid against the oracle"""
+    sv = _solvent(nv, seed=nv + sum(shape))
+    chi = synthetic_chi(nv, sv.rho, n_k=3000, dk=0.02, k0=0.02, seed=nv, amp=0.5)
+    sol = _small_solute(seed=shape[0], n=3)
+    orc, gpu, _, _ = make_pair(n=shape, spacing=0.4, solvent=sv, chi=chi, M=M, solute=sol)
+    W, Wo = gpu.get_field("W"), orc.get_field("W")
+    finite = np.abs(Wo) < 600.0
+    assert np.max(np.abs(W - Wo)[finite]) < 1e-10
+    orc.iterate(12, 0.0)
+    gpu.iterate(12, 0.0)
+    np.testing.assert_allclose(gpu.rms_history(), orc.rms_history, rtol=1e-6, atol=1e-12)
+    assert np.max(np.abs(gpu.get_field("G") - orc.get_field("G"))) <= 1e-9
+    assert np.max(np.abs(gpu.get_field("TAU") - orc.get_field("TAU"))) <= 1e-9
+    gpu.close()

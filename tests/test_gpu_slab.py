@@ -53,6 +53,10 @@ def _gather(ranks, which):
     (4, (32, 64, 16), "water", 7.0, False),
     (4, (64, 32, 32), "water_nacl_0.1M", 0.0, True),
     (8, (64, 64, 16), "water", 0.0, True),
+    (2, (128, 16, 8), "water", 0.0, True),             # 128-point x lines on 8 rows per rank
+    (4, (32, 256, 8), "water", 0.0, False),            # 256-point y lines through the row map; the three-pass k-space kernel
+    (2, (512, 16, 8), "water", 5.0, True),             # the 512-point k-space kernel on a slab
+    (2, (16, 128, 16), "water_nacl_0.1M", 0.0, False),
 ])
 def test_slab_ranks_match_oracle(P, shape, solvent, rcut, peer):
     import paper_2403_01039_b200 as lib
