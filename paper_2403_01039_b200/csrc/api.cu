@@ -300,7 +300,7 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
   }
   if (y_uses_tma(g.ny, g.n_ranks)) {
     const uint64_t row = (uint64_t)g.q() * 2;                                                // doubles per (ix, iy) row
-    if (!make_tensor_map_2d(&ctx->b.tm_ywork, ctx->b.work, row, (uint64_t)g.nxl * g.ny, row * 8, 16, (uint32_t)g.ny)) {
+    if (!make_tensor_map_2d(&ctx->b.tm_ywork, ctx->b.work, row, (uint64_t)g.nxl * g.ny, row * 8, 2 * (uint32_t)y_tile_cols(g), (uint32_t)g.ny)) {
       delete ctx;
       return RISM3D_ERR_CUDA;
     }

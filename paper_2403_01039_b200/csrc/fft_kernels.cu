@@ -173,7 +173,7 @@ static int launch_strided_n(const Grid& gr, const Buffers& b, bool x_axis, bool 
 
 // ------------------------------------------------------------------------------------------------
 // Two-pass y transform for the long lines (64 = 8 x 8, 128 = 16 x 8, 256 = 16 x 16), single-rank runs: the scheme of the
-// k-space pass (kspace_kernel.cu) without its arithmetic.  Tiles of N rows x 128 bytes arrive by TMA (one request per
+// k-space pass (kspace_kernel.cu) without its arithmetic.  Tiles of N rows x 128 (or 256) bytes arrive by TMA (one request per
 // tile, two stages, no LDGSTS issue slots and no staging registers), each thread does one radix-R1 butterfly per outer
 // pass with twiddles generated from two seeds, the other pass runs on registers and the results leave from registers as
 // 128-byte rows: 2 loads + 1 store of the tile in shared memory per work item instead of 3 + 3 (cp.async staging
@@ -184,21 +184,21 @@ template <> struct YPlan2<64>  { enum { OK = 1, R1 = 8,  R2 = 8 }; };
 template <> struct YPlan2<128> { enum { OK = 1, R1 = 16, R2 = 8 }; };
 template <> struct YPlan2<256> { enum { OK = 1, R1 = 16, R2 = 16 }; };
 
-template <int N>
+template <int N, int CC>
 struct Y2Cfg {
-  enum { R1 = YPlan2<N>::R1, R2 = YPlan2<N>::R2, T = N / R1, NT = T * COLS, NB = N / R2, IB = NB / T,
-         ITEM = N * COLS, TILE_BYTES = ITEM * (int)sizeof(cplx), SHM = 2 * TILE_BYTES + 64,
+  enum { R1 = YPlan2<N>::R1, R2 = YPlan2<N>::R2, T = N / R1, NT = T * CC, NB = N / R2, IB = NB / T,
+         ITEM = N * CC, TILE_BYTES = ITEM * (int)sizeof(cplx), SHM = 2 * TILE_BYTES + 64,
          FIT = 227 * 1024 / (SHM + 1024), CAP = (N >= 256) ? 2 : 4, MINB = FIT < CAP ? FIT : CAP };
 };
 
-template <int N, bool INV>
-__global__ void __launch_bounds__(Y2Cfg<N>::NT, Y2Cfg<N>::MINB)
+template <int N, bool INV, int CC>
+__global__ void __launch_bounds__(Y2Cfg<N, CC>::NT, Y2Cfg<N, CC>::MINB)
     fft_y2_kernel(const __grid_constant__ CUtensorMap tm, cplx* __restrict__ data, Twiddle tw,
                   const DevState* __restrict__ st, unsigned chunks_per_plane, size_t plane_stride, size_t es,
                   unsigned nitems) {
   if (st != nullptr && st->done) return;
-  using K = Y2Cfg<N>;
-  constexpr int R1 = K::R1, R2 = K::R2, T = K::T, C = COLS, S1 = N / R1, NB = K::NB, IB = K::IB;
+  using K = Y2Cfg<N, CC>;
+  constexpr int R1 = K::R1, R2 = K::R2, T = K::T, C = CC, S1 = N / R1, NB = K::NB, IB = K::IB;
   const int tid = threadIdx.x;
   const int col = tid % C, t = tid / C;
   const cplx a0 = tw(t), astep = tw(2 * t);          // exp(-i pi t / N) and its square: a[k1] = a0 * astep^k1
@@ -278,13 +278,18 @@ __global__ void __launch_bounds__(Y2Cfg<N>::NT, Y2Cfg<N>::MINB)
   }
 }
 
-template <int N, bool INV>
-static int launch_y2_n(const Grid& gr, const Buffers& b, bool use_state, cudaStream_t s) {
+// complex columns per tile: 16 (256-byte rows, one 256-thread CTA per SM) for the 256-point lines -- fewer, longer
+// requests in flight suit the memory system better than two CTAs fetching 128-byte rows (C4: 0.199 -> 0.177 ms per
+// pass; profiles/README.md) -- 8 otherwise (at 128 points the two are level, at 512 the tile would not fit)
+int y_tile_cols(const Grid& gr) { return (gr.ny == 256 && gr.q() % 16 == 0) ? 16 : COLS; }
+
+template <int N, bool INV, int CC>
+static int launch_y2_cc(const Grid& gr, const Buffers& b, bool use_state, cudaStream_t s) {
   if constexpr (YPlan2<N>::OK) {
-    using K = Y2Cfg<N>;
+    using K = Y2Cfg<N, CC>;
     const size_t Q = gr.q();
-    const unsigned cpp = (unsigned)(Q / COLS), nitems = (unsigned)gr.nxl * cpp;
-    auto kern = fft_y2_kernel<N, INV>;
+    const unsigned cpp = (unsigned)(Q / CC), nitems = (unsigned)gr.nxl * cpp;
+    auto kern = fft_y2_kernel<N, INV, CC>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SHM) != cudaSuccess) return 0;
     Twiddle tw{b.tw, gr.nmax / N, 2 * gr.nmax - 1};
     unsigned grid = (unsigned)(gr.num_sms * K::MINB);
@@ -294,6 +299,13 @@ static int launch_y2_n(const Grid& gr, const Buffers& b, bool use_state, cudaStr
   } else {
     return 0;
   }
+}
+template <int N, bool INV>
+static int launch_y2_n(const Grid& gr, const Buffers& b, bool use_state, cudaStream_t s) {
+  if constexpr (N == 256) {
+    if (y_tile_cols(gr) == 16) return launch_y2_cc<N, INV, 16>(gr, b, use_state, s);
+  }
+  return launch_y2_cc<N, INV, COLS>(gr, b, use_state, s);
 }
 
 // true when the y passes of this grid take the two-pass TMA kernel (the API layer then builds its tensor map)

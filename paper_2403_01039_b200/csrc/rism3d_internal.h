@@ -129,6 +129,7 @@ struct SolverParams {
 int kspace_smem_bytes(int nx, int nv);
 bool kspace_uses_tma(int nx);
 bool y_uses_tma(int ny, int n_ranks);
+int y_tile_cols(const Grid&);
 
 // ---- launchers (each returns the number of kernels it launched; errors surface via cudaGetLastError) ----
 // fft_kernels.cu
