@@ -380,7 +380,7 @@ constexpr int ZP = COLS + 1;
 template <int NZ> struct ZPlan : FftCfg<NZ> { enum { GF = FftCfg<NZ>::G, MBF = 1, GI = FftCfg<NZ>::G, MBI = 1, MBG = 1 }; };
 template <> struct ZPlan<64>  { enum { R1 = 8, R2 = 8, R3 = 1, T = 8, G = 4, GF = 2, MBF = 4, GI = 2, MBI = 8, MBG = 5 }; };
 template <> struct ZPlan<128> { enum { R1 = 4, R2 = 4, R3 = 8, T = 16, G = 2, GF = 1, MBF = 4, GI = 1, MBI = 8, MBG = 5 }; };
-template <> struct ZPlan<256> { enum { R1 = 16, R2 = 16, R3 = 1, T = 16, G = 2, GF = 2, MBF = 2, GI = 2, MBI = 2, MBG = 2 }; };
+template <> struct ZPlan<256> { enum { R1 = 4, R2 = 8, R3 = 8, T = 32, G = 1, GF = 1, MBF = 3, GI = 1, MBI = 4, MBG = 3 }; };
 
 __device__ __forceinline__ double2 ld2(const double* p) { return *reinterpret_cast<const double2*>(p); }
 __device__ __forceinline__ void st2(double* p, double2 v) { *reinterpret_cast<double2*>(p) = v; }
