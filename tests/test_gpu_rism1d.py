@@ -125,3 +125,29 @@ def test_full_size_table_feeds_the_3d_solver():
     ref.iterate(400, 1e-6)
     assert abs(s.free_energy()[0] - ref.free_energy()[0]) <= 1e-5 * abs(ref.free_energy()[0])
     gpu.close()
+
+
+def test_argument_and_order_checks():
+    import paper_2403_01039_b200 as lib
+    sv = solvent_by_name("water")
+    one = lib.Solver1d(sv.n_s, n_points=512, dr=0.05)
+    with pytest.raises(lib.Rism3dError) as e:
+        one.solve(1.0, 5, 0.0)                               # no solvent yet
+    assert e.value.status == -3
+    args = [sv.q[sv.site_type], sv.sigma[sv.site_type], sv.eps[sv.site_type], sv.species_rho[sv.site_species],
+            sv.site_species, sv.bond]
+    bad_q = np.array(args[0], dtype=float)
+    bad_q[0] += 0.1                                          # not neutral any more
+    with pytest.raises(lib.Rism3dError) as e:
+        one.set_solvent(bad_q, *args[1:])
+    assert e.value.status == -5
+    no_bond = np.zeros_like(sv.bond)
+    with pytest.raises(lib.Rism3dError) as e:
+        one.set_solvent(*args[:5], no_bond)                  # bonded sites need a distance
+    assert e.value.status == -1
+    one.set_solvent(*args)
+    nd, rms = one.solve(0.0, 3, 0.0)
+    assert nd == 3 and rms > 0
+    with pytest.raises(lib.Rism3dError):
+        lib.rism1d_get_pair(one.ctx, 7, sv.n_s, 512)         # unknown pair function
+    one.close()

@@ -265,3 +265,26 @@ def test_bench_decompose_slab_two_processes(tmp_path):
     assert outs[1].strip() == ""
     assert line["scaling"] == "strong" and line["n_gpus"] == 2 and line["value"] > 0 and line["gpu_launches"] > 0
     assert line["e2e"]["converged"] and 300 < line["e2e"]["iterations_to_converge"] < 450      # a single rank needs 359
+
+
+def test_slab_peer_table_checks():
+    import torch
+    import paper_2403_01039_b200 as lib
+    stream = torch.cuda.Stream()
+    a = lib.SlabSolver(32, 0.5, 2, 2, 0, stream=stream)
+    b = lib.SlabSolver(32, 0.5, 2, 2, 1, stream=stream)
+    la, lb = a.local, b.local
+    with pytest.raises(lib.Rism3dError):                     # entry `rank` must be the rank's own arrays
+        a.connect_peers([lb["K"], la["K"]], [lb["gram"], la["gram"]], [lb["flags"], la["flags"]])
+    with pytest.raises(lib.Rism3dError):
+        a.connect_peers([la["K"], 0], [la["gram"], lb["gram"]], [la["flags"], lb["flags"]])
+    with pytest.raises(lib.Rism3dError):
+        a.phase(4)
+    with pytest.raises(lib.Rism3dError):
+        a.phase(0)                                           # no solute yet
+    with pytest.raises(RuntimeError):
+        a.iterate_host_ordered(1)                            # not in peer mode
+    a.connect_peers([la["K"], lb["K"]], [la["gram"], lb["gram"]], [la["flags"], lb["flags"]])
+    assert a.peer_mode
+    a.close()
+    b.close()
