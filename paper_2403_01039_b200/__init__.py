@@ -17,4 +17,5 @@ from .binding import (  # noqa: F401
     EXPORTED_SYMBOLS_1D, Rism1dParams, Solver1d, rism1d_workspace_bytes, rism1d_init, rism1d_set_solvent, rism1d_solve,
     rism1d_get_pair, rism1d_get_chi, rism1d_get_chi_types, rism1d_thermo, rism1d_launch_count, rism1d_last_error,
     rism1d_destroy,
+    EXPORTED_SYMBOLS_NOALLOC, NOALLOC_MAX_SITES, NOALLOC_MAX_POINTS, NOALLOC_SCRATCH_BYTES, rism3d_noalloc_free_energy,
 )

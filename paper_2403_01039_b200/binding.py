@@ -31,6 +31,8 @@ EXPORTED_SYMBOLS_1D = [
     "rism1d_workspace_bytes", "rism1d_init", "rism1d_set_solvent", "rism1d_solve", "rism1d_get_pair", "rism1d_get_chi",
     "rism1d_get_chi_types", "rism1d_thermo", "rism1d_launch_count", "rism1d_last_error", "rism1d_destroy",
 ]
+EXPORTED_SYMBOLS_NOALLOC = ["rism3d_noalloc_free_energy"]          # include/rism3d_noalloc.h
+NOALLOC_MAX_SITES, NOALLOC_MAX_POINTS, NOALLOC_SCRATCH_BYTES = 8, 134217728, 151552
 
 
 class Rism3dError(RuntimeError):
@@ -182,6 +184,11 @@ def load_library():
     lib.rism1d_last_error.argtypes = [C.c_void_p]
     lib.rism1d_destroy.restype = None
     lib.rism1d_destroy.argtypes = [C.c_void_p]
+    # rism3d_noalloc.h
+    lib.rism3d_noalloc_free_energy.restype = C.c_int
+    lib.rism3d_noalloc_free_energy.argtypes = [C.c_int, C.c_void_p, C.c_size_t, C.c_double, C.c_int, C.c_int, C.c_int,
+                                               C.c_double, dp, dp, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                               C.c_char_p, C.c_size_t]
     _LIB = lib
     return lib
 
@@ -248,6 +255,27 @@ def rism3d_free_energy(ctx, n_sites: int):
     site = np.zeros(n_sites)
     _check(ctx, load_library().rism3d_free_energy(ctx, C.byref(tot), _dptr(site)))
     return float(tot.value), site
+
+
+def rism3d_noalloc_free_energy(device: int, cuda_stream: int, n_points: int, spacing: float, n_sites: int, closure: int,
+                               pse_order: int, temperature: float, q, rho, d_tau: int, d_w: int, d_phi: int, d_out: int):
+    """The free-energy sum for callers that cannot give the library a workspace (their host program's pool owns the
+    whole GPU, or they must not stall the device with cudaMalloc / cudaFree): the partial sums live in a fixed 148 KiB
+    array inside the library image, so this call allocates nothing.  d_tau, d_w: device addresses of
+    [n_sites][n_points] doubles, d_phi: [n_points], d_out: [2][n_sites] (dmu per site in kcal/mol, then dV sum c_sr in
+    A^3).  Enqueued on `cuda_stream` (a cudaStream_t as an integer, 0 = default stream) and NOT waited for.  At most 8
+    site types and 512^3 points; one array per GPU shared by all calls -- calls that overlap on one GPU race.  Make
+    the first call on each device during start-up, outside stream capture (include/rism3d_noalloc.h)."""
+    q, rho = _f64(q), _f64(rho)
+    if q.shape != (int(n_sites),) or rho.shape != (int(n_sites),):
+        raise ValueError(f"q and rho must have shape ({int(n_sites)},), got {q.shape} and {rho.shape}")
+    err = C.create_string_buffer(512)
+    st = load_library().rism3d_noalloc_free_energy(int(device), C.c_void_p(cuda_stream), int(n_points), float(spacing),
+                                                   int(n_sites), int(closure), int(pse_order), float(temperature),
+                                                   _dptr(q), _dptr(rho), C.c_void_p(d_tau), C.c_void_p(d_w),
+                                                   C.c_void_p(d_phi), C.c_void_p(d_out), err, len(err))
+    if st != 0:
+        raise Rism3dError(st, err.value.decode() or rism3d_status_string(st))
 
 
 def rism3d_pmv(ctx, chi_t: float, n_sites: int):

@@ -16,9 +16,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "librism3d.so")
-SOURCES = ["api.cu", "fft_kernels.cu", "kspace_kernel.cu", "mdiis_kernels.cu", "setup_kernels.cu", "rism1d.cu"]
+SOURCES = ["api.cu", "fft_kernels.cu", "kspace_kernel.cu", "mdiis_kernels.cu", "setup_kernels.cu", "rism1d.cu", "noalloc.cu"]
 HEADERS = ["fft_core.cuh", "async_copy.cuh", "tma.cuh", "mdiis_device.cuh", "rism3d_internal.h",
-           os.path.join("..", "..", "include", "rism3d.h"), os.path.join("..", "..", "include", "rism1d.h")]
+           os.path.join("..", "..", "include", "rism3d.h"), os.path.join("..", "..", "include", "rism1d.h"),
+           os.path.join("..", "..", "include", "rism3d_noalloc.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-O2"]
