@@ -274,7 +274,8 @@ __global__ void __launch_bounds__(Y2Cfg<N, CC>::NT, Y2Cfg<N, CC>::MINB)
         for (int m1 = 0; m1 < R1; ++m1) base[(size_t)(m1 * S1 + t) * es] = cscale(x[m1], scale);
       }
     }
-    __syncthreads();                                 // stage b is free again
+    fence_proxy_async();                             // this item's st.shared writes to stage b come before the TMA load that
+    __syncthreads();                                 // refills it (generic -> async proxy);  stage b is free again
   }
 }
 

@@ -357,7 +357,10 @@ __global__ void __launch_bounds__(Kspace2Cfg<N, NV>::NT, Kspace2Cfg<N, NV>::MINB
       for (int k1 = 0; k1 < R1; ++k1) x[k1] = cmulc(ld_sm(k1 * S1 + t), a.get(k1));
       if constexpr (STAGES == 1) {
         // single-buffered tiles (n = 512): once every thread holds its values the stage is free -- the next tile is
-        // requested now and lands under this pass's arithmetic; the results leave from registers (128-byte rows)
+        // requested now and lands under this pass's arithmetic; the results leave from registers (128-byte rows).
+        // The stage was last written with ordinary st.shared (pass B): order those generic-proxy writes before the
+        // async-proxy write of the TMA load (a CTA barrier alone does not order the two proxies in the PTX model)
+        fence_proxy_async();
         __syncthreads();
         if (tid == 0 && next < nitems) issue(next, 0);
       }
