@@ -55,7 +55,9 @@ typedef enum {
   RISM3D_ERR_NEUTRAL   = -5,   /* sum_g rho_g q_g != 0 (1e-12)                                     */
   RISM3D_ERR_WORKSPACE = -6,   /* workspace smaller than rism3d_workspace_bytes()                  */
   RISM3D_ERR_CUDA      = -7,   /* a CUDA call failed; message carries cudaGetErrorString           */
-  RISM3D_ERR_DIVERGED  = -8    /* non-finite residual; tau is left at the last input               */
+  RISM3D_ERR_DIVERGED  = -8,   /* non-finite residual; tau is left at the last input               */
+  RISM3D_ERR_PEER      = -9    /* peer mode: another rank did not reach an in-stream barrier within the wait limit
+                                  (rism3d_slab_set_peer_timeout); the iteration was abandoned on this rank          */
 } rism3d_status;
 
 typedef enum { RISM3D_KH = 1, RISM3D_PSE = 2, RISM3D_HNC = 3 } rism3d_closure;
@@ -192,6 +194,8 @@ int rism3d_measure_dfma_peak(rism3d_ctx* ctx, double* tflops);
  * loop kernel k over *n_iterations profiled iterations, in launch order (names: rism3d_loop_kernel_name). */
 #define RISM3D_N_LOOP_KERNELS 5
 int rism3d_set_profiling(rism3d_ctx* ctx, int enable);
+/* (SURVEY.md section 8(b) sketched this call as (float*, int); it returns double sums and the iteration count instead, so
+ * that a caller can form per-iteration means without a second call.) */
 int rism3d_get_timings(rism3d_ctx* ctx, double* ms_total, int cap, long long* n_iterations);
 const char* rism3d_loop_kernel_name(int k);             /* static strings; "" when k is out of range */
 
@@ -255,8 +259,31 @@ int rism3d_slab_local(rism3d_ctx* ctx, void** d_K, void** d_stage, void** d_gram
                       size_t* gram_row_bytes);
 
 /* Switch to peer mode: d_K[r], d_gram[r], d_flags[r] are the arrays rism3d_slab_local returned on rank r, as DEVICE
- * pointers valid in this process (HOST arrays of n_ranks pointers; entry `rank` is this rank's own). */
+ * pointers valid in this process (HOST arrays of n_ranks pointers; entry `rank` is this rank's own).
+ * EXPERIMENTAL: peer mode has been checked for numerics with the ranks' phases ordered by the host, and its barrier by
+ * the self-test below; a peer-mode rism3d_iterate has not yet run on two GPUs.
+ * The call also zeroes this rank's barrier flags and epoch counter.  EVERY rank must call it (again) whenever any rank's
+ * context has been (re)created, and the ranks must then meet on the host (a process-group barrier) before the first
+ * rism3d_iterate: the in-stream barriers count epochs from that point and rely on every rank enqueueing the same
+ * sequence of iterations (same max_iter and tol on every rank). */
 int rism3d_slab_set_peers(rism3d_ctx* ctx, void* const* d_K, void* const* d_gram, void* const* d_flags);
+
+/* Longest time one in-stream barrier of a peer-mode rism3d_iterate waits for the other ranks, seconds (0.001..3600;
+ * default 30).  When a rank does not arrive in time -- its process died, it enqueued fewer iterations, it was re-created
+ * without a new rism3d_slab_set_peers everywhere -- the waiting rank stops iterating instead of spinning inside a kernel
+ * for ever: the remaining kernels of the call return at once and rism3d_iterate returns RISM3D_ERR_PEER.  tau is then
+ * undefined for the abandoned iteration, and further rism3d_iterate calls fail with RISM3D_ERR_PEER until every rank has
+ * called rism3d_slab_set_peers again. */
+int rism3d_slab_set_peer_timeout(rism3d_ctx* ctx, double seconds);
+
+/* Test hook: runs the barrier code of peer mode on ONE GPU, the n_ranks (1..8) ranks being the blocks of one cooperative
+ * launch (kernels that wait on one another must not be separate launches on one device).  `epochs` barriers in a row;
+ * before each, every rank publishes a value that every other rank must see after it.  absent_rank >= 0: that rank never
+ * arrives and every other rank must give up after timeout_s (0.001..60).  d_scratch: DEVICE, >= 4096 bytes, overwritten.
+ * *n_errors: ordering violations seen (must be 0); *n_timeouts: ranks that gave up (0, or n_ranks - 1 with an absent
+ * rank).  Synchronises cuda_stream. */
+int rism3d_debug_peer_barrier_selftest(int device, void* d_scratch, size_t bytes, void* cuda_stream, int n_ranks, int epochs,
+                                       int absent_rank, double timeout_s, int* n_errors, int* n_timeouts);
 
 /* Mapping the peers' arrays into this process (CUDA IPC; one GPU per process on one node).  A workspace that is to
  * be exported must be an allocation of its own: peer_alloc is a plain cudaMalloc on `device` (a sub-block of a caching

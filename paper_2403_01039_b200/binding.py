@@ -24,7 +24,7 @@ EXPORTED_SYMBOLS = [
     "rism3d_loop_kernel_name", "rism3d_debug_fft_forward",
     "rism3d_debug_fft_inverse", "rism3d_last_error", "rism3d_status_string", "rism3d_destroy",
     "rism3d_slab_plan", "rism3d_slab_local", "rism3d_slab_set_peers", "rism3d_slab_begin", "rism3d_slab_phase",
-    "rism3d_slab_status", "rism3d_slab_end",
+    "rism3d_slab_status", "rism3d_slab_end", "rism3d_slab_set_peer_timeout", "rism3d_debug_peer_barrier_selftest",
     "rism3d_peer_alloc", "rism3d_peer_free", "rism3d_peer_export", "rism3d_peer_open", "rism3d_peer_close",
 ]
 EXPORTED_SYMBOLS_1D = [
@@ -143,6 +143,11 @@ def load_library():
     lib.rism3d_slab_local.argtypes = [C.c_void_p, vpp, vpp, vpp, vpp, szp, szp]
     lib.rism3d_slab_set_peers.restype = C.c_int
     lib.rism3d_slab_set_peers.argtypes = [C.c_void_p, vpp, vpp, vpp]
+    lib.rism3d_slab_set_peer_timeout.restype = C.c_int
+    lib.rism3d_slab_set_peer_timeout.argtypes = [C.c_void_p, C.c_double]
+    lib.rism3d_debug_peer_barrier_selftest.restype = C.c_int
+    lib.rism3d_debug_peer_barrier_selftest.argtypes = [C.c_int, C.c_void_p, C.c_size_t, C.c_void_p, C.c_int, C.c_int, C.c_int,
+                                                       C.c_double, ip, ip]
     lib.rism3d_slab_begin.restype = C.c_int
     lib.rism3d_slab_begin.argtypes = [C.c_void_p, C.c_double]
     lib.rism3d_slab_phase.restype = C.c_int
@@ -379,6 +384,22 @@ def rism3d_slab_set_peers(ctx, d_K, d_gram, d_flags):
     n = len(d_K)
     arr = lambda v: (C.c_void_p * n)(*[int(x) for x in v])
     _check(ctx, load_library().rism3d_slab_set_peers(ctx, arr(d_K), arr(d_gram), arr(d_flags)))
+
+
+def rism3d_slab_set_peer_timeout(ctx, seconds: float):
+    _check(ctx, load_library().rism3d_slab_set_peer_timeout(ctx, float(seconds)))
+
+
+def rism3d_debug_peer_barrier_selftest(device: int, d_scratch: int, nbytes: int, cuda_stream: int, n_ranks: int, epochs: int,
+                                       absent_rank: int = -1, timeout_s: float = 5.0):
+    """-> (ordering errors, ranks that timed out) of the peer-mode barrier run as ONE cooperative launch on one GPU"""
+    ne, nt = C.c_int(-1), C.c_int(-1)
+    st = load_library().rism3d_debug_peer_barrier_selftest(int(device), C.c_void_p(d_scratch), int(nbytes),
+                                                           C.c_void_p(cuda_stream), int(n_ranks), int(epochs),
+                                                           int(absent_rank), float(timeout_s), C.byref(ne), C.byref(nt))
+    if st != 0:
+        raise Rism3dError(st, rism3d_status_string(st))
+    return int(ne.value), int(nt.value)
 
 
 def rism3d_peer_alloc(device: int, nbytes: int) -> int:
@@ -677,6 +698,9 @@ class SlabSolver(Solver):
     def connect_peers(self, d_K, d_gram, d_flags):
         rism3d_slab_set_peers(self.ctx, d_K, d_gram, d_flags)
         self.peer_mode = True
+
+    def set_peer_timeout(self, seconds: float):
+        rism3d_slab_set_peer_timeout(self.ctx, seconds)
 
     def connect_peers_ipc(self):
         """Peer mode across processes (one GPU each, one node): every rank exports its workspace (created with

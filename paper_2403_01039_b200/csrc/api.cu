@@ -42,6 +42,7 @@ struct rism3d_ctx {
   float phi_ms;              // GPU time of that deferred phi kernel
   StateHeader* h_hdr;        // pinned
   double* d_out;             // small device array for scalar results (inside workspace)
+  bool peer_broken;          // an in-stream barrier of a peer-mode iterate timed out: reconnect before iterating again
   char err[512];
 };
 
@@ -223,6 +224,7 @@ extern "C" const char* rism3d_status_string(int s) {
     case RISM3D_ERR_WORKSPACE: return "workspace too small";
     case RISM3D_ERR_CUDA: return "CUDA error";
     case RISM3D_ERR_DIVERGED: return "iteration diverged";
+    case RISM3D_ERR_PEER: return "a peer rank did not reach an in-stream barrier in time";
     default: return "unknown status";
   }
 }
@@ -297,6 +299,7 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
     ctx->b.gram_dst[0] = ctx->b.gram_x;
     ctx->b.n_gram_dst = 1;
     ctx->b.peer_mode = false;
+    ctx->b.peer_timeout_ns = 30ull * 1000000000ull;        // rism3d_slab_set_peer_timeout
   }
   if (y_uses_tma(g.ny, g.n_ranks)) {
     const uint64_t row = (uint64_t)g.q() * 2;                                                // doubles per (ix, iy) row
@@ -676,6 +679,9 @@ extern "C" int rism3d_iterate(rism3d_ctx* ctx, int max_iter, double tol, int* n_
   if (!ctx->have_solute) return fail(ctx, RISM3D_ERR_ORDER, "set_solute must come before iterate");
   if (ctx->g.n_ranks > 1 && !ctx->b.peer_mode)
     return fail(ctx, RISM3D_ERR_ORDER, "a staged slab run is driven by rism3d_slab_phase (or call rism3d_slab_set_peers)");
+  if (ctx->peer_broken)
+    return fail(ctx, RISM3D_ERR_PEER, "an earlier iterate gave up at an in-stream barrier: the ranks' barrier epochs no longer "
+                                      "agree; call rism3d_slab_set_peers on every rank (then a host-side barrier) first");
   iterate_begin_kernel<<<1, 1, 0, ctx->stream>>>(ctx->b.state, tol);
   ctx->launches += 1;
   // packs of GRAPH_PACK iterations (one graph launch each) with a look at the device state in between when a
@@ -702,6 +708,11 @@ extern "C" int rism3d_iterate(rism3d_ctx* ctx, int max_iter, double tol, int* n_
   if (rms) *rms = ctx->h_hdr->rms_last;
   if (ctx->h_hdr->status == RISM3D_ERR_DIVERGED)
     return fail(ctx, RISM3D_ERR_DIVERGED, "non-finite residual after %d iterations", ctx->h_hdr->n_done);
+  if (ctx->h_hdr->status == RISM3D_ERR_PEER) {
+    ctx->peer_broken = true;
+    return fail(ctx, RISM3D_ERR_PEER, "a peer rank did not reach an in-stream barrier within %.3g s (after %d iterations): "
+                "the iteration was abandoned on this rank", (double)ctx->b.peer_timeout_ns * 1e-9, ctx->h_hdr->n_done);
+  }
   return RISM3D_OK;
 }
 
@@ -920,7 +931,11 @@ extern "C" int rism3d_slab_set_peers(rism3d_ctx* ctx, void* const* d_K, void* co
     if (!d_K[r] || !d_gram[r] || !d_flags[r]) return fail(ctx, RISM3D_ERR_ARG, "peer %d: NULL pointer", r);
   if (d_K[g.rank] != (void*)ctx->b.kbuf || d_gram[g.rank] != (void*)ctx->b.gram_x || d_flags[g.rank] != (void*)ctx->b.xflags)
     return fail(ctx, RISM3D_ERR_ARG, "entry %d must be this rank's own arrays (rism3d_slab_local)", g.rank);
+  // every (re)connection starts the barrier epochs from zero on every rank: a rank whose context was re-created would
+  // otherwise count from 0 while the others keep their old epochs (all ranks call set_peers, then meet on the host)
+  CU(cudaMemsetAsync(ctx->b.xflags, 0, (MAX_RANKS + 1) * sizeof(unsigned long long), ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
+  ctx->peer_broken = false;
   // rank r's rows of the spectrum sit in block `rank` of rank r's K: stores on the way in, loads on the way out
   const size_t blk = (size_t)g.nxl * g.nyl * g.q();
   for (int r = 0; r < g.n_ranks; ++r) {
@@ -935,6 +950,40 @@ extern "C" int rism3d_slab_set_peers(rism3d_ctx* ctx, void* const* d_K, void* co
   if (ctx->graph1) { cudaGraphExecDestroy(ctx->graph1); ctx->graph1 = nullptr; }
   if (ctx->graph_pack) { cudaGraphExecDestroy(ctx->graph_pack); ctx->graph_pack = nullptr; }
   ctx->graph_tried = false;
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_slab_set_peer_timeout(rism3d_ctx* ctx, double seconds) {
+  if (!ctx) return RISM3D_ERR_ARG;
+  ON_CTX_DEVICE(ctx);
+  if (ctx->g.n_ranks <= 1) return fail(ctx, RISM3D_ERR_ORDER, "not a slab run (rism3d_params.n_ranks <= 1)");
+  if (!(seconds >= 1e-3) || !(seconds <= 3600.0)) return fail(ctx, RISM3D_ERR_ARG, "timeout %g s outside 0.001..3600", seconds);
+  CU(cudaStreamSynchronize(ctx->stream));
+  ctx->b.peer_timeout_ns = (unsigned long long)(seconds * 1e9);
+  // the limit is a launch parameter of the captured barrier kernels
+  if (ctx->graph1) { cudaGraphExecDestroy(ctx->graph1); ctx->graph1 = nullptr; }
+  if (ctx->graph_pack) { cudaGraphExecDestroy(ctx->graph_pack); ctx->graph_pack = nullptr; }
+  ctx->graph_tried = false;
+  return RISM3D_OK;
+}
+
+extern "C" int rism3d_debug_peer_barrier_selftest(int device, void* d_scratch, size_t bytes, void* cuda_stream, int n_ranks,
+                                                  int epochs, int absent_rank, double timeout_s, int* n_errors,
+                                                  int* n_timeouts) {
+  if (!d_scratch || bytes < 4096 || !n_errors || !n_timeouts) return RISM3D_ERR_ARG;
+  if (n_ranks < 1 || n_ranks > MAX_RANKS || epochs < 1 || absent_rank >= n_ranks) return RISM3D_ERR_ARG;
+  if (!(timeout_s >= 1e-3) || !(timeout_s <= 60.0)) return RISM3D_ERR_ARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return RISM3D_ERR_CUDA;
+  DeviceGuard guard(device);
+  int res[2] = {-1, -1};
+  if (run_xbarrier_selftest(d_scratch, n_ranks, epochs, absent_rank, (unsigned long long)(timeout_s * 1e9), res,
+                            (cudaStream_t)cuda_stream) != cudaSuccess) {
+    cudaGetLastError();
+    return RISM3D_ERR_CUDA;
+  }
+  *n_errors = res[0];
+  *n_timeouts = res[1];
   return RISM3D_OK;
 }
 

@@ -819,32 +819,107 @@ int launch_gram_solve(const Grid& gr, const Buffers& b, const SolverParams& sp, 
 // every rank's flag array (release, system scope: the stores of the kernels before it in the stream are visible to
 // whoever sees the flag) and waits until all slots of its own array have reached that epoch.  All ranks enqueue the same
 // sequence of kernels, so epochs agree without any host involvement; the kernel is graph-capturable.
+// The wait is BOUNDED: a rank that never arrives (its process died, it enqueued fewer barriers, its context was
+// re-created without a new rism3d_slab_set_peers on every rank) would otherwise leave the others spinning inside a
+// kernel for ever.  After timeout_ns without all arrivals the function gives up and returns false.
 struct FlagPtrs { unsigned long long* p[MAX_RANKS]; };
-__global__ void __launch_bounds__(32)
-    xbarrier_kernel(unsigned long long* __restrict__ mine, FlagPtrs peers, int n_ranks, int rank) {
-  __shared__ unsigned long long s_epoch;
+
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;\n" : "=l"(t));
+  return t;
+}
+
+// one warp per rank (blockDim.x == 32); `mine` = this rank's [MAX_RANKS + 1] flags (the last entry is its epoch counter)
+__device__ __forceinline__ bool xbarrier_arrive_and_wait(unsigned long long* mine, const FlagPtrs& peers, int n_ranks,
+                                                         int rank, unsigned long long timeout_ns) {
   const int lane = threadIdx.x;
+  unsigned long long epoch = 0;
   if (lane == 0) {
-    s_epoch = mine[MAX_RANKS] + 1;
-    mine[MAX_RANKS] = s_epoch;
+    epoch = mine[MAX_RANKS] + 1;
+    mine[MAX_RANKS] = epoch;
   }
-  __syncwarp();
-  const unsigned long long epoch = s_epoch;
+  epoch = __shfl_sync(0xffffffffu, epoch, 0);
   __threadfence_system();
+  bool ok = true;
   if (lane < n_ranks) {
     asm volatile("st.release.sys.global.u64 [%0], %1;\n" ::"l"(peers.p[lane] + rank), "l"(epoch) : "memory");
-    unsigned long long seen;
-    do {
+    const unsigned long long t0 = global_timer_ns();
+    unsigned spins = 0;
+    for (;;) {
+      unsigned long long seen;
       asm volatile("ld.acquire.sys.global.u64 %0, [%1];\n" : "=l"(seen) : "l"(mine + lane) : "memory");
-    } while (seen < epoch);
+      if (seen >= epoch) break;
+      if ((++spins & 63u) == 0u && global_timer_ns() - t0 > timeout_ns) { ok = false; break; }
+    }
+  }
+  return __all_sync(0xffffffffu, ok);
+}
+
+// On a timeout the rank's solver state is marked: done = 1 makes every later loop kernel of the call return at once,
+// status = RISM3D_ERR_PEER is what rism3d_iterate reports; later barriers of the same call do not wait again (the epochs
+// of the ranks no longer agree: the run has to be reconnected with rism3d_slab_set_peers on every rank).
+__global__ void __launch_bounds__(32)
+    xbarrier_kernel(unsigned long long* __restrict__ mine, FlagPtrs peers, int n_ranks, int rank, DevState* st,
+                    unsigned long long timeout_ns) {
+  if (st->status == RISM3D_ERR_PEER) return;
+  const bool ok = xbarrier_arrive_and_wait(mine, peers, n_ranks, rank, timeout_ns);
+  if (!ok && threadIdx.x == 0) {
+    st->status = RISM3D_ERR_PEER;
+    st->done = 1;
   }
 }
 
 int launch_xbarrier(const Grid& gr, const Buffers& b, cudaStream_t s) {
   FlagPtrs fp{};
   for (int r = 0; r < gr.n_ranks; ++r) fp.p[r] = b.flag_dst[r];
-  xbarrier_kernel<<<1, 32, 0, s>>>(b.xflags, fp, gr.n_ranks, gr.rank);
+  xbarrier_kernel<<<1, 32, 0, s>>>(b.xflags, fp, gr.n_ranks, gr.rank, b.state, b.peer_timeout_ns);
   return 1;
+}
+
+// Self-test of the barrier on ONE GPU (rism3d_debug_peer_barrier_selftest).  Kernels that wait on one another must not be
+// run as separate launches on one device -- nothing guarantees that they are resident together -- so the ranks are the
+// blocks of one cooperative launch: block r is rank r, with its own flag array in `flags` ([n_ranks][MAX_RANKS + 1],
+// zero on entry), and runs the same xbarrier_arrive_and_wait as the production kernel `epochs` times.  Before barrier e
+// rank r publishes data[r] = e * 1000 + r with a plain store; after it, every rank must see at least that value from
+// every other rank (the release / acquire pair orders it).  absent_rank >= 0: that block leaves at once, every other
+// rank must give up within timeout_ns and reports it.  result[0] += ordering errors, result[1] += ranks that timed out.
+__global__ void __launch_bounds__(32)
+    xbarrier_selftest_kernel(unsigned long long* flags, volatile unsigned long long* data, int* result, int n_ranks,
+                             int epochs, int absent_rank, unsigned long long timeout_ns) {
+  const int rank = blockIdx.x, lane = threadIdx.x;
+  if (rank == absent_rank) return;
+  FlagPtrs fp{};
+  for (int r = 0; r < n_ranks; ++r) fp.p[r] = flags + (size_t)r * (MAX_RANKS + 1);
+  for (int e = 1; e <= epochs; ++e) {
+    if (lane == 0) data[rank] = (unsigned long long)e * 1000ull + rank;
+    __syncwarp();
+    if (!xbarrier_arrive_and_wait(fp.p[rank], fp, n_ranks, rank, timeout_ns)) {
+      if (lane == 0) atomicAdd(result + 1, 1);
+      return;
+    }
+    if (lane < n_ranks) {
+      const unsigned long long v = data[lane];
+      if (v < (unsigned long long)e * 1000ull + lane || v % 1000ull != (unsigned long long)lane) atomicAdd(result, 1);
+    }
+    __syncwarp();
+  }
+}
+
+// d_scratch: >= 4096 bytes, zeroed here on `s`; h_result[2] (pinned or pageable) receives (errors, timeouts) after a sync
+cudaError_t run_xbarrier_selftest(void* d_scratch, int n_ranks, int epochs, int absent_rank, unsigned long long timeout_ns,
+                                  int h_result[2], cudaStream_t s) {
+  cudaError_t e = cudaMemsetAsync(d_scratch, 0, 4096, s);
+  if (e != cudaSuccess) return e;
+  unsigned long long* flags = (unsigned long long*)d_scratch;                       // 8 x 9 x 8 = 576 bytes
+  unsigned long long* data = flags + (size_t)MAX_RANKS * (MAX_RANKS + 1);            // 64 bytes
+  int* result = (int*)(data + MAX_RANKS);
+  void* args[] = {&flags, &data, &result, &n_ranks, &epochs, &absent_rank, &timeout_ns};
+  e = cudaLaunchCooperativeKernel((const void*)xbarrier_selftest_kernel, dim3(n_ranks), dim3(32), args, 0, s);
+  if (e != cudaSuccess) return e;
+  e = cudaMemcpyAsync(h_result, result, 2 * sizeof(int), cudaMemcpyDeviceToHost, s);
+  if (e != cudaSuccess) return e;
+  return cudaStreamSynchronize(s);
 }
 
 }  // namespace r3d

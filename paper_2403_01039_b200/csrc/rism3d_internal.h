@@ -105,6 +105,7 @@ struct Buffers {
   unsigned long long* flag_dst[MAX_RANKS];   // peer mode: xflags of every rank
   int n_gram_dst;
   bool peer_mode;
+  unsigned long long peer_timeout_ns;        // longest wait of one in-stream barrier (rism3d_slab_set_peer_timeout)
   // TMA descriptors of the k-space pass (built by rism3d_init when kspace_uses_tma(n)): `work` as a 2D array of doubles
   // [jx][2 n Q] with boxes of n rows x 128 bytes, `phik` as [jx][2 n n/2] with boxes of n rows x (8 / nv) complex
   CUtensorMap tm_work, tm_phik;
@@ -142,6 +143,8 @@ int launch_y_inv(const Grid&, const Buffers&, bool use_state, cudaStream_t);   /
 int launch_gram_solve(const Grid&, const Buffers&, const SolverParams&, cudaStream_t);   // slab runs: sum the ranks' rows, solve
 int launch_gram_solve_rows(DevState*, const double* rows, int n_rows, const SolverParams&, double n_values, cudaStream_t);
 int launch_xbarrier(const Grid&, const Buffers&, cudaStream_t);                // peer mode: all ranks have reached this point
+cudaError_t run_xbarrier_selftest(void* d_scratch, int n_ranks, int epochs, int absent_rank, unsigned long long timeout_ns,
+                                  int h_result[2], cudaStream_t);
 int launch_zinv_residual(const Grid&, const Buffers&, const SolverParams&, double* d_raw_out, cudaStream_t);
 int zinv_ctas(const Grid&);                      // CTAs of zinv_residual (it writes one Gram partial per CTA)
 // mdiis_kernels.cu

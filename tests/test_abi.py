@@ -108,6 +108,7 @@ def test_workspace_bytes_and_argument_checks_without_a_device(lib):
     assert handle.rism3d_launch_count(None) == 0
     handle.rism3d_destroy(None)
     assert lib.rism3d_status_string(-8) == "iteration diverged"
+    assert "barrier" in lib.rism3d_status_string(-9)
     assert lib.rism3d_loop_kernel_name(0) != "" and lib.rism3d_loop_kernel_name(99) == ""
 
 

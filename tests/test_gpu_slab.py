@@ -288,3 +288,55 @@ def test_slab_peer_table_checks():
     assert a.peer_mode
     a.close()
     b.close()
+
+
+# ---- the in-stream barrier of peer mode ---------------------------------------------------------------------------
+# Kernels that wait on one another must not be run as separate launches on one GPU (nothing guarantees that they are
+# resident together), so the barrier is exercised as ONE cooperative launch whose blocks are the ranks and run the
+# production barrier function (rism3d_debug_peer_barrier_selftest); the wait is bounded either way.
+@pytest.mark.parametrize("P", [1, 2, 4, 8])
+def test_peer_barrier_orders_the_ranks(P):
+    import torch
+    import paper_2403_01039_b200 as lib
+    scratch = torch.empty(4096, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    errors, timeouts = lib.rism3d_debug_peer_barrier_selftest(0, scratch.data_ptr(), scratch.numel(), stream.cuda_stream,
+                                                              P, 500, -1, 5.0)
+    assert (errors, timeouts) == (0, 0)
+
+
+def test_peer_barrier_gives_up_on_an_absent_rank():
+    import time
+    import torch
+    import paper_2403_01039_b200 as lib
+    scratch = torch.empty(4096, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.Stream()
+    stream.wait_stream(torch.cuda.current_stream())
+    t0 = time.time()
+    errors, timeouts = lib.rism3d_debug_peer_barrier_selftest(0, scratch.data_ptr(), scratch.numel(), stream.cuda_stream,
+                                                              4, 10, 2, 0.05)
+    assert (errors, timeouts) == (0, 3)                      # the three ranks that did arrive all report the missing one
+    assert time.time() - t0 < 5.0                            # ... after the 50 ms limit, not never
+    with pytest.raises(lib.Rism3dError):
+        lib.rism3d_debug_peer_barrier_selftest(0, scratch.data_ptr(), 1024, stream.cuda_stream, 2, 1)     # scratch too small
+    with pytest.raises(lib.Rism3dError):
+        lib.rism3d_debug_peer_barrier_selftest(0, scratch.data_ptr(), 4096, stream.cuda_stream, 9, 1)     # > 8 ranks
+
+
+def test_peer_timeout_setting_and_status():
+    import torch
+    import paper_2403_01039_b200 as lib
+    assert "barrier" in lib.rism3d_status_string(-9)
+    a = lib.SlabSolver(32, 0.5, 2, 2, 0, stream=torch.cuda.Stream())
+    a.set_peer_timeout(2.0)
+    for bad in (0.0, -1.0, 1e5, float("nan")):
+        with pytest.raises(lib.Rism3dError) as e:
+            a.set_peer_timeout(bad)
+        assert e.value.status == -1
+    a.close()
+    one = lib.Solver(32, 0.5, 2)
+    with pytest.raises(lib.Rism3dError) as e:
+        lib.rism3d_slab_set_peer_timeout(one.ctx, 1.0)       # not a slab run
+    assert e.value.status == -3
+    one.close()
