@@ -359,7 +359,10 @@ def run_ours(args):
     dominant = max(kernels, key=lambda k: kernels[k]["ms"])
     traffic = ncu_traffic(dominant, args.workload)
     roofline = {"bound": "hbm", "kernel": dominant, "achieved": kernels[dominant]["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": kernels[dominant]["frac"], "traffic": traffic, "peak_source": peak_src,
+                "frac": kernels[dominant]["frac"], "traffic": traffic,
+                # NOT measured by this run: the stored figure of one committed ncu --set full capture of the same kernel
+                "traffic_source": "profiles/traffic.json (static: copied from a committed ncu --set full capture, not re-measured by this run)" if traffic is not None else None,
+                "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": kernels[dominant]["algorithmic_gb"] * 1e9,
                 "iteration": {"ms_sum_of_kernels": sum(k["ms"] for k in kernels.values()),
                               "algorithmic_gb": sum(k["algorithmic_gb"] for k in kernels.values()),
