@@ -294,6 +294,7 @@ struct rism1d_ctx {
   int ns, M, L, npairs, n_rows;
   size_t field;
   double beta, lam;
+  bool lam_set;              // a solve has fixed the charge scale (until then the getters build w with lam = 1)
   Solvent1d sv;
   bool have_solvent, w_valid;
   DevState* state;
@@ -393,7 +394,8 @@ extern "C" int rism1d_init(rism1d_ctx** out, const rism1d_params* p, void* d_ws,
   ctx->field = (size_t)ctx->npairs * ctx->M;
   ctx->n_rows = rows_of(p);
   ctx->beta = 1.0 / (K_BOLTZMANN * p->temperature);
-  ctx->lam = -1.0;
+  ctx->lam = 1.0;
+  ctx->lam_set = false;
   carve1(p, (char*)d_ws, ctx);
   SolverParams& sp = ctx->sp;
   memset(&sp, 0, sizeof(sp));
@@ -432,19 +434,29 @@ extern "C" int rism1d_set_solvent(rism1d_ctx* ctx, const double* q, const double
   if (!ctx) return RISM3D_ERR_ARG;
   if (!q || !sigma || !eps || !rho || !species || !bond) return fail1(ctx, RISM3D_ERR_ARG, "bad argument");
   const int ns = ctx->ns;
+  // everything is checked on a local copy: a refused call leaves the context's solvent (and its flags) as they were
+  Solvent1d sv;
+  memset(&sv, 0, sizeof(sv));
   double neutral = 0.0;
-  for (int a = 0; a < ns; ++a) neutral += rho[a] * q[a];
-  if (fabs(neutral) > 1e-12) return fail1(ctx, RISM3D_ERR_NEUTRAL, "sum rho_a q_a = %.3e", neutral);
-  memset(&ctx->sv, 0, sizeof(ctx->sv));
   for (int a = 0; a < ns; ++a) {
-    ctx->sv.q[a] = q[a]; ctx->sv.sigma[a] = sigma[a]; ctx->sv.eps[a] = eps[a]; ctx->sv.rho[a] = rho[a];
-    ctx->sv.species[a] = species[a];
+    if (!isfinite(q[a]) || !isfinite(eps[a]) || !(eps[a] >= 0.0))
+      return fail1(ctx, RISM3D_ERR_ARG, "site %d: q and eps must be finite, eps >= 0 (q = %g, eps = %g)", a, q[a], eps[a]);
+    if (!isfinite(sigma[a]) || !(sigma[a] > 0.0) || !isfinite(rho[a]) || !(rho[a] > 0.0))
+      return fail1(ctx, RISM3D_ERR_ARG, "site %d: sigma and rho must be positive (sigma = %g, rho = %g)", a, sigma[a], rho[a]);
+    if (species[a] < 0 || species[a] >= ns) return fail1(ctx, RISM3D_ERR_ARG, "site %d: species %d outside 0..%d", a, species[a], ns - 1);
+    neutral += rho[a] * q[a];
+  }
+  if (fabs(neutral) > 1e-12) return fail1(ctx, RISM3D_ERR_NEUTRAL, "sum rho_a q_a = %.3e", neutral);
+  for (int a = 0; a < ns; ++a) {
+    sv.q[a] = q[a]; sv.sigma[a] = sigma[a]; sv.eps[a] = eps[a]; sv.rho[a] = rho[a];
+    sv.species[a] = species[a];
     for (int b = 0; b < ns; ++b) {
-      ctx->sv.bond[a][b] = bond[a * ns + b];
-      if (a != b && species[a] == species[b] && !(bond[a * ns + b] > 0.0))
+      sv.bond[a][b] = bond[a * ns + b];
+      if (a != b && species[a] == species[b] && !(bond[a * ns + b] > 0.0 && isfinite(bond[a * ns + b])))
         return fail1(ctx, RISM3D_ERR_ARG, "sites %d and %d share a species but have no bond length", a, b);
     }
   }
+  ctx->sv = sv;
   ctx->have_solvent = true;
   ctx->w_valid = false;
   return RISM3D_OK;
@@ -481,6 +493,7 @@ static int ensure_w(rism1d_ctx* ctx, double lam) {
   ctx->launches += 1;
   CU1(cudaGetLastError());
   ctx->lam = lam;
+  ctx->lam_set = true;
   ctx->w_valid = true;
   return RISM3D_OK;
 }
@@ -515,6 +528,7 @@ extern "C" int rism1d_solve(rism1d_ctx* ctx, double charge_scale, int max_iter, 
   if (!ctx) return RISM3D_ERR_ARG;
   DeviceGuard1 guard(ctx->p.device);
   if (max_iter < 0) return fail1(ctx, RISM3D_ERR_ARG, "max_iter < 0");
+  if (!isfinite(charge_scale) || charge_scale < 0.0) return fail1(ctx, RISM3D_ERR_ARG, "charge_scale = %g (must be finite and >= 0)", charge_scale);
   if (!ctx->have_solvent) return fail1(ctx, RISM3D_ERR_ORDER, "set_solvent must come before solve");
   int rc = ensure_w(ctx, charge_scale);
   if (rc) return rc;
@@ -556,7 +570,7 @@ extern "C" int rism1d_get_pair(rism1d_ctx* ctx, int which, double* dst) {
   DeviceGuard1 guard(ctx->p.device);
   if (!dst || which < 0 || which > 2) return fail1(ctx, RISM3D_ERR_ARG, "bad argument");
   if (!ctx->have_solvent) return fail1(ctx, RISM3D_ERR_ORDER, "set_solvent must come first");
-  int rc = ensure_w(ctx, ctx->lam < 0.0 ? 1.0 : ctx->lam);
+  int rc = ensure_w(ctx, ctx->lam_set ? ctx->lam : 1.0);
   if (rc) return rc;
   const int n = ctx->npairs * (ctx->M - 1);
   double* d = (double*)ctx->bufA;                                          // scratch between iterations
@@ -574,7 +588,7 @@ extern "C" int rism1d_get_chi(rism1d_ctx* ctx, double* dst) {
   DeviceGuard1 guard(ctx->p.device);
   if (!dst) return fail1(ctx, RISM3D_ERR_ARG, "dst is NULL");
   if (!ctx->have_solvent) return fail1(ctx, RISM3D_ERR_ORDER, "set_solvent must come first");
-  int rc = ensure_w(ctx, ctx->lam < 0.0 ? 1.0 : ctx->lam);
+  int rc = ensure_w(ctx, ctx->lam_set ? ctx->lam : 1.0);
   if (rc) return rc;
   CU1(cudaMemsetAsync(&ctx->state->done, 0, sizeof(int), ctx->stream));     // the transform kernels skip a finished solve
   rc = forward_half(ctx, true);
@@ -614,7 +628,7 @@ extern "C" int rism1d_thermo(rism1d_ctx* ctx, double* chi_t, double* pressure, d
   if (!ctx) return RISM3D_ERR_ARG;
   DeviceGuard1 guard(ctx->p.device);
   if (!ctx->have_solvent) return fail1(ctx, RISM3D_ERR_ORDER, "set_solvent must come first");
-  int rc = ensure_w(ctx, ctx->lam < 0.0 ? 1.0 : ctx->lam);
+  int rc = ensure_w(ctx, ctx->lam_set ? ctx->lam : 1.0);
   if (rc) return rc;
   c_integral1d_kernel<<<ctx->npairs, 256, 0, ctx->stream>>>(ctx->c0, ctx->tau, ctx->w, ctx->M, ctx->p.dr, ctx->sp.closure,
                                                            ctx->sp.pse_order);

@@ -150,4 +150,21 @@ def test_argument_and_order_checks():
     assert nd == 3 and rms > 0
     with pytest.raises(lib.Rism3dError):
         lib.rism1d_get_pair(one.ctx, 7, sv.n_s, 512)         # unknown pair function
+    # a refused set_solvent leaves the accepted solvent in place: same iterations, same numbers, before and after
+    g_before = lib.rism1d_get_pair(one.ctx, 0, sv.n_s, 512)
+    for k, bad in ((1, 0.0), (1, -1.0), (3, 0.0), (2, -0.1), (1, float("nan"))):     # sigma, rho, eps
+        a = [np.array(x, dtype=float) if i < 4 else x for i, x in enumerate(args)]
+        a[k][0] = bad
+        with pytest.raises(lib.Rism3dError) as e:
+            one.set_solvent(*a)
+        assert e.value.status == -1
+    with pytest.raises(lib.Rism3dError) as e:
+        one.set_solvent(*args[:5], no_bond)
+    assert e.value.status == -1
+    g_after = lib.rism1d_get_pair(one.ctx, 0, sv.n_s, 512)
+    assert np.array_equal(np.asarray(g_before), np.asarray(g_after))
+    for bad in (-0.5, float("nan"), float("inf")):           # a negative scale used to double as "never solved"
+        with pytest.raises(lib.Rism3dError) as e:
+            one.solve(bad, 1, 0.0)
+        assert e.value.status == -1
     one.close()
