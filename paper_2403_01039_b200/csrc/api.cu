@@ -67,8 +67,14 @@ static int fail(rism3d_ctx* c, int code, const char* fmt, ...) {
 struct DeviceGuard {
   int prev = -1;
   bool switched = false;
+  bool ok = true;            // false: `dev` could not be made current -- the caller must not go on (it would work on
+                             // whatever device happens to be current)
   explicit DeviceGuard(int dev) {
-    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = (cudaSetDevice(dev) == cudaSuccess);
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+    if (prev != dev) {
+      switched = (cudaSetDevice(dev) == cudaSuccess);
+      ok = switched;
+    }
   }
   ~DeviceGuard() {
     if (switched) cudaSetDevice(prev);
@@ -76,7 +82,33 @@ struct DeviceGuard {
   DeviceGuard(const DeviceGuard&) = delete;
   DeviceGuard& operator=(const DeviceGuard&) = delete;
 };
-#define ON_CTX_DEVICE(ctx) DeviceGuard device_guard_((ctx)->p.device)
+#define ON_CTX_DEVICE(ctx)                        \
+  DeviceGuard device_guard_((ctx)->p.device);     \
+  if (!device_guard_.ok) return fail(ctx, RISM3D_ERR_CUDA, "device %d could not be made current", (ctx)->p.device)
+
+// small RAII holders so that an early return through CU() does not leak
+struct ScopedEvents {
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  cudaError_t create() {
+    cudaError_t e = cudaEventCreate(&e0);
+    return e != cudaSuccess ? e : cudaEventCreate(&e1);
+  }
+  ~ScopedEvents() {
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+  }
+};
+struct ScopedDeviceAlloc {
+  void* p = nullptr;
+  ~ScopedDeviceAlloc() {
+    if (p) cudaFree(p);
+  }
+};
+
+static bool device_exists(int device) {
+  int n = 0;
+  return cudaGetDeviceCount(&n) == cudaSuccess && device >= 0 && device < n;
+}
 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -326,8 +358,8 @@ extern "C" int rism3d_init(rism3d_ctx** out, const rism3d_params* p, void* d_wor
 
 extern "C" void rism3d_destroy(rism3d_ctx* ctx) {
   if (!ctx) return;
-  ON_CTX_DEVICE(ctx);
-  cudaStreamSynchronize(ctx->stream);
+  DeviceGuard device_guard_(ctx->p.device);
+  if (device_guard_.ok) cudaStreamSynchronize(ctx->stream);
   if (ctx->ev_pool) {
     for (cudaEvent_t e : *ctx->ev_pool) cudaEventDestroy(e);
     delete ctx->ev_pool;
@@ -373,10 +405,10 @@ extern "C" int rism3d_set_solvent_chi(rism3d_ctx* ctx, const double* q, const do
   // the radial table is only needed until chi_shell is built: it goes through the history span (rebuilt by set_solute
   // anyway) or, on grids too small to hold it, through a temporary allocation of the library's own
   double* d_table = ctx->b.Z;
-  double* d_tmp = nullptr;
+  ScopedDeviceAlloc tmp;                             // freed on every way out, also an early CU() return
   if (tbytes > ctx->scratch_bytes) {
-    CU(cudaMalloc((void**)&d_tmp, tbytes));
-    d_table = d_tmp;
+    CU(cudaMalloc(&tmp.p, tbytes));
+    d_table = (double*)tmp.p;
   }
   CU(cudaMemcpyAsync(d_table, table, tbytes, cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaMemcpyAsync(ctx->b.qv, ctx->qv, g.nv * 8, cudaMemcpyHostToDevice, ctx->stream));
@@ -385,8 +417,7 @@ extern "C" int rism3d_set_solvent_chi(rism3d_ctx* ctx, const double* q, const do
     ctx->gramw[i] = (ctx->sp.accel == RISM3D_ACCEL_ANDERSON) ? (i < nu ? 1.0 / rho[i] : 0.0) : 1.0;
   CU(cudaMemcpyAsync(ctx->b.gram_w, ctx->gramw, g.nv * 8, cudaMemcpyHostToDevice, ctx->stream));
   ctx->launches += launch_chi_shell(g, ctx->b, d_table, n_k, k0, dk, ctx->stream);
-  const cudaError_t e_launch = cudaGetLastError(), e_sync = cudaStreamSynchronize(ctx->stream);
-  if (d_tmp) cudaFree(d_tmp);
+  const cudaError_t e_launch = cudaGetLastError(), e_sync = cudaStreamSynchronize(ctx->stream);   // before tmp goes away
   CU(e_launch);
   CU(e_sync);
   ctx->have_solvent = true;
@@ -488,9 +519,9 @@ extern "C" int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz
   double* d_pair = (double*)(scr + b_atoms);
   double2* d_phase = (double2*)(scr + b_atoms + b_pair);
   int* d_cells = (int*)(scr + b_atoms + b_pair + b_phase);
-  cudaEvent_t e0, e1;
-  CU(cudaEventCreate(&e0));
-  CU(cudaEventCreate(&e1));
+  ScopedEvents ev;
+  CU(ev.create());
+  cudaEvent_t e0 = ev.e0, e1 = ev.e1;
   if (na) {
     CU(cudaMemcpyAsync(d_atoms, up_atoms.data(), na * 4 * 8, cudaMemcpyHostToDevice, ctx->stream));
     // raw charges right after the atom records (phi~ reads them there)
@@ -518,8 +549,6 @@ extern "C" int rism3d_set_solute(rism3d_ctx* ctx, int n_atoms, const double* xyz
   CU(cudaStreamSynchronize(ctx->stream));
   float ms = 0.f;
   CU(cudaEventElapsedTime(&ms, e0, e1));
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
   if (setup_ms) *setup_ms = ms;
   if (!ctx->h_atoms) ctx->h_atoms = new std::vector<double>();
   if (!ctx->h_pair) ctx->h_pair = new std::vector<double>();
@@ -724,9 +753,9 @@ static int ensure_phi(rism3d_ctx* ctx) {
   const size_t na = (size_t)ctx->n_atoms;
   if (na * 4 * 8 > ctx->g.field * 8) return fail(ctx, RISM3D_ERR_WORKSPACE, "%d atoms do not fit the work array", ctx->n_atoms);
   double* d_atoms = (double*)ctx->b.work;
-  cudaEvent_t e0, e1;
-  CU(cudaEventCreate(&e0));
-  CU(cudaEventCreate(&e1));
+  ScopedEvents ev;
+  CU(ev.create());
+  cudaEvent_t e0 = ev.e0, e1 = ev.e1;
   CU(cudaMemcpyAsync(d_atoms, ctx->h_atoms->data(), na * 4 * 8, cudaMemcpyHostToDevice, ctx->stream));
   CU(cudaEventRecord(e0, ctx->stream));
   ctx->launches += launch_phi(ctx->g, ctx->b, ctx->sp, ctx->n_atoms, d_atoms, ctx->stream);
@@ -734,8 +763,6 @@ static int ensure_phi(rism3d_ctx* ctx) {
   CU(cudaEventRecord(e1, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   CU(cudaEventElapsedTime(&ctx->phi_ms, e0, e1));
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
   ctx->phi_valid = true;
   return RISM3D_OK;
 }
@@ -992,18 +1019,24 @@ static_assert(sizeof(cudaIpcMemHandle_t) == 64, "the ABI passes IPC handles as 6
 
 extern "C" int rism3d_peer_alloc(int device, size_t bytes, void** d_ptr) {
   if (!d_ptr || bytes == 0) return RISM3D_ERR_ARG;
+  if (!device_exists(device)) return RISM3D_ERR_ARG;
   DeviceGuard guard(device);
+  if (!guard.ok) return RISM3D_ERR_CUDA;
   return cudaMalloc(d_ptr, bytes) == cudaSuccess ? RISM3D_OK : RISM3D_ERR_CUDA;
 }
 
 extern "C" int rism3d_peer_free(int device, void* d_ptr) {
+  if (!device_exists(device)) return RISM3D_ERR_ARG;
   DeviceGuard guard(device);
+  if (!guard.ok) return RISM3D_ERR_CUDA;
   return cudaFree(d_ptr) == cudaSuccess ? RISM3D_OK : RISM3D_ERR_CUDA;
 }
 
 extern "C" int rism3d_peer_export(int device, void* d_ptr, unsigned char handle[64]) {
   if (!d_ptr || !handle) return RISM3D_ERR_ARG;
+  if (!device_exists(device)) return RISM3D_ERR_ARG;
   DeviceGuard guard(device);
+  if (!guard.ok) return RISM3D_ERR_CUDA;
   cudaIpcMemHandle_t h;
   if (cudaIpcGetMemHandle(&h, d_ptr) != cudaSuccess) return RISM3D_ERR_CUDA;
   memcpy(handle, &h, 64);
@@ -1012,14 +1045,18 @@ extern "C" int rism3d_peer_export(int device, void* d_ptr, unsigned char handle[
 
 extern "C" int rism3d_peer_open(int device, const unsigned char handle[64], void** d_ptr) {
   if (!d_ptr || !handle) return RISM3D_ERR_ARG;
+  if (!device_exists(device)) return RISM3D_ERR_ARG;
   DeviceGuard guard(device);
+  if (!guard.ok) return RISM3D_ERR_CUDA;
   cudaIpcMemHandle_t h;
   memcpy(&h, handle, 64);
   return cudaIpcOpenMemHandle(d_ptr, h, cudaIpcMemLazyEnablePeerAccess) == cudaSuccess ? RISM3D_OK : RISM3D_ERR_CUDA;
 }
 
 extern "C" int rism3d_peer_close(int device, void* d_ptr) {
+  if (!device_exists(device)) return RISM3D_ERR_ARG;
   DeviceGuard guard(device);
+  if (!guard.ok) return RISM3D_ERR_CUDA;
   return cudaIpcCloseMemHandle(d_ptr) == cudaSuccess ? RISM3D_OK : RISM3D_ERR_CUDA;
 }
 

@@ -324,8 +324,13 @@ static int fail1(rism1d_ctx* ctx, int code, const char* fmt, ...) {
 struct DeviceGuard1 {
   int prev = -1;
   bool switched = false;
+  bool ok = true;            // false: the context's device could not be made current
   explicit DeviceGuard1(int dev) {
-    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = (cudaSetDevice(dev) == cudaSuccess);
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+    if (prev != dev) {
+      switched = (cudaSetDevice(dev) == cudaSuccess);
+      ok = switched;
+    }
   }
   ~DeviceGuard1() {
     if (switched) cudaSetDevice(prev);
@@ -386,6 +391,7 @@ extern "C" int rism1d_init(rism1d_ctx** out, const rism1d_params* p, void* d_ws,
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || p->device < 0 || ndev <= p->device) return RISM3D_ERR_CUDA;
   DeviceGuard1 guard(p->device);
+  if (!guard.ok) return RISM3D_ERR_CUDA;
   rism1d_ctx* ctx = new rism1d_ctx();
   memset(ctx, 0, sizeof(*ctx));
   ctx->p = *p;
@@ -527,6 +533,7 @@ static int read_header1(rism1d_ctx* ctx) {
 extern "C" int rism1d_solve(rism1d_ctx* ctx, double charge_scale, int max_iter, double tol, int* n_done, double* rms) {
   if (!ctx) return RISM3D_ERR_ARG;
   DeviceGuard1 guard(ctx->p.device);
+  if (!guard.ok) return fail1(ctx, RISM3D_ERR_CUDA, "device %d could not be made current", ctx->p.device);
   if (max_iter < 0) return fail1(ctx, RISM3D_ERR_ARG, "max_iter < 0");
   if (!isfinite(charge_scale) || charge_scale < 0.0) return fail1(ctx, RISM3D_ERR_ARG, "charge_scale = %g (must be finite and >= 0)", charge_scale);
   if (!ctx->have_solvent) return fail1(ctx, RISM3D_ERR_ORDER, "set_solvent must come before solve");
@@ -568,6 +575,7 @@ extern "C" int rism1d_solve(rism1d_ctx* ctx, double charge_scale, int max_iter, 
 extern "C" int rism1d_get_pair(rism1d_ctx* ctx, int which, double* dst) {
   if (!ctx) return RISM3D_ERR_ARG;
   DeviceGuard1 guard(ctx->p.device);
+  if (!guard.ok) return fail1(ctx, RISM3D_ERR_CUDA, "device %d could not be made current", ctx->p.device);
   if (!dst || which < 0 || which > 2) return fail1(ctx, RISM3D_ERR_ARG, "bad argument");
   if (!ctx->have_solvent) return fail1(ctx, RISM3D_ERR_ORDER, "set_solvent must come first");
   int rc = ensure_w(ctx, ctx->lam_set ? ctx->lam : 1.0);
@@ -586,6 +594,7 @@ extern "C" int rism1d_get_pair(rism1d_ctx* ctx, int which, double* dst) {
 extern "C" int rism1d_get_chi(rism1d_ctx* ctx, double* dst) {
   if (!ctx) return RISM3D_ERR_ARG;
   DeviceGuard1 guard(ctx->p.device);
+  if (!guard.ok) return fail1(ctx, RISM3D_ERR_CUDA, "device %d could not be made current", ctx->p.device);
   if (!dst) return fail1(ctx, RISM3D_ERR_ARG, "dst is NULL");
   if (!ctx->have_solvent) return fail1(ctx, RISM3D_ERR_ORDER, "set_solvent must come first");
   int rc = ensure_w(ctx, ctx->lam_set ? ctx->lam : 1.0);
@@ -627,6 +636,7 @@ extern "C" int rism1d_get_chi_types(rism1d_ctx* ctx, int n_types, const int* sit
 extern "C" int rism1d_thermo(rism1d_ctx* ctx, double* chi_t, double* pressure, double* c0) {
   if (!ctx) return RISM3D_ERR_ARG;
   DeviceGuard1 guard(ctx->p.device);
+  if (!guard.ok) return fail1(ctx, RISM3D_ERR_CUDA, "device %d could not be made current", ctx->p.device);
   if (!ctx->have_solvent) return fail1(ctx, RISM3D_ERR_ORDER, "set_solvent must come first");
   int rc = ensure_w(ctx, ctx->lam_set ? ctx->lam : 1.0);
   if (rc) return rc;

@@ -109,6 +109,11 @@ def test_workspace_bytes_and_argument_checks_without_a_device(lib):
     handle.rism3d_destroy(None)
     assert lib.rism3d_status_string(-8) == "iteration diverged"
     assert "barrier" in lib.rism3d_status_string(-9)
+    # the IPC helpers take a device ordinal, not a context: one that does not exist is refused before any CUDA call on it
+    ptr = C.c_void_p()
+    assert handle.rism3d_peer_alloc(4096, 1024, C.byref(ptr)) == -1 and not ptr.value
+    assert handle.rism3d_peer_free(-1, None) == -1
+    assert handle.rism3d_peer_close(4096, None) == -1
     assert lib.rism3d_loop_kernel_name(0) != "" and lib.rism3d_loop_kernel_name(99) == ""
 
 
