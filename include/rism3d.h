@@ -306,6 +306,12 @@ int rism3d_slab_phase(rism3d_ctx* ctx, int phase);
 int rism3d_slab_status(rism3d_ctx* ctx, int* done, int* n_done, double* rms);
 int rism3d_slab_end(rism3d_ctx* ctx, int* n_done, double* rms);
 
+/* Slab runs: free_energy, pmv, pressure_correction and gradient return THIS rank's share of a grid sum; the whole-grid
+ * value is the sum of the ranks' shares.  The caller gathers the shares (an all-gather: data movement only) and this call
+ * adds them, in rank order, so that every rank gets the same bits whatever the collective library does:
+ * per_rank: HOST [n_ranks][n_values], out: HOST [n_values], out[j] = sum_r per_rank[r][j] (r = 0, 1, ...).  Host-only. */
+int rism3d_slab_combine(const double* per_rank, int n_ranks, int n_values, double* out);
+
 const char* rism3d_last_error(const rism3d_ctx* ctx);   /* valid until the next call on ctx */
 const char* rism3d_status_string(int status);           /* static strings                    */
 

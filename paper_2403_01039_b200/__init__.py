@@ -12,7 +12,7 @@ from .binding import (  # noqa: F401
     rism3d_set_profiling, rism3d_get_timings, rism3d_loop_kernel_name, N_LOOP_KERNELS,
     rism3d_debug_fft_forward, rism3d_debug_fft_inverse, rism3d_last_error, rism3d_status_string,
     rism3d_destroy, EXPORTED_SYMBOLS, Rism3dSlabInfo, rism3d_slab_plan, rism3d_slab_local, rism3d_slab_set_peers,
-    rism3d_slab_begin, rism3d_slab_phase, rism3d_slab_set_peer_timeout, rism3d_debug_peer_barrier_selftest, rism3d_slab_status, rism3d_slab_end, SlabSolver, iterate_in_lockstep,
+    rism3d_slab_begin, rism3d_slab_phase, rism3d_slab_set_peer_timeout, rism3d_slab_combine, rism3d_debug_peer_barrier_selftest, rism3d_slab_status, rism3d_slab_end, SlabSolver, iterate_in_lockstep,
     rism3d_peer_alloc, rism3d_peer_free, rism3d_peer_export, rism3d_peer_open, rism3d_peer_close,
     EXPORTED_SYMBOLS_1D, Rism1dParams, Solver1d, rism1d_workspace_bytes, rism1d_init, rism1d_set_solvent, rism1d_solve,
     rism1d_get_pair, rism1d_get_chi, rism1d_get_chi_types, rism1d_thermo, rism1d_launch_count, rism1d_last_error,

@@ -25,6 +25,7 @@ EXPORTED_SYMBOLS = [
     "rism3d_debug_fft_inverse", "rism3d_last_error", "rism3d_status_string", "rism3d_destroy",
     "rism3d_slab_plan", "rism3d_slab_local", "rism3d_slab_set_peers", "rism3d_slab_begin", "rism3d_slab_phase",
     "rism3d_slab_status", "rism3d_slab_end", "rism3d_slab_set_peer_timeout", "rism3d_debug_peer_barrier_selftest",
+    "rism3d_slab_combine",
     "rism3d_peer_alloc", "rism3d_peer_free", "rism3d_peer_export", "rism3d_peer_open", "rism3d_peer_close",
 ]
 EXPORTED_SYMBOLS_1D = [
@@ -148,6 +149,8 @@ def load_library():
     lib.rism3d_debug_peer_barrier_selftest.restype = C.c_int
     lib.rism3d_debug_peer_barrier_selftest.argtypes = [C.c_int, C.c_void_p, C.c_size_t, C.c_void_p, C.c_int, C.c_int, C.c_int,
                                                        C.c_double, ip, ip]
+    lib.rism3d_slab_combine.restype = C.c_int
+    lib.rism3d_slab_combine.argtypes = [dp, C.c_int, C.c_int, dp]
     lib.rism3d_slab_begin.restype = C.c_int
     lib.rism3d_slab_begin.argtypes = [C.c_void_p, C.c_double]
     lib.rism3d_slab_phase.restype = C.c_int
@@ -384,6 +387,18 @@ def rism3d_slab_set_peers(ctx, d_K, d_gram, d_flags):
     n = len(d_K)
     arr = lambda v: (C.c_void_p * n)(*[int(x) for x in v])
     _check(ctx, load_library().rism3d_slab_set_peers(ctx, arr(d_K), arr(d_gram), arr(d_flags)))
+
+
+def rism3d_slab_combine(per_rank) -> np.ndarray:
+    """[n_ranks][n_values] shares of the ranks -> their sums in rank order (the addition happens in the library)"""
+    rows = _f64(per_rank)
+    if rows.ndim != 2:
+        raise ValueError(f"per_rank must be [n_ranks][n_values], got shape {rows.shape}")
+    out = np.zeros(rows.shape[1])
+    st = load_library().rism3d_slab_combine(_dptr(rows), int(rows.shape[0]), int(rows.shape[1]), _dptr(out))
+    if st != 0:
+        raise Rism3dError(st, rism3d_status_string(st))
+    return out
 
 
 def rism3d_slab_set_peer_timeout(ctx, seconds: float):
@@ -801,13 +816,15 @@ class SlabSolver(Solver):
         return self.end()
 
     def _sum_over_ranks(self, values):
+        """all-gather the ranks' shares (data movement), add them in rank order inside the library (rism3d_slab_combine)"""
         import torch
         import torch.distributed as dist
-        t = torch.as_tensor(np.asarray(values, dtype=np.float64))
+        t = torch.as_tensor(np.ascontiguousarray(np.asarray(values, dtype=np.float64).reshape(-1)))
         if self._device_collectives():
             t = t.to(self.device)
-        dist.all_reduce(t, group=self.group)
-        return t.cpu().numpy()
+        rows = torch.empty(self.n_ranks * t.numel(), dtype=torch.float64, device=t.device)     # flat: rank r's share at r * n
+        dist.all_gather_into_tensor(rows, t, group=self.group)
+        return rism3d_slab_combine(rows.cpu().numpy().reshape(self.n_ranks, t.numel())).reshape(np.shape(values))
 
     def free_energy(self):
         mu, site = rism3d_free_energy(self.ctx, self.n_sites)
@@ -820,8 +837,10 @@ class SlabSolver(Solver):
         return float(tot[0]), tot[1:]
 
     def pressure_correction(self, chi_t: float, pressure: float):
-        v, _ = self.pmv(chi_t)
-        return -pressure * v, v
+        # every rank's call returns its share of -P V (Eq. 21) and of V: both are sums over the slabs
+        pc, v = rism3d_pressure_correction(self.ctx, chi_t, pressure)
+        tot = self._sum_over_ranks(np.array([pc, v]))
+        return float(tot[0]), float(tot[1])
 
     def gradient(self) -> np.ndarray:
         return self._sum_over_ranks(rism3d_gradient(self.ctx, self.n_atoms))

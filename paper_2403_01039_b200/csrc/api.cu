@@ -980,6 +980,16 @@ extern "C" int rism3d_slab_set_peers(rism3d_ctx* ctx, void* const* d_K, void* co
   return RISM3D_OK;
 }
 
+extern "C" int rism3d_slab_combine(const double* per_rank, int n_ranks, int n_values, double* out) {
+  if (!per_rank || !out || n_ranks < 1 || n_ranks > MAX_RANKS || n_values < 0) return RISM3D_ERR_ARG;
+  for (int j = 0; j < n_values; ++j) {
+    double acc = 0.0;
+    for (int r = 0; r < n_ranks; ++r) acc += per_rank[(size_t)r * n_values + j];   // fixed rank order, as the Gram rows
+    out[j] = acc;
+  }
+  return RISM3D_OK;
+}
+
 extern "C" int rism3d_slab_set_peer_timeout(rism3d_ctx* ctx, double seconds) {
   if (!ctx) return RISM3D_ERR_ARG;
   ON_CTX_DEVICE(ctx);
